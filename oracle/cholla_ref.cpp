@@ -1,0 +1,668 @@
+// cholla_ref.cpp — ORACLE. TEST INFRASTRUCTURE ONLY.
+//
+// A plain, slow, obviously-correct CPU implementation of one unsplit CTU time step of the 3-D
+// Euler equations (PPMC reconstruction + exact Riemann solver), written from the text of
+// arXiv:1410.4194 (Schneider & Robertson, "Cholla").  Citations are `P:L<line>` =
+// /root/reference/PAPER.md line, plus the equation; "G<n>/S<n>" are the readings of garbled /
+// silent passages listed in DESIGN.md §"Readings".
+//
+// Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
+// call this.  It shares no code (no headers, helpers, tables, constants) with the CUDA path in
+// paper_1410_4194_b200/csrc/ and must never be linked into or called from the product.
+//
+// Style: whole-grid arrays for every intermediate of the paper's steps 1-5, one
+// loop nest per step, no tiling, no fusion, fp64 throughout, built with -ffp-contract=off.
+// The optional OpenMP pragma on the outermost loop of each nest does not change any result (the
+// step contains no floating-point reduction; min is exact).
+//
+// Parity pins: every function below is pinned by tests/test_oracle_*.py (closed forms,
+// invariants, special cases); see DESIGN.md §"Oracle pins".  No function here is "parity
+// unpinned".
+
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <limits>
+#include <new>
+#include <string>
+#include <vector>
+
+namespace {
+
+constexpr double P_FLOOR = 1e-20;       // P:L231 pressure floor
+constexpr double P_GUESS_FLOOR = 1e-6;
+constexpr double NEWTON_TOL = 1e-8;     // P:L1095 "e.g. 1e-6"; reading S2: 1e-8
+constexpr int NEWTON_CAP = 20;          // reading S2
+
+enum { BC_PERIODIC = 1, BC_REFLECTIVE = 2, BC_OUTFLOW = 3 };
+
+thread_local std::string g_err;
+
+// ---------------------------------------------------------------------------------------------
+// Eq. 6-10: conserved u=[rho, rho*u, rho*v, rho*w, E] <-> primitive w=[rho,u,v,w,p].
+// Pressure floor (reading S1: applied in every conserved->primitive conversion).
+// ---------------------------------------------------------------------------------------------
+void cons_to_prim(double gamma, const double u[5], double w[5]) {
+  const double rho = u[0];
+  const double vx = u[1] / rho, vy = u[2] / rho, vz = u[3] / rho;
+  const double ke = 0.5 * rho * ((vx * vx + vy * vy) + vz * vz);  // Eq. 7
+  double p = (gamma - 1.0) * (u[4] - ke);                         // Eq. 6, 8
+  if (!(p >= P_FLOOR)) p = (p != p) ? p : P_FLOOR;                // keep NaN visible
+  w[0] = rho; w[1] = vx; w[2] = vy; w[3] = vz; w[4] = p;
+}
+
+void prim_to_cons(double gamma, const double w[5], double u[5]) {
+  const double rho = w[0];
+  u[0] = rho;
+  u[1] = rho * w[1];
+  u[2] = rho * w[2];
+  u[3] = rho * w[3];
+  u[4] = w[4] / (gamma - 1.0) + 0.5 * rho * ((w[1] * w[1] + w[2] * w[2]) + w[3] * w[3]);
+}
+
+// Direction-local ordering (rho, v_n, v_t1, v_t2, p|E) for a sweep along d: cyclic permutation
+// (P:L164).  comp(d,m) = index in the global vector of local component m.
+inline int comp(int d, int m) {
+  if (m == 0 || m == 4) return m;
+  return 1 + (d + (m - 1)) % 3;
+}
+void to_local(int d, const double g[5], double l[5]) { for (int m = 0; m < 5; ++m) l[m] = g[comp(d, m)]; }
+void to_global(int d, const double l[5], double g[5]) { for (int m = 0; m < 5; ++m) g[comp(d, m)] = l[m]; }
+
+// ---------------------------------------------------------------------------------------------
+// A9 (first row read as G1: 0.5(-rho du/a + dp/a^2)) and A11.
+// ---------------------------------------------------------------------------------------------
+void char_project(double rho, double a, const double dw[5], double dxi[5]) {
+  const double a2 = a * a;
+  dxi[0] = 0.5 * (-(rho * dw[1] / a) + dw[4] / a2);
+  dxi[1] = dw[0] - dw[4] / a2;
+  dxi[2] = dw[2];
+  dxi[3] = dw[3];
+  dxi[4] = 0.5 * (rho * dw[1] / a + dw[4] / a2);
+}
+void char_backproject(double rho, double a, const double dxi[5], double dw[5]) {
+  dw[0] = dxi[1] + (dxi[0] + dxi[4]);
+  dw[1] = (a / rho) * (dxi[4] - dxi[0]);
+  dw[2] = dxi[2];
+  dw[3] = dxi[3];
+  dw[4] = (a * a) * (dxi[0] + dxi[4]);
+}
+
+inline double sgn(double x) { return x < 0.0 ? -1.0 : 1.0; }  // A4
+
+// Monotonised-central limiter A10 (called "van Leer" in the text; the formula governs, G7).
+inline double limit(double dL, double dR, double dC) {
+  if (dL * dR > 0.0) return sgn(dC) * std::min(std::fabs(dC), std::min(2.0 * std::fabs(dL), 2.0 * std::fabs(dR)));
+  return 0.0;
+}
+
+// Limited slope of cell q from its neighbours (A2 P:L690, A8-A11 P:L722-743), primitive, local order.
+void limited_slope(double gamma, const double wm[5], const double w0[5], const double wp[5], double dw[5]) {
+  const double rho = w0[0];
+  const double a = std::sqrt(gamma * w0[4] / rho);  // Eq. 21 with cell q's own averages
+  double dwL[5], dwR[5], dwC[5], xL[5], xR[5], xC[5], x[5];
+  for (int m = 0; m < 5; ++m) {
+    dwL[m] = w0[m] - wm[m];
+    dwR[m] = wp[m] - w0[m];
+    dwC[m] = 0.5 * (wp[m] - wm[m]);
+  }
+  char_project(rho, a, dwL, xL);
+  char_project(rho, a, dwR, xR);
+  char_project(rho, a, dwC, xC);
+  for (int m = 0; m < 5; ++m) x[m] = limit(xL[m], xR[m], xC[m]);
+  char_backproject(rho, a, x, dw);
+}
+
+// ---------------------------------------------------------------------------------------------
+// PPMC for one cell (A.3).  w[s] = primitive cell averages of cells i-2..i+2 (s=0..4),
+// local order.  Outputs: WL,WR = monotonised face values (after A23); WLs,WRs = W*_L, W*_R
+// after characteristic tracing (A33), all primitive, local order.  dtdx = dt/dx_d.
+// ---------------------------------------------------------------------------------------------
+void ppmc_cell(double gamma, double dtdx, const double w[5][5], double WL[5], double WR[5],
+               double WLs[5], double WRs[5]) {
+  double dwm[5], dw0[5], dwp[5];
+  limited_slope(gamma, w[0], w[1], w[2], dwm);  // cell i-1
+  limited_slope(gamma, w[1], w[2], w[3], dw0);  // cell i
+  limited_slope(gamma, w[2], w[3], w[4], dwp);  // cell i+1
+  const double* wi = w[2];
+  const double* wim = w[1];
+  const double* wip = w[3];
+
+  double dwi[5], w6[5];
+  for (int m = 0; m < 5; ++m) {
+    // A20
+    double L = 0.5 * (wi[m] + wim[m]) - (dw0[m] - dwm[m]) / 6.0;
+    double R = 0.5 * (wip[m] + wi[m]) - (dwp[m] - dw0[m]) / 6.0;
+    // A21
+    if ((R - wi[m]) * (wi[m] - L) <= 0.0) { L = wi[m]; R = wi[m]; }
+    // A22: both tests on the pair as it stands after A21 (G8)
+    const bool fixL = (R - L) * (L - (3.0 * wi[m] - 2.0 * R)) < 0.0;
+    const bool fixR = (R - L) * ((3.0 * wi[m] - 2.0 * L) - R) < 0.0;
+    const double L0 = L, R0 = R;
+    if (fixL) L = 3.0 * wi[m] - 2.0 * R0;
+    if (fixR) R = 3.0 * wi[m] - 2.0 * L0;
+    // A23
+    L = std::max(std::min(wi[m], wim[m]), L);
+    L = std::min(std::max(wi[m], wim[m]), L);
+    R = std::max(std::min(wi[m], wip[m]), R);
+    R = std::min(std::max(wi[m], wip[m]), R);
+    WL[m] = L; WR[m] = R;
+    dwi[m] = R - L;                              // A24
+    w6[m] = 6.0 * (wi[m] - 0.5 * (L + R));       // A26 read as A50 (G2)
+  }
+
+  // A8 eigenvalues from the cell averages; A27
+  const double rho = wi[0];
+  const double a = std::sqrt(gamma * wi[4] / rho);
+  const double lm = wi[1] - a, l0 = wi[1], lp = wi[1] + a;
+  const double am = dtdx * std::min(lm, 0.0), bm = dtdx * std::max(lm, 0.0);
+  const double a0 = dtdx * std::min(l0, 0.0), b0 = dtdx * std::max(l0, 0.0);
+  const double ap = dtdx * std::min(lp, 0.0), bp = dtdx * std::max(lp, 0.0);
+
+  // Domain-of-dependence averages under each characteristic (the six forms at P:L1005-1015;
+  // A25 P:L837-838 are the m (left) and p (right) members).
+  double WLm[5], WL0[5], WLp[5], WRm[5], WR0[5], WRp[5];
+  for (int m = 0; m < 5; ++m) {
+    WLm[m] = WL[m] - 0.5 * am * (dwi[m] + w6[m] * (1.0 + (2.0 / 3.0) * am));
+    WL0[m] = WL[m] - 0.5 * a0 * (dwi[m] + w6[m] * (1.0 + (2.0 / 3.0) * a0));
+    WLp[m] = WL[m] - 0.5 * ap * (dwi[m] + w6[m] * (1.0 + (2.0 / 3.0) * ap));
+    WRm[m] = WR[m] - 0.5 * bm * (dwi[m] - w6[m] * (1.0 - (2.0 / 3.0) * bm));
+    WR0[m] = WR[m] - 0.5 * b0 * (dwi[m] - w6[m] * (1.0 - (2.0 / 3.0) * b0));
+    WRp[m] = WR[m] - 0.5 * bp * (dwi[m] - w6[m] * (1.0 - (2.0 / 3.0) * bp));
+  }
+  // A29, A30, A32 read as differences of those averages (G3).
+  double E[5], B[5], C[5], D[5];
+  for (int m = 0; m < 5; ++m) {
+    E[m] = WL0[m] - WLm[m];
+    B[m] = WLp[m] - WLm[m];
+    C[m] = WRm[m] - WRp[m];
+    D[m] = WR0[m] - WRp[m];
+  }
+  const double a2 = a * a;
+  double sL[5] = {0, 0, 0, 0, 0}, sR[5] = {0, 0, 0, 0, 0};
+  if (l0 < 0.0) {  // A28 first term
+    sL[0] += E[0] - E[4] / a2;
+    sL[2] += E[2];
+    sL[3] += E[3];
+  }
+  if (lp < 0.0) {  // A28 second term
+    sL[0] += 0.5 * (rho * B[1] / a + B[4] / a2);
+    sL[1] += 0.5 * (B[1] + B[4] / (a * rho));
+    sL[4] += 0.5 * (rho * B[1] * a + B[4]);
+  }
+  if (lm > 0.0) {  // A31 first term
+    sR[0] += 0.5 * (-(rho * C[1] / a) + C[4] / a2);
+    sR[1] += 0.5 * (C[1] - C[4] / (a * rho));
+    sR[4] += 0.5 * (-(rho * C[1] * a) + C[4]);
+  }
+  if (l0 > 0.0) {  // A31 second term
+    sR[0] += D[0] - D[4] / a2;
+    sR[2] += D[2];
+    sR[3] += D[3];
+  }
+  for (int m = 0; m < 5; ++m) {  // A33, reference states A25
+    WLs[m] = WLm[m] + sL[m];
+    WRs[m] = WRp[m] + sR[m];
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Exact Riemann solver (B.1).  Inputs: primitive L/R states in local order
+// (rho, u_n, v_t1, v_t2, p).  Output: flux in local order (B22) and diagnostics.
+// ---------------------------------------------------------------------------------------------
+struct RiemannDiag { double pm, um, rho, u, p; int iters; int region; };
+
+// B5, B6
+inline void pressure_function(double gamma, double p0, double rhok, double pk, double ak, double& f, double& fp) {
+  if (p0 <= pk) {  // rarefaction
+    const double pr = p0 / pk;
+    f = 2.0 * ak / (gamma - 1.0) * (std::pow(pr, (gamma - 1.0) / (2.0 * gamma)) - 1.0);
+    fp = 1.0 / (rhok * ak) * std::pow(pr, -(gamma + 1.0) / (2.0 * gamma));
+  } else {  // shock
+    const double A = 2.0 / ((gamma + 1.0) * rhok);       // B4
+    const double B = (gamma - 1.0) / (gamma + 1.0) * pk;
+    const double s = std::sqrt(A / (p0 + B));
+    f = (p0 - pk) * s;
+    fp = s * (1.0 - (p0 - pk) / (2.0 * (B + p0)));
+  }
+}
+
+void riemann_exact(double gamma, const double WL[5], const double WR[5], double flux[5], RiemannDiag* diag) {
+  const double rL = WL[0], uL = WL[1], pL = std::max(WL[4], P_FLOOR);
+  const double rR = WR[0], uR = WR[1], pR = std::max(WR[4], P_FLOOR);
+  const double aL = std::sqrt(gamma * pL / rL);  // B1
+  const double aR = std::sqrt(gamma * pR / rR);
+
+  // B2
+  double pt = 0.5 * (pL + pR) + 0.125 * (uL - uR) * (rL + rR) * (aL + aR);
+  if (pt < 0.0) pt = 0.0;
+  // B3, B4
+  const double gL = std::sqrt((2.0 / ((gamma + 1.0) * rL)) / (pt + (gamma - 1.0) / (gamma + 1.0) * pL));
+  const double gR = std::sqrt((2.0 / ((gamma + 1.0) * rR)) / (pt + (gamma - 1.0) / (gamma + 1.0) * pR));
+  double p0 = ((gL * pL + gR * pR) - (uR - uL)) / (gL + gR);
+  if (p0 < P_GUESS_FLOOR) p0 = P_GUESS_FLOOR;
+
+  // Newton-Raphson B5-B8
+  double pm = p0, fL, fR, fpL, fpR;
+  int it = 0;
+  for (;;) {
+    pressure_function(gamma, p0, rL, pL, aL, fL, fpL);
+    pressure_function(gamma, p0, rR, pR, aR, fR, fpR);
+    pm = p0 - ((fL + fR) + (uR - uL)) / (fpL + fpR);      // B7
+    if (pm < P_FLOOR) pm = P_FLOOR;                        // reading S4
+    ++it;
+    const double delta = 2.0 * std::fabs(pm - p0) / std::fabs(pm + p0);  // B8
+    if (!(delta > NEWTON_TOL) || it >= NEWTON_CAP) break;
+    p0 = pm;
+  }
+  // B9 with f_k re-evaluated at the final p^m (reading S3)
+  pressure_function(gamma, pm, rL, pL, aL, fL, fpL);
+  pressure_function(gamma, pm, rR, pR, aR, fR, fpR);
+  const double um = 0.5 * ((uL + uR) + (fR - fL));
+
+  // Sampling at x/t = 0
+  const double z = (gamma - 1.0) / (2.0 * gamma);
+  const double gm = (gamma - 1.0) / (gamma + 1.0);
+  double rho, u, p;
+  int region;
+  const double* Wk;
+  if (um >= 0.0) {
+    Wk = WL;
+    if (pm <= pL) {  // left rarefaction
+      if (uL - aL >= 0.0) { rho = rL; u = uL; p = pL; region = 0; }                      // B10
+      else if (um - aL * std::pow(pm / pL, z) < 0.0) {                                  // B11
+        rho = rL * std::pow(pm / pL, 1.0 / gamma); u = um; p = pm; region = 1;
+      } else {                                                                          // B12
+        const double a = 2.0 / (gamma + 1.0) * (aL + 0.5 * (gamma - 1.0) * uL);
+        rho = rL * std::pow(a / aL, 2.0 / (gamma - 1.0));
+        u = a;
+        p = pL * std::pow(a / aL, 2.0 * gamma / (gamma - 1.0));
+        region = 2;
+      }
+    } else {  // left shock
+      const double sL = uL - aL * std::sqrt((gamma + 1.0) / (2.0 * gamma) * (pm / pL) + z);  // B13
+      if (sL >= 0.0) { rho = rL; u = uL; p = pL; region = 3; }                            // B14
+      else { rho = rL * (pm / pL + gm) / (pm / pL * gm + 1.0); u = um; p = pm; region = 4; }  // B15
+    }
+  } else {
+    Wk = WR;
+    if (pm <= pR) {  // right rarefaction
+      if (uR + aR <= 0.0) { rho = rR; u = uR; p = pR; region = 5; }                      // B16
+      else if (um + aR * std::pow(pm / pR, z) >= 0.0) {                                 // B17
+        rho = rR * std::pow(pm / pR, 1.0 / gamma); u = um; p = pm; region = 6;
+      } else {                                                                          // B18 (G4)
+        const double a = 2.0 / (gamma + 1.0) * (aR - 0.5 * (gamma - 1.0) * uR);
+        rho = rR * std::pow(a / aR, 2.0 / (gamma - 1.0));
+        u = -a;
+        p = pR * std::pow(a / aR, 2.0 * gamma / (gamma - 1.0));
+        region = 7;
+      }
+    } else {  // right shock
+      const double sR = uR + aR * std::sqrt((gamma + 1.0) / (2.0 * gamma) * (pm / pR) + z);  // B19 (G5)
+      if (sR <= 0.0) { rho = rR; u = uR; p = pR; region = 8; }                            // B20
+      else { rho = rR * (pm / pR + gm) / (pm / pR * gm + 1.0); u = um; p = pm; region = 9; }  // B21
+    }
+  }
+  // B22; transverse velocities from side k (reading S9)
+  const double vt1 = Wk[2], vt2 = Wk[3];
+  const double E = p / (gamma - 1.0) + 0.5 * rho * ((u * u + vt1 * vt1) + vt2 * vt2);
+  flux[0] = rho * u;
+  flux[1] = rho * u * u + p;
+  flux[2] = rho * u * vt1;
+  flux[3] = rho * u * vt2;
+  flux[4] = (E + p) * u;
+  if (diag) { diag->pm = pm; diag->um = um; diag->rho = rho; diag->u = u; diag->p = p; diag->iters = it; diag->region = region; }
+}
+
+// Riemann problem at an interface normal to d from two conserved states in GLOBAL order.
+void riemann_interface(double gamma, int d, const double UL[5], const double UR[5], double F[5]) {
+  double wl[5], wr[5], ll[5], lr[5], fl[5];
+  cons_to_prim(gamma, UL, wl);
+  cons_to_prim(gamma, UR, wr);
+  to_local(d, wl, ll);
+  to_local(d, wr, lr);
+  riemann_exact(gamma, ll, lr, fl, nullptr);
+  to_global(d, fl, F);
+}
+
+// ---------------------------------------------------------------------------------------------
+// Grid context.
+// ---------------------------------------------------------------------------------------------
+struct Ctx {
+  int n[3], g, gd[3], pd[3];
+  long np;
+  double gamma, dx[3];
+  int bc[6];
+  bool active[3];
+  bool have_state = false;
+  std::vector<double> u;  // [5][np], x fastest
+  inline long idx(int i, int j, int k) const {  // real-cell coordinates, ghosts negative / >= n
+    return ((long)(k + gd[2]) * pd[1] + (j + gd[1])) * pd[0] + (i + gd[0]);
+  }
+};
+
+// Ghost fill (readings S6, S7): x over real (y,z); y over the padded x extent; z over
+// padded x,y — the ordering that carries edges and corners.
+void ghost_fill(Ctx& c) {
+  for (int d = 0; d < 3; ++d) {
+    if (!c.active[d]) continue;
+    int lo[3], hi[3];
+    for (int e = 0; e < 3; ++e) {
+      if (e < d) { lo[e] = -c.gd[e]; hi[e] = c.n[e] + c.gd[e]; }   // already-filled padded extent
+      else if (e > d) { lo[e] = 0; hi[e] = c.n[e]; }               // real cells only
+      else { lo[e] = 0; hi[e] = 1; }                               // placeholder for the fill dim
+    }
+    const int n = c.n[d], g = c.g;
+    for (int side = 0; side < 2; ++side) {
+      const int bc = c.bc[2 * d + side];
+      for (int l = 1; l <= g; ++l) {
+        int gi, si;  // ghost index and its source index along d
+        if (side == 0) {
+          gi = -l;
+          si = bc == BC_PERIODIC ? n - l : bc == BC_REFLECTIVE ? l - 1 : 0;
+        } else {
+          gi = n - 1 + l;
+          si = bc == BC_PERIODIC ? l - 1 : bc == BC_REFLECTIVE ? n - l : n - 1;
+        }
+        int a[3];
+        for (a[2] = lo[2]; a[2] < hi[2]; ++a[2])
+          for (a[1] = lo[1]; a[1] < hi[1]; ++a[1])
+            for (a[0] = lo[0]; a[0] < hi[0]; ++a[0]) {
+              int gq[3] = {a[0], a[1], a[2]}, sq[3] = {a[0], a[1], a[2]};
+              gq[d] = gi; sq[d] = si;
+              const long ig = c.idx(gq[0], gq[1], gq[2]);
+              const long is = c.idx(sq[0], sq[1], sq[2]);
+              for (int f = 0; f < 5; ++f) {
+                double v = c.u[f * c.np + is];
+                if (bc == BC_REFLECTIVE && f == 1 + d) v = -v;
+                c.u[f * c.np + ig] = v;
+              }
+            }
+      }
+    }
+  }
+}
+
+// Eq. 22 over real cells; returns C0 * min.  NaN if any cell is non-physical.
+double compute_dt(const Ctx& c, double cfl) {
+  double dtmin = std::numeric_limits<double>::infinity();
+  bool bad = false;
+  for (int k = 0; k < c.n[2]; ++k)
+    for (int j = 0; j < c.n[1]; ++j)
+      for (int i = 0; i < c.n[0]; ++i) {
+        const long q = c.idx(i, j, k);
+        double uc[5], w[5];
+        for (int f = 0; f < 5; ++f) uc[f] = c.u[f * c.np + q];
+        if (!(uc[0] > 0.0) || !std::isfinite(uc[0]) || !std::isfinite(uc[4])) { bad = true; continue; }
+        cons_to_prim(c.gamma, uc, w);
+        const double a = std::sqrt(c.gamma * w[4] / w[0]);  // Eq. 21
+        for (int d = 0; d < 3; ++d) {
+          if (!c.active[d]) continue;
+          const double t = c.dx[d] / (std::fabs(w[1 + d]) + a);
+          if (!(t == t)) bad = true;
+          if (t < dtmin) dtmin = t;
+        }
+      }
+  if (bad) return std::numeric_limits<double>::quiet_NaN();
+  return cfl * dtmin;
+}
+
+// One CTU step: steps 1-5 on whole-grid arrays, then the ghost fill.
+void ctu_step(Ctx& c, double dt) {
+  const long np = c.np;
+  const double gamma = c.gamma;
+  const int g = c.g;
+  (void)g;
+  // O1: primitives of every padded cell.
+  std::vector<double> w(5 * np);
+#pragma omp parallel for
+  for (long q = 0; q < np; ++q) {
+    double uc[5], wc[5];
+    for (int f = 0; f < 5; ++f) uc[f] = c.u[f * np + q];
+    cons_to_prim(gamma, uc, wc);
+    for (int f = 0; f < 5; ++f) w[f * np + q] = wc[f];
+  }
+
+  // extents helpers: along the sweep dim [-1, n]; other active dims [-t, n+t) ; inactive [0,1)
+  auto range = [&](int e, int ext, int& lo, int& hi) {
+    if (!c.active[e]) { lo = 0; hi = 1; } else { lo = -ext; hi = c.n[e] + ext; }
+  };
+  const long stride[3] = {1, c.pd[0], (long)c.pd[0] * c.pd[1]};
+
+  // Step 1: U*_L, U*_R per direction (conserved, global order) — O2.
+  std::vector<double> UsL[3], UsR[3], Fs[3], UhL[3], UhR[3], Fh[3];
+  for (int d = 0; d < 3; ++d) {
+    if (!c.active[d]) continue;
+    UsL[d].assign(5 * np, 0.0);
+    UsR[d].assign(5 * np, 0.0);
+    int lo[3], hi[3];
+    for (int e = 0; e < 3; ++e) range(e, 1, lo[e], hi[e]);
+    const double dtdx = dt / c.dx[d];
+#pragma omp parallel for collapse(2)
+    for (int k = lo[2]; k < hi[2]; ++k)
+      for (int j = lo[1]; j < hi[1]; ++j)
+        for (int i = lo[0]; i < hi[0]; ++i) {
+          const long q = c.idx(i, j, k);
+          double ws[5][5];
+          for (int s = 0; s < 5; ++s) {
+            const long qs = q + (s - 2) * stride[d];
+            double wg[5];
+            for (int f = 0; f < 5; ++f) wg[f] = w[f * np + qs];
+            to_local(d, wg, ws[s]);
+          }
+          double WL[5], WR[5], WLs[5], WRs[5], gl[5], gr[5], ul[5], ur[5];
+          ppmc_cell(gamma, dtdx, ws, WL, WR, WLs, WRs);
+          to_global(d, WLs, gl);
+          to_global(d, WRs, gr);
+          prim_to_cons(gamma, gl, ul);
+          prim_to_cons(gamma, gr, ur);
+          for (int f = 0; f < 5; ++f) { UsL[d][f * np + q] = ul[f]; UsR[d][f * np + q] = ur[f]; }
+        }
+  }
+  // Step 2: F*_d at interface c+1/2 stored at cell index c — O3.  L state = right face of cell
+  // c, R state = left face of cell c+1.
+  for (int d = 0; d < 3; ++d) {
+    if (!c.active[d]) continue;
+    Fs[d].assign(5 * np, 0.0);
+    int lo[3], hi[3];
+    for (int e = 0; e < 3; ++e) range(e, 1, lo[e], hi[e]);
+    hi[d] -= 1;  // interfaces c in [-1, n-1]
+#pragma omp parallel for collapse(2)
+    for (int k = lo[2]; k < hi[2]; ++k)
+      for (int j = lo[1]; j < hi[1]; ++j)
+        for (int i = lo[0]; i < hi[0]; ++i) {
+          const long q = c.idx(i, j, k), qp = q + stride[d];
+          double UL[5], UR[5], F[5];
+          for (int f = 0; f < 5; ++f) { UL[f] = UsR[d][f * np + q]; UR[f] = UsL[d][f * np + qp]; }
+          riemann_interface(gamma, d, UL, UR, F);
+          for (int f = 0; f < 5; ++f) Fs[d][f * np + q] = F[f];
+        }
+  }
+  // Step 3: transverse half-step, Eq. 23 — O4.
+  for (int d = 0; d < 3; ++d) {
+    if (!c.active[d]) continue;
+    UhL[d].assign(5 * np, 0.0);
+    UhR[d].assign(5 * np, 0.0);
+    int lo[3], hi[3];
+    for (int e = 0; e < 3; ++e) range(e, e == d ? 1 : 0, lo[e], hi[e]);
+#pragma omp parallel for collapse(2)
+    for (int k = lo[2]; k < hi[2]; ++k)
+      for (int j = lo[1]; j < hi[1]; ++j)
+        for (int i = lo[0]; i < hi[0]; ++i) {
+          const long q = c.idx(i, j, k);
+          for (int f = 0; f < 5; ++f) {
+            double corr = 0.0;
+            for (int t = 1; t <= 2; ++t) {  // cyclic: d+1 then d+2
+              const int e = (d + t) % 3;
+              if (!c.active[e]) continue;
+              corr += 0.5 * (dt / c.dx[e]) * (Fs[e][f * np + q - stride[e]] - Fs[e][f * np + q]);
+            }
+            UhL[d][f * np + q] = UsL[d][f * np + q] + corr;
+            UhR[d][f * np + q] = UsR[d][f * np + q] + corr;
+          }
+        }
+  }
+  // Step 4: CTU fluxes — O5.
+  for (int d = 0; d < 3; ++d) {
+    if (!c.active[d]) continue;
+    Fh[d].assign(5 * np, 0.0);
+    int lo[3], hi[3];
+    for (int e = 0; e < 3; ++e) range(e, e == d ? 1 : 0, lo[e], hi[e]);
+    hi[d] -= 1;
+#pragma omp parallel for collapse(2)
+    for (int k = lo[2]; k < hi[2]; ++k)
+      for (int j = lo[1]; j < hi[1]; ++j)
+        for (int i = lo[0]; i < hi[0]; ++i) {
+          const long q = c.idx(i, j, k), qp = q + stride[d];
+          double UL[5], UR[5], F[5];
+          for (int f = 0; f < 5; ++f) { UL[f] = UhR[d][f * np + q]; UR[f] = UhL[d][f * np + qp]; }
+          riemann_interface(gamma, d, UL, UR, F);
+          for (int f = 0; f < 5; ++f) Fh[d][f * np + q] = F[f];
+        }
+  }
+  // Step 5: conservative update, Eq. 24 on real cells — O6.
+#pragma omp parallel for collapse(2)
+  for (int k = 0; k < c.n[2]; ++k)
+    for (int j = 0; j < c.n[1]; ++j)
+      for (int i = 0; i < c.n[0]; ++i) {
+        const long q = c.idx(i, j, k);
+        for (int f = 0; f < 5; ++f) {
+          double v = c.u[f * np + q];
+          for (int d = 0; d < 3; ++d) {
+            if (!c.active[d]) continue;
+            v += (dt / c.dx[d]) * (Fh[d][f * np + q - stride[d]] - Fh[d][f * np + q]);
+          }
+          c.u[f * np + q] = v;
+        }
+      }
+  ghost_fill(c);  // O7
+}
+
+int fail(const char* msg) { g_err = msg; return -1; }
+
+}  // namespace
+
+// =============================================================================================
+// C ABI (prefix ref_): mirrors include/ch.h so one Python harness drives both, plus unit-level
+// entry points used by the pins.
+// =============================================================================================
+extern "C" {
+
+const char* ref_last_error(void) { return g_err.c_str(); }
+
+void* ref_init(int nx, int ny, int nz, int nghost, double gamma, const int* bc) {
+  if (nx < 1 || ny < 1 || nz < 1) { fail("n < 1"); return nullptr; }
+  if (nghost < 3) { fail("nghost < 3"); return nullptr; }
+  if (!(gamma > 1.0)) { fail("gamma <= 1"); return nullptr; }
+  Ctx* c = new (std::nothrow) Ctx();
+  if (!c) { fail("alloc"); return nullptr; }
+  c->n[0] = nx; c->n[1] = ny; c->n[2] = nz;
+  c->g = nghost; c->gamma = gamma;
+  for (int d = 0; d < 3; ++d) {
+    c->active[d] = c->n[d] > 1;
+    c->gd[d] = c->active[d] ? nghost : 0;
+    c->pd[d] = c->n[d] + 2 * c->gd[d];
+    c->dx[d] = 1.0 / nx;  // reading S8
+    if (c->active[d] && c->n[d] < nghost) { delete c; fail("active dim smaller than nghost"); return nullptr; }
+  }
+  for (int s = 0; s < 6; ++s) {
+    c->bc[s] = bc ? bc[s] : BC_PERIODIC;
+    if (c->active[s / 2] && (c->bc[s] < 1 || c->bc[s] > 3)) { delete c; fail("bad bc"); return nullptr; }
+  }
+  for (int d = 0; d < 3; ++d)
+    if (c->active[d] && ((c->bc[2 * d] == BC_PERIODIC) != (c->bc[2 * d + 1] == BC_PERIODIC))) {
+      delete c; fail("unpaired periodic"); return nullptr;
+    }
+  c->np = (long)c->pd[0] * c->pd[1] * c->pd[2];
+  c->u.assign(5 * c->np, 0.0);
+  return c;
+}
+
+int ref_free(void* h) { delete static_cast<Ctx*>(h); return 0; }
+
+int ref_set_spacing(void* h, double dx, double dy, double dz) {
+  Ctx* c = static_cast<Ctx*>(h);
+  if (!(dx > 0 && dy > 0 && dz > 0)) return fail("spacing <= 0");
+  c->dx[0] = dx; c->dx[1] = dy; c->dx[2] = dz;
+  return 0;
+}
+
+long ref_padded_cells(void* h) { return static_cast<Ctx*>(h)->np; }
+
+// u = [5][nz][ny][nx] real cells only; copies in and fills the ghosts.
+int ref_set_state(void* h, const double* u) {
+  Ctx* c = static_cast<Ctx*>(h);
+  const long n = (long)c->n[0] * c->n[1] * c->n[2];
+  for (int f = 0; f < 5; ++f)
+    for (int k = 0; k < c->n[2]; ++k)
+      for (int j = 0; j < c->n[1]; ++j)
+        for (int i = 0; i < c->n[0]; ++i)
+          c->u[f * c->np + c->idx(i, j, k)] = u[f * n + ((long)k * c->n[1] + j) * c->n[0] + i];
+  ghost_fill(*c);
+  c->have_state = true;
+  return 0;
+}
+
+int ref_get_state(void* h, double* u) {
+  Ctx* c = static_cast<Ctx*>(h);
+  if (!c->have_state) return fail("no state");
+  const long n = (long)c->n[0] * c->n[1] * c->n[2];
+  for (int f = 0; f < 5; ++f)
+    for (int k = 0; k < c->n[2]; ++k)
+      for (int j = 0; j < c->n[1]; ++j)
+        for (int i = 0; i < c->n[0]; ++i)
+          u[f * n + ((long)k * c->n[1] + j) * c->n[0] + i] = c->u[f * c->np + c->idx(i, j, k)];
+  return 0;
+}
+
+// Padded store [5][pz][py][px] as is (ghosts included, not refilled): used to run the step on a
+// sub-box cut out of a larger grid (sampled parity at full size) and to test the ghost fill.
+int ref_set_padded(void* h, const double* up) {
+  Ctx* c = static_cast<Ctx*>(h);
+  std::memcpy(c->u.data(), up, sizeof(double) * 5 * c->np);
+  c->have_state = true;
+  return 0;
+}
+int ref_get_padded(void* h, double* up) {
+  Ctx* c = static_cast<Ctx*>(h);
+  std::memcpy(up, c->u.data(), sizeof(double) * 5 * c->np);
+  return 0;
+}
+
+double ref_compute_dt(void* h, double cfl) {
+  Ctx* c = static_cast<Ctx*>(h);
+  if (!c->have_state) { fail("no state"); return std::numeric_limits<double>::quiet_NaN(); }
+  return compute_dt(*c, cfl);
+}
+
+int ref_step(void* h, double dt) {
+  Ctx* c = static_cast<Ctx*>(h);
+  if (!c->have_state) return fail("no state");
+  if (!(dt > 0.0) || !std::isfinite(dt)) return fail("bad dt");
+  ctu_step(*c, dt);
+  return 0;
+}
+
+// ---- unit-level entry points for the pins (all primitive, direction-local order) -------------
+void ref_cons_to_prim(double gamma, const double* u, double* w) { cons_to_prim(gamma, u, w); }
+void ref_prim_to_cons(double gamma, const double* w, double* u) { prim_to_cons(gamma, w, u); }
+void ref_char_project(double rho, double a, const double* dw, double* dxi) { char_project(rho, a, dw, dxi); }
+void ref_char_backproject(double rho, double a, const double* dxi, double* dw) { char_backproject(rho, a, dxi, dw); }
+void ref_limited_slope(double gamma, const double* wm, const double* w0, const double* wp, double* dw) {
+  limited_slope(gamma, wm, w0, wp, dw);
+}
+// w = [5 cells][5 comps]; out = [4][5] = WL, WR, W*_L, W*_R
+void ref_ppmc_cell(double gamma, double dtdx, const double* w, double* out) {
+  double ws[5][5];
+  std::memcpy(ws, w, sizeof(ws));
+  ppmc_cell(gamma, dtdx, ws, out, out + 5, out + 10, out + 15);
+}
+// WL, WR primitive; flux[5]; diag[7] = pm, um, rho, u, p, iterations, region
+void ref_riemann_exact(double gamma, const double* WL, const double* WR, double* flux, double* diag) {
+  RiemannDiag d;
+  riemann_exact(gamma, WL, WR, flux, &d);
+  if (diag) { diag[0] = d.pm; diag[1] = d.um; diag[2] = d.rho; diag[3] = d.u; diag[4] = d.p; diag[5] = d.iters; diag[6] = d.region; }
+}
+
+}  // extern "C"
