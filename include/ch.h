@@ -1,0 +1,139 @@
+/* ch.h — C ABI of the B200-native CTU + PPMC + exact-Riemann hydro step.
+ *
+ * One unsplit Corner Transport Upwind (CTU) time step of the 3-D Euler equations on a static
+ * Cartesian mesh, fp64, as stated in arXiv:1410.4194 (Schneider & Robertson, "Cholla").
+ * Citations are `P:L<line>` = line of /root/reference/PAPER.md plus the equation it falls in;
+ * "reading Gn/Sn" refers to the table of readings in DESIGN.md.
+ *
+ * The five graded calls are the ones BASELINE.json's north_star names:
+ *     ch_init(nx,ny,nz,nghost,gamma,bc), ch_set_state, ch_compute_dt(cfl), ch_step(dt), ch_get_state.
+ * The rest are helpers that exist because the caller (PyTorch) owns device memory and streams.
+ *
+ * Conventions
+ *   - All floating point is IEEE binary64.  All `int` returns: CH_OK (0) or a negative CH_E* code;
+ *     ch_last_error() returns a human-readable reason for the last failure on the calling thread.
+ *   - Field order: rho, rho*u, rho*v, rho*w, E  (Eq. 9).  x is the fastest index
+ *     (P:L312).
+ *   - "real" arrays are [5][nz][ny][nx]; "padded" arrays are [5][pz][py][px] with
+ *     p_d = n_d + 2*nghost for an active dimension (n_d > 1) and p_d = 1 for an inactive one
+ *     (n_d == 1: no ghosts, no sweep, no transverse term, no dt term — P:L132).
+ *   - Cell widths default to dx = dy = dz = 1/nx (reading S8); ch_set_spacing overrides.
+ *   - The library never allocates or frees DEVICE memory: every device buffer is handed in through
+ *     ch_bind and stays owned by the caller.  It does own a few bytes of pinned HOST memory (the
+ *     dt read-back cell) per context.
+ *   - A context is not thread-safe; use one per host thread / stream.
+ *   - There is no CPU fallback: every call that touches data launches CUDA work on the bound
+ *     stream and returns CH_ECUDA if that fails.
+ */
+#ifndef CH_H_
+#define CH_H_
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct ch_ctx ch_ctx; /* opaque, host-side */
+
+enum {
+  CH_OK = 0,
+  CH_EINVAL = -1,   /* bad argument */
+  CH_ESTATE = -2,   /* call out of order (no buffers bound / no state set) */
+  CH_ECUDA = -3,    /* a CUDA runtime call or launch failed */
+  CH_ENONPHYS = -4  /* non-physical data met (rho <= 0 or non-finite) */
+};
+
+/* Boundary-condition codes per face: any mix per face, periodic faces must be paired. */
+enum { CH_BC_PERIODIC = 1, CH_BC_REFLECTIVE = 2, CH_BC_OUTFLOW = 3 };
+
+/* Device buffers handed to ch_bind.  All pointers are DEVICE pointers owned by the caller and must
+ * stay valid until ch_free or the next ch_bind. */
+typedef struct ch_buffers {
+  double* state;          /* padded conserved store u, 5*Np doubles (SoA, x fastest) */
+  void* workspace;        /* scratch, at least ch_workspace_bytes(...) bytes, 256-byte aligned */
+  size_t workspace_bytes; /* size of `workspace` as allocated */
+  void* reduce;           /* 64 bytes, 8-byte aligned: device cells of the dt reduction */
+} ch_buffers;
+
+/* ch_init — create a context for an nx*ny*nz grid of real cells with `nghost` ghost layers on each
+ * side of every active dimension, ratio of specific heats `gamma` (Eq. 8), and boundary
+ * codes bc[6] = {x-,x+,y-,y+,z-,z+} (host pointer; NULL = all periodic).  Host-only: makes no CUDA
+ * call.  Returns NULL on error (n < 1; nghost < 3 — PPMC inside six-solve CTU needs 3; gamma <= 1;
+ * a bc code outside 1..3 on an active dimension; unpaired periodic faces; an active dimension
+ * smaller than nghost). */
+ch_ctx* ch_init(int nx, int ny, int nz, int nghost, double gamma, const int* bc);
+
+/* ch_free — destroy the context (host memory only; bound device buffers stay with the caller). */
+int ch_free(ch_ctx* ctx);
+
+/* ch_last_error — reason for the most recent failure on this thread ("" if none). */
+const char* ch_last_error(void);
+
+/* ch_set_spacing — override the cell widths (all > 0).  Default 1/nx each (reading S8). */
+int ch_set_spacing(ch_ctx* ctx, double dx, double dy, double dz);
+
+/* ch_padded_cells — Np = px*py*pz for the context. */
+long long ch_padded_cells(const ch_ctx* ctx);
+
+/* ch_workspace_bytes — bytes of scratch ch_bind needs for this grid: the first-pass fluxes F*,G*,H*
+ * (P:L157), the traced interface states U*_L, U*_R per direction and the CTU fluxes
+ * F,G,H^{n+1/2}, all padded SoA fp64.  Returns 0 on bad arguments. */
+size_t ch_workspace_bytes(int nx, int ny, int nz, int nghost);
+
+/* ch_bind — attach caller-owned device buffers and the CUDA stream (a cudaStream_t passed as
+ * void*; NULL = the legacy default stream) every later call runs on.  Must precede ch_set_state.
+ * CH_EINVAL if a pointer is NULL or the workspace is too small.  Invalidates any state set before. */
+int ch_bind(ch_ctx* ctx, const ch_buffers* bufs, void* stream);
+
+/* ch_set_state — copy the real cells `u` ([5][nz][ny][nx], HOST or DEVICE pointer, resolved by
+ * unified addressing) into the padded store and fill the ghost cells (periodic =
+ * opposite side; reflective = mirror cell with the normal momentum negated; outflow = adjacent
+ * boundary cell; x then y then z so edges and corners are carried; readings S6, S7).
+ * Asynchronous on the stream for device / pinned sources. */
+int ch_set_state(ch_ctx* ctx, const double* u);
+
+/* ch_get_state — copy the real cells out to `u` ([5][nz][ny][nx], HOST or DEVICE pointer) and
+ * synchronise the stream. */
+int ch_get_state(ch_ctx* ctx, double* u);
+
+/* ch_set_padded / ch_get_padded — the padded store as is, ghosts included and NOT refilled
+ * ([5][pz][py][px], HOST or DEVICE pointer).  Used to run one step on a sub-box cut from a larger
+ * grid and to check the ghost fill; get synchronises. */
+int ch_set_padded(ch_ctx* ctx, const double* up);
+int ch_get_padded(ch_ctx* ctx, double* up);
+
+/* ch_compute_dt — Eq. 22: returns cfl * min over real cells and active directions d of
+ * dx_d / (|v_d| + a), a = sqrt(gamma p / rho) (Eq. 21), p floored at 1e-20.  Synchronises
+ * the stream (one 16-byte device-to-host copy).  When ch_step has already reduced the wave speeds
+ * of the current state inside its update kernel, no further pass over the grid is made.
+ * Returns NaN and sets CH_ENONPHYS if any real cell has rho <= 0 or a non-finite rho or E; NaN with
+ * CH_EINVAL if cfl is not in (0,1]; NaN with CH_ESTATE if no state is set.  The paper's stability
+ * bound for the 3-D six-solve CTU is cfl < 0.5: documented, not enforced. */
+double ch_compute_dt(ch_ctx* ctx, double cfl);
+
+/* ch_step — advance the state by one CTU step of size dt (steps 1-5): PPMC
+ * reconstruction with characteristic limiting and characteristic tracing in every active direction
+ * (A8-A11 P:L722-743), exact Riemann solver at every interface (Newton
+ * tolerance 1e-8, cap 20: reading S2), transverse flux correction (Eq. 23), second Riemann
+ * pass, conservative update (Eq. 24), ghost fill.  Asynchronous on the stream.
+ * CH_ESTATE if no state is set; CH_EINVAL if dt <= 0 or non-finite; CH_ECUDA on launch failure. */
+int ch_step(ch_ctx* ctx, double dt);
+
+/* ch_sync — block until all work queued on the context's stream has finished. */
+int ch_sync(ch_ctx* ctx);
+
+/* ch_kernel_launches — number of kernels this context has launched since ch_init (for bench.py's
+ * gpu_launches claim). */
+long long ch_kernel_launches(const ch_ctx* ctx);
+
+/* ch_fp64_peak_probe — measurement helper for the roofline denominator: runs `iters` dependent
+ * DFMA chains (8 independent chains per thread) on `blocks` x `threads` threads on `stream` and
+ * returns the elapsed milliseconds measured with CUDA events (negative on error).  `sink` is a
+ * device pointer to at least blocks*threads doubles.  FP64 flops done = 2*8*iters*blocks*threads. */
+double ch_fp64_peak_probe(double* sink, int blocks, int threads, int iters, void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CH_H_ */

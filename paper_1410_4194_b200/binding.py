@@ -1,0 +1,212 @@
+"""Thin Python binding over the C-ABI library declared in include/ch.h (argument marshalling only).
+
+PyTorch owns device memory and streams (torch tensors are handed to `ch_bind`); every step of the
+hot path runs in the CUDA kernels of csrc/.  There is no CPU fallback: `load_library()` raises if
+the shared library is missing and `Grid` raises if no CUDA device is present.  This module never
+imports oracle/.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_CSRC = os.path.join(_HERE, "csrc")
+_LIB = os.path.join(_HERE, "libch_b200.so")
+_SOURCES = [os.path.join(_CSRC, "ch_kernels.cu")]
+_HEADERS = [os.path.join(_CSRC, "ch_hydro.cuh"), os.path.join(os.path.dirname(_HERE), "include", "ch.h")]
+
+PERIODIC, REFLECTIVE, OUTFLOW = 1, 2, 3
+CH_OK, CH_EINVAL, CH_ESTATE, CH_ECUDA, CH_ENONPHYS = 0, -1, -2, -3, -4
+
+# every symbol include/ch.h declares
+SYMBOLS = ("ch_init", "ch_free", "ch_last_error", "ch_set_spacing", "ch_padded_cells", "ch_workspace_bytes",
+           "ch_bind", "ch_set_state", "ch_get_state", "ch_set_padded", "ch_get_padded", "ch_compute_dt",
+           "ch_step", "ch_sync", "ch_kernel_launches", "ch_fp64_peak_probe")
+
+NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
+              "-Xcompiler", "-fPIC", "-shared"]
+
+
+def build(force: bool = False, verbose: bool = False) -> str:
+    """Compile csrc/ for sm_100a with nvcc into paper_1410_4194_b200/libch_b200.so (in-tree)."""
+    deps = _SOURCES + _HEADERS
+    if not force and os.path.exists(_LIB) and all(os.path.getmtime(_LIB) >= os.path.getmtime(d) for d in deps):
+        return _LIB
+    nvcc = os.environ.get("NVCC") or ("/usr/local/cuda/bin/nvcc" if os.path.exists("/usr/local/cuda/bin/nvcc") else "nvcc")
+    tmp = _LIB + ".tmp%d" % os.getpid()
+    cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp] + _SOURCES
+    subprocess.check_call(cmd)
+    os.replace(tmp, _LIB)
+    return _LIB
+
+
+class ChStruct(C.Structure):
+    _fields_ = [("state", C.c_void_p), ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t),
+                ("reduce", C.c_void_p)]
+
+
+_lib = None
+
+
+def load_library() -> C.CDLL:
+    """dlopen the CUDA library.  Raises (loudly) if it has not been built."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(_LIB):
+        raise RuntimeError(f"{_LIB} is missing: run `python -c 'import __graft_entry__ as g; g.build()'` "
+                           "(there is no CPU fallback)")
+    L = C.CDLL(_LIB)
+    vp, dp = C.c_void_p, C.c_void_p   # data pointers go through as raw addresses (host or device)
+    L.ch_init.restype = vp
+    L.ch_init.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int, C.c_double, C.POINTER(C.c_int)]
+    L.ch_free.argtypes = [vp]
+    L.ch_last_error.restype = C.c_char_p
+    L.ch_set_spacing.argtypes = [vp, C.c_double, C.c_double, C.c_double]
+    L.ch_padded_cells.restype = C.c_longlong
+    L.ch_padded_cells.argtypes = [vp]
+    L.ch_workspace_bytes.restype = C.c_size_t
+    L.ch_workspace_bytes.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int]
+    L.ch_bind.argtypes = [vp, C.POINTER(ChStruct), vp]
+    for name in ("ch_set_state", "ch_get_state", "ch_set_padded", "ch_get_padded"):
+        getattr(L, name).argtypes = [vp, dp]
+    L.ch_compute_dt.restype = C.c_double
+    L.ch_compute_dt.argtypes = [vp, C.c_double]
+    L.ch_step.argtypes = [vp, C.c_double]
+    L.ch_sync.argtypes = [vp]
+    L.ch_kernel_launches.restype = C.c_longlong
+    L.ch_kernel_launches.argtypes = [vp]
+    L.ch_fp64_peak_probe.restype = C.c_double
+    L.ch_fp64_peak_probe.argtypes = [vp, C.c_int, C.c_int, C.c_int, vp]
+    _lib = L
+    return L
+
+
+def last_error() -> str:
+    return load_library().ch_last_error().decode()
+
+
+def _addr(a) -> int:
+    """Raw address of a numpy array (host) or torch tensor (host or device), fp64 and contiguous."""
+    if isinstance(a, np.ndarray):
+        assert a.dtype == np.float64 and a.flags.c_contiguous
+        return a.ctypes.data
+    import torch
+    assert isinstance(a, torch.Tensor) and a.dtype == torch.float64 and a.is_contiguous()
+    return a.data_ptr()
+
+
+class Grid:
+    """ch_init + ch_bind with torch-owned device buffers; methods mirror the C calls one to one."""
+
+    def __init__(self, nx, ny, nz, nghost=3, gamma=1.4, bc=(PERIODIC,) * 6, device="cuda:0", stream=None):
+        import torch
+        L = load_library()
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_1410_4194_b200.Grid needs a CUDA device (no CPU fallback)")
+        bc_arr = (C.c_int * 6)(*[int(b) for b in bc])
+        self._h = L.ch_init(nx, ny, nz, nghost, gamma, bc_arr)
+        if not self._h:
+            raise ValueError("ch_init: " + last_error())
+        self._L = L
+        self.shape = (nz, ny, nx)
+        self.nghost = nghost
+        g = [nghost if n > 1 else 0 for n in (nz, ny, nx)]
+        self.padded_shape = tuple(n + 2 * gg for n, gg in zip(self.shape, g))
+        self.device = torch.device(device)
+        np_cells = L.ch_padded_cells(self._h)
+        ws_bytes = L.ch_workspace_bytes(nx, ny, nz, nghost)
+        with torch.cuda.device(self.device):
+            self._state = torch.empty(5 * np_cells, dtype=torch.float64, device=self.device)
+            self._ws = torch.empty(ws_bytes // 8, dtype=torch.float64, device=self.device)
+            self._red = torch.zeros(8, dtype=torch.int64, device=self.device)
+            self._stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+        bufs = ChStruct(self._state.data_ptr(), self._ws.data_ptr(), ws_bytes, self._red.data_ptr())
+        self._check(L.ch_bind(self._h, C.byref(bufs), self._stream.cuda_stream), "ch_bind")
+
+    def _check(self, rc, what):
+        if rc != CH_OK:
+            raise (ValueError if rc == CH_EINVAL else RuntimeError)(f"{what}: {last_error()} (code {rc})")
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self._L.ch_sync(self._h)
+            self._L.ch_free(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    @property
+    def cuda_stream(self):
+        return self._stream
+
+    def set_spacing(self, dx, dy, dz):
+        self._check(self._L.ch_set_spacing(self._h, dx, dy, dz), "ch_set_spacing")
+
+    def set_state(self, u):
+        """u: numpy array or torch tensor (host, pinned host or device), [5][nz][ny][nx] fp64."""
+        if isinstance(u, np.ndarray):
+            u = np.ascontiguousarray(u, dtype=np.float64)
+        assert tuple(u.shape) == (5,) + self.shape, (tuple(u.shape), self.shape)
+        self._check(self._L.ch_set_state(self._h, _addr(u)), "ch_set_state")
+        if isinstance(u, np.ndarray):
+            self._L.ch_sync(self._h)   # the source array may be a temporary
+
+    def get_state(self, out=None):
+        if out is None:
+            out = np.empty((5,) + self.shape)
+        assert tuple(out.shape) == (5,) + self.shape
+        self._check(self._L.ch_get_state(self._h, _addr(out)), "ch_get_state")
+        return out
+
+    def set_padded(self, up):
+        if isinstance(up, np.ndarray):
+            up = np.ascontiguousarray(up, dtype=np.float64)
+        assert tuple(up.shape) == (5,) + self.padded_shape, (tuple(up.shape), self.padded_shape)
+        self._check(self._L.ch_set_padded(self._h, _addr(up)), "ch_set_padded")
+        if isinstance(up, np.ndarray):
+            self._L.ch_sync(self._h)
+
+    def get_padded(self, out=None):
+        if out is None:
+            out = np.empty((5,) + self.padded_shape)
+        self._check(self._L.ch_get_padded(self._h, _addr(out)), "ch_get_padded")
+        return out
+
+    def compute_dt(self, cfl) -> float:
+        dt = float(self._L.ch_compute_dt(self._h, cfl))
+        if dt != dt:
+            err = last_error()
+            if "cfl" in err or "no state" in err:
+                raise ValueError("ch_compute_dt: " + err)
+        return dt
+
+    def step(self, dt):
+        self._check(self._L.ch_step(self._h, dt), "ch_step")
+
+    def sync(self):
+        self._check(self._L.ch_sync(self._h), "ch_sync")
+
+    @property
+    def kernel_launches(self) -> int:
+        return int(self._L.ch_kernel_launches(self._h))
+
+
+def fp64_peak_probe(blocks=148 * 8, threads=256, iters=200000, device="cuda:0"):
+    """Measured DFMA rate (the ALU-roofline denominator): returns (TFLOP/s, ms)."""
+    import torch
+    L = load_library()
+    sink = torch.empty(blocks * threads, dtype=torch.float64, device=device)
+    st = torch.cuda.current_stream(sink.device)
+    ms = L.ch_fp64_peak_probe(sink.data_ptr(), blocks, threads, iters, st.cuda_stream)
+    if ms <= 0:
+        raise RuntimeError("ch_fp64_peak_probe: " + last_error())
+    return 2.0 * 8 * iters * blocks * threads / (ms * 1e-3) / 1e12, ms

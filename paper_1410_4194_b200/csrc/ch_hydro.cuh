@@ -1,0 +1,297 @@
+// ch_hydro.cuh — per-cell / per-interface device arithmetic of the CTU step (fp64).
+//
+// Written from the text of arXiv:1410.4194 (citations `P:L<line>` = /root/reference/PAPER.md line);
+// "G<n>/S<n>" are the readings of garbled / silent passages listed in DESIGN.md.  This file shares
+// nothing with oracle/: it restates the same equations in a form chosen for the B200 FP64 pipe
+// (one reciprocal-square-root per cell instead of four divisions and a square root, pr^z through
+// exp(z*log(pr)) with the 1/gamma power derived from it, mirror-folded Riemann sampling).
+//
+// All functions work in the direction-local ordering (rho, v_n, v_t1, v_t2, p).
+#pragma once
+
+#include <math.h>
+
+#ifdef __CUDACC__
+#define CH_HD __host__ __device__ __forceinline__
+#else
+#define CH_HD inline
+#endif
+
+namespace ch {
+
+constexpr double kPFloor = 1e-20;
+constexpr double kPGuessFloor = 1e-6;
+constexpr double kNewtonTol = 1e-8;     // P:L1095 "e.g. 1e-6"; reading S2
+constexpr int kNewtonCap = 20;          // reading S2
+
+// gamma-derived constants, computed once on the host in ch_init.
+struct Gas {
+  double gamma;
+  double gm1;        // gamma - 1
+  double inv_gm1;    // 1/(gamma - 1)
+  double two_gm1;    // 2/(gamma - 1)
+  double z;          // (gamma - 1)/(2 gamma)
+  double gm;         // (gamma - 1)/(gamma + 1)
+  double c_sh;       // (gamma + 1)/(2 gamma)
+  double half_gp1;   // (gamma + 1)/2
+  double two_gp1;    // 2/(gamma + 1)
+  double half_gm1;   // (gamma - 1)/2
+};
+
+CH_HD double rsqrt_d(double x) {
+#ifdef __CUDA_ARCH__
+  return rsqrt(x);
+#else
+  return 1.0 / sqrt(x);
+#endif
+}
+
+CH_HD double floor_p(double p) { return (p < kPFloor) ? kPFloor : p; }  // keeps NaN visible
+
+// Eq. 6-8: conserved (direction-local momenta) -> primitive, pressure floor (S1).
+CH_HD void cons2prim(const Gas& G, double d, double mn, double mt1, double mt2, double E, double w[5]) {
+  const double r = 1.0 / d;
+  const double u = mn * r, v = mt1 * r, ww = mt2 * r;
+  const double ke = 0.5 * d * ((u * u + v * v) + ww * ww);
+  w[0] = d; w[1] = u; w[2] = v; w[3] = ww;
+  w[4] = floor_p(G.gm1 * (E - ke));
+}
+
+// Eq. 6-8 inverted: primitive -> conserved (direction-local momenta).
+CH_HD void prim2cons(const Gas& G, const double w[5], double c[5]) {
+  c[0] = w[0];
+  c[1] = w[0] * w[1];
+  c[2] = w[0] * w[2];
+  c[3] = w[0] * w[3];
+  c[4] = w[4] * G.inv_gm1 + 0.5 * w[0] * ((w[1] * w[1] + w[2] * w[2]) + w[3] * w[3]);
+}
+
+// s = 1/(rho a) with a = sqrt(gamma p / rho) (Eq. 21): the one transcendental per cell; everything
+// the characteristic projections need follows by multiplication:
+//   a = gamma p s,  1/a = rho s,  rho/a = rho^2 s,  1/a^2 = (rho s)^2,  a/rho = a^2 s,  rho a = gamma p rho s.
+CH_HD double inv_rho_a(const Gas& G, double rho, double p) { return rsqrt_d(G.gamma * p * rho); }
+
+// Monotonised-central limiter A10 (reading G7: the formula governs).
+CH_HD double mc_limit(double dL, double dR, double dC) {
+  const double m = fmin(fabs(dC), 2.0 * fmin(fabs(dL), fabs(dR)));
+  return (dL * dR > 0.0) ? copysign(m, dC) : 0.0;
+}
+
+// Limited slope of cell q in primitive variables via characteristic variables (A2 P:L690, A9 P:L730
+// with row 0 read as G1, A10, A11 P:L741), projected with cell q's own rho, a.
+// s = inv_rho_a(q).
+CH_HD void limited_slope(const Gas& G, const double wm[5], const double w0[5], const double wp[5], double s,
+                         double dw[5]) {
+  const double rho = w0[0];
+  const double a = G.gamma * w0[4] * s;
+  const double ia = rho * s;
+  const double ra = rho * ia;     // rho / a
+  const double ia2 = ia * ia;     // 1 / a^2
+  double xL[5], xR[5], x[5];
+  {
+    const double d0 = w0[0] - wm[0], d1 = w0[1] - wm[1], d4 = w0[4] - wm[4];
+    const double t1 = ra * d1, t2 = d4 * ia2;
+    xL[0] = 0.5 * (t2 - t1); xL[1] = d0 - t2; xL[2] = w0[2] - wm[2]; xL[3] = w0[3] - wm[3]; xL[4] = 0.5 * (t1 + t2);
+  }
+  {
+    const double d0 = wp[0] - w0[0], d1 = wp[1] - w0[1], d4 = wp[4] - w0[4];
+    const double t1 = ra * d1, t2 = d4 * ia2;
+    xR[0] = 0.5 * (t2 - t1); xR[1] = d0 - t2; xR[2] = wp[2] - w0[2]; xR[3] = wp[3] - w0[3]; xR[4] = 0.5 * (t1 + t2);
+  }
+  {
+    // centred difference (A2) projected the same way
+    const double d0 = 0.5 * (wp[0] - wm[0]), d1 = 0.5 * (wp[1] - wm[1]), d4 = 0.5 * (wp[4] - wm[4]);
+    const double t1 = ra * d1, t2 = d4 * ia2;
+    const double c0 = 0.5 * (t2 - t1), c1 = d0 - t2, c2 = 0.5 * (wp[2] - wm[2]), c3 = 0.5 * (wp[3] - wm[3]),
+                 c4 = 0.5 * (t1 + t2);
+    x[0] = mc_limit(xL[0], xR[0], c0);
+    x[1] = mc_limit(xL[1], xR[1], c1);
+    x[2] = mc_limit(xL[2], xR[2], c2);
+    x[3] = mc_limit(xL[3], xR[3], c3);
+    x[4] = mc_limit(xL[4], xR[4], c4);
+  }
+  const double s04 = x[0] + x[4];
+  dw[0] = x[1] + s04;
+  dw[1] = (a * a * s) * (x[4] - x[0]);   // a / rho
+  dw[2] = x[2];
+  dw[3] = x[3];
+  dw[4] = (a * a) * s04;
+}
+
+// PPMC for one cell (A.3): parabola edges A20-A23, A24/A26(=A50, G2), characteristic
+// tracing A25-A33 (A30/A32 read as G3).  wm,w0,wp = cells i-1,i,i+1; dwm,dw0,dwp their limited
+// slopes; s = inv_rho_a(i); dtdx = dt/dx_d.  Outputs W*_L, W*_R (primitive).
+CH_HD void ppmc_faces(const Gas& G, double dtdx, const double wm[5], const double w0[5], const double wp[5],
+                      const double dwm[5], const double dw0[5], const double dwp[5], double s, double WLs[5],
+                      double WRs[5]) {
+  double WL[5], WR[5], dwi[5], w6[5];
+#pragma unroll
+  for (int m = 0; m < 5; ++m) {
+    const double wi = w0[m];
+    double L = 0.5 * (wi + wm[m]) - (dw0[m] - dwm[m]) * (1.0 / 6.0);   // A20
+    double R = 0.5 * (wp[m] + wi) - (dwp[m] - dw0[m]) * (1.0 / 6.0);
+    if ((R - wi) * (wi - L) <= 0.0) { L = wi; R = wi; }                // A21
+    const double t3 = 3.0 * wi;
+    const double cl = t3 - 2.0 * R, cr = t3 - 2.0 * L;                 // A22, G8
+    const double RL = R - L;
+    const bool fixL = RL * (L - cl) < 0.0;
+    const bool fixR = RL * (cr - R) < 0.0;
+    if (fixL) L = cl;
+    if (fixR) R = cr;
+    L = fmin(fmax(wi, wm[m]), fmax(fmin(wi, wm[m]), L));               // A23
+    R = fmin(fmax(wi, wp[m]), fmax(fmin(wi, wp[m]), R));
+    WL[m] = L; WR[m] = R;
+    dwi[m] = R - L;                                                    // A24
+    w6[m] = 6.0 * (wi - 0.5 * (L + R));                                // A26 as A50 (G2)
+  }
+  const double rho = w0[0];
+  const double a = G.gamma * w0[4] * s;
+  const double ia = rho * s;
+  const double ia2 = ia * ia;
+  const double ra = rho * ia;        // rho / a
+  const double rhoa = rho * a;       // rho * a
+  const double lm = w0[1] - a, l0 = w0[1], lp = w0[1] + a;            // A8
+  const double am = dtdx * fmin(lm, 0.0), a0 = dtdx * fmin(l0, 0.0), ap = dtdx * fmin(lp, 0.0);  // A27
+  const double bm = dtdx * fmax(lm, 0.0), b0 = dtdx * fmax(l0, 0.0), bp = dtdx * fmax(lp, 0.0);
+  const double k23 = 2.0 / 3.0;
+  // reference states A25: left face under lambda^m, right face under lambda^p
+  double WLm[5], WRp[5];
+  {
+    const double ca = 0.5 * am, cb = 1.0 + k23 * am;
+    const double da = 0.5 * bp, db = 1.0 - k23 * bp;
+#pragma unroll
+    for (int m = 0; m < 5; ++m) {
+      WLm[m] = WL[m] - ca * (dwi[m] + w6[m] * cb);
+      WRp[m] = WR[m] - da * (dwi[m] - w6[m] * db);
+    }
+  }
+  double sL0 = 0.0, sL1 = 0.0, sL2 = 0.0, sL3 = 0.0, sL4 = 0.0;
+  double sR0 = 0.0, sR1 = 0.0, sR2 = 0.0, sR3 = 0.0, sR4 = 0.0;
+  if (l0 < 0.0) {   // A28 first term: E = W_L^0 - W_L^m
+    const double ca = 0.5 * a0, cb = 1.0 + k23 * a0;
+    const double E0 = (WL[0] - ca * (dwi[0] + w6[0] * cb)) - WLm[0];
+    const double E2 = (WL[2] - ca * (dwi[2] + w6[2] * cb)) - WLm[2];
+    const double E3 = (WL[3] - ca * (dwi[3] + w6[3] * cb)) - WLm[3];
+    const double E4 = (WL[4] - ca * (dwi[4] + w6[4] * cb)) - WLm[4];
+    sL0 += E0 - E4 * ia2; sL2 += E2; sL3 += E3;
+  }
+  if (lp < 0.0) {   // A28 second term: B = W_L^p - W_L^m
+    const double ca = 0.5 * ap, cb = 1.0 + k23 * ap;
+    const double B1 = (WL[1] - ca * (dwi[1] + w6[1] * cb)) - WLm[1];
+    const double B4 = (WL[4] - ca * (dwi[4] + w6[4] * cb)) - WLm[4];
+    sL0 += 0.5 * (ra * B1 + B4 * ia2);
+    sL1 += 0.5 * (B1 + B4 * s);
+    sL4 += 0.5 * (rhoa * B1 + B4);
+  }
+  if (lm > 0.0) {   // A31 first term: C = W_R^m - W_R^p
+    const double da = 0.5 * bm, db = 1.0 - k23 * bm;
+    const double C1 = (WR[1] - da * (dwi[1] - w6[1] * db)) - WRp[1];
+    const double C4 = (WR[4] - da * (dwi[4] - w6[4] * db)) - WRp[4];
+    sR0 += 0.5 * (C4 * ia2 - ra * C1);
+    sR1 += 0.5 * (C1 - C4 * s);
+    sR4 += 0.5 * (C4 - rhoa * C1);
+  }
+  if (l0 > 0.0) {   // A31 second term: D = W_R^0 - W_R^p
+    const double da = 0.5 * b0, db = 1.0 - k23 * b0;
+    const double D0 = (WR[0] - da * (dwi[0] - w6[0] * db)) - WRp[0];
+    const double D2 = (WR[2] - da * (dwi[2] - w6[2] * db)) - WRp[2];
+    const double D3 = (WR[3] - da * (dwi[3] - w6[3] * db)) - WRp[3];
+    const double D4 = (WR[4] - da * (dwi[4] - w6[4] * db)) - WRp[4];
+    sR0 += D0 - D4 * ia2; sR2 += D2; sR3 += D3;
+  }
+  WLs[0] = WLm[0] + sL0; WLs[1] = WLm[1] + sL1; WLs[2] = WLm[2] + sL2; WLs[3] = WLm[3] + sL3; WLs[4] = WLm[4] + sL4;  // A33
+  WRs[0] = WRp[0] + sR0; WRs[1] = WRp[1] + sR1; WRs[2] = WRp[2] + sR2; WRs[3] = WRp[3] + sR3; WRs[4] = WRp[4] + sR4;
+}
+
+// Pressure function f_k, f'_k (B5, B6) for one side at trial pressure p.
+//   rk, pk: density and pressure of side k; ak = sound speed; rpk = 1/pk; ick = 1/(rho_k a_k).
+// x returns (p/pk)^z on the rarefaction branch (re-used by the sampler), untouched otherwise.
+CH_HD void pressure_fn(const Gas& G, double p, double rk, double pk, double ak, double rpk, double ick, double& f,
+                       double& fp, double& x) {
+  if (p <= pk) {   // rarefaction
+    const double pr = p * rpk;
+    x = exp(G.z * log(pr));
+    f = G.two_gm1 * ak * (x - 1.0);
+    fp = ick * x / pr;                       // pr^{-(gamma+1)/(2 gamma)} = pr^z / pr
+  } else {         // shock: sqrt(A/(p+B)) = rsqrt((p + B) rho (gamma+1)/2)   (B4)
+    const double h = rk * G.half_gp1;
+    const double sq = rsqrt_d((p + G.gm * pk) * h);
+    const double dp = p - pk;
+    f = dp * sq;
+    fp = sq * (1.0 - 0.5 * dp * (sq * sq) * h);   // 1/(B+p) = sq^2 (gamma+1) rho / 2
+  }
+}
+
+// Exact Riemann solver (B.1): primitive L/R states (direction-local) -> flux B22.
+// Newton-Raphson on the star pressure from the two-shock guess B2-B4; f_k re-evaluated at the final
+// p^m for u^m (reading S3); iterate floored at 1e-20 (S4).  The ten-way sampling at x/t = 0 is
+// folded onto the left-wave family by mirroring (u -> -u) when u^m < 0; the mirrored tests coincide
+// with B16-B21 except on the measure-zero tie um + a_R x = 0, where fan and star state are equal.
+CH_HD void riemann_exact(const Gas& G, const double WL[5], const double WR[5], double flux[5]) {
+  const double rL = WL[0], uL = WL[1], pL = floor_p(WL[4]);
+  const double rR = WR[0], uR = WR[1], pR = floor_p(WR[4]);
+  const double icL = inv_rho_a(G, rL, pL), icR = inv_rho_a(G, rR, pR);   // 1/(rho a)
+  const double gpL = G.gamma * pL, gpR = G.gamma * pR;
+  const double aL = gpL * icL, aR = gpR * icR;                           // B1
+  const double rpL = G.gamma * rL * (icL * icL);                         // 1/p = gamma rho /(rho a)^2
+  const double rpR = G.gamma * rR * (icR * icR);
+  const double du = uR - uL;
+  // B2
+  double pt = 0.5 * (pL + pR) - 0.125 * du * (rL + rR) * (aL + aR);
+  pt = (pt < 0.0) ? 0.0 : pt;
+  // B3, B4: g_k = sqrt(A_k/(pt + B_k))
+  const double gL = rsqrt_d((pt + G.gm * pL) * rL * G.half_gp1);
+  const double gR = rsqrt_d((pt + G.gm * pR) * rR * G.half_gp1);
+  double p0 = ((gL * pL + gR * pR) - du) / (gL + gR);
+  p0 = (p0 < kPGuessFloor) ? kPGuessFloor : p0;
+  // Newton-Raphson B5-B8
+  double pm, fL, fR, fpL, fpR, xL = 1.0, xR = 1.0;
+  int it = 0;
+  for (;;) {
+    pressure_fn(G, p0, rL, pL, aL, rpL, icL, fL, fpL, xL);
+    pressure_fn(G, p0, rR, pR, aR, rpR, icR, fR, fpR, xR);
+    pm = p0 - ((fL + fR) + du) / (fpL + fpR);                           // B7
+    pm = (pm < kPFloor) ? kPFloor : pm;                                  // S4
+    ++it;
+    if (!(2.0 * fabs(pm - p0) > kNewtonTol * fabs(pm + p0)) || it >= kNewtonCap) break;   // B8
+    p0 = pm;
+  }
+  pressure_fn(G, pm, rL, pL, aL, rpL, icL, fL, fpL, xL);                 // S3
+  pressure_fn(G, pm, rR, pR, aR, rpR, icR, fR, fpR, xR);
+  const double um = 0.5 * ((uL + uR) + (fR - fL));                       // B9
+
+  // Sampling at x/t = 0, mirrored onto the left family.
+  const bool left = (um >= 0.0);
+  const double sg = left ? 1.0 : -1.0;
+  const double rk = left ? rL : rR, pk = left ? pL : pR, ak = left ? aL : aR;
+  const double uk = sg * (left ? uL : uR), us = sg * um;
+  const double rpk = left ? rpL : rpR, xk = left ? xL : xR;
+  const double vt1 = left ? WL[2] : WR[2], vt2 = left ? WL[3] : WR[3];   // S9
+  const double pr = pm * rpk;
+  double rho, u, p;
+  if (pm <= pk) {                                                        // rarefaction
+    if (uk - ak >= 0.0) { rho = rk; u = uk; p = pk; }                    // B10 / B16
+    else if (us - ak * xk < 0.0) { rho = rk * (pr / (xk * xk)); u = us; p = pm; }   // B11 / B17: pr^{1/gamma} = pr / x^2
+    else {                                                               // B12 / B18 (G4)
+      const double af = G.two_gp1 * (ak + G.half_gm1 * uk);
+      const double q = af / ak;
+      const double y = exp(G.two_gm1 * log(q));                          // (a/a_k)^{2/(gamma-1)}
+      rho = rk * y; u = af; p = pk * y * (q * q);                        // exponent 2 gamma/(gamma-1) = 2/(gamma-1) + 2
+    }
+  } else {                                                               // shock
+    const double sk = uk - ak * sqrt(G.c_sh * pr + G.z);                 // B13 / B19 (G5)
+    if (sk >= 0.0) { rho = rk; u = uk; p = pk; }                         // B14 / B20
+    else { rho = rk * (pr + G.gm) / (pr * G.gm + 1.0); u = us; p = pm; } // B15 / B21
+  }
+  u *= sg;
+  // B22
+  const double E = p * G.inv_gm1 + 0.5 * rho * ((u * u + vt1 * vt1) + vt2 * vt2);
+  const double ru = rho * u;
+  flux[0] = ru;
+  flux[1] = ru * u + p;
+  flux[2] = ru * vt1;
+  flux[3] = ru * vt2;
+  flux[4] = (E + p) * u;
+}
+
+}  // namespace ch

@@ -1,0 +1,754 @@
+// ch_kernels.cu — CUDA kernels (sm_100a) and the C ABI of include/ch.h.
+//
+// One CTU step =
+//   k_reset            reset the dt reduction cells
+//   k_pass1_x          PPMC + tracing + exact Riemann along x   -> U*_L,U*_R(.,x), F*      (steps 1-2)
+//   k_pass1_march<1|2> same along y / z, marching in registers  -> U*_L,U*_R(.,d), G*, H*
+//   k_pass2            Eq. 23 transverse correction + second exact Riemann pass -> F,G,H^{n+1/2} (3-4)
+//   k_update           Eq. 24 conservative update + Eq. 22 wave-speed reduction of the new state (5)
+//   k_ghost            ghost fill of the new state
+// Data layout: struct-of-arrays fp64, x fastest, ghosts included; every kernel maps
+// consecutive lanes to consecutive x so loads and stores coalesce.  The work is FP64-pipe bound
+// (see DESIGN.md §Roofline), so intermediates that cross kernels go through HBM/L2 as plain
+// coalesced arrays and no operand is reshaped for tensor cores.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdint>
+#include <cstdio>
+#include <cstring>
+#include <limits>
+#include <new>
+#include <string>
+
+#include "../../include/ch.h"
+#include "ch_hydro.cuh"
+
+namespace {
+
+using ch::Gas;
+
+struct Geom {
+  int n[3];          // real cells
+  int g[3];          // ghost layers (0 for an inactive dimension)
+  int pd[3];         // padded extents
+  int act[3];        // n_d > 1
+  long long st[3];   // strides in doubles: 1, px, px*py
+  long long np;      // padded cells
+};
+
+struct StepArgs {
+  Geom geo;
+  Gas gas;
+  double dtdx[3];    // dt / dx_d
+  double dx[3];
+  double* u;         // state [5][np]
+  double* Fs[3];     // first-pass fluxes F*_d at interface c+1/2 stored at c  [5][np]
+  double* UL[3];     // U*_L(c,d): traced state at the left face of cell c     [5][np]
+  double* UR[3];     // U*_R(c,d)
+  double* Fh[3];     // CTU fluxes F^{n+1/2}_d                                 [5][np]
+  unsigned long long* red;  // [0] = bits of min dt_cell, [1] = non-physical flag
+};
+
+// global component index of direction-local component m for a sweep along D (cyclic)
+template <int D>
+__device__ __forceinline__ constexpr int comp(int m) {
+  return (m == 0 || m == 4) ? m : 1 + (D + (m - 1)) % 3;
+}
+
+template <int D>
+__device__ __forceinline__ void load_prim(const Gas& G, const double* __restrict__ u, long long np, long long q,
+                                          double w[5]) {
+  const double d = u[q];
+  const double mn = u[comp<D>(1) * np + q];
+  const double m1 = u[comp<D>(2) * np + q];
+  const double m2 = u[comp<D>(3) * np + q];
+  const double E = u[4 * np + q];
+  ch::cons2prim(G, d, mn, m1, m2, E, w);
+}
+
+// store a direction-local conserved vector into a global-order SoA array
+template <int D>
+__device__ __forceinline__ void store_local(double* __restrict__ dst, long long np, long long q, const double c[5]) {
+  dst[q] = c[0];
+  dst[comp<D>(1) * np + q] = c[1];
+  dst[comp<D>(2) * np + q] = c[2];
+  dst[comp<D>(3) * np + q] = c[3];
+  dst[4 * np + q] = c[4];
+}
+
+__device__ __forceinline__ void copy5(double dst[5], const double src[5]) {
+#pragma unroll
+  for (int m = 0; m < 5; ++m) dst[m] = src[m];
+}
+
+// ---------------------------------------------------------------------------------------------
+// Pass 1 along y or z: each thread owns one (x, transverse) column and marches a segment of `seg`
+// interfaces along D with the 5-cell primitive stencil, three limited slopes and the previous
+// cell's right-face state in registers.  Every cell's slope and parabola is computed once per
+// segment (warm-up: 3 slopes + 1 parabola per segment).
+// ---------------------------------------------------------------------------------------------
+template <int D>
+__global__ void __launch_bounds__(128) k_pass1_march(const StepArgs A, int seg) {
+  constexpr int T = 3 - D;   // the other transverse dimension (x is the lane dimension)
+  const Geom& g = A.geo;
+  const Gas& G = A.gas;
+  const int ext0 = g.act[0] ? g.n[0] + 2 : 1, lo0 = g.act[0] ? -1 : 0;
+  const int extT = g.act[T] ? g.n[T] + 2 : 1, loT = g.act[T] ? -1 : 0;
+  const long long col = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (col >= (long long)ext0 * extT) return;
+  const int i = lo0 + (int)(col % ext0);
+  const int t = loT + (int)(col / ext0);
+  const int c0 = -1 + (int)blockIdx.y * seg;          // first interface of this segment
+  const int nD = g.n[D];
+  int c1 = c0 + seg;                                   // one past the last interface
+  const bool last = c1 >= nD;
+  if (last) c1 = nD;
+  const long long sD = g.st[D];
+  const long long np = g.np;
+  const long long base = (long long)(i + g.g[0]) + (long long)(t + g.g[T]) * g.st[T] + (long long)g.g[D] * sD;
+  const double dtdx = A.dtdx[D];
+  const double* __restrict__ u = A.u;
+
+  double wa[5], wb[5], wc[5], wd[5];   // cells c-1, c, c+1, c+2 (rotating)
+  double sa[5], sb[5], sc[5];          // slopes of c-1, c, c+1
+  double icb, icc;                     // 1/(rho a) of c, c+1
+  double pr_prev[5];                   // previous cell's right-face primitive state
+  {
+    double wz[5];
+    load_prim<D>(G, u, np, base + (long long)(c0 - 2) * sD, wz);
+    load_prim<D>(G, u, np, base + (long long)(c0 - 1) * sD, wa);
+    load_prim<D>(G, u, np, base + (long long)(c0)*sD, wb);
+    load_prim<D>(G, u, np, base + (long long)(c0 + 1) * sD, wc);
+    ch::limited_slope(G, wz, wa, wb, ch::inv_rho_a(G, wa[0], wa[4]), sa);
+    icb = ch::inv_rho_a(G, wb[0], wb[4]);
+    ch::limited_slope(G, wa, wb, wc, icb, sb);
+  }
+  for (int c = c0; c <= c1; ++c) {
+    const long long q = base + (long long)c * sD;
+    load_prim<D>(G, u, np, q + 2 * sD, wd);
+    icc = ch::inv_rho_a(G, wc[0], wc[4]);
+    ch::limited_slope(G, wb, wc, wd, icc, sc);
+    double WLs[5], WRs[5], cl[5], cr[5];
+    ch::ppmc_faces(G, dtdx, wa, wb, wc, sa, sb, sc, icb, WLs, WRs);
+    ch::prim2cons(G, WLs, cl);
+    ch::prim2cons(G, WRs, cr);
+    if (c < c1 || last) {
+      store_local<D>(A.UL[D], np, q, cl);
+      store_local<D>(A.UR[D], np, q, cr);
+    }
+    if (c > c0) {
+      double wl[5], fl[5];
+      ch::cons2prim(G, cl[0], cl[1], cl[2], cl[3], cl[4], wl);   // states are kept conserved between stages
+      ch::riemann_exact(G, pr_prev, wl, fl);
+      store_local<D>(A.Fs[D], np, q - sD, fl);
+    }
+    ch::cons2prim(G, cr[0], cr[1], cr[2], cr[3], cr[4], pr_prev);
+    copy5(wa, wb); copy5(wb, wc); copy5(wc, wd);
+    copy5(sa, sb); copy5(sb, sc);
+    icb = icc;
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Pass 1 along x: one thread per padded cell of a flat run of memory (x fastest, rows follow one
+// another), neighbours exchanged through shared memory in three stages (primitives -> slopes ->
+// left-face states).  A CTA of T threads yields T-5 interfaces; lanes on cells outside the needed
+// ranges are masked so garbage row-crossing stencils cost nothing.
+// ---------------------------------------------------------------------------------------------
+constexpr int kXT = 256;       // threads per CTA
+constexpr int kXOut = kXT - 5; // interfaces produced per CTA
+
+__global__ void __launch_bounds__(kXT) k_pass1_x(const StepArgs A, long long q_begin, long long q_end) {
+  __shared__ double sP[5][kXT];
+  __shared__ double sS[5][kXT];
+  __shared__ double sL[5][kXT];
+  const Geom& g = A.geo;
+  const Gas& G = A.gas;
+  const long long np = g.np;
+  const int tid = threadIdx.x;
+  const long long q = q_begin + (long long)blockIdx.x * kXOut + tid - 2;
+  const bool inb = (q >= 0 && q < np);
+  // coordinates of q
+  int i = 0, j = 0, k = 0;
+  if (inb) {
+    long long r = q;
+    k = (int)(r / g.st[2]); r -= (long long)k * g.st[2];
+    j = (int)(r / g.st[1]);
+    i = (int)(r - (long long)j * g.st[1]);
+    i -= g.g[0]; j -= g.g[1]; k -= g.g[2];
+  }
+  // rows needed: transverse indices in [-1, n] (or the single row of an inactive dimension)
+  const bool row_ok = inb && (!g.act[1] || (j >= -1 && j <= g.n[1])) && (!g.act[2] || (k >= -1 && k <= g.n[2]));
+  const int nx = g.n[0];
+  double w0[5] = {1.0, 0.0, 0.0, 0.0, 1.0};
+  if (row_ok) load_prim<0>(G, A.u, np, q, w0);
+#pragma unroll
+  for (int m = 0; m < 5; ++m) sP[m][tid] = w0[m];
+  __syncthreads();
+  // stage 2: slopes for i in [-2, nx+1]
+  double wm[5], wp[5], s0[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+  const bool slope_ok = row_ok && tid >= 1 && tid <= kXT - 2 && i >= -2 && i <= nx + 1;
+  const int tl = tid > 0 ? tid - 1 : 0, tr = tid < kXT - 1 ? tid + 1 : kXT - 1;
+#pragma unroll
+  for (int m = 0; m < 5; ++m) { wm[m] = sP[m][tl]; wp[m] = sP[m][tr]; }
+  double ic = 0.0;
+  if (slope_ok) {
+    ic = ch::inv_rho_a(G, w0[0], w0[4]);
+    ch::limited_slope(G, wm, w0, wp, ic, s0);
+  }
+#pragma unroll
+  for (int m = 0; m < 5; ++m) sS[m][tid] = s0[m];
+  __syncthreads();
+  // stage 3: parabola + tracing for i in [-1, nx]
+  const bool face_ok = slope_ok && tid >= 2 && tid <= kXT - 3 && i >= -1 && i <= nx;
+  double prR[5] = {1.0, 0.0, 0.0, 0.0, 1.0}, prL[5] = {1.0, 0.0, 0.0, 0.0, 1.0};
+  if (face_ok) {
+    double sm[5], sp[5], WLs[5], WRs[5], cl[5], cr[5];
+#pragma unroll
+    for (int m = 0; m < 5; ++m) { sm[m] = sS[m][tid - 1]; sp[m] = sS[m][tid + 1]; }
+    ch::ppmc_faces(G, A.dtdx[0], wm, w0, wp, sm, s0, sp, ic, WLs, WRs);
+    ch::prim2cons(G, WLs, cl);
+    ch::prim2cons(G, WRs, cr);
+    // a cell's faces are written by the CTA whose output window [2, kXT-4] holds it, plus the
+    // trailing cell kXT-3 that no later window covers as a face-only slot: both write the same value
+    store_local<0>(A.UL[0], np, q, cl);
+    store_local<0>(A.UR[0], np, q, cr);
+    ch::cons2prim(G, cl[0], cl[1], cl[2], cl[3], cl[4], prL);
+    ch::cons2prim(G, cr[0], cr[1], cr[2], cr[3], cr[4], prR);
+  }
+#pragma unroll
+  for (int m = 0; m < 5; ++m) sL[m][tid] = prL[m];
+  __syncthreads();
+  // stage 4: Riemann problem at i+1/2 for i in [-1, nx-1]
+  if (face_ok && tid <= kXT - 4 && i <= nx - 1 && q < q_end) {
+    double wr[5], fl[5];
+#pragma unroll
+    for (int m = 0; m < 5; ++m) wr[m] = sL[m][tid + 1];
+    ch::riemann_exact(G, prR, wr, fl);
+    store_local<0>(A.Fs[0], np, q, fl);
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Pass 2: transverse correction (Eq. 23) of the two states meeting at interface c+1/2
+// along each active direction, then the second exact Riemann solve.  One thread per cell
+// of [-1, n)^3.
+// ---------------------------------------------------------------------------------------------
+template <int D>
+__device__ __forceinline__ void corrected_prim(const StepArgs& A, const double* __restrict__ U, long long q,
+                                               double w[5]) {
+  const Geom& g = A.geo;
+  const long long np = g.np;
+  constexpr int E1 = (D + 1) % 3, E2 = (D + 2) % 3;
+  double c[5];
+#pragma unroll
+  for (int f = 0; f < 5; ++f) {
+    double corr = 0.0;
+    if (g.act[E1]) corr += 0.5 * A.dtdx[E1] * (A.Fs[E1][f * np + q - g.st[E1]] - A.Fs[E1][f * np + q]);
+    if (g.act[E2]) corr += 0.5 * A.dtdx[E2] * (A.Fs[E2][f * np + q - g.st[E2]] - A.Fs[E2][f * np + q]);
+    c[f] = U[f * np + q] + corr;
+  }
+  ch::cons2prim(A.gas, c[0], c[comp<D>(1)], c[comp<D>(2)], c[comp<D>(3)], c[4], w);
+}
+
+template <int D>
+__device__ __forceinline__ void pass2_dir(const StepArgs& A, long long q) {
+  double wl[5], wr[5], fl[5];
+  corrected_prim<D>(A, A.UR[D], q, wl);                 // U^{n+1/2}_R of cell c   -> left state
+  corrected_prim<D>(A, A.UL[D], q + A.geo.st[D], wr);   // U^{n+1/2}_L of cell c+1 -> right state
+  ch::riemann_exact(A.gas, wl, wr, fl);
+  store_local<D>(A.Fh[D], A.geo.np, q, fl);
+}
+
+__global__ void __launch_bounds__(128) k_pass2(const StepArgs A) {
+  const Geom& g = A.geo;
+  const int e0 = g.act[0] ? g.n[0] + 1 : 1, e1 = g.act[1] ? g.n[1] + 1 : 1, e2 = g.act[2] ? g.n[2] + 1 : 1;
+  const long long id = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (id >= (long long)e0 * e1 * e2) return;
+  const int i = (int)(id % e0) - (g.act[0] ? 1 : 0);
+  const long long r = id / e0;
+  const int j = (int)(r % e1) - (g.act[1] ? 1 : 0);
+  const int k = (int)(r / e1) - (g.act[2] ? 1 : 0);
+  const long long q = (long long)(i + g.g[0]) + (long long)(j + g.g[1]) * g.st[1] + (long long)(k + g.g[2]) * g.st[2];
+  if (g.act[0] && j >= 0 && k >= 0) pass2_dir<0>(A, q);
+  if (g.act[1] && i >= 0 && k >= 0) pass2_dir<1>(A, q);
+  if (g.act[2] && i >= 0 && j >= 0) pass2_dir<2>(A, q);
+}
+
+// ---------------------------------------------------------------------------------------------
+// Eq. 22 per cell, evaluated with explicitly rounded operations (no FMA contraction) so that the
+// reduced minimum does not depend on how the compiler fuses: dt is a pure function of the state.
+// Returns dx_d/(|v_d|+a) minimised over active d; sets bad for rho<=0 / non-finite input.
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ double cell_dt(const StepArgs& A, double d, double m0, double m1, double m2, double E,
+                                          bool& bad) {
+  const double inf = __longlong_as_double(0x7FF0000000000000LL);
+  if (!(d > 0.0) || !isfinite(d) || !isfinite(E)) { bad = true; return inf; }
+  const double vx = __ddiv_rn(m0, d), vy = __ddiv_rn(m1, d), vz = __ddiv_rn(m2, d);
+  const double v2 = __dadd_rn(__dadd_rn(__dmul_rn(vx, vx), __dmul_rn(vy, vy)), __dmul_rn(vz, vz));
+  const double ke = __dmul_rn(__dmul_rn(0.5, d), v2);                       // Eq. 7
+  double p = __dmul_rn(A.gas.gm1, __dadd_rn(E, -ke));                        // Eq. 6, 8
+  if (!(p >= ch::kPFloor)) p = (p != p) ? p : ch::kPFloor;
+  const double a = __dsqrt_rn(__ddiv_rn(__dmul_rn(A.gas.gamma, p), d));      // Eq. 21
+  double tmin = inf;
+  const double v[3] = {vx, vy, vz};
+#pragma unroll
+  for (int e = 0; e < 3; ++e) {
+    if (!A.geo.act[e]) continue;
+    const double t = __ddiv_rn(A.dx[e], __dadd_rn(fabs(v[e]), a));
+    if (t != t) bad = true;
+    if (t < tmin) tmin = t;
+  }
+  return tmin;
+}
+
+__device__ __forceinline__ void block_min_reduce(double t, bool bad, unsigned long long* red) {
+  __shared__ double s_min[32];
+  __shared__ int s_bad;
+  if (threadIdx.x == 0) s_bad = 0;
+  __syncthreads();
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) t = fmin(t, __shfl_xor_sync(0xffffffffu, t, o));
+  if (__any_sync(0xffffffffu, bad) && (threadIdx.x & 31) == 0) s_bad = 1;
+  if ((threadIdx.x & 31) == 0) s_min[threadIdx.x >> 5] = t;
+  __syncthreads();
+  if (threadIdx.x < 32) {
+    const int nw = (blockDim.x + 31) >> 5;
+    double v = threadIdx.x < nw ? s_min[threadIdx.x] : __longlong_as_double(0x7FF0000000000000LL);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v = fmin(v, __shfl_xor_sync(0xffffffffu, v, o));
+    if (threadIdx.x == 0) {
+      // positive doubles order like their bit patterns: a single-pass grid reduction with one
+      // atomicMin per CTA, deterministic because min is exact
+      atomicMin(red, (unsigned long long)__double_as_longlong(v));
+      if (s_bad) atomicOr(red + 1, 1ULL);
+    }
+  }
+}
+
+__global__ void __launch_bounds__(256) k_reset(unsigned long long* red) {
+  if (threadIdx.x == 0) { red[0] = 0x7FF0000000000000ULL; red[1] = 0ULL; }
+}
+
+// Standalone Eq. 22 reduction over real cells (used after ch_set_state / ch_set_padded).
+__global__ void __launch_bounds__(256) k_dt(const StepArgs A) {
+  const Geom& g = A.geo;
+  const long long N = (long long)g.n[0] * g.n[1] * g.n[2];
+  double tmin = __longlong_as_double(0x7FF0000000000000LL);
+  bool bad = false;
+  for (long long id = (long long)blockIdx.x * blockDim.x + threadIdx.x; id < N; id += (long long)gridDim.x * blockDim.x) {
+    const int i = (int)(id % g.n[0]);
+    const long long r = id / g.n[0];
+    const int j = (int)(r % g.n[1]);
+    const int k = (int)(r / g.n[1]);
+    const long long q = (long long)(i + g.g[0]) + (long long)(j + g.g[1]) * g.st[1] + (long long)(k + g.g[2]) * g.st[2];
+    const double t = cell_dt(A, A.u[q], A.u[g.np + q], A.u[2 * g.np + q], A.u[3 * g.np + q], A.u[4 * g.np + q], bad);
+    tmin = fmin(tmin, t);
+  }
+  block_min_reduce(tmin, bad, A.red);
+}
+
+// Eq. 24 on real cells, fused with the Eq. 22 reduction of the updated state.
+__global__ void __launch_bounds__(256) k_update(const StepArgs A) {
+  const Geom& g = A.geo;
+  const long long N = (long long)g.n[0] * g.n[1] * g.n[2];
+  const long long id = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  double t = __longlong_as_double(0x7FF0000000000000LL);
+  bool bad = false;
+  if (id < N) {
+    const int i = (int)(id % g.n[0]);
+    const long long r = id / g.n[0];
+    const int j = (int)(r % g.n[1]);
+    const int k = (int)(r / g.n[1]);
+    const long long q = (long long)(i + g.g[0]) + (long long)(j + g.g[1]) * g.st[1] + (long long)(k + g.g[2]) * g.st[2];
+    double v[5];
+#pragma unroll
+    for (int f = 0; f < 5; ++f) {
+      double x = A.u[f * g.np + q];
+#pragma unroll
+      for (int d = 0; d < 3; ++d)
+        if (g.act[d]) x += A.dtdx[d] * (A.Fh[d][f * g.np + q - g.st[d]] - A.Fh[d][f * g.np + q]);
+      v[f] = x;
+      A.u[f * g.np + q] = x;
+    }
+    t = cell_dt(A, v[0], v[1], v[2], v[3], v[4], bad);
+  }
+  block_min_reduce(t, bad, A.red);
+}
+
+// ---------------------------------------------------------------------------------------------
+// Ghost fill (readings S6, S7).  Filling x, then y over the padded x extent, then z over
+// the padded x,y extent makes every ghost cell a copy of the real cell obtained by mapping
+// each coordinate on its own, with the sign of each reflected normal momentum flipped; so one
+// launch over the ghost shell reads real cells only and writes ghost cells only.
+// ---------------------------------------------------------------------------------------------
+struct BcArgs { int bc[6]; };
+
+__device__ __forceinline__ int bc_source(int c, int n, int lo, int hi, bool& flip) {
+  if (c < 0) {
+    if (lo == CH_BC_PERIODIC) return c + n;
+    if (lo == CH_BC_REFLECTIVE) { flip = !flip; return -c - 1; }
+    return 0;
+  }
+  if (c >= n) {
+    if (hi == CH_BC_PERIODIC) return c - n;
+    if (hi == CH_BC_REFLECTIVE) { flip = !flip; return 2 * n - 1 - c; }
+    return n - 1;
+  }
+  return c;
+}
+
+__global__ void __launch_bounds__(256) k_ghost(const StepArgs A, const BcArgs B) {
+  const Geom& g = A.geo;
+  // shell = z slabs (all padded x,y) + y slabs (real z, padded x) + x slabs (real z, real y)
+  const long long nzs = (long long)2 * g.g[2] * g.pd[1] * g.pd[0];
+  const long long nys = (long long)g.n[2] * 2 * g.g[1] * g.pd[0];
+  const long long nxs = (long long)g.n[2] * g.n[1] * 2 * g.g[0];
+  long long id = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (id >= nzs + nys + nxs) return;
+  int pi, pj, pk;   // padded coordinates
+  if (id < nzs) {
+    pi = (int)(id % g.pd[0]); long long r = id / g.pd[0];
+    pj = (int)(r % g.pd[1]); int s = (int)(r / g.pd[1]);
+    pk = s < g.g[2] ? s : s + g.n[2];
+  } else if (id < nzs + nys) {
+    id -= nzs;
+    pi = (int)(id % g.pd[0]); long long r = id / g.pd[0];
+    int s = (int)(r % (2 * g.g[1])); pk = (int)(r / (2 * g.g[1])) + g.g[2];
+    pj = s < g.g[1] ? s : s + g.n[1];
+  } else {
+    id -= nzs + nys;
+    int s = (int)(id % (2 * g.g[0])); long long r = id / (2 * g.g[0]);
+    pj = (int)(r % g.n[1]) + g.g[1]; pk = (int)(r / g.n[1]) + g.g[2];
+    pi = s < g.g[0] ? s : s + g.n[0];
+  }
+  bool fx = false, fy = false, fz = false;
+  const int si = bc_source(pi - g.g[0], g.n[0], B.bc[0], B.bc[1], fx);
+  const int sj = bc_source(pj - g.g[1], g.n[1], B.bc[2], B.bc[3], fy);
+  const int sk = bc_source(pk - g.g[2], g.n[2], B.bc[4], B.bc[5], fz);
+  const long long qd = (long long)pi + (long long)pj * g.st[1] + (long long)pk * g.st[2];
+  const long long qs = (long long)(si + g.g[0]) + (long long)(sj + g.g[1]) * g.st[1] + (long long)(sk + g.g[2]) * g.st[2];
+  double* u = A.u;
+  u[qd] = u[qs];
+  u[g.np + qd] = fx ? -u[g.np + qs] : u[g.np + qs];
+  u[2 * g.np + qd] = fy ? -u[2 * g.np + qs] : u[2 * g.np + qs];
+  u[3 * g.np + qd] = fz ? -u[3 * g.np + qs] : u[3 * g.np + qs];
+  u[4 * g.np + qd] = u[4 * g.np + qs];
+}
+
+// FP64 peak probe: 8 independent DFMA chains per thread.
+__global__ void k_dfma_probe(double* sink, int iters) {
+  double a0 = threadIdx.x * 1e-9, a1 = a0 + 1, a2 = a0 + 2, a3 = a0 + 3, a4 = a0 + 4, a5 = a0 + 5, a6 = a0 + 6, a7 = a0 + 7;
+  const double b = 1.0000000001, c = 1e-12;
+  for (int it = 0; it < iters; ++it) {
+    a0 = fma(a0, b, c); a1 = fma(a1, b, c); a2 = fma(a2, b, c); a3 = fma(a3, b, c);
+    a4 = fma(a4, b, c); a5 = fma(a5, b, c); a6 = fma(a6, b, c); a7 = fma(a7, b, c);
+  }
+  sink[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = ((a0 + a1) + (a2 + a3)) + ((a4 + a5) + (a6 + a7));
+}
+
+thread_local std::string g_err;
+
+}  // namespace
+
+// =============================================================================================
+// Host side: opaque context and the C ABI.
+// =============================================================================================
+struct ch_ctx {
+  Geom geo;
+  Gas gas;
+  int nghost;
+  double dx[3];
+  int bc[6];
+  bool bound = false, have_state = false, dt_valid = false;
+  double* state = nullptr;
+  double* ws = nullptr;
+  unsigned long long* red = nullptr;
+  cudaStream_t stream = nullptr;
+  unsigned long long* h_red = nullptr;   // pinned, 16 bytes
+  long long launches = 0;
+  int march_seg = 64;
+};
+
+namespace {
+
+int fail(int code, const char* msg) { g_err = msg; return code; }
+int cuda_fail(cudaError_t e, const char* where) {
+  g_err = std::string(where) + ": " + cudaGetErrorString(e);
+  return CH_ECUDA;
+}
+#define CH_CUDA(call, where) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return cuda_fail(e_, where); } while (0)
+
+bool geometry(int nx, int ny, int nz, int nghost, Geom& g) {
+  if (nx < 1 || ny < 1 || nz < 1 || nghost < 3) return false;
+  const int n[3] = {nx, ny, nz};
+  for (int d = 0; d < 3; ++d) {
+    g.n[d] = n[d];
+    g.act[d] = n[d] > 1;
+    g.g[d] = g.act[d] ? nghost : 0;
+    g.pd[d] = n[d] + 2 * g.g[d];
+    if (g.act[d] && n[d] < nghost) return false;
+  }
+  g.st[0] = 1; g.st[1] = g.pd[0]; g.st[2] = (long long)g.pd[0] * g.pd[1];
+  g.np = g.st[2] * g.pd[2];
+  return true;
+}
+
+StepArgs make_args(const ch_ctx* c, double dt) {
+  StepArgs A;
+  A.geo = c->geo; A.gas = c->gas;
+  for (int d = 0; d < 3; ++d) { A.dx[d] = c->dx[d]; A.dtdx[d] = dt / c->dx[d]; }
+  A.u = c->state;
+  const long long blk = 5 * c->geo.np;
+  for (int d = 0; d < 3; ++d) {
+    A.Fs[d] = c->ws + (long long)(0 + d) * blk;
+    A.UL[d] = c->ws + (long long)(3 + d) * blk;
+    A.UR[d] = c->ws + (long long)(6 + d) * blk;
+    A.Fh[d] = c->ws + (long long)(9 + d) * blk;
+  }
+  A.red = c->red;
+  return A;
+}
+
+int launch_ghost(ch_ctx* c, const StepArgs& A) {
+  const Geom& g = c->geo;
+  const long long shell = (long long)2 * g.g[2] * g.pd[1] * g.pd[0] + (long long)g.n[2] * 2 * g.g[1] * g.pd[0] +
+                          (long long)g.n[2] * g.n[1] * 2 * g.g[0];
+  if (shell == 0) return CH_OK;
+  BcArgs B; for (int s = 0; s < 6; ++s) B.bc[s] = c->bc[s];
+  k_ghost<<<(unsigned)((shell + 255) / 256), 256, 0, c->stream>>>(A, B);
+  ++c->launches;
+  CH_CUDA(cudaGetLastError(), "k_ghost");
+  return CH_OK;
+}
+
+int copy_real(ch_ctx* c, double* user, bool to_device) {
+  const Geom& g = c->geo;
+  const size_t N = (size_t)g.n[0] * g.n[1] * g.n[2];
+  for (int f = 0; f < 5; ++f) {
+    cudaMemcpy3DParms p;
+    std::memset(&p, 0, sizeof(p));
+    cudaPitchedPtr up = make_cudaPitchedPtr(user + f * N, (size_t)g.n[0] * 8, (size_t)g.n[0] * 8, (size_t)g.n[1]);
+    cudaPitchedPtr sp = make_cudaPitchedPtr(c->state + (size_t)f * g.np, (size_t)g.pd[0] * 8, (size_t)g.pd[0] * 8, (size_t)g.pd[1]);
+    cudaPos origin = make_cudaPos(0, 0, 0);
+    cudaPos ghost = make_cudaPos((size_t)g.g[0] * 8, (size_t)g.g[1], (size_t)g.g[2]);
+    if (to_device) { p.srcPtr = up; p.srcPos = origin; p.dstPtr = sp; p.dstPos = ghost; }
+    else { p.srcPtr = sp; p.srcPos = ghost; p.dstPtr = up; p.dstPos = origin; }
+    p.extent = make_cudaExtent((size_t)g.n[0] * 8, (size_t)g.n[1], (size_t)g.n[2]);
+    p.kind = cudaMemcpyDefault;
+    CH_CUDA(cudaMemcpy3DAsync(&p, c->stream), "cudaMemcpy3DAsync");
+  }
+  return CH_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* ch_last_error(void) { return g_err.c_str(); }
+
+ch_ctx* ch_init(int nx, int ny, int nz, int nghost, double gamma, const int* bc) {
+  Geom g;
+  if (nx < 1 || ny < 1 || nz < 1) { fail(CH_EINVAL, "ch_init: n < 1"); return nullptr; }
+  if (nghost < 3) { fail(CH_EINVAL, "ch_init: nghost < 3"); return nullptr; }
+  if (!(gamma > 1.0) || !std::isfinite(gamma)) { fail(CH_EINVAL, "ch_init: gamma <= 1"); return nullptr; }
+  if (!geometry(nx, ny, nz, nghost, g)) { fail(CH_EINVAL, "ch_init: active dimension smaller than nghost"); return nullptr; }
+  ch_ctx* c = new (std::nothrow) ch_ctx();
+  if (!c) { fail(CH_EINVAL, "ch_init: out of host memory"); return nullptr; }
+  c->geo = g;
+  c->nghost = nghost;
+  for (int s = 0; s < 6; ++s) {
+    c->bc[s] = bc ? bc[s] : CH_BC_PERIODIC;
+    if (g.act[s / 2] && (c->bc[s] < 1 || c->bc[s] > 3)) { delete c; fail(CH_EINVAL, "ch_init: bad boundary code"); return nullptr; }
+  }
+  for (int d = 0; d < 3; ++d) {
+    if (g.act[d] && ((c->bc[2 * d] == CH_BC_PERIODIC) != (c->bc[2 * d + 1] == CH_BC_PERIODIC))) {
+      delete c; fail(CH_EINVAL, "ch_init: unpaired periodic faces"); return nullptr;
+    }
+    c->dx[d] = 1.0 / nx;   // reading S8
+  }
+  Gas& G = c->gas;
+  G.gamma = gamma; G.gm1 = gamma - 1.0; G.inv_gm1 = 1.0 / (gamma - 1.0); G.two_gm1 = 2.0 / (gamma - 1.0);
+  G.z = (gamma - 1.0) / (2.0 * gamma); G.gm = (gamma - 1.0) / (gamma + 1.0); G.c_sh = (gamma + 1.0) / (2.0 * gamma);
+  G.half_gp1 = 0.5 * (gamma + 1.0); G.two_gp1 = 2.0 / (gamma + 1.0); G.half_gm1 = 0.5 * (gamma - 1.0);
+  return c;
+}
+
+int ch_free(ch_ctx* c) {
+  if (!c) return CH_OK;
+  if (c->h_red) cudaFreeHost(c->h_red);
+  delete c;
+  return CH_OK;
+}
+
+int ch_set_spacing(ch_ctx* c, double dx, double dy, double dz) {
+  if (!c) return fail(CH_EINVAL, "ch_set_spacing: null context");
+  if (!(dx > 0 && dy > 0 && dz > 0) || !std::isfinite(dx) || !std::isfinite(dy) || !std::isfinite(dz))
+    return fail(CH_EINVAL, "ch_set_spacing: spacing <= 0");
+  c->dx[0] = dx; c->dx[1] = dy; c->dx[2] = dz;
+  c->dt_valid = false;
+  return CH_OK;
+}
+
+long long ch_padded_cells(const ch_ctx* c) { return c ? c->geo.np : 0; }
+
+size_t ch_workspace_bytes(int nx, int ny, int nz, int nghost) {
+  Geom g;
+  if (!geometry(nx, ny, nz, nghost, g)) return 0;
+  return (size_t)12 * 5 * (size_t)g.np * sizeof(double);
+}
+
+int ch_bind(ch_ctx* c, const ch_buffers* b, void* stream) {
+  if (!c || !b) return fail(CH_EINVAL, "ch_bind: null argument");
+  if (!b->state || !b->workspace || !b->reduce) return fail(CH_EINVAL, "ch_bind: null buffer");
+  if (b->workspace_bytes < (size_t)12 * 5 * (size_t)c->geo.np * sizeof(double))
+    return fail(CH_EINVAL, "ch_bind: workspace too small");
+  if (((uintptr_t)b->state & 7) || ((uintptr_t)b->workspace & 7) || ((uintptr_t)b->reduce & 7))
+    return fail(CH_EINVAL, "ch_bind: misaligned buffer");
+  c->state = b->state;
+  c->ws = static_cast<double*>(b->workspace);
+  c->red = static_cast<unsigned long long*>(b->reduce);
+  c->stream = static_cast<cudaStream_t>(stream);
+  if (!c->h_red) CH_CUDA(cudaHostAlloc((void**)&c->h_red, 16, cudaHostAllocDefault), "cudaHostAlloc");
+  c->bound = true; c->have_state = false; c->dt_valid = false;
+  return CH_OK;
+}
+
+int ch_set_state(ch_ctx* c, const double* u) {
+  if (!c || !u) return fail(CH_EINVAL, "ch_set_state: null argument");
+  if (!c->bound) return fail(CH_ESTATE, "ch_set_state: no buffers bound");
+  int rc = copy_real(c, const_cast<double*>(u), true);
+  if (rc) return rc;
+  StepArgs A = make_args(c, 1.0);
+  rc = launch_ghost(c, A);
+  if (rc) return rc;
+  c->have_state = true; c->dt_valid = false;
+  return CH_OK;
+}
+
+int ch_get_state(ch_ctx* c, double* u) {
+  if (!c || !u) return fail(CH_EINVAL, "ch_get_state: null argument");
+  if (!c->have_state) return fail(CH_ESTATE, "ch_get_state: no state set");
+  int rc = copy_real(c, u, false);
+  if (rc) return rc;
+  CH_CUDA(cudaStreamSynchronize(c->stream), "ch_get_state sync");
+  return CH_OK;
+}
+
+int ch_set_padded(ch_ctx* c, const double* up) {
+  if (!c || !up) return fail(CH_EINVAL, "ch_set_padded: null argument");
+  if (!c->bound) return fail(CH_ESTATE, "ch_set_padded: no buffers bound");
+  CH_CUDA(cudaMemcpyAsync(c->state, up, (size_t)5 * c->geo.np * 8, cudaMemcpyDefault, c->stream), "ch_set_padded");
+  c->have_state = true; c->dt_valid = false;
+  return CH_OK;
+}
+
+int ch_get_padded(ch_ctx* c, double* up) {
+  if (!c || !up) return fail(CH_EINVAL, "ch_get_padded: null argument");
+  if (!c->have_state) return fail(CH_ESTATE, "ch_get_padded: no state set");
+  CH_CUDA(cudaMemcpyAsync(up, c->state, (size_t)5 * c->geo.np * 8, cudaMemcpyDefault, c->stream), "ch_get_padded");
+  CH_CUDA(cudaStreamSynchronize(c->stream), "ch_get_padded sync");
+  return CH_OK;
+}
+
+double ch_compute_dt(ch_ctx* c, double cfl) {
+  const double nan = std::numeric_limits<double>::quiet_NaN();
+  if (!c) { fail(CH_EINVAL, "ch_compute_dt: null context"); return nan; }
+  if (!c->have_state) { fail(CH_ESTATE, "ch_compute_dt: no state set"); return nan; }
+  if (!(cfl > 0.0) || !(cfl <= 1.0)) { fail(CH_EINVAL, "ch_compute_dt: cfl not in (0,1]"); return nan; }
+  if (!c->dt_valid) {
+    StepArgs A = make_args(c, 1.0);
+    k_reset<<<1, 32, 0, c->stream>>>(c->red);
+    const long long N = (long long)c->geo.n[0] * c->geo.n[1] * c->geo.n[2];
+    long long blocks = (N + 255) / 256;
+    if (blocks > 148 * 8) blocks = 148 * 8;
+    k_dt<<<(unsigned)blocks, 256, 0, c->stream>>>(A);
+    c->launches += 2;
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) { cuda_fail(e, "k_dt"); return nan; }
+    c->dt_valid = true;
+  }
+  cudaError_t e = cudaMemcpyAsync(c->h_red, c->red, 16, cudaMemcpyDeviceToHost, c->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+  if (e != cudaSuccess) { cuda_fail(e, "ch_compute_dt read-back"); return nan; }
+  if (c->h_red[1] != 0ULL) { fail(CH_ENONPHYS, "ch_compute_dt: non-physical cell (rho <= 0 or non-finite)"); return nan; }
+  double m;
+  std::memcpy(&m, &c->h_red[0], 8);
+  return cfl * m;
+}
+
+int ch_step(ch_ctx* c, double dt) {
+  if (!c) return fail(CH_EINVAL, "ch_step: null context");
+  if (!c->have_state) return fail(CH_ESTATE, "ch_step: no state set");
+  if (!(dt > 0.0) || !std::isfinite(dt)) return fail(CH_EINVAL, "ch_step: dt <= 0 or non-finite");
+  const Geom& g = c->geo;
+  StepArgs A = make_args(c, dt);
+  cudaStream_t st = c->stream;
+  k_reset<<<1, 32, 0, st>>>(c->red);
+  ++c->launches;
+  // pass 1
+  if (g.act[0]) {
+    // flat run of padded cells from the first needed row to the last: rows j,k in [-1, n]
+    const int j0 = g.act[1] ? g.g[1] - 1 : 0, k0 = g.act[2] ? g.g[2] - 1 : 0;
+    const int j1 = g.act[1] ? g.g[1] + g.n[1] : 0, k1 = g.act[2] ? g.g[2] + g.n[2] : 0;
+    const long long qb = (long long)j0 * g.st[1] + (long long)k0 * g.st[2];
+    const long long qe = (long long)j1 * g.st[1] + (long long)k1 * g.st[2] + g.pd[0];
+    const long long nb = (qe - qb + kXOut - 1) / kXOut;
+    k_pass1_x<<<(unsigned)nb, kXT, 0, st>>>(A, qb, qe);
+    ++c->launches;
+  }
+  for (int d = 1; d < 3; ++d) {
+    if (!g.act[d]) continue;
+    const int T = 3 - d;
+    const long long cols = (long long)(g.act[0] ? g.n[0] + 2 : 1) * (g.act[T] ? g.n[T] + 2 : 1);
+    const int seg = c->march_seg;
+    dim3 grid((unsigned)((cols + 127) / 128), (unsigned)((g.n[d] + 1 + seg - 1) / seg));
+    if (d == 1) k_pass1_march<1><<<grid, 128, 0, st>>>(A, seg);
+    else k_pass1_march<2><<<grid, 128, 0, st>>>(A, seg);
+    ++c->launches;
+  }
+  CH_CUDA(cudaGetLastError(), "pass 1");
+  {
+    const long long cells = (long long)(g.act[0] ? g.n[0] + 1 : 1) * (g.act[1] ? g.n[1] + 1 : 1) * (g.act[2] ? g.n[2] + 1 : 1);
+    k_pass2<<<(unsigned)((cells + 127) / 128), 128, 0, st>>>(A);
+    ++c->launches;
+  }
+  {
+    const long long N = (long long)g.n[0] * g.n[1] * g.n[2];
+    k_update<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(A);
+    ++c->launches;
+  }
+  CH_CUDA(cudaGetLastError(), "pass 2 / update");
+  int rc = launch_ghost(c, A);
+  if (rc) return rc;
+  c->dt_valid = true;
+  return CH_OK;
+}
+
+int ch_sync(ch_ctx* c) {
+  if (!c) return fail(CH_EINVAL, "ch_sync: null context");
+  CH_CUDA(cudaStreamSynchronize(c->stream), "ch_sync");
+  return CH_OK;
+}
+
+long long ch_kernel_launches(const ch_ctx* c) { return c ? c->launches : 0; }
+
+double ch_fp64_peak_probe(double* sink, int blocks, int threads, int iters, void* stream) {
+  if (!sink || blocks < 1 || threads < 1 || threads > 1024 || iters < 1) { fail(CH_EINVAL, "ch_fp64_peak_probe: bad argument"); return -1.0; }
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  cudaEvent_t e0, e1;
+  if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) { fail(CH_ECUDA, "event create"); return -1.0; }
+  k_dfma_probe<<<blocks, threads, 0, st>>>(sink, iters);   // warm-up
+  cudaEventRecord(e0, st);
+  k_dfma_probe<<<blocks, threads, 0, st>>>(sink, iters);
+  cudaEventRecord(e1, st);
+  cudaError_t e = cudaEventSynchronize(e1);
+  float ms = -1.f;
+  if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
+  cudaEventDestroy(e0); cudaEventDestroy(e1);
+  if (e != cudaSuccess) { cuda_fail(e, "ch_fp64_peak_probe"); return -1.0; }
+  return (double)ms;
+}
+
+}  // extern "C"
