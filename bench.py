@@ -1,0 +1,307 @@
+#!/usr/bin/env python
+"""bench.py — cell-updates/s of the full CTU + PPMC + exact-Riemann step (fp64) on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--size 512] [--impl reference]
+
+A "step" is one pass of the whole hot path over the grid: `dt = ch_compute_dt(cfl)` (Eq. 22) then
+`ch_step(dt)` (PPMC + exact Riemann in x, y, z; transverse correction; second Riemann pass; update;
+ghost fill).  Workload: BASELINE.json's throughput-sweep configuration (periodic box, gamma = 5/3,
+seeded sum of 8 random-phase sinusoids) at `--size`^3 (default 512, the largest size the metric is
+quoted on; 256^3 is reported beside it under "other_sizes").  The state (5.6 GB at 512^3) is far
+larger than the 126 MB L2, so no L2 flush is needed between steps.
+
+N > 1 (torchrun): the path does not shard in this build ("replicas only"): every rank
+steps its own replica with no data-path collective; value = all ranks' cell-updates / max-over-ranks
+time.
+
+`--impl reference`: the oracle (oracle/, plain C++ on the host cores) on a bounded sample of the
+same workload; rank 0 only.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "cell-updates/sec (fp64 CTU+PPM+exact Riemann)"
+UNIT = "cell-updates/s"
+CPU_SAMPLE_N = 128          # the oracle is timed on a 128^3 corner of the workload
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--size", type=int, default=512)
+    ap.add_argument("--other-sizes", type=str, default="256")
+    ap.add_argument("--impl", type=str, default="b200", choices=["b200", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    return ap.parse_args()
+
+
+# ---- clocks ---------------------------------------------------------------------------------------
+class ClockSampler:
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.p = None
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), "--query-gpu=" + self.Q,
+                                       "--format=csv,noheader,nounits", "-lms", "100"],
+                                      stdout=self.f, stderr=subprocess.DEVNULL)
+        except OSError:
+            pass
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.p is None:
+            return out
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.p.kill()
+        self.f.flush()
+        self.f.seek(0)
+        sm, mx, power, reasons = [], [], [], set()
+        for line in self.f:
+            c = [x.strip() for x in line.split(",")]
+            if len(c) < 9:
+                continue
+            try:
+                sm.append(float(c[1])); mx.append(float(c[2])); power.append(float(c[3]))
+            except ValueError:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), c[5:9]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        self.f.close()
+        os.unlink(self.f.name)
+        if sm:
+            out.update(sm_mhz=statistics.median(sm), sm_max_mhz=max(mx), reasons=sorted(reasons), samples=len(sm),
+                       power_w_max=max(power))
+        return out
+
+
+# ---- the oracle arm ---------------------------------------------------------------------------------
+def corner_sample(w, m):
+    """A bounded sample of the workload: the m^3 corner of its initial state, outflow faces, the
+    workload's own cell width."""
+    import numpy as np
+    return np.ascontiguousarray(w.u[:, :m, :m, :m])
+
+
+def time_oracle(w, steps, warmup, m=CPU_SAMPLE_N):
+    from oracle import ref
+    from paper_1410_4194_b200 import workloads as wl
+    nx = w.shape[0]
+    m = min(m, nx)
+    u = corner_sample(w, m)
+    G = ref.RefGrid(m, m, m, 3, w.gamma, (wl.OUTFLOW,) * 6)
+    G.set_spacing(1.0 / nx, 1.0 / nx, 1.0 / nx)
+    G.set_state(u)
+    for _ in range(warmup):
+        G.step(G.compute_dt(w.cfl))
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        G.step(G.compute_dt(w.cfl))
+    el = time.perf_counter() - t0
+    cores = len(os.sched_getaffinity(0)) if hasattr(os, "sched_getaffinity") else os.cpu_count()
+    omp = os.environ.get("OMP_NUM_THREADS")
+    if omp:
+        cores = min(cores, int(omp))
+    return dict(value=m ** 3 * steps / el, unit=UNIT, cores=cores, kind="oracle",
+                sample=f"{m}^3 corner of the {nx}^3 sweep initial state (outflow faces, dx=1/{nx}), "
+                       f"{steps} steps of compute_dt+step after {warmup} warm-up, OpenMP over the outer loops",
+                ms_per_step=el / steps * 1e3)
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from paper_1410_4194_b200 import workloads as wl
+    w = wl.sweep(args.size)
+    r = time_oracle(w, args.steps, args.warmup)
+    line = {"impl": "reference", "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": r["ms_per_step"], "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"throughput sweep (BASELINE.json config 5), {CPU_SAMPLE_N}^3 corner sample per step",
+                       "gamma": w.gamma, "cfl": w.cfl, "bc": "outflow (sample faces)"},
+            "cpu_baseline": {k: r[k] for k in ("value", "unit", "cores", "kind", "sample")},
+            "e2e": {"value": r["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+# ---- the CUDA arm -----------------------------------------------------------------------------------
+def timed_steps(G, cfl, steps, stream_events):
+    """K steps of compute_dt + step, timed with CUDA events on the library's stream."""
+    import torch
+    e0, e1 = stream_events
+    torch.cuda.synchronize()
+    e0.record(G.cuda_stream)
+    for _ in range(steps):
+        G.step(G.compute_dt(cfl))
+    e1.record(G.cuda_stream)
+    torch.cuda.synchronize()
+    return e0.elapsed_time(e1) * 1e-3
+
+
+def bench_size(pkg, wl, n, steps, warmup, device, dist=None, profile=True, e2e=True):
+    import numpy as np
+    import torch
+    w = wl.sweep(n)
+    N = n ** 3
+    G = pkg.Grid(n, n, n, 3, w.gamma, w.bc, device=device)
+    u_dev = torch.from_numpy(w.u).to(device)
+    G.set_state(u_dev)
+    ev = (torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+    for _ in range(max(warmup, 3)):
+        G.step(G.compute_dt(w.cfl))
+    n0 = G.kernel_launches
+    if dist is not None:
+        dist.barrier()
+    el = timed_steps(G, w.cfl, steps, ev)
+    launches = G.kernel_launches - n0
+    if dist is not None:
+        t = torch.tensor([el], dtype=torch.float64, device=device)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dist.barrier()
+        el = float(t.item())
+    out = dict(n=n, seconds=el, launches=launches, cells=N, gamma=w.gamma, cfl=w.cfl)
+    if profile:
+        # same K steps again with an event pair around every kernel (ch_profile): per-kernel durations
+        G.profile(True)
+        for _ in range(steps):
+            G.step(G.compute_dt(w.cfl))
+        prof = G.profile_read()
+        G.profile(False)
+        out["kernels"] = {k: {"ms_avg": ms / c, "launches_per_step": c / steps}
+                          for k, (ms, c) in prof.items() if c}
+        out["kernel_ms_per_step"] = sum(ms for ms, c in prof.values()) / steps
+    if e2e:
+        # the user's call sequence with HOST buffers: H2D of the state, dt, step, D2H of the result
+        k_e2e = max(1, min(steps, 5))
+        h_in = torch.from_numpy(w.u).pin_memory()
+        h_out = torch.empty_like(h_in).pin_memory()
+        G.set_state(h_in); G.step(G.compute_dt(w.cfl)); G.get_state(h_out)       # warm-up
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+        t0 = time.perf_counter()
+        for _ in range(k_e2e):
+            G.set_state(h_in)
+            G.step(G.compute_dt(w.cfl))
+            G.get_state(h_out)                                                  # synchronises
+        t_e2e = time.perf_counter() - t0
+        if dist is not None:
+            t = torch.tensor([t_e2e], dtype=torch.float64, device=device)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            t_e2e = float(t.item())
+        out["e2e"] = dict(seconds=t_e2e, steps=k_e2e, h2d=h_in.numel() * 8, d2h=h_out.numel() * 8)
+        assert bool(torch.isfinite(h_out).all())
+        del h_in, h_out
+    G.close()
+    del G, u_dev
+    torch.cuda.empty_cache()
+    return out, w
+
+
+def main():
+    args = parse()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    import paper_1410_4194_b200 as pkg
+    from paper_1410_4194_b200 import roofline as rf
+    from paper_1410_4194_b200 import workloads as wl
+    from paper_1410_4194_b200.binding import fp64_peak_probe
+
+    pkg.load_library()                      # no CPU fallback: raises if the CUDA library is missing
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
+    torch.cuda.set_device(local)
+    device = f"cuda:{local}"
+
+    sampler = ClockSampler(local) if rank == 0 else None
+    peak_tf, _ = fp64_peak_probe(device=device)                 # measured DFMA rate, burst
+    main_res, w = bench_size(pkg, wl, args.size, args.steps, args.warmup, device, dist,
+                             profile=True, e2e=not args.no_e2e)
+    clocks = sampler.stop() if sampler else None
+    others = {}
+    if world == 1:
+        for s in [int(x) for x in args.other_sizes.split(",") if x]:
+            if s != args.size:
+                r, _ = bench_size(pkg, wl, s, args.steps, args.warmup, device, None, profile=False, e2e=False)
+                others[str(s)] = {"value": r["cells"] * args.steps / r["seconds"], "unit": UNIT,
+                                  "ms_per_step": r["seconds"] / args.steps * 1e3}
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    N, K = main_res["cells"], args.steps
+    value = world * N * K / main_res["seconds"]
+    # dominant kernel and its ALU roofline
+    kern = main_res["kernels"]
+    top = max((k for k in kern if k in rf.ALG_FLOPS), key=lambda k: kern[k]["ms_avg"] * kern[k]["launches_per_step"])
+    t_top = kern[top]["ms_avg"] * 1e-3
+    achieved = rf.ALG_FLOPS[top] * N / t_top / 1e12
+    sm_mhz = (clocks or {}).get("sm_mhz") or 1965.0
+    roofline = {"bound": "alu", "kernel": top, "achieved": achieved, "peak": peak_tf, "unit": "TFLOP/s",
+                "frac": achieved / peak_tf, "traffic": None,
+                "peak_source": "measured: ch_fp64_peak_probe DFMA chains in this run (burst); nominal "
+                               f"148 SM x 64 lanes x 2 x {sm_mhz:.0f} MHz = {rf.nominal_fp64_tflops(sm_mhz):.1f}",
+                "alg_flops_per_cell": rf.ALG_FLOPS[top],
+                "kernel_ms": kern[top]["ms_avg"],
+                "kernel_share_of_step": kern[top]["ms_avg"] * kern[top]["launches_per_step"] / main_res["kernel_ms_per_step"],
+                "step": {"alg_flops_per_cell": sum(rf.ALG_FLOPS.values()),
+                         "achieved": sum(rf.ALG_FLOPS.values()) * N * K / main_res["seconds"] / 1e12,
+                         "frac": sum(rf.ALG_FLOPS.values()) * N * K / main_res["seconds"] / 1e12 / peak_tf},
+                "kernels": kern}
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": args.warmup,
+            "ms_per_step": main_res["seconds"] / K * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"throughput sweep (BASELINE.json config 5) {args.size}^3 periodic, "
+                                   "sum of 8 seeded sinusoids, 1 replica per GPU",
+                       "gamma": w.gamma, "cfl": w.cfl, "nghost": 3, "l2": "state (5 fields) larger than L2, no flush",
+                       "parallelism": "replicas only" if world > 1 else "single GPU"},
+            "gpu_launches": main_res["launches"], "clocks": clocks, "roofline": roofline}
+    if others:
+        line["other_sizes"] = others
+    if "e2e" in main_res:
+        e = main_res["e2e"]
+        line["e2e"] = {"value": world * N * e["steps"] / e["seconds"], "unit": UNIT,
+                       "h2d_bytes_per_step": e["h2d"], "d2h_bytes_per_step": e["d2h"], "steps": e["steps"],
+                       "how": "ch_set_state(pinned host) + ch_compute_dt + ch_step + ch_get_state(pinned host) per step"}
+    if world == 1 and not args.no_cpu_baseline:
+        r = time_oracle(w, steps=3, warmup=1)
+        line["cpu_baseline"] = {k: r[k] for k in ("value", "unit", "cores", "kind", "sample")}
+    print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -127,6 +127,25 @@ int ch_sync(ch_ctx* ctx);
  * gpu_launches claim). */
 long long ch_kernel_launches(const ch_ctx* ctx);
 
+/* Kernel kinds of one step, for ch_profile_read / ch_kernel_name. */
+enum {
+  CH_K_RESET = 0, CH_K_PASS1_X, CH_K_PASS1_Y, CH_K_PASS1_Z, CH_K_PASS2, CH_K_UPDATE, CH_K_GHOST, CH_K_DT,
+  CH_K_COUNT
+};
+
+/* ch_profile — measurement helper (P:L427 keeps wall-clock timers per phase; this is the per-kernel
+ * equivalent).  enable != 0: every later ch_step / ch_compute_dt brackets each of its kernel launches
+ * with CUDA events on the bound stream, blocks until the step has finished and adds the elapsed
+ * times to per-kind totals; enable == 0: back to asynchronous steps.  Either call zeroes the totals. */
+int ch_profile(ch_ctx* ctx, int enable);
+
+/* ch_profile_read — copy the totals out: ms[CH_K_COUNT] (milliseconds) and calls[CH_K_COUNT]
+ * (launches timed), HOST pointers. */
+int ch_profile_read(const ch_ctx* ctx, double* ms, long long* calls);
+
+/* ch_kernel_name — static name of kernel kind `kind` ("" if out of range). */
+const char* ch_kernel_name(int kind);
+
 /* ch_fp64_peak_probe — measurement helper for the roofline denominator: runs `iters` dependent
  * DFMA chains (8 independent chains per thread) on `blocks` x `threads` threads on `stream` and
  * returns the elapsed milliseconds measured with CUDA events (negative on error).  `sink` is a

@@ -25,7 +25,9 @@ CH_OK, CH_EINVAL, CH_ESTATE, CH_ECUDA, CH_ENONPHYS = 0, -1, -2, -3, -4
 # every symbol include/ch.h declares
 SYMBOLS = ("ch_init", "ch_free", "ch_last_error", "ch_set_spacing", "ch_padded_cells", "ch_workspace_bytes",
            "ch_bind", "ch_set_state", "ch_get_state", "ch_set_padded", "ch_get_padded", "ch_compute_dt",
-           "ch_step", "ch_sync", "ch_kernel_launches", "ch_fp64_peak_probe")
+           "ch_step", "ch_sync", "ch_kernel_launches", "ch_profile", "ch_profile_read", "ch_kernel_name",
+           "ch_fp64_peak_probe")
+K_COUNT = 8
 
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-shared"]
@@ -80,6 +82,10 @@ def load_library() -> C.CDLL:
     L.ch_sync.argtypes = [vp]
     L.ch_kernel_launches.restype = C.c_longlong
     L.ch_kernel_launches.argtypes = [vp]
+    L.ch_profile.argtypes = [vp, C.c_int]
+    L.ch_profile_read.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
+    L.ch_kernel_name.restype = C.c_char_p
+    L.ch_kernel_name.argtypes = [C.c_int]
     L.ch_fp64_peak_probe.restype = C.c_double
     L.ch_fp64_peak_probe.argtypes = [vp, C.c_int, C.c_int, C.c_int, vp]
     _lib = L
@@ -194,6 +200,16 @@ class Grid:
 
     def sync(self):
         self._check(self._L.ch_sync(self._h), "ch_sync")
+
+    def profile(self, enable=True):
+        self._check(self._L.ch_profile(self._h, 1 if enable else 0), "ch_profile")
+
+    def profile_read(self) -> dict:
+        """{kernel name: (total ms, launches timed)} since the last profile() call."""
+        ms = (C.c_double * K_COUNT)()
+        calls = (C.c_longlong * K_COUNT)()
+        self._check(self._L.ch_profile_read(self._h, ms, calls), "ch_profile_read")
+        return {self._L.ch_kernel_name(k).decode(): (ms[k], calls[k]) for k in range(K_COUNT)}
 
     @property
     def kernel_launches(self) -> int:

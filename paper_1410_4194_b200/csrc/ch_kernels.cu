@@ -469,6 +469,12 @@ struct ch_ctx {
   unsigned long long* h_red = nullptr;   // pinned, 16 bytes
   long long launches = 0;
   int march_seg = 64;
+  // optional per-kernel timing (ch_profile): one event pair per kernel kind
+  bool profiling = false;
+  cudaEvent_t ev[2 * CH_K_COUNT] = {};
+  bool ev_used[CH_K_COUNT] = {};
+  double prof_ms[CH_K_COUNT] = {};
+  long long prof_calls[CH_K_COUNT] = {};
 };
 
 namespace {
@@ -511,14 +517,40 @@ StepArgs make_args(const ch_ctx* c, double dt) {
   return A;
 }
 
+const char* const kKernelNames[CH_K_COUNT] = {"k_reset", "k_pass1_x", "k_pass1_march<y>", "k_pass1_march<z>",
+                                              "k_pass2", "k_update", "k_ghost", "k_dt"};
+
+// event brackets around one launch when profiling is on (no-ops otherwise)
+struct Bracket {
+  ch_ctx* c; int kind;
+  Bracket(ch_ctx* c_, int kind_) : c(c_), kind(kind_) {
+    if (c->profiling) { cudaEventRecord(c->ev[2 * kind], c->stream); }
+  }
+  ~Bracket() {
+    ++c->launches;
+    if (c->profiling) { cudaEventRecord(c->ev[2 * kind + 1], c->stream); c->ev_used[kind] = true; }
+  }
+};
+
+int profile_collect(ch_ctx* c) {
+  if (!c->profiling) return CH_OK;
+  CH_CUDA(cudaStreamSynchronize(c->stream), "profile sync");
+  for (int k = 0; k < CH_K_COUNT; ++k) {
+    if (!c->ev_used[k]) continue;
+    float ms = 0.f;
+    CH_CUDA(cudaEventElapsedTime(&ms, c->ev[2 * k], c->ev[2 * k + 1]), "cudaEventElapsedTime");
+    c->prof_ms[k] += ms; ++c->prof_calls[k]; c->ev_used[k] = false;
+  }
+  return CH_OK;
+}
+
 int launch_ghost(ch_ctx* c, const StepArgs& A) {
   const Geom& g = c->geo;
   const long long shell = (long long)2 * g.g[2] * g.pd[1] * g.pd[0] + (long long)g.n[2] * 2 * g.g[1] * g.pd[0] +
                           (long long)g.n[2] * g.n[1] * 2 * g.g[0];
   if (shell == 0) return CH_OK;
   BcArgs B; for (int s = 0; s < 6; ++s) B.bc[s] = c->bc[s];
-  k_ghost<<<(unsigned)((shell + 255) / 256), 256, 0, c->stream>>>(A, B);
-  ++c->launches;
+  { Bracket b(c, CH_K_GHOST); k_ghost<<<(unsigned)((shell + 255) / 256), 256, 0, c->stream>>>(A, B); }
   CH_CUDA(cudaGetLastError(), "k_ghost");
   return CH_OK;
 }
@@ -578,6 +610,7 @@ ch_ctx* ch_init(int nx, int ny, int nz, int nghost, double gamma, const int* bc)
 int ch_free(ch_ctx* c) {
   if (!c) return CH_OK;
   if (c->h_red) cudaFreeHost(c->h_red);
+  for (int k = 0; k < 2 * CH_K_COUNT; ++k) if (c->ev[k]) cudaEventDestroy(c->ev[k]);
   delete c;
   return CH_OK;
 }
@@ -659,14 +692,14 @@ double ch_compute_dt(ch_ctx* c, double cfl) {
   if (!(cfl > 0.0) || !(cfl <= 1.0)) { fail(CH_EINVAL, "ch_compute_dt: cfl not in (0,1]"); return nan; }
   if (!c->dt_valid) {
     StepArgs A = make_args(c, 1.0);
-    k_reset<<<1, 32, 0, c->stream>>>(c->red);
+    { Bracket b(c, CH_K_RESET); k_reset<<<1, 32, 0, c->stream>>>(c->red); }
     const long long N = (long long)c->geo.n[0] * c->geo.n[1] * c->geo.n[2];
     long long blocks = (N + 255) / 256;
     if (blocks > 148 * 8) blocks = 148 * 8;
-    k_dt<<<(unsigned)blocks, 256, 0, c->stream>>>(A);
-    c->launches += 2;
+    { Bracket b(c, CH_K_DT); k_dt<<<(unsigned)blocks, 256, 0, c->stream>>>(A); }
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) { cuda_fail(e, "k_dt"); return nan; }
+    if (profile_collect(c) != CH_OK) return nan;
     c->dt_valid = true;
   }
   cudaError_t e = cudaMemcpyAsync(c->h_red, c->red, 16, cudaMemcpyDeviceToHost, c->stream);
@@ -685,8 +718,7 @@ int ch_step(ch_ctx* c, double dt) {
   const Geom& g = c->geo;
   StepArgs A = make_args(c, dt);
   cudaStream_t st = c->stream;
-  k_reset<<<1, 32, 0, st>>>(c->red);
-  ++c->launches;
+  { Bracket b(c, CH_K_RESET); k_reset<<<1, 32, 0, st>>>(c->red); }
   // pass 1
   if (g.act[0]) {
     // flat run of padded cells from the first needed row to the last: rows j,k in [-1, n]
@@ -695,8 +727,8 @@ int ch_step(ch_ctx* c, double dt) {
     const long long qb = (long long)j0 * g.st[1] + (long long)k0 * g.st[2];
     const long long qe = (long long)j1 * g.st[1] + (long long)k1 * g.st[2] + g.pd[0];
     const long long nb = (qe - qb + kXOut - 1) / kXOut;
+    Bracket b(c, CH_K_PASS1_X);
     k_pass1_x<<<(unsigned)nb, kXT, 0, st>>>(A, qb, qe);
-    ++c->launches;
   }
   for (int d = 1; d < 3; ++d) {
     if (!g.act[d]) continue;
@@ -704,26 +736,26 @@ int ch_step(ch_ctx* c, double dt) {
     const long long cols = (long long)(g.act[0] ? g.n[0] + 2 : 1) * (g.act[T] ? g.n[T] + 2 : 1);
     const int seg = c->march_seg;
     dim3 grid((unsigned)((cols + 127) / 128), (unsigned)((g.n[d] + 1 + seg - 1) / seg));
+    Bracket b(c, d == 1 ? CH_K_PASS1_Y : CH_K_PASS1_Z);
     if (d == 1) k_pass1_march<1><<<grid, 128, 0, st>>>(A, seg);
     else k_pass1_march<2><<<grid, 128, 0, st>>>(A, seg);
-    ++c->launches;
   }
   CH_CUDA(cudaGetLastError(), "pass 1");
   {
     const long long cells = (long long)(g.act[0] ? g.n[0] + 1 : 1) * (g.act[1] ? g.n[1] + 1 : 1) * (g.act[2] ? g.n[2] + 1 : 1);
+    Bracket b(c, CH_K_PASS2);
     k_pass2<<<(unsigned)((cells + 127) / 128), 128, 0, st>>>(A);
-    ++c->launches;
   }
   {
     const long long N = (long long)g.n[0] * g.n[1] * g.n[2];
+    Bracket b(c, CH_K_UPDATE);
     k_update<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(A);
-    ++c->launches;
   }
   CH_CUDA(cudaGetLastError(), "pass 2 / update");
   int rc = launch_ghost(c, A);
   if (rc) return rc;
   c->dt_valid = true;
-  return CH_OK;
+  return profile_collect(c);
 }
 
 int ch_sync(ch_ctx* c) {
@@ -733,6 +765,24 @@ int ch_sync(ch_ctx* c) {
 }
 
 long long ch_kernel_launches(const ch_ctx* c) { return c ? c->launches : 0; }
+
+int ch_profile(ch_ctx* c, int enable) {
+  if (!c) return fail(CH_EINVAL, "ch_profile: null context");
+  if (enable && !c->ev[0]) {
+    for (int k = 0; k < 2 * CH_K_COUNT; ++k) CH_CUDA(cudaEventCreate(&c->ev[k]), "cudaEventCreate");
+  }
+  c->profiling = enable != 0;
+  for (int k = 0; k < CH_K_COUNT; ++k) { c->prof_ms[k] = 0.0; c->prof_calls[k] = 0; c->ev_used[k] = false; }
+  return CH_OK;
+}
+
+int ch_profile_read(const ch_ctx* c, double* ms, long long* calls) {
+  if (!c || !ms || !calls) return fail(CH_EINVAL, "ch_profile_read: null argument");
+  for (int k = 0; k < CH_K_COUNT; ++k) { ms[k] = c->prof_ms[k]; calls[k] = c->prof_calls[k]; }
+  return CH_OK;
+}
+
+const char* ch_kernel_name(int kind) { return (kind >= 0 && kind < CH_K_COUNT) ? kKernelNames[kind] : ""; }
 
 double ch_fp64_peak_probe(double* sink, int blocks, int threads, int iters, void* stream) {
   if (!sink || blocks < 1 || threads < 1 || threads > 1024 || iters < 1) { fail(CH_EINVAL, "ch_fp64_peak_probe: bad argument"); return -1.0; }

@@ -164,14 +164,18 @@ def _sinusoid_sum(nx, ny, nz, seed):
                      if 1 <= a * a + b * b + c * c <= 64])
     ks = cand[rng.integers(0, len(cand), size=8)]
     ph = rng.uniform(0.0, 2.0 * np.pi, size=8)
-    # unit box in every direction for this workload: coordinates (i+1/2)/n_d so the field is periodic
+    # unit box in every direction for this workload: coordinates (i+1/2)/n_d so the field is periodic.
+    # sin(tx + ty + tz + ph) = sin(tx+ty+ph) cos(tz) + cos(tx+ty+ph) sin(tz): the sum over the 8 modes
+    # is one [nz,16] x [16,ny*nx] product (keeps 512^3 generation to seconds).
     x = ((np.arange(nx) + 0.5) / nx).reshape(1, 1, nx)
     y = ((np.arange(ny) + 0.5) / ny).reshape(1, ny, 1)
-    z = ((np.arange(nz) + 0.5) / nz).reshape(nz, 1, 1)
-    S = np.zeros((nz, ny, nx))
-    for (ka, kb, kc), p in zip(ks, ph):
-        S += np.sin(2.0 * np.pi * (ka * x + kb * y + kc * z) + p)
-    return S / 8.0
+    z = ((np.arange(nz) + 0.5) / nz).reshape(nz, 1)
+    kx, ky, kz = (ks[:, d].astype(np.float64).reshape(8, 1, 1) for d in range(3))
+    txy = 2.0 * np.pi * (kx * x + ky * y) + ph.reshape(8, 1, 1)           # [8,ny,nx]
+    tz = 2.0 * np.pi * z * kz.reshape(1, 8)                                  # [nz,8]
+    A = np.concatenate([np.cos(tz), np.sin(tz)], axis=1)                    # [nz,16]
+    B = np.concatenate([np.sin(txy), np.cos(txy)], axis=0).reshape(16, ny * nx)
+    return (A @ B).reshape(nz, ny, nx) / 8.0
 
 
 def sweep(n=256, steps=100, shape=None) -> Workload:
@@ -209,3 +213,37 @@ def riemann_tube(nx, left, right, gamma=1.4, t_end=0.2, x0=0.5) -> Workload:
     vx = np.where(L, left[1], right[1])
     p = np.where(L, left[2], right[2])
     return Workload("riemann_tube", conserved(rho, vx, 0.0, 0.0, p, gamma), gamma, (OUTFLOW,) * 6, 0.4, t_end=t_end)
+
+
+def smooth_random(nx, ny=1, nz=1, seed=0, gamma=5.0 / 3.0, amp=0.2, bc=(PERIODIC,) * 6, steps=1, cfl=0.4) -> Workload:
+    """Seeded smooth state of O(1) density/pressure with `amp`-sized variations in every primitive
+    field (three random low-|k| sinusoids each): the generic parity-test input, any grid shape."""
+    rng = np.random.default_rng(seed)
+    x = ((np.arange(nx) + 0.5) / nx).reshape(1, 1, nx)
+    y = ((np.arange(ny) + 0.5) / ny).reshape(1, ny, 1)
+    z = ((np.arange(nz) + 0.5) / nz).reshape(nz, 1, 1)
+
+    def f():
+        out = np.zeros((nz, ny, nx))
+        for _ in range(3):
+            k = rng.integers(-2, 3, 3)
+            ph = rng.uniform(0.0, 2.0 * np.pi)
+            out += np.sin(2.0 * np.pi * (k[0] * x + k[1] * y + k[2] * z) + ph)
+        return out / 3.0
+
+    u = conserved(1.0 + amp * f(), amp * f(), amp * f(), amp * f(), 1.0 + amp * f(), gamma)
+    return Workload("smooth_random", u, gamma, tuple(bc), cfl, steps=steps)
+
+
+def rough_random(nx, ny=1, nz=1, seed=0, gamma=1.4, mach=2.0, bc=(OUTFLOW,) * 6, steps=1, cfl=0.3) -> Workload:
+    """Seeded cell-wise random state (log-uniform density and pressure over two decades, velocities up
+    to `mach` sound speeds): every interface is a strong Riemann problem, so every sampling branch,
+    limiter branch and many Newton iteration counts are exercised in one step."""
+    rng = np.random.default_rng(seed)
+    shp = (nz, ny, nx)
+    rho = 10.0 ** rng.uniform(-1.0, 1.0, shp)
+    p = 10.0 ** rng.uniform(-1.0, 1.0, shp)
+    a = np.sqrt(gamma * p / rho)
+    v = [mach * a * rng.uniform(-1.0, 1.0, shp) for _ in range(3)]
+    u = conserved(rho, v[0], v[1], v[2], p, gamma)
+    return Workload("rough_random", u, gamma, tuple(bc), cfl, steps=steps)

@@ -1,0 +1,116 @@
+"""Parity at BASELINE.json's full sizes, in the launch configuration bench.py times (`-m gpu`).
+
+The oracle cannot step 256^3 / 512^3 in seconds, so full-size parity is taken on SAMPLED outputs
+the oracle can compute one by one: after one GPU step of the whole grid, sub-boxes of m^3 real cells
+(with their 3-deep halo cut from the GPU's pre-step padded store, whose ghost fill is checked
+bit-exactly elsewhere) are stepped by the oracle with the same dt and cell widths, and every cell of
+every sub-box must agree to <= 1e-12 (north_star's one-step gate; a cell's update depends on nothing
+outside its radius-3 neighbourhood).  Sub-boxes sit on domain corners, edges and faces
+(so periodic / outflow ghosts take part), across CTA tile seams of every kernel, and at seeded
+random interior positions.  Conservation (periodic) holds at any size and is checked on the whole grid.
+"""
+import math
+
+import numpy as np
+import pytest
+
+from paper_1410_4194_b200 import workloads as wl
+from paper_1410_4194_b200.driver import run
+from tests.parity import ONE_STEP_TOL, RUN_L1_TOL, max_rel_error, rel_l1_error
+
+pytestmark = pytest.mark.gpu
+
+
+def subbox_origins(n, m, rng, extra=6):
+    lo, hi, mid = 0, n - m, (n - m) // 2
+    seams = [251 - m // 2, 64 - m // 2, 128 - m // 2]     # x-tile seam, march-segment seam, column-block seam
+    pts = [(lo, lo, lo), (hi, hi, hi), (lo, hi, mid), (hi, lo, mid), (mid, mid, lo), (mid, mid, hi),
+           (min(seams[0], hi), min(seams[1], hi), min(seams[2], hi))]
+    for _ in range(extra):
+        pts.append(tuple(int(v) for v in rng.integers(0, n - m + 1, 3)))
+    return pts
+
+
+def sampled_one_step(ref, w, m=12, extra=6, seed=0):
+    import paper_1410_4194_b200 as ch
+    nx, ny, nz = w.shape
+    g = 3
+    G = ch.Grid(nx, ny, nz, g, w.gamma, w.bc)
+    G.set_state(w.u)
+    dt = G.compute_dt(w.cfl)
+    pre = G.get_padded()
+    G.step(dt)
+    post = G.get_state()
+    G.close()
+    dx = 1.0 / nx
+    worst = 0.0
+    rng = np.random.default_rng(seed)
+    for (i0, j0, k0) in subbox_origins(nx, m, rng, extra):
+        Rg = ref.RefGrid(m, m, m, g, w.gamma, (wl.OUTFLOW,) * 6)     # its own ghost fill runs after the update only
+        Rg.set_spacing(dx, dx, dx)
+        Rg.set_padded(pre[:, k0:k0 + m + 2 * g, j0:j0 + m + 2 * g, i0:i0 + m + 2 * g])
+        Rg.step(dt)
+        ur = Rg.get_state()
+        ug = post[:, k0:k0 + m, j0:j0 + m, i0:i0 + m]
+        worst = max(worst, max(max_rel_error(ug, ur, w.gamma)))
+    return worst, post, dt
+
+
+@pytest.mark.parametrize("n", [256, 512])
+def test_sweep_full_size_sampled_parity_and_conservation(ref, n):
+    """Throughput-sweep workload (BASELINE.json config 5) at the sizes the metric is quoted on."""
+    w = wl.sweep(n)
+    worst, post, _ = sampled_one_step(ref, w)
+    assert worst <= ONE_STEP_TOL, worst
+    for f in range(5):
+        s0, s1 = float(np.sum(w.u[f], dtype=np.longdouble)), float(np.sum(post[f], dtype=np.longdouble))
+        scale = float(np.sum(np.abs(w.u[f]), dtype=np.longdouble)) + (w.u[0].size if f in (1, 2, 3) else 0)
+        assert abs(s1 - s0) <= 1e-13 * scale, (f, s0, s1)
+
+
+def test_shock_cloud_256_sampled_parity(ref):
+    """BASELINE.json config 4 at full size: one step, sub-boxes on the shock front and in the cloud."""
+    w = wl.shock_cloud(256)
+    worst, post, _ = sampled_one_step(ref, w, extra=10, seed=4)
+    assert worst <= ONE_STEP_TOL, worst
+    assert np.all(np.isfinite(post)) and post[0].min() > 0
+
+
+def test_sedov_128_sampled_parity(ref):
+    """BASELINE.json config 3 at full size: one step; the centre sub-box holds the hot cells."""
+    w = wl.sedov(128)
+    nx = 128
+    import paper_1410_4194_b200 as ch
+    worst, post, dt = sampled_one_step(ref, w, extra=4, seed=3)
+    assert worst <= ONE_STEP_TOL, worst
+    # the blast centre itself
+    g, m, o = 3, 16, 56
+    G = ch.Grid(nx, nx, nx, g, w.gamma, w.bc)
+    G.set_state(w.u)
+    pre = G.get_padded()
+    G.step(dt)
+    ug = G.get_state()[:, o:o + m, o:o + m, o:o + m]
+    G.close()
+    Rg = ref.RefGrid(m, m, m, g, w.gamma, (wl.OUTFLOW,) * 6)
+    Rg.set_spacing(1.0 / nx, 1.0 / nx, 1.0 / nx)
+    Rg.set_padded(pre[:, o:o + m + 2 * g, o:o + m + 2 * g, o:o + m + 2 * g])
+    Rg.step(dt)
+    assert max(max_rel_error(ug, Rg.get_state(), w.gamma)) <= ONE_STEP_TOL
+
+
+def test_kelvin_helmholtz_256_200_steps(ref):
+    """BASELINE.json config 2 in full: 256^2, 200 steps at CFL 0.4, lock-step and free-running."""
+    import paper_1410_4194_b200 as ch
+    w = wl.kelvin_helmholtz(256, steps=200)
+    Rg = ref.RefGrid(256, 256, 1, 3, w.gamma, w.bc)
+    dts = []
+    run(Rg, w, record_dts=dts)
+    ur = Rg.get_state()
+    G = ch.Grid(256, 256, 1, 3, w.gamma, w.bc)
+    run(G, w, dts=dts)
+    e_lock = rel_l1_error(G.get_state(), ur, w.gamma)
+    run(G, w)
+    e_free = rel_l1_error(G.get_state(), ur, w.gamma)
+    G.close()
+    assert max(e_lock) <= RUN_L1_TOL, e_lock
+    assert max(e_free) <= RUN_L1_TOL, e_free
