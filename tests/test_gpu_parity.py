@@ -134,9 +134,9 @@ ONE_STEP_CASES = {
     "sweep_yz_2d": lambda: wl.sweep(shape=(1, 40, 48)),           # inactive x
     "sweep_min_size": lambda: wl.sweep(shape=(3, 3, 3)),
     "smooth_mixed_bc": lambda: wl.smooth_random(41, 29, 23, seed=5, bc=(R, O, P, P, O, R)),
-    "rough_3d": lambda: wl.rough_random(37, 21, 13, seed=11),
+    "rough_3d": lambda: wl.rough_random(37, 21, 13, seed=11, decades=0.5),
     "rough_1d": lambda: wl.rough_random(1000, seed=12, mach=3.0),
-    "rough_reflective": lambda: wl.rough_random(24, 24, 24, seed=13, bc=(R,) * 6, mach=1.0),
+    "rough_reflective": lambda: wl.rough_random(24, 24, 24, seed=13, bc=(R,) * 6, mach=1.0, decades=0.5),
 }
 
 
