@@ -159,7 +159,7 @@ def test_one_step_parity_four_ghosts(ch, ref):
 
 
 def test_uniform_state_is_preserved(ch):
-    u = wl.conserved(1.3, 0.4, -0.2, 0.7, 2.1, 1.4) * np.ones((5, 9, 10, 11))
+    u = wl.conserved(1.3, 0.4, -0.2, 0.7, 2.1, 1.4).reshape(5, 1, 1, 1) * np.ones((5, 9, 10, 11))
     for bc in [(P,) * 6, (O,) * 6, (R, O, P, P, O, R)]:
         G = ch.Grid(11, 10, 9, 3, 1.4, bc)
         G.set_state(u)
@@ -257,14 +257,14 @@ def test_error_codes(ch):
     assert math.isnan(L.ch_compute_dt(h, 0.4))
     L.ch_free(h)
     G = ch.Grid(8, 8, 8)
-    G.set_state(wl.conserved(1.0, 0.0, 0.0, 0.0, 1.0, 1.4) * np.ones((5, 8, 8, 8)))
+    G.set_state(wl.conserved(1.0, 0.0, 0.0, 0.0, 1.0, 1.4).reshape(5, 1, 1, 1) * np.ones((5, 8, 8, 8)))
     with pytest.raises(ValueError):
         G.step(0.0)
     with pytest.raises(ValueError):
         G.step(float("nan"))
     with pytest.raises(ValueError):
         G.compute_dt(1.5)
-    u = wl.conserved(1.0, 0.0, 0.0, 0.0, 1.0, 1.4) * np.ones((5, 8, 8, 8))
+    u = wl.conserved(1.0, 0.0, 0.0, 0.0, 1.0, 1.4).reshape(5, 1, 1, 1) * np.ones((5, 8, 8, 8))
     u[0, 3, 3, 3] = -1.0
     G.set_state(u)
     assert math.isnan(G.compute_dt(0.4)) and "non-physical" in B.last_error()
