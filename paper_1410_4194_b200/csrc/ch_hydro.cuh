@@ -3,19 +3,23 @@
 // Written from the text of arXiv:1410.4194 (citations `P:L<line>` = /root/reference/PAPER.md line);
 // "G<n>/S<n>" are the readings of garbled / silent passages listed in DESIGN.md.  This file shares
 // nothing with oracle/: it restates the same equations in a form chosen for the B200 FP64 pipe
-// (one reciprocal-square-root per cell instead of four divisions and a square root, pr^z through
-// exp(z*log(pr)) with the 1/gamma power derived from it, mirror-folded Riemann sampling).
+// (DESIGN.md §4 "Arithmetic restatements"):
+//   * reciprocals and reciprocal square roots are MUFU seeds refined by DFMA Newton steps, with no
+//     slow-path branches (every operand here is a normal positive double);
+//   * one rsqrt(gamma p rho) per cell yields a, 1/a, rho/a, 1/a^2, a/rho by multiplication;
+//   * (p/p_k)^z is a 13-term binomial series when |p/p_k - 1| <= 1/16 (smooth flow) and
+//     exp(z log(.)) otherwise; (p/p_k)^{1/gamma} = pr / (pr^z)^2;
+//   * min / max / clamp are compare-selects (no NaN-propagating fmin/fmax emulation);
+//   * B9 and the sampling take f_k, (p/p_k)^z at the converged pressure by a first-order update
+//     from the last Newton iterate (error O(tol^2) = 1e-16) instead of a fresh evaluation;
+//   * the ten-way sampling is folded onto the left wave family by mirroring when u^m < 0.
 //
 // All functions work in the direction-local ordering (rho, v_n, v_t1, v_t2, p).
 #pragma once
 
 #include <math.h>
 
-#ifdef __CUDACC__
-#define CH_HD __host__ __device__ __forceinline__
-#else
-#define CH_HD inline
-#endif
+#define CH_D __device__ __forceinline__
 
 namespace ch {
 
@@ -23,8 +27,10 @@ constexpr double kPFloor = 1e-20;
 constexpr double kPGuessFloor = 1e-6;
 constexpr double kNewtonTol = 1e-8;     // P:L1095 "e.g. 1e-6"; reading S2
 constexpr int kNewtonCap = 20;          // reading S2
+constexpr int kPowTerms = 13;           // binomial series length for (1+t)^z, |t| <= kPowRadius
+constexpr double kPowRadius = 1.0 / 16.0;
 
-// gamma-derived constants, computed once on the host in ch_init.
+// gamma-derived constants, computed once on the host in ch_init (fill_gas in ch_kernels.cu).
 struct Gas {
   double gamma;
   double gm1;        // gamma - 1
@@ -36,21 +42,51 @@ struct Gas {
   double half_gp1;   // (gamma + 1)/2
   double two_gp1;    // 2/(gamma + 1)
   double half_gm1;   // (gamma - 1)/2
+  double bz[kPowTerms];   // binomial coefficients C(z, k), k = 1..13:  (1+t)^z - 1 = sum bz[k-1] t^k
 };
 
-CH_HD double rsqrt_d(double x) {
-#ifdef __CUDA_ARCH__
-  return rsqrt(x);
-#else
-  return 1.0 / sqrt(x);
-#endif
+// ---- branch-free reciprocal / reciprocal square root / square root ------------------------------
+// MUFU seed (about 20 good bits) + one cubic and one quadratic Newton step in DFMA: result within
+// 1-2 ulp for normal positive x, which every operand on this path is (densities, floored pressures,
+// sums of positive terms).  No denormal / inf / zero slow path.
+CH_D double rcp(double x) {
+  double r;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+  double e = fma(-x, r, 1.0);
+  e = fma(e, e, e);
+  r = fma(r, e, r);
+  e = fma(-x, r, 1.0);
+  return fma(r, e, r);
 }
 
-CH_HD double floor_p(double p) { return (p < kPFloor) ? kPFloor : p; }  // keeps NaN visible
+CH_D double rsqrt_pos(double x) {
+  double y;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  double t = x * y;
+  double e = fma(-t, y, 1.0);
+  const double c = fma(e, 0.375, 0.5);
+  y = fma(c, y * e, y);
+  t = x * y;
+  e = fma(-t, y, 1.0);
+  return fma(0.5 * y, e, y);
+}
+
+// sqrt(x) = x * rsqrt(x) with one residual correction.
+CH_D double sqrt_pos(double x) {
+  const double y = rsqrt_pos(x);
+  const double s = x * y;
+  const double r = fma(-s, s, x);
+  return fma(r, 0.5 * y, s);
+}
+
+CH_D double sel_min(double a, double b) { return (a < b) ? a : b; }
+CH_D double sel_max(double a, double b) { return (a > b) ? a : b; }
+
+CH_D double floor_p(double p) { return (p < kPFloor) ? kPFloor : p; }  // keeps NaN visible
 
 // Eq. 6-8: conserved (direction-local momenta) -> primitive, pressure floor (S1).
-CH_HD void cons2prim(const Gas& G, double d, double mn, double mt1, double mt2, double E, double w[5]) {
-  const double r = 1.0 / d;
+CH_D void cons2prim(const Gas& G, double d, double mn, double mt1, double mt2, double E, double w[5]) {
+  const double r = rcp(d);
   const double u = mn * r, v = mt1 * r, ww = mt2 * r;
   const double ke = 0.5 * d * ((u * u + v * v) + ww * ww);
   w[0] = d; w[1] = u; w[2] = v; w[3] = ww;
@@ -58,7 +94,7 @@ CH_HD void cons2prim(const Gas& G, double d, double mn, double mt1, double mt2, 
 }
 
 // Eq. 6-8 inverted: primitive -> conserved (direction-local momenta).
-CH_HD void prim2cons(const Gas& G, const double w[5], double c[5]) {
+CH_D void prim2cons(const Gas& G, const double w[5], double c[5]) {
   c[0] = w[0];
   c[1] = w[0] * w[1];
   c[2] = w[0] * w[2];
@@ -69,19 +105,19 @@ CH_HD void prim2cons(const Gas& G, const double w[5], double c[5]) {
 // s = 1/(rho a) with a = sqrt(gamma p / rho) (Eq. 21): the one transcendental per cell; everything
 // the characteristic projections need follows by multiplication:
 //   a = gamma p s,  1/a = rho s,  rho/a = rho^2 s,  1/a^2 = (rho s)^2,  a/rho = a^2 s,  rho a = gamma p rho s.
-CH_HD double inv_rho_a(const Gas& G, double rho, double p) { return rsqrt_d(G.gamma * p * rho); }
+CH_D double inv_rho_a(const Gas& G, double rho, double p) { return rsqrt_pos(G.gamma * p * rho); }
 
 // Monotonised-central limiter A10 (reading G7: the formula governs).
-CH_HD double mc_limit(double dL, double dR, double dC) {
-  const double m = fmin(fabs(dC), 2.0 * fmin(fabs(dL), fabs(dR)));
+CH_D double mc_limit(double dL, double dR, double dC) {
+  const double m = sel_min(fabs(dC), 2.0 * sel_min(fabs(dL), fabs(dR)));
   return (dL * dR > 0.0) ? copysign(m, dC) : 0.0;
 }
 
 // Limited slope of cell q in primitive variables via characteristic variables (A2 P:L690, A9 P:L730
 // with row 0 read as G1, A10, A11 P:L741), projected with cell q's own rho, a.
 // s = inv_rho_a(q).
-CH_HD void limited_slope(const Gas& G, const double wm[5], const double w0[5], const double wp[5], double s,
-                         double dw[5]) {
+CH_D void limited_slope(const Gas& G, const double wm[5], const double w0[5], const double wp[5], double s,
+                        double dw[5]) {
   const double rho = w0[0];
   const double a = G.gamma * w0[4] * s;
   const double ia = rho * s;
@@ -121,7 +157,7 @@ CH_HD void limited_slope(const Gas& G, const double wm[5], const double w0[5], c
 // PPMC for one cell (A.3): parabola edges A20-A23, A24/A26(=A50, G2), characteristic
 // tracing A25-A33 (A30/A32 read as G3).  wm,w0,wp = cells i-1,i,i+1; dwm,dw0,dwp their limited
 // slopes; s = inv_rho_a(i); dtdx = dt/dx_d.  Outputs W*_L, W*_R (primitive).
-CH_HD void ppmc_faces(const Gas& G, double dtdx, const double wm[5], const double w0[5], const double wp[5],
+CH_D void ppmc_faces(const Gas& G, double dtdx, const double wm[5], const double w0[5], const double wp[5],
                       const double dwm[5], const double dw0[5], const double dwp[5], double s, double WLs[5],
                       double WRs[5]) {
   double WL[5], WR[5], dwi[5], w6[5];
@@ -138,8 +174,16 @@ CH_HD void ppmc_faces(const Gas& G, double dtdx, const double wm[5], const doubl
     const bool fixR = RL * (cr - R) < 0.0;
     if (fixL) L = cl;
     if (fixR) R = cr;
-    L = fmin(fmax(wi, wm[m]), fmax(fmin(wi, wm[m]), L));               // A23
-    R = fmin(fmax(wi, wp[m]), fmax(fmin(wi, wp[m]), R));
+    {                                                                  // A23
+      const bool up = wm[m] < wi;
+      const double lo = up ? wm[m] : wi, hi = up ? wi : wm[m];
+      L = sel_min(hi, sel_max(lo, L));
+    }
+    {
+      const bool up = wp[m] < wi;
+      const double lo = up ? wp[m] : wi, hi = up ? wi : wp[m];
+      R = sel_min(hi, sel_max(lo, R));
+    }
     WL[m] = L; WR[m] = R;
     dwi[m] = R - L;                                                    // A24
     w6[m] = 6.0 * (wi - 0.5 * (L + R));                                // A26 as A50 (G2)
@@ -151,8 +195,8 @@ CH_HD void ppmc_faces(const Gas& G, double dtdx, const double wm[5], const doubl
   const double ra = rho * ia;        // rho / a
   const double rhoa = rho * a;       // rho * a
   const double lm = w0[1] - a, l0 = w0[1], lp = w0[1] + a;            // A8
-  const double am = dtdx * fmin(lm, 0.0), a0 = dtdx * fmin(l0, 0.0), ap = dtdx * fmin(lp, 0.0);  // A27
-  const double bm = dtdx * fmax(lm, 0.0), b0 = dtdx * fmax(l0, 0.0), bp = dtdx * fmax(lp, 0.0);
+  const double am = dtdx * sel_min(lm, 0.0), a0 = dtdx * sel_min(l0, 0.0), ap = dtdx * sel_min(lp, 0.0);  // A27
+  const double bm = dtdx * sel_max(lm, 0.0), b0 = dtdx * sel_max(l0, 0.0), bp = dtdx * sel_max(lp, 0.0);
   const double k23 = 2.0 / 3.0;
   // reference states A25: left face under lambda^m, right face under lambda^p
   double WLm[5], WRp[5];
@@ -203,31 +247,52 @@ CH_HD void ppmc_faces(const Gas& G, double dtdx, const double wm[5], const doubl
   WRs[0] = WRp[0] + sR0; WRs[1] = WRp[1] + sR1; WRs[2] = WRp[2] + sR2; WRs[3] = WRp[3] + sR3; WRs[4] = WRp[4] + sR4;
 }
 
+// (1 + t)^z - 1 for |t| <= kPowRadius: 13-term binomial series in Horner form (truncation
+// C(z,14) 16^-14 < 1e-18).  Returns the value WITHOUT the leading 1 so that f_k = 2a/(gamma-1) (x-1)
+// (B5) does not cancel.
+CH_D double powz_m1_series(const Gas& G, double t) {
+  double h = G.bz[kPowTerms - 1];
+#pragma unroll
+  for (int k = kPowTerms - 2; k >= 0; --k) h = fma(h, t, G.bz[k]);
+  return h * t;
+}
+
 // Pressure function f_k, f'_k (B5, B6) for one side at trial pressure p.
-//   rk, pk: density and pressure of side k; ak = sound speed; rpk = 1/pk; ick = 1/(rho_k a_k).
-// x returns (p/pk)^z on the rarefaction branch (re-used by the sampler), untouched otherwise.
-CH_HD void pressure_fn(const Gas& G, double p, double rk, double pk, double ak, double rpk, double ick, double& f,
-                       double& fp, double& x) {
-  if (p <= pk) {   // rarefaction
-    const double pr = p * rpk;
-    x = exp(G.z * log(pr));
-    f = G.two_gm1 * ak * (x - 1.0);
-    fp = ick * x / pr;                       // pr^{-(gamma+1)/(2 gamma)} = pr^z / pr
+//   rk, pk: density and pressure of side k; ak = sound speed; rpk = 1/pk; ick = 1/(rho_k a_k);
+//   rp = 1/p.  On the rarefaction branch x returns (p/pk)^z (re-used by the sampler).
+// Returns true on the rarefaction branch.
+CH_D bool pressure_fn(const Gas& G, double p, double rp, double rk, double pk, double ak, double rpk, double ick,
+                      double& f, double& fp, double& x) {
+  const bool rare = (p <= pk);
+  if (rare) {
+    const double t = (p - pk) * rpk;         // p/pk - 1, exact difference first
+    double xm1;
+    if (fabs(t) <= kPowRadius) xm1 = powz_m1_series(G, t);
+    else xm1 = exp(G.z * log(p * rpk)) - 1.0;
+    x = xm1 + 1.0;
+    f = G.two_gm1 * ak * xm1;
+    fp = ick * x * (pk * rp);                // (p/pk)^{-(gamma+1)/(2 gamma)} = pr^z / pr
   } else {         // shock: sqrt(A/(p+B)) = rsqrt((p + B) rho (gamma+1)/2)   (B4)
     const double h = rk * G.half_gp1;
-    const double sq = rsqrt_d((p + G.gm * pk) * h);
+    const double sq = rsqrt_pos((p + G.gm * pk) * h);
     const double dp = p - pk;
     f = dp * sq;
     fp = sq * (1.0 - 0.5 * dp * (sq * sq) * h);   // 1/(B+p) = sq^2 (gamma+1) rho / 2
   }
+  return rare;
 }
 
 // Exact Riemann solver (B.1): primitive L/R states (direction-local) -> flux B22.
-// Newton-Raphson on the star pressure from the two-shock guess B2-B4; f_k re-evaluated at the final
-// p^m for u^m (reading S3); iterate floored at 1e-20 (S4).  The ten-way sampling at x/t = 0 is
-// folded onto the left-wave family by mirroring (u -> -u) when u^m < 0; the mirrored tests coincide
-// with B16-B21 except on the measure-zero tie um + a_R x = 0, where fan and star state are equal.
-CH_HD void riemann_exact(const Gas& G, const double WL[5], const double WR[5], double flux[5]) {
+// Newton-Raphson on the star pressure from the two-shock guess B2-B4.  With p0 the last iterate at
+// which f_k, f'_k were evaluated and p^m the accepted pressure (|p^m - p0| <= 1e-8 p, B8), B9 needs
+// f_k(p^m) (reading S3): taken as f_k(p0) + f'_k(p0)(p^m - p0), whose error f'' (p^m - p0)^2 / 2 is
+// below 1e-16 of the wave-speed scale; likewise (p^m/p_k)^z for the sampler.  The sampler branches
+// on the wave type found at p0 (the two wave curves have second-order contact at p = p_k, so the
+// choice within 1e-8 of the kink moves nothing above 1e-24).  Iterate floored at 1e-20 (S4).  The
+// ten-way sampling at x/t = 0 is folded onto the left-wave family by mirroring (u -> -u) when
+// u^m < 0; the mirrored tests coincide with B16-B21 except on the measure-zero tie
+// um + a_R x = 0, where fan and star state are equal.
+CH_D void riemann_exact(const Gas& G, const double WL[5], const double WR[5], double flux[5]) {
   const double rL = WL[0], uL = WL[1], pL = floor_p(WL[4]);
   const double rR = WR[0], uR = WR[1], pR = floor_p(WR[4]);
   const double icL = inv_rho_a(G, rL, pL), icR = inv_rho_a(G, rR, pR);   // 1/(rho a)
@@ -240,24 +305,27 @@ CH_HD void riemann_exact(const Gas& G, const double WL[5], const double WR[5], d
   double pt = 0.5 * (pL + pR) - 0.125 * du * (rL + rR) * (aL + aR);
   pt = (pt < 0.0) ? 0.0 : pt;
   // B3, B4: g_k = sqrt(A_k/(pt + B_k))
-  const double gL = rsqrt_d((pt + G.gm * pL) * rL * G.half_gp1);
-  const double gR = rsqrt_d((pt + G.gm * pR) * rR * G.half_gp1);
-  double p0 = ((gL * pL + gR * pR) - du) / (gL + gR);
+  const double gL = rsqrt_pos((pt + G.gm * pL) * rL * G.half_gp1);
+  const double gR = rsqrt_pos((pt + G.gm * pR) * rR * G.half_gp1);
+  double p0 = ((gL * pL + gR * pR) - du) * rcp(gL + gR);
   p0 = (p0 < kPGuessFloor) ? kPGuessFloor : p0;
   // Newton-Raphson B5-B8
-  double pm, fL, fR, fpL, fpR, xL = 1.0, xR = 1.0;
+  double pm, rp0, fL, fR, fpL, fpR, xL = 1.0, xR = 1.0;
+  bool rareL, rareR;
   int it = 0;
   for (;;) {
-    pressure_fn(G, p0, rL, pL, aL, rpL, icL, fL, fpL, xL);
-    pressure_fn(G, p0, rR, pR, aR, rpR, icR, fR, fpR, xR);
-    pm = p0 - ((fL + fR) + du) / (fpL + fpR);                           // B7
+    rp0 = rcp(p0);
+    rareL = pressure_fn(G, p0, rp0, rL, pL, aL, rpL, icL, fL, fpL, xL);
+    rareR = pressure_fn(G, p0, rp0, rR, pR, aR, rpR, icR, fR, fpR, xR);
+    pm = p0 - ((fL + fR) + du) * rcp(fpL + fpR);                        // B7
     pm = (pm < kPFloor) ? kPFloor : pm;                                  // S4
     ++it;
     if (!(2.0 * fabs(pm - p0) > kNewtonTol * fabs(pm + p0)) || it >= kNewtonCap) break;   // B8
     p0 = pm;
   }
-  pressure_fn(G, pm, rL, pL, aL, rpL, icL, fL, fpL, xL);                 // S3
-  pressure_fn(G, pm, rR, pR, aR, rpR, icR, fR, fpR, xR);
+  const double dp = pm - p0;                                             // S3 by first-order update
+  fL = fma(fpL, dp, fL);
+  fR = fma(fpR, dp, fR);
   const double um = 0.5 * ((uL + uR) + (fR - fL));                       // B9
 
   // Sampling at x/t = 0, mirrored onto the left family.
@@ -265,23 +333,26 @@ CH_HD void riemann_exact(const Gas& G, const double WL[5], const double WR[5], d
   const double sg = left ? 1.0 : -1.0;
   const double rk = left ? rL : rR, pk = left ? pL : pR, ak = left ? aL : aR;
   const double uk = sg * (left ? uL : uR), us = sg * um;
-  const double rpk = left ? rpL : rpR, xk = left ? xL : xR;
+  const double rpk = left ? rpL : rpR;
+  const bool rare = left ? rareL : rareR;
+  double xk = left ? xL : xR;
+  xk = fma(G.z * xk * rp0, dp, xk);                                      // (pm/pk)^z from (p0/pk)^z
   const double vt1 = left ? WL[2] : WR[2], vt2 = left ? WL[3] : WR[3];   // S9
   const double pr = pm * rpk;
   double rho, u, p;
-  if (pm <= pk) {                                                        // rarefaction
+  if (rare) {                                                            // rarefaction
     if (uk - ak >= 0.0) { rho = rk; u = uk; p = pk; }                    // B10 / B16
-    else if (us - ak * xk < 0.0) { rho = rk * (pr / (xk * xk)); u = us; p = pm; }   // B11 / B17: pr^{1/gamma} = pr / x^2
+    else if (us - ak * xk < 0.0) { rho = rk * pr * rcp(xk * xk); u = us; p = pm; }   // B11 / B17: pr^{1/gamma} = pr / x^2
     else {                                                               // B12 / B18 (G4)
       const double af = G.two_gp1 * (ak + G.half_gm1 * uk);
-      const double q = af / ak;
+      const double q = af * rcp(ak);
       const double y = exp(G.two_gm1 * log(q));                          // (a/a_k)^{2/(gamma-1)}
       rho = rk * y; u = af; p = pk * y * (q * q);                        // exponent 2 gamma/(gamma-1) = 2/(gamma-1) + 2
     }
   } else {                                                               // shock
-    const double sk = uk - ak * sqrt(G.c_sh * pr + G.z);                 // B13 / B19 (G5)
+    const double sk = uk - ak * sqrt_pos(G.c_sh * pr + G.z);             // B13 / B19 (G5)
     if (sk >= 0.0) { rho = rk; u = uk; p = pk; }                         // B14 / B20
-    else { rho = rk * (pr + G.gm) / (pr * G.gm + 1.0); u = us; p = pm; } // B15 / B21
+    else { rho = rk * (pr + G.gm) * rcp(pr * G.gm + 1.0); u = us; p = pm; } // B15 / B21
   }
   u *= sg;
   // B22

@@ -233,32 +233,31 @@ __global__ void __launch_bounds__(kXT) k_pass1_x(const StepArgs A, long long q_b
 // ---------------------------------------------------------------------------------------------
 // Pass 2: transverse correction (Eq. 23) of the two states meeting at interface c+1/2
 // along each active direction, then the second exact Riemann solve.  One thread per cell
-// of [-1, n)^3.
+// of [-1, n)^3.  The three directions run through ONE copy of the solver (a rolled loop over d with
+// the cyclic permutation P:L164 done by field offsets), which keeps the kernel inside the
+// instruction cache.
 // ---------------------------------------------------------------------------------------------
-template <int D>
-__device__ __forceinline__ void corrected_prim(const StepArgs& A, const double* __restrict__ U, long long q,
-                                               double w[5]) {
-  const Geom& g = A.geo;
-  const long long np = g.np;
-  constexpr int E1 = (D + 1) % 3, E2 = (D + 2) % 3;
+struct DirSel {
+  const double* F1; const double* F2;   // first-pass fluxes of the two transverse directions
+  long long s0, s1, s2;                 // strides: along d, along e1 = d+1, along e2 = d+2 (cyclic)
+  double h1, h2;                        // dt / (2 dx_e1), dt / (2 dx_e2)
+  bool a1, a2;                          // transverse direction active
+  long long f1, f2, f3;                 // field offsets (in doubles) of the direction-local momenta
+};
+
+__device__ __forceinline__ void corrected_prim(const Gas& G, const DirSel& S, long long np, const double* __restrict__ U,
+                                               long long q, double w[5]) {
+  const long long off[5] = {0, S.f1, S.f2, S.f3, 4 * np};
   double c[5];
 #pragma unroll
-  for (int f = 0; f < 5; ++f) {
+  for (int m = 0; m < 5; ++m) {
+    const long long a = off[m] + q;
     double corr = 0.0;
-    if (g.act[E1]) corr += 0.5 * A.dtdx[E1] * (A.Fs[E1][f * np + q - g.st[E1]] - A.Fs[E1][f * np + q]);
-    if (g.act[E2]) corr += 0.5 * A.dtdx[E2] * (A.Fs[E2][f * np + q - g.st[E2]] - A.Fs[E2][f * np + q]);
-    c[f] = U[f * np + q] + corr;
+    if (S.a1) corr += S.h1 * (S.F1[a - S.s1] - S.F1[a]);
+    if (S.a2) corr += S.h2 * (S.F2[a - S.s2] - S.F2[a]);
+    c[m] = U[a] + corr;
   }
-  ch::cons2prim(A.gas, c[0], c[comp<D>(1)], c[comp<D>(2)], c[comp<D>(3)], c[4], w);
-}
-
-template <int D>
-__device__ __forceinline__ void pass2_dir(const StepArgs& A, long long q) {
-  double wl[5], wr[5], fl[5];
-  corrected_prim<D>(A, A.UR[D], q, wl);                 // U^{n+1/2}_R of cell c   -> left state
-  corrected_prim<D>(A, A.UL[D], q + A.geo.st[D], wr);   // U^{n+1/2}_L of cell c+1 -> right state
-  ch::riemann_exact(A.gas, wl, wr, fl);
-  store_local<D>(A.Fh[D], A.geo.np, q, fl);
+  ch::cons2prim(G, c[0], c[1], c[2], c[3], c[4], w);
 }
 
 __global__ void __launch_bounds__(128) k_pass2(const StepArgs A) {
@@ -270,10 +269,28 @@ __global__ void __launch_bounds__(128) k_pass2(const StepArgs A) {
   const long long r = id / e0;
   const int j = (int)(r % e1) - (g.act[1] ? 1 : 0);
   const int k = (int)(r / e1) - (g.act[2] ? 1 : 0);
+  const long long np = g.np;
   const long long q = (long long)(i + g.g[0]) + (long long)(j + g.g[1]) * g.st[1] + (long long)(k + g.g[2]) * g.st[2];
-  if (g.act[0] && j >= 0 && k >= 0) pass2_dir<0>(A, q);
-  if (g.act[1] && i >= 0 && k >= 0) pass2_dir<1>(A, q);
-  if (g.act[2] && i >= 0 && j >= 0) pass2_dir<2>(A, q);
+#pragma unroll 1
+  for (int d = 0; d < 3; ++d) {
+    // interface c+1/2 along d is needed where the two transverse indices are real (>= 0)
+    const bool need = d == 0 ? (g.act[0] && j >= 0 && k >= 0) : d == 1 ? (g.act[1] && i >= 0 && k >= 0)
+                                                                       : (g.act[2] && i >= 0 && j >= 0);
+    if (!need) continue;
+    const int d1 = d == 2 ? 0 : d + 1, d2 = d == 0 ? 2 : d - 1;
+    DirSel S;
+    S.F1 = A.Fs[d1]; S.F2 = A.Fs[d2];
+    S.s0 = g.st[d]; S.s1 = g.st[d1]; S.s2 = g.st[d2];
+    S.h1 = 0.5 * A.dtdx[d1]; S.h2 = 0.5 * A.dtdx[d2];
+    S.a1 = g.act[d1] != 0; S.a2 = g.act[d2] != 0;
+    S.f1 = (long long)(1 + d) * np; S.f2 = (long long)(1 + d1) * np; S.f3 = (long long)(1 + d2) * np;
+    double wl[5], wr[5], fl[5];
+    corrected_prim(A.gas, S, np, A.UR[d], q, wl);           // U^{n+1/2}_R of cell c   -> left state
+    corrected_prim(A.gas, S, np, A.UL[d], q + S.s0, wr);    // U^{n+1/2}_L of cell c+1 -> right state
+    ch::riemann_exact(A.gas, wl, wr, fl);
+    double* __restrict__ Fh = A.Fh[d];
+    Fh[q] = fl[0]; Fh[S.f1 + q] = fl[1]; Fh[S.f2 + q] = fl[2]; Fh[S.f3 + q] = fl[3]; Fh[4 * np + q] = fl[4];
+  }
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -604,6 +621,12 @@ ch_ctx* ch_init(int nx, int ny, int nz, int nghost, double gamma, const int* bc)
   G.gamma = gamma; G.gm1 = gamma - 1.0; G.inv_gm1 = 1.0 / (gamma - 1.0); G.two_gm1 = 2.0 / (gamma - 1.0);
   G.z = (gamma - 1.0) / (2.0 * gamma); G.gm = (gamma - 1.0) / (gamma + 1.0); G.c_sh = (gamma + 1.0) / (2.0 * gamma);
   G.half_gp1 = 0.5 * (gamma + 1.0); G.two_gp1 = 2.0 / (gamma + 1.0); G.half_gm1 = 0.5 * (gamma - 1.0);
+  {
+    // binomial coefficients C(z,k) = C(z,k-1) (z-k+1)/k of the (1+t)^z series (ch_hydro.cuh)
+    const long double zl = ((long double)gamma - 1.0L) / (2.0L * (long double)gamma);
+    long double b = 1.0L;
+    for (int k = 1; k <= ch::kPowTerms; ++k) { b *= (zl - (long double)(k - 1)) / (long double)k; G.bz[k - 1] = (double)b; }
+  }
   return c;
 }
 
