@@ -130,6 +130,7 @@ long long ch_kernel_launches(const ch_ctx* ctx);
 /* Kernel kinds of one step, for ch_profile_read / ch_kernel_name. */
 enum {
   CH_K_RESET = 0, CH_K_PASS1_X, CH_K_PASS1_Y, CH_K_PASS1_Z, CH_K_PASS2, CH_K_UPDATE, CH_K_GHOST, CH_K_DT,
+  CH_K_FINAL,
   CH_K_COUNT
 };
 

@@ -27,7 +27,7 @@ SYMBOLS = ("ch_init", "ch_free", "ch_last_error", "ch_set_spacing", "ch_padded_c
            "ch_bind", "ch_set_state", "ch_get_state", "ch_set_padded", "ch_get_padded", "ch_compute_dt",
            "ch_step", "ch_sync", "ch_kernel_launches", "ch_profile", "ch_profile_read", "ch_kernel_name",
            "ch_fp64_peak_probe")
-K_COUNT = 8
+K_COUNT = 9
 
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-shared"]

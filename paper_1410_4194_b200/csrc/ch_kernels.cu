@@ -16,6 +16,7 @@
 #include <cmath>
 #include <cstdint>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <limits>
 #include <new>
@@ -88,8 +89,24 @@ __device__ __forceinline__ void copy5(double dst[5], const double src[5]) {
 // cell's right-face state in registers.  Every cell's slope and parabola is computed once per
 // segment (warm-up: 3 slopes + 1 parabola per segment).
 // ---------------------------------------------------------------------------------------------
+#ifndef CH_MARCH_T
+#define CH_MARCH_T 128   // threads per CTA of the marching kernels
+#endif
+#ifndef CH_MARCH_MINB
+#define CH_MARCH_MINB 1
+#endif
+#ifndef CH_X_MINB
+#define CH_X_MINB 1
+#endif
+#ifndef CH_P2_T
+#define CH_P2_T 128
+#endif
+#ifndef CH_P2_MINB
+#define CH_P2_MINB 1
+#endif
+
 template <int D>
-__global__ void __launch_bounds__(128) k_pass1_march(const StepArgs A, int seg) {
+__global__ void __launch_bounds__(CH_MARCH_T, CH_MARCH_MINB) k_pass1_march(const StepArgs A, int seg) {
   constexpr int T = 3 - D;   // the other transverse dimension (x is the lane dimension)
   const Geom& g = A.geo;
   const Gas& G = A.gas;
@@ -159,7 +176,7 @@ __global__ void __launch_bounds__(128) k_pass1_march(const StepArgs A, int seg) 
 constexpr int kXT = 256;       // threads per CTA
 constexpr int kXOut = kXT - 5; // interfaces produced per CTA
 
-__global__ void __launch_bounds__(kXT) k_pass1_x(const StepArgs A, long long q_begin, long long q_end) {
+__global__ void __launch_bounds__(kXT, CH_X_MINB) k_pass1_x(const StepArgs A, long long q_begin, long long q_end) {
   __shared__ double sP[5][kXT];
   __shared__ double sS[5][kXT];
   __shared__ double sL[5][kXT];
@@ -260,7 +277,7 @@ __device__ __forceinline__ void corrected_prim(const Gas& G, const DirSel& S, lo
   ch::cons2prim(G, c[0], c[1], c[2], c[3], c[4], w);
 }
 
-__global__ void __launch_bounds__(128) k_pass2(const StepArgs A) {
+__global__ void __launch_bounds__(CH_P2_T, CH_P2_MINB) k_pass2(const StepArgs A) {
   const Geom& g = A.geo;
   const int e0 = g.act[0] ? g.n[0] + 1 : 1, e1 = g.act[1] ? g.n[1] + 1 : 1, e2 = g.act[2] ? g.n[2] + 1 : 1;
   const long long id = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -395,6 +412,142 @@ __global__ void __launch_bounds__(256) k_update(const StepArgs A) {
 }
 
 // ---------------------------------------------------------------------------------------------
+// Fused second half of the step for 3-D grids: Eq. 23 transverse correction, second exact Riemann
+// pass, Eq. 24 update and the Eq. 22 reduction of the new state in ONE kernel, so the CTU fluxes
+// F,G,H^{n+1/2} never touch HBM (steps 3-5).
+//
+// A CTA is a 32 (x) by kFY (y) tile of threads that marches a segment of z.  Every thread owns one
+// cell column; at step k it forms the corrected face states of cell (i,j,k), solves the Riemann
+// problems on the cell's LOW faces (the left state comes from the neighbour: lane-1 through shared
+// memory for x, row-1 for y, its own previous step for z) and differences them against the low-face
+// flux of the neighbour on the high side.  Lane 0 / row 0 only supply states, lane 31 / row kFY-1
+// only supply fluxes: a tile updates 30 x (kFY-2) columns.  The z flux of a cell's high face arrives
+// one step later, so a cell is finished (stored, and its Eq. 22 time step reduced) at step k+1 from
+// the x,y-updated partial sum and its low-face z flux kept in shared memory.  The three directions
+// run through one rolled copy of the solver (instruction cache).
+// ---------------------------------------------------------------------------------------------
+#ifndef CH_F_TY
+#define CH_F_TY 8
+#endif
+#ifndef CH_F_MINB
+#define CH_F_MINB 3
+#endif
+constexpr int kFX = 32, kFY = CH_F_TY, kFT = kFX * kFY;
+
+__global__ void __launch_bounds__(kFT, CH_F_MINB) k_final3d(const StepArgs A, int seg) {
+  extern __shared__ double s_final[];
+  typedef double (*Arr)[kFT];
+  Arr sX = reinterpret_cast<Arr>(s_final);              // exchanged right-face primitive state of the sweep direction
+  Arr sF = reinterpret_cast<Arr>(s_final + 5 * kFT);    // exchanged low-face flux
+  Arr zU = reinterpret_cast<Arr>(s_final + 10 * kFT);   // carried: U^{n+1/2}_R(., z) of cell k-1, primitive, z-local order
+  Arr zF = reinterpret_cast<Arr>(s_final + 15 * kFT);   // carried: H^{n+1/2} on the low z face of cell k-1, z-local order
+  Arr zP = reinterpret_cast<Arr>(s_final + 20 * kFT);   // carried: u + x and y flux differences of cell k-1, global order
+  const Geom& g = A.geo;
+  const Gas& G = A.gas;
+  const int tid = threadIdx.x, lane = tid & 31, row = tid >> 5;
+  const int nx = g.n[0], ny = g.n[1], nz = g.n[2];
+  const int i = (int)blockIdx.x * (kFX - 2) - 1 + lane;
+  const int j = (int)blockIdx.y * (kFY - 2) - 1 + row;
+  const int k0 = (int)blockIdx.z * seg;
+  const int k1 = min(k0 + seg, nz);
+  const bool valid = i <= nx && j <= ny;
+  const bool realI = i >= 0 && i < nx, realJ = j >= 0 && j < ny;
+  const bool updL = lane >= 1 && lane <= kFX - 2 && realI, updR = row >= 1 && row <= kFY - 2 && realJ;
+  const bool need0 = valid && updR, need1 = valid && updL, need2 = updL && updR;
+  const bool solve0 = need0 && lane >= 1 && i >= 0, solve1 = need1 && row >= 1 && j >= 0;
+  const long long np = g.np;
+  const long long qcol = (long long)(i + g.g[0]) + (long long)(j + g.g[1]) * g.st[1] + (long long)g.g[2] * g.st[2];
+  double tmin = __longlong_as_double(0x7FF0000000000000LL);
+  bool bad = false;
+
+  for (int k = k0 - 1; k <= k1; ++k) {
+    const bool first = k == k0 - 1, tail = k == k1;
+    const long long q = qcol + (long long)k * g.st[2];
+    double part[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+    if (need2 && !first && !tail) {
+#pragma unroll
+      for (int f = 0; f < 5; ++f) part[f] = A.u[f * np + q];
+    }
+#pragma unroll 1
+    for (int d = (first || tail) ? 2 : 0; d < 3; ++d) {
+      const int d1 = d == 2 ? 0 : d + 1, d2 = d == 0 ? 2 : d - 1;
+      const bool need = d == 0 ? need0 : d == 1 ? need1 : need2;
+      const bool solve = d == 0 ? solve0 : d == 1 ? solve1 : (need2 && !first);
+      const long long f1 = (long long)(1 + d) * np, f2 = (long long)(1 + d1) * np, f3 = (long long)(1 + d2) * np;
+      double wl[5] = {1.0, 0.0, 0.0, 0.0, 1.0}, wr[5] = {1.0, 0.0, 0.0, 0.0, 1.0};
+      if (need) {
+        // Eq. 23: both face states of cell c along d get the same two transverse flux differences
+        const double* __restrict__ F1 = A.Fs[d1];
+        const double* __restrict__ F2 = A.Fs[d2];
+        const double* __restrict__ UL = A.UL[d];
+        const double* __restrict__ UR = A.UR[d];
+        const long long s1 = g.st[d1], s2 = g.st[d2];
+        const double h1 = 0.5 * A.dtdx[d1], h2 = 0.5 * A.dtdx[d2];
+        const long long off[5] = {0, f1, f2, f3, 4 * np};
+        double cl[5], cr[5];
+#pragma unroll
+        for (int m = 0; m < 5; ++m) {
+          const long long a = off[m] + q;
+          const double corr = h1 * (F1[a - s1] - F1[a]) + h2 * (F2[a - s2] - F2[a]);
+          cl[m] = UL[a] + corr;
+          cr[m] = UR[a] + corr;
+        }
+        ch::cons2prim(G, cl[0], cl[1], cl[2], cl[3], cl[4], wl);   // U^{n+1/2}_L(c,d): right state of the low face
+        ch::cons2prim(G, cr[0], cr[1], cr[2], cr[3], cr[4], wr);   // U^{n+1/2}_R(c,d): left state of the high face
+      }
+      double nb[5], fl[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+      if (d < 2) {
+#pragma unroll
+        for (int m = 0; m < 5; ++m) sX[m][tid] = wr[m];
+        __syncthreads();
+        const int src = d == 0 ? (tid > 0 ? tid - 1 : 0) : (tid >= kFX ? tid - kFX : tid);
+#pragma unroll
+        for (int m = 0; m < 5; ++m) nb[m] = sX[m][src];
+      } else {
+#pragma unroll
+        for (int m = 0; m < 5; ++m) nb[m] = zU[m][tid];
+      }
+      if (solve) ch::riemann_exact(G, nb, wl, fl);
+      if (d < 2) {
+#pragma unroll
+        for (int m = 0; m < 5; ++m) sF[m][tid] = fl[m];
+        __syncthreads();
+        if (need2) {
+          const int dst = d == 0 ? tid + 1 : tid + kFX;
+          const double dtd = A.dtdx[d];
+          double t[5];
+#pragma unroll
+          for (int m = 0; m < 5; ++m) t[m] = dtd * (fl[m] - sF[m][dst]);
+          // direction-local -> global momentum order: x: (1,2,3), y: (3,1,2)
+          part[0] += t[0];
+          part[1] += d == 0 ? t[1] : t[3];
+          part[2] += d == 0 ? t[2] : t[1];
+          part[3] += d == 0 ? t[3] : t[2];
+          part[4] += t[4];
+        }
+      } else if (need2) {
+        if (k > k0) {
+          // finish cell k-1 (Eq. 24): z-local order (rho, mz, mx, my, E)
+          const double dtd = A.dtdx[2];
+          const long long qm = q - g.st[2];
+          const double v0 = zP[0][tid] + dtd * (zF[0][tid] - fl[0]);
+          const double v1 = zP[1][tid] + dtd * (zF[2][tid] - fl[2]);
+          const double v2 = zP[2][tid] + dtd * (zF[3][tid] - fl[3]);
+          const double v3 = zP[3][tid] + dtd * (zF[1][tid] - fl[1]);
+          const double v4 = zP[4][tid] + dtd * (zF[4][tid] - fl[4]);
+          A.u[qm] = v0; A.u[np + qm] = v1; A.u[2 * np + qm] = v2; A.u[3 * np + qm] = v3; A.u[4 * np + qm] = v4;
+          const double t = cell_dt(A, v0, v1, v2, v3, v4, bad);
+          tmin = t < tmin ? t : tmin;
+        }
+#pragma unroll
+        for (int m = 0; m < 5; ++m) { zU[m][tid] = wr[m]; zF[m][tid] = fl[m]; zP[m][tid] = part[m]; }
+      }
+    }
+  }
+  block_min_reduce(tmin, bad, A.red);
+}
+
+// ---------------------------------------------------------------------------------------------
 // Ghost fill (readings S6, S7).  Filling x, then y over the padded x extent, then z over
 // the padded x,y extent makes every ghost cell a copy of the real cell obtained by mapping
 // each coordinate on its own, with the sign of each reflected normal momentum flipped; so one
@@ -486,6 +639,7 @@ struct ch_ctx {
   unsigned long long* h_red = nullptr;   // pinned, 16 bytes
   long long launches = 0;
   int march_seg = 64;
+  int final_seg = 64;
   // optional per-kernel timing (ch_profile): one event pair per kernel kind
   bool profiling = false;
   cudaEvent_t ev[2 * CH_K_COUNT] = {};
@@ -535,7 +689,7 @@ StepArgs make_args(const ch_ctx* c, double dt) {
 }
 
 const char* const kKernelNames[CH_K_COUNT] = {"k_reset", "k_pass1_x", "k_pass1_march<y>", "k_pass1_march<z>",
-                                              "k_pass2", "k_update", "k_ghost", "k_dt"};
+                                              "k_pass2", "k_update", "k_ghost", "k_dt", "k_final3d"};
 
 // event brackets around one launch when profiling is on (no-ops otherwise)
 struct Bracket {
@@ -607,6 +761,8 @@ ch_ctx* ch_init(int nx, int ny, int nz, int nghost, double gamma, const int* bc)
   if (!c) { fail(CH_EINVAL, "ch_init: out of host memory"); return nullptr; }
   c->geo = g;
   c->nghost = nghost;
+  if (const char* e = std::getenv("CH_MARCH_SEG")) { const int v = std::atoi(e); if (v >= 4) c->march_seg = v; }   // tuning knob
+  if (const char* e = std::getenv("CH_FINAL_SEG")) { const int v = std::atoi(e); if (v >= 4) c->final_seg = v; }
   for (int s = 0; s < 6; ++s) {
     c->bc[s] = bc ? bc[s] : CH_BC_PERIODIC;
     if (g.act[s / 2] && (c->bc[s] < 1 || c->bc[s] > 3)) { delete c; fail(CH_EINVAL, "ch_init: bad boundary code"); return nullptr; }
@@ -758,22 +914,36 @@ int ch_step(ch_ctx* c, double dt) {
     const int T = 3 - d;
     const long long cols = (long long)(g.act[0] ? g.n[0] + 2 : 1) * (g.act[T] ? g.n[T] + 2 : 1);
     const int seg = c->march_seg;
-    dim3 grid((unsigned)((cols + 127) / 128), (unsigned)((g.n[d] + 1 + seg - 1) / seg));
+    dim3 grid((unsigned)((cols + CH_MARCH_T - 1) / CH_MARCH_T), (unsigned)((g.n[d] + 1 + seg - 1) / seg));
     Bracket b(c, d == 1 ? CH_K_PASS1_Y : CH_K_PASS1_Z);
-    if (d == 1) k_pass1_march<1><<<grid, 128, 0, st>>>(A, seg);
-    else k_pass1_march<2><<<grid, 128, 0, st>>>(A, seg);
+    if (d == 1) k_pass1_march<1><<<grid, CH_MARCH_T, 0, st>>>(A, seg);
+    else k_pass1_march<2><<<grid, CH_MARCH_T, 0, st>>>(A, seg);
   }
   CH_CUDA(cudaGetLastError(), "pass 1");
-  {
-    const long long cells = (long long)(g.act[0] ? g.n[0] + 1 : 1) * (g.act[1] ? g.n[1] + 1 : 1) * (g.act[2] ? g.n[2] + 1 : 1);
-    Bracket b(c, CH_K_PASS2);
-    k_pass2<<<(unsigned)((cells + 127) / 128), 128, 0, st>>>(A);
-  }
-  {
-    const long long N = (long long)g.n[0] * g.n[1] * g.n[2];
-    Bracket b(c, CH_K_UPDATE);
-    k_update<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(A);
-  }
+  if (g.act[0] && g.act[1] && g.act[2]) {
+    const int seg = c->final_seg;
+    dim3 grid((unsigned)((g.n[0] + kFX - 3) / (kFX - 2)), (unsigned)((g.n[1] + kFY - 3) / (kFY - 2)),
+              (unsigned)((g.n[2] + seg - 1) / seg));
+    const size_t smem = (size_t)25 * kFT * sizeof(double);
+    static bool attr_set = false;
+    if (!attr_set) {
+      CH_CUDA(cudaFuncSetAttribute(k_final3d, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem), "k_final3d smem attribute");
+      attr_set = true;
+    }
+    Bracket b(c, CH_K_FINAL);
+    k_final3d<<<grid, kFT, smem, st>>>(A, seg);
+  } else {
+    {
+      const long long cells = (long long)(g.act[0] ? g.n[0] + 1 : 1) * (g.act[1] ? g.n[1] + 1 : 1) * (g.act[2] ? g.n[2] + 1 : 1);
+      Bracket b(c, CH_K_PASS2);
+      k_pass2<<<(unsigned)((cells + CH_P2_T - 1) / CH_P2_T), CH_P2_T, 0, st>>>(A);
+    }
+    {
+      const long long N = (long long)g.n[0] * g.n[1] * g.n[2];
+      Bracket b(c, CH_K_UPDATE);
+      k_update<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(A);
+    }
+}
   CH_CUDA(cudaGetLastError(), "pass 2 / update");
   int rc = launch_ghost(c, A);
   if (rc) return rc;

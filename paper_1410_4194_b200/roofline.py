@@ -23,6 +23,7 @@ ALG_FLOPS = {
     "k_pass1_march<z>": 0.0,
     "k_pass2": 0.0,
     "k_update": 0.0,
+    "k_final3d": 0.0,
 }
 # FP64-pipe instructions (DADD + DMUL + DFMA) per real cell-update, same provenance.
 ALG_INST = dict(ALG_FLOPS)
