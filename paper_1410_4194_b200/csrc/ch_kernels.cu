@@ -427,23 +427,46 @@ __global__ void __launch_bounds__(256) k_update(const StepArgs A) {
 // run through one rolled copy of the solver (instruction cache).
 // ---------------------------------------------------------------------------------------------
 #ifndef CH_F_TY
-#define CH_F_TY 8
+#define CH_F_TY 16
 #endif
 #ifndef CH_F_MINB
-#define CH_F_MINB 3
+#define CH_F_MINB 1
 #endif
 constexpr int kFX = 32, kFY = CH_F_TY, kFT = kFX * kFY;
+
+// Corrected face states of cell q along D (Eq. 23): U^{n+1/2}_{L,R}(c,D) = U*_{L,R}(c,D) + dF_{D+1} + dF_{D+2}
+// with dF_e[f] = dt/(2 dx_e) [F*_e(c - e) - F*_e(c)] in global field order; primitive, D-local order out.
+template <int D>
+__device__ __forceinline__ void face_states(const StepArgs& A, long long q, const double (&dF)[3][5], double wl[5],
+                                            double wr[5]) {
+  constexpr int D1 = (D + 1) % 3, D2 = (D + 2) % 3;
+  const long long np = A.geo.np;
+  const double* __restrict__ UL = A.UL[D];
+  const double* __restrict__ UR = A.UR[D];
+  double cl[5], cr[5];
+#pragma unroll
+  for (int m = 0; m < 5; ++m) {
+    constexpr int dummy = 0; (void)dummy;
+    const int f = comp<D>(m);
+    const double corr = dF[D1][f] + dF[D2][f];
+    cl[m] = UL[f * np + q] + corr;
+    cr[m] = UR[f * np + q] + corr;
+  }
+  ch::cons2prim(A.gas, cl[0], cl[1], cl[2], cl[3], cl[4], wl);
+  ch::cons2prim(A.gas, cr[0], cr[1], cr[2], cr[3], cr[4], wr);
+}
 
 __global__ void __launch_bounds__(kFT, CH_F_MINB) k_final3d(const StepArgs A, int seg) {
   extern __shared__ double s_final[];
   typedef double (*Arr)[kFT];
-  Arr sX = reinterpret_cast<Arr>(s_final);              // exchanged right-face primitive state of the sweep direction
-  Arr sF = reinterpret_cast<Arr>(s_final + 5 * kFT);    // exchanged low-face flux
+  Arr sX = reinterpret_cast<Arr>(s_final);              // exchanged right-face primitive state along y
+  Arr sF = reinterpret_cast<Arr>(s_final + 5 * kFT);    // exchanged low-face y flux
   Arr zU = reinterpret_cast<Arr>(s_final + 10 * kFT);   // carried: U^{n+1/2}_R(., z) of cell k-1, primitive, z-local order
   Arr zF = reinterpret_cast<Arr>(s_final + 15 * kFT);   // carried: H^{n+1/2} on the low z face of cell k-1, z-local order
   Arr zP = reinterpret_cast<Arr>(s_final + 20 * kFT);   // carried: u + x and y flux differences of cell k-1, global order
   const Geom& g = A.geo;
   const Gas& G = A.gas;
+  const unsigned full = 0xffffffffu;
   const int tid = threadIdx.x, lane = tid & 31, row = tid >> 5;
   const int nx = g.n[0], ny = g.n[1], nz = g.n[2];
   const int i = (int)blockIdx.x * (kFX - 2) - 1 + lane;
@@ -456,92 +479,91 @@ __global__ void __launch_bounds__(kFT, CH_F_MINB) k_final3d(const StepArgs A, in
   const bool need0 = valid && updR, need1 = valid && updL, need2 = updL && updR;
   const bool solve0 = need0 && lane >= 1 && i >= 0, solve1 = need1 && row >= 1 && j >= 0;
   const long long np = g.np;
-  const long long qcol = (long long)(i + g.g[0]) + (long long)(j + g.g[1]) * g.st[1] + (long long)g.g[2] * g.st[2];
+  const long long s1 = g.st[1], s2 = g.st[2];
+  const long long qcol = (long long)(i + g.g[0]) + (long long)(j + g.g[1]) * s1 + (long long)g.g[2] * s2;
+  const double hx = 0.5 * A.dtdx[0], hy = 0.5 * A.dtdx[1], hz = 0.5 * A.dtdx[2];
   double tmin = __longlong_as_double(0x7FF0000000000000LL);
   bool bad = false;
 
   for (int k = k0 - 1; k <= k1; ++k) {
-    const bool first = k == k0 - 1, tail = k == k1;
-    const long long q = qcol + (long long)k * g.st[2];
-    double part[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
-    if (need2 && !first && !tail) {
+    const bool first = k == k0 - 1, tail = k == k1, mid = !first && !tail;
+    const long long q = qcol + (long long)k * s2;
+    // transverse flux differences of this cell (each feeds four of its six face states)
+    double dF[3][5];
+    if (need0 || need1) {
 #pragma unroll
-      for (int f = 0; f < 5; ++f) part[f] = A.u[f * np + q];
+      for (int f = 0; f < 5; ++f) {
+        const long long a = f * np + q;
+        dF[0][f] = hx * (A.Fs[0][a - 1] - A.Fs[0][a]);
+        dF[1][f] = hy * (A.Fs[1][a - s1] - A.Fs[1][a]);
+        dF[2][f] = hz * (A.Fs[2][a - s2] - A.Fs[2][a]);
+      }
     }
-#pragma unroll 1
-    for (int d = (first || tail) ? 2 : 0; d < 3; ++d) {
-      const int d1 = d == 2 ? 0 : d + 1, d2 = d == 0 ? 2 : d - 1;
-      const bool need = d == 0 ? need0 : d == 1 ? need1 : need2;
-      const bool solve = d == 0 ? solve0 : d == 1 ? solve1 : (need2 && !first);
-      const long long f1 = (long long)(1 + d) * np, f2 = (long long)(1 + d1) * np, f3 = (long long)(1 + d2) * np;
-      double wl[5] = {1.0, 0.0, 0.0, 0.0, 1.0}, wr[5] = {1.0, 0.0, 0.0, 0.0, 1.0};
-      if (need) {
-        // Eq. 23: both face states of cell c along d get the same two transverse flux differences
-        const double* __restrict__ F1 = A.Fs[d1];
-        const double* __restrict__ F2 = A.Fs[d2];
-        const double* __restrict__ UL = A.UL[d];
-        const double* __restrict__ UR = A.UR[d];
-        const long long s1 = g.st[d1], s2 = g.st[d2];
-        const double h1 = 0.5 * A.dtdx[d1], h2 = 0.5 * A.dtdx[d2];
-        const long long off[5] = {0, f1, f2, f3, 4 * np};
-        double cl[5], cr[5];
+    double part[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+    if (mid) {
+      if (need2) {
+#pragma unroll
+        for (int f = 0; f < 5; ++f) part[f] = A.u[f * np + q];
+      }
+      {   // ---- x: neighbours are lanes of the same warp
+        double wl[5] = {1.0, 0.0, 0.0, 0.0, 1.0}, wr[5] = {1.0, 0.0, 0.0, 0.0, 1.0}, nb[5], fl[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+        if (need0) face_states<0>(A, q, dF, wl, wr);
+#pragma unroll
+        for (int m = 0; m < 5; ++m) nb[m] = __shfl_up_sync(full, wr[m], 1);
+        if (solve0) ch::riemann_exact(G, nb, wl, fl);
 #pragma unroll
         for (int m = 0; m < 5; ++m) {
-          const long long a = off[m] + q;
-          const double corr = h1 * (F1[a - s1] - F1[a]) + h2 * (F2[a - s2] - F2[a]);
-          cl[m] = UL[a] + corr;
-          cr[m] = UR[a] + corr;
+          const double hi = __shfl_down_sync(full, fl[m], 1);
+          part[m] += A.dtdx[0] * (fl[m] - hi);      // x-local order is the global order
         }
-        ch::cons2prim(G, cl[0], cl[1], cl[2], cl[3], cl[4], wl);   // U^{n+1/2}_L(c,d): right state of the low face
-        ch::cons2prim(G, cr[0], cr[1], cr[2], cr[3], cr[4], wr);   // U^{n+1/2}_R(c,d): left state of the high face
       }
-      double nb[5], fl[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
-      if (d < 2) {
+      {   // ---- y: neighbours are rows of the CTA
+        double wl[5] = {1.0, 0.0, 0.0, 0.0, 1.0}, wr[5] = {1.0, 0.0, 0.0, 0.0, 1.0}, nb[5], fl[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+        if (need1) face_states<1>(A, q, dF, wl, wr);
 #pragma unroll
         for (int m = 0; m < 5; ++m) sX[m][tid] = wr[m];
         __syncthreads();
-        const int src = d == 0 ? (tid > 0 ? tid - 1 : 0) : (tid >= kFX ? tid - kFX : tid);
+        const int src = tid >= kFX ? tid - kFX : tid;
 #pragma unroll
         for (int m = 0; m < 5; ++m) nb[m] = sX[m][src];
-      } else {
-#pragma unroll
-        for (int m = 0; m < 5; ++m) nb[m] = zU[m][tid];
-      }
-      if (solve) ch::riemann_exact(G, nb, wl, fl);
-      if (d < 2) {
+        if (solve1) ch::riemann_exact(G, nb, wl, fl);
 #pragma unroll
         for (int m = 0; m < 5; ++m) sF[m][tid] = fl[m];
         __syncthreads();
         if (need2) {
-          const int dst = d == 0 ? tid + 1 : tid + kFX;
-          const double dtd = A.dtdx[d];
-          double t[5];
-#pragma unroll
-          for (int m = 0; m < 5; ++m) t[m] = dtd * (fl[m] - sF[m][dst]);
-          // direction-local -> global momentum order: x: (1,2,3), y: (3,1,2)
-          part[0] += t[0];
-          part[1] += d == 0 ? t[1] : t[3];
-          part[2] += d == 0 ? t[2] : t[1];
-          part[3] += d == 0 ? t[3] : t[2];
-          part[4] += t[4];
+          const int dst = tid + kFX;
+          // y-local order (rho, my, mz, mx, E) -> global
+          part[0] += A.dtdx[1] * (fl[0] - sF[0][dst]);
+          part[2] += A.dtdx[1] * (fl[1] - sF[1][dst]);
+          part[3] += A.dtdx[1] * (fl[2] - sF[2][dst]);
+          part[1] += A.dtdx[1] * (fl[3] - sF[3][dst]);
+          part[4] += A.dtdx[1] * (fl[4] - sF[4][dst]);
         }
-      } else if (need2) {
-        if (k > k0) {
-          // finish cell k-1 (Eq. 24): z-local order (rho, mz, mx, my, E)
-          const double dtd = A.dtdx[2];
-          const long long qm = q - g.st[2];
-          const double v0 = zP[0][tid] + dtd * (zF[0][tid] - fl[0]);
-          const double v1 = zP[1][tid] + dtd * (zF[2][tid] - fl[2]);
-          const double v2 = zP[2][tid] + dtd * (zF[3][tid] - fl[3]);
-          const double v3 = zP[3][tid] + dtd * (zF[1][tid] - fl[1]);
-          const double v4 = zP[4][tid] + dtd * (zF[4][tid] - fl[4]);
-          A.u[qm] = v0; A.u[np + qm] = v1; A.u[2 * np + qm] = v2; A.u[3 * np + qm] = v3; A.u[4 * np + qm] = v4;
-          const double t = cell_dt(A, v0, v1, v2, v3, v4, bad);
-          tmin = t < tmin ? t : tmin;
-        }
-#pragma unroll
-        for (int m = 0; m < 5; ++m) { zU[m][tid] = wr[m]; zF[m][tid] = fl[m]; zP[m][tid] = part[m]; }
       }
+    }
+    if (need2) {   // ---- z: the neighbour is this thread's previous step
+      double wl[5], wr[5], nb[5], fl[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+      face_states<2>(A, q, dF, wl, wr);
+      if (!first) {
+#pragma unroll
+        for (int m = 0; m < 5; ++m) nb[m] = zU[m][tid];
+        ch::riemann_exact(G, nb, wl, fl);
+      }
+      if (k > k0) {
+        // finish cell k-1 (Eq. 24): z-local order (rho, mz, mx, my, E)
+        const double dtd = A.dtdx[2];
+        const long long qm = q - s2;
+        const double v0 = zP[0][tid] + dtd * (zF[0][tid] - fl[0]);
+        const double v1 = zP[1][tid] + dtd * (zF[2][tid] - fl[2]);
+        const double v2 = zP[2][tid] + dtd * (zF[3][tid] - fl[3]);
+        const double v3 = zP[3][tid] + dtd * (zF[1][tid] - fl[1]);
+        const double v4 = zP[4][tid] + dtd * (zF[4][tid] - fl[4]);
+        A.u[qm] = v0; A.u[np + qm] = v1; A.u[2 * np + qm] = v2; A.u[3 * np + qm] = v3; A.u[4 * np + qm] = v4;
+        const double t = cell_dt(A, v0, v1, v2, v3, v4, bad);
+        tmin = t < tmin ? t : tmin;
+      }
+#pragma unroll
+      for (int m = 0; m < 5; ++m) { zU[m][tid] = wr[m]; zF[m][tid] = fl[m]; zP[m][tid] = part[m]; }
     }
   }
   block_min_reduce(tmin, bad, A.red);
