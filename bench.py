@@ -35,6 +35,8 @@ if ROOT not in sys.path:
 METRIC = "cell-updates/sec (fp64 CTU+PPM+exact Riemann)"
 UNIT = "cell-updates/s"
 CPU_SAMPLE_N = 128          # the oracle is timed on a 128^3 corner of the workload
+# DRAM bytes per launch at 512^3 from the committed ncu --set full capture (profiles/r01e_*); None = not captured
+TRAFFIC_NCU = {}
 
 
 def parse():
@@ -263,23 +265,43 @@ def main():
 
     N, K = main_res["cells"], args.steps
     value = world * N * K / main_res["seconds"]
-    # dominant kernel and its ALU roofline
+    # per-kernel rooflines: the slower of HBM (algorithmic bytes / measured copy bandwidth) and FP64 ALU
+    # (algorithmic flops / DFMA rate measured above); DESIGN.md section 6
     kern = main_res["kernels"]
-    top = max((k for k in kern if k in rf.ALG_FLOPS), key=lambda k: kern[k]["ms_avg"] * kern[k]["launches_per_step"])
-    t_top = kern[top]["ms_avg"] * 1e-3
-    achieved = rf.ALG_FLOPS[top] * N / t_top / 1e12
+    hbm_gbs, hbm_src = rf.hbm_peak_gbs(ROOT)
     sm_mhz = (clocks or {}).get("sm_mhz") or 1965.0
-    roofline = {"bound": "alu", "kernel": top, "achieved": achieved, "peak": peak_tf, "unit": "TFLOP/s",
-                "frac": achieved / peak_tf, "traffic": None,
-                "peak_source": "measured: ch_fp64_peak_probe DFMA chains in this run (burst); nominal "
-                               f"148 SM x 64 lanes x 2 x {sm_mhz:.0f} MHz = {rf.nominal_fp64_tflops(sm_mhz):.1f}",
-                "alg_flops_per_cell": rf.ALG_FLOPS[top],
+    per_kernel, t_roof_step = {}, 0.0
+    for k, v in kern.items():
+        if k not in rf.ALG_BYTES:
+            continue
+        t = v["ms_avg"] * 1e-3
+        gbs = rf.ALG_BYTES[k] * N / t / 1e9
+        tfs = rf.ALG_FLOPS[k] * N / t / 1e12
+        t_h, t_a = rf.ALG_BYTES[k] * N / (hbm_gbs * 1e9), rf.ALG_FLOPS[k] * N / (peak_tf * 1e12)
+        t_roof_step += max(t_h, t_a) * v["launches_per_step"]
+        per_kernel[k] = {"ms": v["ms_avg"], "bound": "hbm" if t_h >= t_a else "alu",
+                         "hbm_GBps": gbs, "hbm_frac": gbs / hbm_gbs, "fp64_TFLOPs": tfs, "fp64_frac": tfs / peak_tf,
+                         "roofline_ms": max(t_h, t_a) * 1e3, "frac": max(t_h, t_a) / t}
+    top = max(per_kernel, key=lambda k: kern[k]["ms_avg"] * kern[k]["launches_per_step"])
+    pk = per_kernel[top]
+    if pk["bound"] == "hbm":
+        ach, peak, unit, psrc = pk["hbm_GBps"], hbm_gbs, "GB/s", hbm_src
+    else:
+        ach, peak, unit = pk["fp64_TFLOPs"], peak_tf, "TFLOP/s"
+        psrc = ("measured: ch_fp64_peak_probe DFMA chains in this run (burst); nominal 148 SM x 64 lanes x 2 x "
+                f"{sm_mhz:.0f} MHz = {rf.nominal_fp64_tflops(sm_mhz):.1f}")
+    step_ms = main_res["seconds"] / K * 1e3
+    roofline = {"bound": pk["bound"], "kernel": top, "achieved": ach, "peak": peak, "unit": unit,
+                "frac": ach / peak, "traffic": TRAFFIC_NCU.get(top),
+                "traffic_note": "dram__bytes_read.sum + dram__bytes_write.sum per launch from profiles/ (ncu --set full, 512^3)",
+                "peak_source": psrc,
+                "alg_bytes_per_cell": rf.ALG_BYTES[top], "alg_flops_per_cell": rf.ALG_FLOPS[top],
                 "kernel_ms": kern[top]["ms_avg"],
                 "kernel_share_of_step": kern[top]["ms_avg"] * kern[top]["launches_per_step"] / main_res["kernel_ms_per_step"],
-                "step": {"alg_flops_per_cell": sum(rf.ALG_FLOPS.values()),
-                         "achieved": sum(rf.ALG_FLOPS.values()) * N * K / main_res["seconds"] / 1e12,
-                         "frac": sum(rf.ALG_FLOPS.values()) * N * K / main_res["seconds"] / 1e12 / peak_tf},
-                "kernels": kern}
+                "fp64_peak_TFLOPs_measured": peak_tf, "hbm_peak_GBps": hbm_gbs,
+                "step": {"alg_bytes_per_cell": sum(rf.ALG_BYTES.values()), "alg_flops_per_cell": sum(rf.ALG_FLOPS.values()),
+                         "roofline_ms": t_roof_step * 1e3, "measured_ms": step_ms, "frac": t_roof_step * 1e3 / step_ms},
+                "kernels": per_kernel, "kernel_times": kern}
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": args.warmup,
             "ms_per_step": main_res["seconds"] / K * 1e3, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",

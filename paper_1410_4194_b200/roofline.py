@@ -1,39 +1,67 @@
-"""Roofline bookkeeping for bench.py: algorithmic FP64 work per cell-update and the peaks.
+"""Roofline bookkeeping for bench.py: algorithmic work per cell-update and the peaks.
 
-No arithmetic of the method lives here, only constants derived in DESIGN.md ("Roofline").
+No arithmetic of the method lives here, only constants derived in DESIGN.md §6 ("Roofline").
 
-The CTU + PPMC + exact-Riemann step is bound by the plain FP64 ALU pipe, not by HBM:
-at >= 4 k FP64-pipe instructions per cell-update and <= 2 kB of HBM traffic per cell-update the
-machine balance (FP64 peak / HBM peak) puts the ALU time well above the memory time.  bench.py
-therefore reports `"bound": "alu"`.
+Two ceilings bound every kernel of the step (north_star: "the slower of the two"):
 
-ALG_FLOPS[kernel] — algorithmic FP64 flops (DADD = DMUL = 1, DFMA = 2; division, square root,
-reciprocal square root, log and exp counted as the FP64-pipe instructions of their CUDA fast paths)
-per REAL cell-update, for the arithmetic each kernel is responsible for, every piece of the method
-done exactly once per cell / interface it is defined on (no halo recomputation).  Frozen from the
-ncu counts of the round-1 unfused kernels, which store every intermediate instead of recomputing it
-(profiles/r01_fp64_inst_counts.md); a later kernel that recomputes to save traffic executes MORE
-than this and is still charged only this.
+* HBM: ALG_BYTES[kernel] = bytes per REAL cell-update the kernel must move given the step's
+  decomposition into kernels (every array it consumes read once, every array it produces written
+  once, no halo re-reads) — against MEASURED_PEAKS.json's copy bandwidth;
+* FP64 ALU: ALG_FLOPS[kernel] = FP64 flops (DADD = DMUL = 1, DFMA = 2) per real cell-update, every
+  piece of the method done exactly once per cell / interface it is defined on (no halo
+  recomputation) — against the DFMA rate measured in the same run (ch_fp64_peak_probe).
+
+ALG_FLOPS / ALG_INST were frozen from the ncu thread-level counts
+(sm__sass_thread_inst_executed_op_{dadd,dmul,dfma}_pred_on.sum) of the round-1 kernels that compute
+each piece once with the present arithmetic (profiles/r01b_full_512_summary.txt: k_pass1_*, and
+k_pass2 + k_update for the second half), divided by 512^3.  k_final3d recomputes halo lanes / rows
+(32/30 x 16/14) and is still charged only the unfused count.
 """
 
-# (DADD + DMUL + 2*DFMA) per real cell-update at 256^3 on the throughput-sweep workload; see module doc.
-ALG_FLOPS = {
-    "k_pass1_x": 0.0,
-    "k_pass1_march<y>": 0.0,
-    "k_pass1_march<z>": 0.0,
-    "k_pass2": 0.0,
-    "k_update": 0.0,
-    "k_final3d": 0.0,
+# bytes per real cell-update (fp64 = 8 B): pass 1 reads u (5) and writes U*_L, U*_R, F* (15);
+# the fused second half reads U*_L, U*_R of three directions (30), F* (15) and u (5), writes u (5).
+ALG_BYTES = {
+    "k_pass1_x": 160.0,
+    "k_pass1_march<y>": 160.0,
+    "k_pass1_march<z>": 160.0,
+    "k_final3d": 440.0,
 }
-# FP64-pipe instructions (DADD + DMUL + DFMA) per real cell-update, same provenance.
-ALG_INST = dict(ALG_FLOPS)
+
+# (DADD + DMUL + 2*DFMA) per real cell-update at 512^3, throughput-sweep workload.
+ALG_FLOPS = {
+    "k_pass1_x": 683.0,
+    "k_pass1_march<y>": 690.7,
+    "k_pass1_march<z>": 690.7,
+    "k_final3d": 1270.5,      # k_pass2 (1094.6) + k_update (175.9) of the unfused path
+}
+
+# FP64-pipe arithmetic instructions (DADD + DMUL + DFMA) per real cell-update, same provenance.
+ALG_INST = {
+    "k_pass1_x": 505.3,
+    "k_pass1_march<y>": 511.3,
+    "k_pass1_march<z>": 511.4,
+    "k_final3d": 864.6,
+}
 
 # B200 plain-FP64 peak: 148 SMs x 64 FP64 lanes x 2 flop (FMA) x SM clock.  At the 1965 MHz
 # maximum that is 37.2 TFLOP/s; the measured figure comes from ch_fp64_peak_probe at run time
 # (8 independent DFMA chains per thread, 8 CTAs of 256 threads per SM).
 SMS = 148
 FP64_LANES_PER_SM = 64
+HBM_FALLBACK_GBS = 6453.1     # MEASURED_PEAKS.json on this pool (used only if the file is absent)
 
 
 def nominal_fp64_tflops(sm_mhz: float) -> float:
     return SMS * FP64_LANES_PER_SM * 2 * sm_mhz * 1e6 / 1e12
+
+
+def hbm_peak_gbs(root: str):
+    """(GB/s, source) — the driver-written measured copy bandwidth if present."""
+    import json
+    import os
+    p = os.path.join(root, "MEASURED_PEAKS.json")
+    try:
+        with open(p) as f:
+            return float(json.load(f)["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs (burst copy bandwidth)"
+    except (OSError, KeyError, ValueError):
+        return HBM_FALLBACK_GBS, "fallback: MEASURED_PEAKS.json absent, last driver-measured value for this pool"
