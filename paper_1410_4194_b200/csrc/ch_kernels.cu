@@ -68,6 +68,15 @@ __device__ __forceinline__ void load_prim(const Gas& G, const double* __restrict
   ch::cons2prim(G, d, mn, m1, m2, E, w);
 }
 
+template <int D>
+__device__ __forceinline__ void load_raw(const double* __restrict__ u, long long np, long long q, double r[5]) {
+  r[0] = u[q];
+  r[1] = u[comp<D>(1) * np + q];
+  r[2] = u[comp<D>(2) * np + q];
+  r[3] = u[comp<D>(3) * np + q];
+  r[4] = u[4 * np + q];
+}
+
 // store a direction-local conserved vector into a global-order SoA array
 template <int D>
 __device__ __forceinline__ void store_local(double* __restrict__ dst, long long np, long long q, const double c[5]) {
@@ -130,37 +139,39 @@ __global__ void __launch_bounds__(CH_MARCH_T, CH_MARCH_MINB) k_pass1_march(const
   double wa[5], wb[5], wc[5], wd[5];   // cells c-1, c, c+1, c+2 (rotating)
   double sa[5], sb[5], sc[5];          // slopes of c-1, c, c+1
   double icb, icc;                     // 1/(rho a) of c, c+1
-  double pr_prev[5];                   // previous cell's right-face primitive state
+  double pr_prev[5];                   // previous cell's right-face primitive state W*_R
+  double raw[5];                       // conserved values of the next cell to enter the stencil (loaded one step ahead)
   {
     double wz[5];
     load_prim<D>(G, u, np, base + (long long)(c0 - 2) * sD, wz);
     load_prim<D>(G, u, np, base + (long long)(c0 - 1) * sD, wa);
     load_prim<D>(G, u, np, base + (long long)(c0)*sD, wb);
     load_prim<D>(G, u, np, base + (long long)(c0 + 1) * sD, wc);
+    load_raw<D>(u, np, base + (long long)(c0 + 2) * sD, raw);
     ch::limited_slope(G, wz, wa, wb, ch::inv_rho_a(G, wa[0], wa[4]), sa);
     icb = ch::inv_rho_a(G, wb[0], wb[4]);
     ch::limited_slope(G, wa, wb, wc, icb, sb);
   }
   for (int c = c0; c <= c1; ++c) {
     const long long q = base + (long long)c * sD;
-    load_prim<D>(G, u, np, q + 2 * sD, wd);
+    ch::cons2prim(G, raw[0], raw[1], raw[2], raw[3], raw[4], wd);
+    if (c < c1) load_raw<D>(u, np, q + 3 * sD, raw);     // cell c+3 <= n_D+2: inside the padded store
     icc = ch::inv_rho_a(G, wc[0], wc[4]);
     ch::limited_slope(G, wb, wc, wd, icc, sc);
     double WLs[5], WRs[5], cl[5], cr[5];
     ch::ppmc_faces(G, dtdx, wa, wb, wc, sa, sb, sc, icb, WLs, WRs);
-    ch::prim2cons(G, WLs, cl);
+    ch::prim2cons(G, WLs, cl);     // states are kept conserved between stages
     ch::prim2cons(G, WRs, cr);
     if (c < c1 || last) {
       store_local<D>(A.UL[D], np, q, cl);
       store_local<D>(A.UR[D], np, q, cr);
     }
     if (c > c0) {
-      double wl[5], fl[5];
-      ch::cons2prim(G, cl[0], cl[1], cl[2], cl[3], cl[4], wl);   // states are kept conserved between stages
-      ch::riemann_exact(G, pr_prev, wl, fl);
+      double fl[5];
+      ch::riemann_exact(G, pr_prev, WLs, fl);      // the solver's first act would be conserved -> primitive
       store_local<D>(A.Fs[D], np, q - sD, fl);
     }
-    ch::cons2prim(G, cr[0], cr[1], cr[2], cr[3], cr[4], pr_prev);
+    copy5(pr_prev, WRs);
     copy5(wa, wb); copy5(wb, wc); copy5(wc, wd);
     copy5(sa, sb); copy5(sb, sc);
     icb = icc;
@@ -231,8 +242,8 @@ __global__ void __launch_bounds__(kXT, CH_X_MINB) k_pass1_x(const StepArgs A, lo
     // trailing cell kXT-3 that no later window covers as a face-only slot: both write the same value
     store_local<0>(A.UL[0], np, q, cl);
     store_local<0>(A.UR[0], np, q, cr);
-    ch::cons2prim(G, cl[0], cl[1], cl[2], cl[3], cl[4], prL);
-    ch::cons2prim(G, cr[0], cr[1], cr[2], cr[3], cr[4], prR);
+    copy5(prL, WLs);     // the solver's first act would be conserved -> primitive
+    copy5(prR, WRs);
   }
 #pragma unroll
   for (int m = 0; m < 5; ++m) sL[m][tid] = prL[m];
