@@ -167,6 +167,7 @@ def timed_steps(G, cfl, steps, stream_events):
 def bench_size(pkg, wl, n, steps, warmup, device, dist=None, profile=True, e2e=True):
     import numpy as np
     import torch
+    from paper_1410_4194_b200.driver import max_over_ranks
     w = wl.sweep(n)
     N = n ** 3
     G = pkg.Grid(n, n, n, 3, w.gamma, w.bc, device=device)
@@ -181,10 +182,8 @@ def bench_size(pkg, wl, n, steps, warmup, device, dist=None, profile=True, e2e=T
     el = timed_steps(G, w.cfl, steps, ev)
     launches = G.kernel_launches - n0
     if dist is not None:
-        t = torch.tensor([el], dtype=torch.float64, device=device)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        el = max_over_ranks(el, dist, device)
         dist.barrier()
-        el = float(t.item())
     out = dict(n=n, seconds=el, launches=launches, cells=N, gamma=w.gamma, cfl=w.cfl)
     if profile:
         # same K steps again with an event pair around every kernel (ch_profile): per-kernel durations
@@ -212,9 +211,7 @@ def bench_size(pkg, wl, n, steps, warmup, device, dist=None, profile=True, e2e=T
             G.get_state(h_out)                                                  # synchronises
         t_e2e = time.perf_counter() - t0
         if dist is not None:
-            t = torch.tensor([t_e2e], dtype=torch.float64, device=device)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            t_e2e = float(t.item())
+            t_e2e = max_over_ranks(t_e2e, dist, device)
         out["e2e"] = dict(seconds=t_e2e, steps=k_e2e, h2d=h_in.numel() * 8, d2h=h_out.numel() * 8)
         assert bool(torch.isfinite(h_out).all())
         del h_in, h_out

@@ -41,3 +41,21 @@ def run(grid, wl, max_steps=None, dts=None, record_dts=None, set_state=True):
         t += dt
         n += 1
     return n, t
+
+
+def max_over_ranks(seconds: float, dist=None, device="cpu") -> float:
+    """Elapsed time of the slowest rank (bench.py: the whole job's time when every rank steps its own
+    replica).  `dist` is torch.distributed once initialised (nccl on GPUs, gloo in the CPU tests), or
+    None for a single process.  The only collective on the path: a MAX all-reduce of one double."""
+    if dist is None or not dist.is_initialized() or dist.get_world_size() == 1:
+        return float(seconds)
+    import torch
+    t = torch.tensor([seconds], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_rate(units_per_rank: float, seconds: float, dist=None, device="cpu") -> float:
+    """Whole-job throughput of N independent replicas: all ranks' units / the slowest rank's time."""
+    world = 1 if dist is None or not dist.is_initialized() else dist.get_world_size()
+    return world * units_per_rank / max_over_ranks(seconds, dist, device)
