@@ -36,7 +36,7 @@ METRIC = "cell-updates/sec (fp64 CTU+PPM+exact Riemann)"
 UNIT = "cell-updates/s"
 CPU_SAMPLE_N = 128          # the oracle is timed on a 128^3 corner of the workload
 # DRAM bytes per launch at 512^3 from the committed ncu --set full capture (profiles/r01e_*); None = not captured
-TRAFFIC_NCU = {}
+TRAFFIC_NCU = {"k_pass1_x": 21.93e9, "k_pass1_march<y>": 22.53e9, "k_pass1_march<z>": 22.75e9, "k_final3d": 64.11e9}
 
 
 def parse():
