@@ -102,10 +102,10 @@ __device__ __forceinline__ void copy5(double dst[5], const double src[5]) {
 #define CH_MARCH_T 128   // threads per CTA of the marching kernels
 #endif
 #ifndef CH_MARCH_MINB
-#define CH_MARCH_MINB 1
+#define CH_MARCH_MINB 3
 #endif
 #ifndef CH_X_MINB
-#define CH_X_MINB 1
+#define CH_X_MINB 3
 #endif
 #ifndef CH_P2_T
 #define CH_P2_T 128
