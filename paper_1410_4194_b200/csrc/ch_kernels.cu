@@ -43,12 +43,13 @@ struct StepArgs {
   Gas gas;
   double dtdx[3];    // dt / dx_d
   double dx[3];
+  double idx[3];     // 1 / dx_d
   double* u;         // state [5][np]
   double* Fs[3];     // first-pass fluxes F*_d at interface c+1/2 stored at c  [5][np]
   double* UL[3];     // U*_L(c,d): traced state at the left face of cell c     [5][np]
   double* UR[3];     // U*_R(c,d)
   double* Fh[3];     // CTU fluxes F^{n+1/2}_d                                 [5][np]
-  unsigned long long* red;  // [0] = bits of min dt_cell, [1] = non-physical flag
+  unsigned long long* red;  // [0] = bits of max cell rate (|v_d|+a)/dx_d, [1] = non-physical flag
 };
 
 // global component index of direction-local component m for a sweep along D (cyclic)
@@ -322,65 +323,79 @@ __global__ void __launch_bounds__(CH_P2_T, CH_P2_MINB) k_pass2(const StepArgs A)
 }
 
 // ---------------------------------------------------------------------------------------------
-// Eq. 22 per cell, evaluated with explicitly rounded operations (no FMA contraction) so that the
-// reduced minimum does not depend on how the compiler fuses: dt is a pure function of the state.
-// Returns dx_d/(|v_d|+a) minimised over active d; sets bad for rho<=0 / non-finite input.
+// Eq. 22 per cell, reduced in inverted form: the grid maximum of
+//     R_cell = max over active d of (|v_d| + a) / dx_d,        dt = cfl / max R_cell,
+// which is Eq. 22's  cfl * min dx_d/(|v_d|+a)  with ONE division for the whole grid instead of three
+// per cell.  Every operation is explicitly rounded (no FMA contraction) and the quotients and the
+// square root are brought to the correctly rounded value by one residual correction on top of the
+// MUFU-seeded reciprocal (Markstein), so |v_d| + a is the IEEE value the oracle computes and R_cell
+// is a pure function of the state: the fused update kernels and the standalone k_dt agree bitwise,
+// and dt agrees with Eq. 22 evaluated in IEEE arithmetic to <= 2 ulp (1/dx_d, the product and the final
+// reciprocal each round once).  Sets bad for rho <= 0 / non-finite input.
 // ---------------------------------------------------------------------------------------------
-__device__ __forceinline__ double cell_dt(const StepArgs& A, double d, double m0, double m1, double m2, double E,
-                                          bool& bad) {
-  const double inf = __longlong_as_double(0x7FF0000000000000LL);
-  if (!(d > 0.0) || !isfinite(d) || !isfinite(E)) { bad = true; return inf; }
-  const double vx = __ddiv_rn(m0, d), vy = __ddiv_rn(m1, d), vz = __ddiv_rn(m2, d);
+__device__ __forceinline__ double div_rn(double n, double d, double r) {   // n/d given r ~ 1/d
+  const double q = __dmul_rn(n, r);
+  return __fma_rn(__fma_rn(-q, d, n), r, q);
+}
+
+__device__ __forceinline__ double cell_rate(const StepArgs& A, double d, double m0, double m1, double m2, double E,
+                                            bool& bad) {
+  if (!(d > 0.0) || !isfinite(d) || !isfinite(E)) { bad = true; return 0.0; }
+  const double r = ch::rcp(d);
+  const double vx = div_rn(m0, d, r), vy = div_rn(m1, d, r), vz = div_rn(m2, d, r);
   const double v2 = __dadd_rn(__dadd_rn(__dmul_rn(vx, vx), __dmul_rn(vy, vy)), __dmul_rn(vz, vz));
   const double ke = __dmul_rn(__dmul_rn(0.5, d), v2);                       // Eq. 7
   double p = __dmul_rn(A.gas.gm1, __dadd_rn(E, -ke));                        // Eq. 6, 8
   if (!(p >= ch::kPFloor)) p = (p != p) ? p : ch::kPFloor;
-  const double a = __dsqrt_rn(__ddiv_rn(__dmul_rn(A.gas.gamma, p), d));      // Eq. 21
-  double tmin = inf;
+  const double a2 = div_rn(__dmul_rn(A.gas.gamma, p), d, r);                 // Eq. 21
+  const double y = ch::rsqrt_pos(a2);
+  const double s0 = __dmul_rn(a2, y);
+  const double a = __fma_rn(__fma_rn(-s0, s0, a2), __dmul_rn(0.5, y), s0);
+  double rmax = 0.0;
   const double v[3] = {vx, vy, vz};
 #pragma unroll
   for (int e = 0; e < 3; ++e) {
     if (!A.geo.act[e]) continue;
-    const double t = __ddiv_rn(A.dx[e], __dadd_rn(fabs(v[e]), a));
+    const double t = __dmul_rn(__dadd_rn(fabs(v[e]), a), A.idx[e]);
     if (t != t) bad = true;
-    if (t < tmin) tmin = t;
+    if (t > rmax) rmax = t;
   }
-  return tmin;
+  return rmax;
 }
 
-__device__ __forceinline__ void block_min_reduce(double t, bool bad, unsigned long long* red) {
-  __shared__ double s_min[32];
+__device__ __forceinline__ void block_max_reduce(double t, bool bad, unsigned long long* red) {
+  __shared__ double s_max[32];
   __shared__ int s_bad;
   if (threadIdx.x == 0) s_bad = 0;
   __syncthreads();
 #pragma unroll
-  for (int o = 16; o > 0; o >>= 1) t = fmin(t, __shfl_xor_sync(0xffffffffu, t, o));
+  for (int o = 16; o > 0; o >>= 1) t = fmax(t, __shfl_xor_sync(0xffffffffu, t, o));
   if (__any_sync(0xffffffffu, bad) && (threadIdx.x & 31) == 0) s_bad = 1;
-  if ((threadIdx.x & 31) == 0) s_min[threadIdx.x >> 5] = t;
+  if ((threadIdx.x & 31) == 0) s_max[threadIdx.x >> 5] = t;
   __syncthreads();
   if (threadIdx.x < 32) {
     const int nw = (blockDim.x + 31) >> 5;
-    double v = threadIdx.x < nw ? s_min[threadIdx.x] : __longlong_as_double(0x7FF0000000000000LL);
+    double v = threadIdx.x < nw ? s_max[threadIdx.x] : 0.0;
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v = fmin(v, __shfl_xor_sync(0xffffffffu, v, o));
+    for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
     if (threadIdx.x == 0) {
-      // positive doubles order like their bit patterns: a single-pass grid reduction with one
-      // atomicMin per CTA, deterministic because min is exact
-      atomicMin(red, (unsigned long long)__double_as_longlong(v));
+      // non-negative doubles order like their bit patterns: a single-pass grid reduction with one
+      // atomicMax per CTA, deterministic because max is exact
+      atomicMax(red, (unsigned long long)__double_as_longlong(v));
       if (s_bad) atomicOr(red + 1, 1ULL);
     }
   }
 }
 
 __global__ void __launch_bounds__(256) k_reset(unsigned long long* red) {
-  if (threadIdx.x == 0) { red[0] = 0x7FF0000000000000ULL; red[1] = 0ULL; }
+  if (threadIdx.x == 0) { red[0] = 0ULL; red[1] = 0ULL; }
 }
 
 // Standalone Eq. 22 reduction over real cells (used after ch_set_state / ch_set_padded).
 __global__ void __launch_bounds__(256) k_dt(const StepArgs A) {
   const Geom& g = A.geo;
   const long long N = (long long)g.n[0] * g.n[1] * g.n[2];
-  double tmin = __longlong_as_double(0x7FF0000000000000LL);
+  double tmin = 0.0;   // running maximum of the cell rates
   bool bad = false;
   for (long long id = (long long)blockIdx.x * blockDim.x + threadIdx.x; id < N; id += (long long)gridDim.x * blockDim.x) {
     const int i = (int)(id % g.n[0]);
@@ -388,10 +403,10 @@ __global__ void __launch_bounds__(256) k_dt(const StepArgs A) {
     const int j = (int)(r % g.n[1]);
     const int k = (int)(r / g.n[1]);
     const long long q = (long long)(i + g.g[0]) + (long long)(j + g.g[1]) * g.st[1] + (long long)(k + g.g[2]) * g.st[2];
-    const double t = cell_dt(A, A.u[q], A.u[g.np + q], A.u[2 * g.np + q], A.u[3 * g.np + q], A.u[4 * g.np + q], bad);
-    tmin = fmin(tmin, t);
+    const double t = cell_rate(A, A.u[q], A.u[g.np + q], A.u[2 * g.np + q], A.u[3 * g.np + q], A.u[4 * g.np + q], bad);
+    tmin = fmax(tmin, t);
   }
-  block_min_reduce(tmin, bad, A.red);
+  block_max_reduce(tmin, bad, A.red);
 }
 
 // Eq. 24 on real cells, fused with the Eq. 22 reduction of the updated state.
@@ -399,7 +414,7 @@ __global__ void __launch_bounds__(256) k_update(const StepArgs A) {
   const Geom& g = A.geo;
   const long long N = (long long)g.n[0] * g.n[1] * g.n[2];
   const long long id = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  double t = __longlong_as_double(0x7FF0000000000000LL);
+  double t = 0.0;
   bool bad = false;
   if (id < N) {
     const int i = (int)(id % g.n[0]);
@@ -417,9 +432,9 @@ __global__ void __launch_bounds__(256) k_update(const StepArgs A) {
       v[f] = x;
       A.u[f * g.np + q] = x;
     }
-    t = cell_dt(A, v[0], v[1], v[2], v[3], v[4], bad);
+    t = cell_rate(A, v[0], v[1], v[2], v[3], v[4], bad);
   }
-  block_min_reduce(t, bad, A.red);
+  block_max_reduce(t, bad, A.red);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -493,7 +508,7 @@ __global__ void __launch_bounds__(kFT, CH_F_MINB) k_final3d(const StepArgs A, in
   const long long s1 = g.st[1], s2 = g.st[2];
   const long long qcol = (long long)(i + g.g[0]) + (long long)(j + g.g[1]) * s1 + (long long)g.g[2] * s2;
   const double hx = 0.5 * A.dtdx[0], hy = 0.5 * A.dtdx[1], hz = 0.5 * A.dtdx[2];
-  double tmin = __longlong_as_double(0x7FF0000000000000LL);
+  double tmin = 0.0;   // running maximum of the cell rates (Eq. 22 inverted)
   bool bad = false;
 
   for (int k = k0 - 1; k <= k1; ++k) {
@@ -570,14 +585,14 @@ __global__ void __launch_bounds__(kFT, CH_F_MINB) k_final3d(const StepArgs A, in
         const double v3 = zP[3][tid] + dtd * (zF[1][tid] - fl[1]);
         const double v4 = zP[4][tid] + dtd * (zF[4][tid] - fl[4]);
         A.u[qm] = v0; A.u[np + qm] = v1; A.u[2 * np + qm] = v2; A.u[3 * np + qm] = v3; A.u[4 * np + qm] = v4;
-        const double t = cell_dt(A, v0, v1, v2, v3, v4, bad);
-        tmin = t < tmin ? t : tmin;
+        const double t = cell_rate(A, v0, v1, v2, v3, v4, bad);
+        tmin = t > tmin ? t : tmin;
       }
 #pragma unroll
       for (int m = 0; m < 5; ++m) { zU[m][tid] = wr[m]; zF[m][tid] = fl[m]; zP[m][tid] = part[m]; }
     }
   }
-  block_min_reduce(tmin, bad, A.red);
+  block_max_reduce(tmin, bad, A.red);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -708,7 +723,7 @@ bool geometry(int nx, int ny, int nz, int nghost, Geom& g) {
 StepArgs make_args(const ch_ctx* c, double dt) {
   StepArgs A;
   A.geo = c->geo; A.gas = c->gas;
-  for (int d = 0; d < 3; ++d) { A.dx[d] = c->dx[d]; A.dtdx[d] = dt / c->dx[d]; }
+  for (int d = 0; d < 3; ++d) { A.dx[d] = c->dx[d]; A.idx[d] = 1.0 / c->dx[d]; A.dtdx[d] = dt / c->dx[d]; }
   A.u = c->state;
   const long long blk = 5 * c->geo.np;
   for (int d = 0; d < 3; ++d) {
@@ -918,9 +933,9 @@ double ch_compute_dt(ch_ctx* c, double cfl) {
   if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
   if (e != cudaSuccess) { cuda_fail(e, "ch_compute_dt read-back"); return nan; }
   if (c->h_red[1] != 0ULL) { fail(CH_ENONPHYS, "ch_compute_dt: non-physical cell (rho <= 0 or non-finite)"); return nan; }
-  double m;
-  std::memcpy(&m, &c->h_red[0], 8);
-  return cfl * m;
+  double rate;                                  // grid maximum of (|v_d| + a) / dx_d
+  std::memcpy(&rate, &c->h_red[0], 8);
+  return cfl * (1.0 / rate);
 }
 
 int ch_step(ch_ctx* c, double dt) {
