@@ -490,6 +490,7 @@ __global__ void __launch_bounds__(kFT, CH_F_MINB) k_final3d(const StepArgs A, in
   Arr zU = reinterpret_cast<Arr>(s_final + 10 * kFT);   // carried: U^{n+1/2}_R(., z) of cell k-1, primitive, z-local order
   Arr zF = reinterpret_cast<Arr>(s_final + 15 * kFT);   // carried: H^{n+1/2} on the low z face of cell k-1, z-local order
   Arr zP = reinterpret_cast<Arr>(s_final + 20 * kFT);   // carried: u + x and y flux differences of cell k-1, global order
+  Arr zS = reinterpret_cast<Arr>(s_final + 25 * kFT);   // carried: F*_z of cell k-1 (global field order)
   const Geom& g = A.geo;
   const Gas& G = A.gas;
   const unsigned full = 0xffffffffu;
@@ -514,15 +515,29 @@ __global__ void __launch_bounds__(kFT, CH_F_MINB) k_final3d(const StepArgs A, in
   for (int k = k0 - 1; k <= k1; ++k) {
     const bool first = k == k0 - 1, tail = k == k1, mid = !first && !tail;
     const long long q = qcol + (long long)k * s2;
-    // transverse flux differences of this cell (each feeds four of its six face states)
+    // transverse flux differences of this cell (each feeds four of its six face states).  Of the six
+    // first-pass fluxes per field only F*_d(c) and F*_y(c - y) are loaded: F*_x(c - x) is lane-1's F*_x(c)
+    // (lane 0 loads it), F*_z(c - z) is what this thread loaded one plane ago (kept in shared memory).
     double dF[3][5];
-    if (need0 || need1) {
+    {
+      double fx[5] = {0.0, 0.0, 0.0, 0.0, 0.0}, fxm[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+      if (valid) {
+#pragma unroll
+        for (int f = 0; f < 5; ++f) {
+          const long long a = f * np + q;
+          fx[f] = A.Fs[0][a];
+          if (lane == 0) fxm[f] = A.Fs[0][a - 1];
+          const double fz = A.Fs[2][a];
+          const double fzm = first ? A.Fs[2][a - s2] : zS[f][tid];
+          zS[f][tid] = fz;
+          dF[1][f] = hy * (A.Fs[1][a - s1] - A.Fs[1][a]);
+          dF[2][f] = hz * (fzm - fz);
+        }
+      }
 #pragma unroll
       for (int f = 0; f < 5; ++f) {
-        const long long a = f * np + q;
-        dF[0][f] = hx * (A.Fs[0][a - 1] - A.Fs[0][a]);
-        dF[1][f] = hy * (A.Fs[1][a - s1] - A.Fs[1][a]);
-        dF[2][f] = hz * (A.Fs[2][a - s2] - A.Fs[2][a]);
+        const double t = __shfl_up_sync(full, fx[f], 1);
+        dF[0][f] = hx * ((lane == 0 ? fxm[f] : t) - fx[f]);
       }
     }
     double part[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
@@ -972,7 +987,7 @@ int ch_step(ch_ctx* c, double dt) {
     const int seg = c->final_seg;
     dim3 grid((unsigned)((g.n[0] + kFX - 3) / (kFX - 2)), (unsigned)((g.n[1] + kFY - 3) / (kFY - 2)),
               (unsigned)((g.n[2] + seg - 1) / seg));
-    const size_t smem = (size_t)25 * kFT * sizeof(double);
+    const size_t smem = (size_t)30 * kFT * sizeof(double);
     static bool attr_set = false;
     if (!attr_set) {
       CH_CUDA(cudaFuncSetAttribute(k_final3d, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem), "k_final3d smem attribute");
