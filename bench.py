@@ -35,8 +35,8 @@ if ROOT not in sys.path:
 METRIC = "cell-updates/sec (fp64 CTU+PPM+exact Riemann)"
 UNIT = "cell-updates/s"
 CPU_SAMPLE_N = 128          # the oracle is timed on a 128^3 corner of the workload
-# DRAM bytes per launch at 512^3 from the committed ncu --set full capture (profiles/r01e_*); None = not captured
-TRAFFIC_NCU = {"k_pass1_x": 21.93e9, "k_pass1_march<y>": 22.53e9, "k_pass1_march<z>": 22.75e9, "k_final3d": 64.11e9}
+# DRAM bytes per launch at 512^3 from the committed ncu --set full capture (profiles/r01f_*); None = not captured
+TRAFFIC_NCU = {"k_pass1_x": 21.98e9, "k_pass1_march<y>": 22.73e9, "k_pass1_march<z>": 22.96e9, "k_final3d": 68.02e9}
 
 
 def parse():
@@ -49,6 +49,7 @@ def parse():
     ap.add_argument("--impl", type=str, default="b200", choices=["b200", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-other-workloads", action="store_true")
     return ap.parse_args()
 
 
@@ -255,6 +256,24 @@ def main():
                 r, _ = bench_size(pkg, wl, s, args.steps, args.warmup, device, None, profile=False, e2e=False)
                 others[str(s)] = {"value": r["cells"] * args.steps / r["seconds"], "unit": UNIT,
                                   "ms_per_step": r["seconds"] / args.steps * 1e3}
+    other_wl = {}
+    if world == 1 and not args.no_other_workloads:
+        # strong shocks change Newton iteration counts and warp divergence: the smooth sweep alone flatters the
+        # solver, so configs 3 and 4 are timed beside it (state after `pre` steps)
+        for name, make, pre, k in (("sedov_128 (config 3)", lambda: wl.sedov(128), 20, 20),
+                                   ("shock_cloud_256 (config 4)", lambda: wl.shock_cloud(256), 10, 10)):
+            ww = make()
+            G = pkg.Grid(*ww.shape, 3, ww.gamma, ww.bc, device=device)
+            G.set_state(torch.from_numpy(ww.u).to(device))
+            for _ in range(pre):
+                G.step(G.compute_dt(ww.cfl))
+            ev = (torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+            sec = timed_steps(G, ww.cfl, k, ev)
+            other_wl[name] = {"value": ww.u[0].size * k / sec, "unit": UNIT, "ms_per_step": sec / k * 1e3,
+                              "steps": k, "after_steps": pre}
+            G.close()
+            del G
+            torch.cuda.empty_cache()
     if rank != 0:
         if dist is not None:
             dist.destroy_process_group()
@@ -309,6 +328,8 @@ def main():
             "gpu_launches": main_res["launches"], "clocks": clocks, "roofline": roofline}
     if others:
         line["other_sizes"] = others
+    if other_wl:
+        line["other_workloads"] = other_wl
     if "e2e" in main_res:
         e = main_res["e2e"]
         line["e2e"] = {"value": world * N * e["steps"] / e["seconds"], "unit": UNIT,

@@ -53,7 +53,7 @@ typedef struct ch_buffers {
   double* state;          /* padded conserved store u, 5*Np doubles (SoA, x fastest) */
   void* workspace;        /* scratch, at least ch_workspace_bytes(...) bytes, 256-byte aligned */
   size_t workspace_bytes; /* size of `workspace` as allocated */
-  void* reduce;           /* 64 bytes, 8-byte aligned: device cells of the dt reduction */
+  void* reduce;           /* 64 bytes, 8-byte aligned: device cells of the dt reduction (max wave rate, flag) */
 } ch_buffers;
 
 /* ch_init — create a context for an nx*ny*nz grid of real cells with `nghost` ghost layers on each
@@ -104,12 +104,15 @@ int ch_set_padded(ch_ctx* ctx, const double* up);
 int ch_get_padded(ch_ctx* ctx, double* up);
 
 /* ch_compute_dt — Eq. 22: returns cfl * min over real cells and active directions d of
- * dx_d / (|v_d| + a), a = sqrt(gamma p / rho) (Eq. 21), p floored at 1e-20.  Synchronises
- * the stream (one 16-byte device-to-host copy).  When ch_step has already reduced the wave speeds
- * of the current state inside its update kernel, no further pass over the grid is made.
- * Returns NaN and sets CH_ENONPHYS if any real cell has rho <= 0 or a non-finite rho or E; NaN with
- * CH_EINVAL if cfl is not in (0,1]; NaN with CH_ESTATE if no state is set.  The paper's stability
- * bound for the 3-D six-solve CTU is cfl < 0.5: documented, not enforced. */
+ * dx_d / (|v_d| + a), a = sqrt(gamma p / rho) (Eq. 21), p floored at 1e-20.  The device
+ * reduces the equivalent grid MAXIMUM of (|v_d| + a) / dx_d (one value per CTA, one atomic) and the
+ * host takes the single reciprocal; |v_d| + a is evaluated with correctly rounded quotients and
+ * square root, so the result agrees with Eq. 22 in IEEE arithmetic to <= 2 ulp and is a pure function
+ * of the state.  Synchronises the stream (one 16-byte device-to-host copy).  When ch_step has already
+ * reduced the wave speeds of the current state inside its update kernel, no further pass over the
+ * grid is made.  Returns NaN and sets CH_ENONPHYS if any real cell has rho <= 0 or a non-finite rho
+ * or E; NaN with CH_EINVAL if cfl is not in (0,1]; NaN with CH_ESTATE if no state is set.  The
+ * paper's stability bound for the 3-D six-solve CTU is cfl < 0.5: documented, not enforced. */
 double ch_compute_dt(ch_ctx* ctx, double cfl);
 
 /* ch_step — advance the state by one CTU step of size dt (steps 1-5): PPMC
@@ -130,7 +133,7 @@ long long ch_kernel_launches(const ch_ctx* ctx);
 /* Kernel kinds of one step, for ch_profile_read / ch_kernel_name. */
 enum {
   CH_K_RESET = 0, CH_K_PASS1_X, CH_K_PASS1_Y, CH_K_PASS1_Z, CH_K_PASS2, CH_K_UPDATE, CH_K_GHOST, CH_K_DT,
-  CH_K_FINAL,
+  CH_K_FINAL, /* fused pass 2 + update of 3-D grids */
   CH_K_COUNT
 };
 

@@ -4,13 +4,13 @@
 //   k_reset            reset the dt reduction cells
 //   k_pass1_x          PPMC + tracing + exact Riemann along x   -> U*_L,U*_R(.,x), F*      (steps 1-2)
 //   k_pass1_march<1|2> same along y / z, marching in registers  -> U*_L,U*_R(.,d), G*, H*
-//   k_pass2            Eq. 23 transverse correction + second exact Riemann pass -> F,G,H^{n+1/2} (3-4)
-//   k_update           Eq. 24 conservative update + Eq. 22 wave-speed reduction of the new state (5)
+//   k_final3d          3-D grids: Eq. 23 transverse correction + second exact Riemann pass + Eq. 24
+//                      update + Eq. 22 reduction of the new state, fused (steps 3-5; F,G,H^{n+1/2} stay on chip)
+//   k_pass2, k_update  the same two halves unfused, for 1-D / 2-D grids
 //   k_ghost            ghost fill of the new state
 // Data layout: struct-of-arrays fp64, x fastest, ghosts included; every kernel maps
-// consecutive lanes to consecutive x so loads and stores coalesce.  The work is FP64-pipe bound
-// (see DESIGN.md §Roofline), so intermediates that cross kernels go through HBM/L2 as plain
-// coalesced arrays and no operand is reshaped for tensor cores.
+// consecutive lanes to consecutive x so loads and stores coalesce.  No operand is reshaped for
+// tensor cores: this is a stencil / ALU path.
 #include <cuda_runtime.h>
 
 #include <cmath>
@@ -453,33 +453,50 @@ __global__ void __launch_bounds__(256) k_update(const StepArgs A) {
 // run through one rolled copy of the solver (instruction cache).
 // ---------------------------------------------------------------------------------------------
 #ifndef CH_F_TY
-#define CH_F_TY 16
+#define CH_F_TY 10
 #endif
 #ifndef CH_F_MINB
-#define CH_F_MINB 1
+#define CH_F_MINB 2
 #endif
 constexpr int kFX = 32, kFY = CH_F_TY, kFT = kFX * kFY;
 
 // Corrected face states of cell q along D (Eq. 23): U^{n+1/2}_{L,R}(c,D) = U*_{L,R}(c,D) + dF_{D+1} + dF_{D+2}
 // with dF_e[f] = dt/(2 dx_e) [F*_e(c - e) - F*_e(c)] in global field order; primitive, D-local order out.
 template <int D>
-__device__ __forceinline__ void face_states(const StepArgs& A, long long q, const double (&dF)[3][5], double wl[5],
-                                            double wr[5]) {
-  constexpr int D1 = (D + 1) % 3, D2 = (D + 2) % 3;
+__device__ __forceinline__ void load_faces(const StepArgs& A, long long q, double ul[5], double ur[5]) {
   const long long np = A.geo.np;
   const double* __restrict__ UL = A.UL[D];
   const double* __restrict__ UR = A.UR[D];
+#pragma unroll
+  for (int m = 0; m < 5; ++m) {
+    const int f = comp<D>(m);
+    ul[m] = UL[f * np + q];
+    ur[m] = UR[f * np + q];
+  }
+}
+
+template <int D>
+__device__ __forceinline__ void correct_faces(const StepArgs& A, const double ul[5], const double ur[5],
+                                              const double (&dF)[3][5], double wl[5], double wr[5]) {
+  constexpr int D1 = (D + 1) % 3, D2 = (D + 2) % 3;
   double cl[5], cr[5];
 #pragma unroll
   for (int m = 0; m < 5; ++m) {
-    constexpr int dummy = 0; (void)dummy;
     const int f = comp<D>(m);
     const double corr = dF[D1][f] + dF[D2][f];
-    cl[m] = UL[f * np + q] + corr;
-    cr[m] = UR[f * np + q] + corr;
+    cl[m] = ul[m] + corr;
+    cr[m] = ur[m] + corr;
   }
   ch::cons2prim(A.gas, cl[0], cl[1], cl[2], cl[3], cl[4], wl);
   ch::cons2prim(A.gas, cr[0], cr[1], cr[2], cr[3], cr[4], wr);
+}
+
+template <int D>
+__device__ __forceinline__ void face_states(const StepArgs& A, long long q, const double (&dF)[3][5], double wl[5],
+                                            double wr[5]) {
+  double ul[5], ur[5];
+  load_faces<D>(A, q, ul, ur);
+  correct_faces<D>(A, ul, ur, dF, wl, wr);
 }
 
 __global__ void __launch_bounds__(kFT, CH_F_MINB) k_final3d(const StepArgs A, int seg) {
@@ -703,6 +720,7 @@ struct ch_ctx {
   long long launches = 0;
   int march_seg = 64;
   int final_seg = 64;
+  bool unfused = false;      // CH_UNFUSED=1: k_pass2 + k_update on 3-D grids too (A/B measurements, instruction counts)
   // optional per-kernel timing (ch_profile): one event pair per kernel kind
   bool profiling = false;
   cudaEvent_t ev[2 * CH_K_COUNT] = {};
@@ -825,6 +843,7 @@ ch_ctx* ch_init(int nx, int ny, int nz, int nghost, double gamma, const int* bc)
   c->geo = g;
   c->nghost = nghost;
   if (const char* e = std::getenv("CH_MARCH_SEG")) { const int v = std::atoi(e); if (v >= 4) c->march_seg = v; }   // tuning knob
+  if (const char* e = std::getenv("CH_UNFUSED")) c->unfused = std::atoi(e) != 0;
   if (const char* e = std::getenv("CH_FINAL_SEG")) { const int v = std::atoi(e); if (v >= 4) c->final_seg = v; }
   for (int s = 0; s < 6; ++s) {
     c->bc[s] = bc ? bc[s] : CH_BC_PERIODIC;
@@ -983,7 +1002,7 @@ int ch_step(ch_ctx* c, double dt) {
     else k_pass1_march<2><<<grid, CH_MARCH_T, 0, st>>>(A, seg);
   }
   CH_CUDA(cudaGetLastError(), "pass 1");
-  if (g.act[0] && g.act[1] && g.act[2]) {
+  if (g.act[0] && g.act[1] && g.act[2] && !c->unfused) {
     const int seg = c->final_seg;
     dim3 grid((unsigned)((g.n[0] + kFX - 3) / (kFX - 2)), (unsigned)((g.n[1] + kFY - 3) / (kFY - 2)),
               (unsigned)((g.n[2] + seg - 1) / seg));

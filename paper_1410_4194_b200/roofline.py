@@ -12,10 +12,11 @@ Two ceilings bound every kernel of the step (north_star: "the slower of the two"
   recomputation) — against the DFMA rate measured in the same run (ch_fp64_peak_probe).
 
 ALG_FLOPS / ALG_INST were frozen from the ncu thread-level counts
-(sm__sass_thread_inst_executed_op_{dadd,dmul,dfma}_pred_on.sum) of the round-1 kernels that compute
-each piece once with the present arithmetic (profiles/r01b_full_512_summary.txt: k_pass1_*, and
-k_pass2 + k_update for the second half), divided by 512^3.  k_final3d recomputes halo lanes / rows
-(32/30 x 16/14) and is still charged only the unfused count.
+(sm__sass_thread_inst_executed_op_{dadd,dmul,dfma}_pred_on.sum) of the kernels that compute each
+piece once with the present arithmetic, divided by 512^3: k_pass1_* from
+profiles/r01f_full_512_summary.txt, and the unfused k_pass2 + k_update (CH_UNFUSED=1,
+profiles/r01f_unfused_counts.csv) for the second half.  k_final3d recomputes halo lanes / rows
+(32/30 x 10/8) and is still charged only the unfused count.  Re-freeze whenever ch_hydro.cuh changes.
 """
 
 # bytes per real cell-update (fp64 = 8 B): pass 1 reads u (5) and writes U*_L, U*_R, F* (15);
@@ -29,18 +30,18 @@ ALG_BYTES = {
 
 # (DADD + DMUL + 2*DFMA) per real cell-update at 512^3, throughput-sweep workload.
 ALG_FLOPS = {
-    "k_pass1_x": 683.0,
-    "k_pass1_march<y>": 690.7,
-    "k_pass1_march<z>": 690.7,
-    "k_final3d": 1270.5,      # k_pass2 (1094.6) + k_update (175.9) of the unfused path
+    "k_pass1_x": 580.4,
+    "k_pass1_march<y>": 586.4,
+    "k_pass1_march<z>": 586.5,
+    "k_final3d": 1030.0,      # k_pass2 (929.0) + k_update (101.0) of the unfused path
 }
 
 # FP64-pipe arithmetic instructions (DADD + DMUL + DFMA) per real cell-update, same provenance.
 ALG_INST = {
-    "k_pass1_x": 505.3,
-    "k_pass1_march<y>": 511.3,
-    "k_pass1_march<z>": 511.4,
-    "k_final3d": 864.6,
+    "k_pass1_x": 442.3,
+    "k_pass1_march<y>": 446.9,
+    "k_pass1_march<z>": 446.9,
+    "k_final3d": 731.4,
 }
 
 # B200 plain-FP64 peak: 148 SMs x 64 FP64 lanes x 2 flop (FMA) x SM clock.  At the 1965 MHz
