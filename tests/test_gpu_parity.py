@@ -279,3 +279,78 @@ def test_kernel_launch_counter(ch):
     G.step(1e-3)
     assert G.kernel_launches - n0 >= 5
     G.close()
+
+
+# ---- determinism, memory safety, fused vs unfused second half ---------------------------------------
+def test_steps_are_bitwise_deterministic(ch):
+    """Two contexts fed the same state take bitwise identical steps (no race in the shared-memory
+    exchanges of k_pass1_x / k_final3d, no order-dependent reduction: min/max are exact)."""
+    for w in (wl.sweep(shape=(70, 45, 37)), wl.rough_random(37, 21, 13, seed=11, decades=0.5), wl.kelvin_helmholtz(64)):
+        outs, dts = [], []
+        for _ in range(2):
+            G = ch.Grid(*w.shape, 3, w.gamma, w.bc)
+            G.set_state(w.u)
+            for _ in range(3):
+                dt = G.compute_dt(w.cfl)
+                G.step(dt)
+            dts.append(G.compute_dt(w.cfl))
+            outs.append(G.get_padded())
+            G.close()
+        assert np.array_equal(outs[0], outs[1]) and dts[0] == dts[1]
+
+
+@pytest.mark.parametrize("shape", [(70, 45, 37), (33, 9, 1), (1, 20, 17), (50, 1, 1), (3, 3, 3)])
+def test_no_write_outside_the_bound_buffers(ch, shape):
+    """Guard bands around every buffer handed to ch_bind stay untouched through set_state, dt, steps, get_state."""
+    import torch
+    from paper_1410_4194_b200 import binding as B
+    L = ch.load_library()
+    nx, ny, nz = shape
+    w = wl.sweep(shape=shape)
+    h = L.ch_init(nx, ny, nz, 3, w.gamma, (B.C.c_int * 6)(*w.bc))
+    assert h
+    npad = L.ch_padded_cells(h)
+    ws_bytes = L.ch_workspace_bytes(nx, ny, nz, 3)
+    guard, sentinel = 4096, -1.2345e300
+    bufs = []
+    for n in (5 * npad, ws_bytes // 8, 8):
+        t = torch.full((n + 2 * guard,), sentinel, dtype=torch.float64, device="cuda")
+        bufs.append(t)
+    st = torch.cuda.current_stream()
+    bs = B.ChStruct(bufs[0][guard:].data_ptr(), bufs[1][guard:].data_ptr(), ws_bytes, bufs[2][guard:].data_ptr())
+    assert L.ch_bind(h, B.C.byref(bs), st.cuda_stream) == 0
+    u = np.ascontiguousarray(w.u)
+    assert L.ch_set_state(h, u.ctypes.data) == 0
+    for _ in range(2):
+        dt = L.ch_compute_dt(h, w.cfl)
+        assert dt > 0 and L.ch_step(h, dt) == 0
+    out = np.empty_like(u)
+    assert L.ch_get_state(h, out.ctypes.data) == 0 and np.all(np.isfinite(out))
+    L.ch_free(h)
+    for t, n in zip(bufs, (5 * npad, ws_bytes // 8, 8)):
+        assert bool((t[:guard] == sentinel).all()) and bool((t[guard + n:] == sentinel).all())
+
+
+def test_fused_and_unfused_second_half_agree(ch, ref, monkeypatch):
+    """k_final3d against k_pass2 + k_update (CH_UNFUSED=1) on the same 3-D state: both within the one-step
+    gate of the oracle, and of each other."""
+    w = wl.rough_random(37, 21, 13, seed=5, decades=0.5)
+    Rg = ref.RefGrid(*w.shape, 3, w.gamma, w.bc)
+    Rg.set_state(w.u)
+    dt = Rg.compute_dt(w.cfl)
+    Rg.step(dt)
+    ur = Rg.get_state()
+    res = {}
+    for mode in ("0", "1"):
+        monkeypatch.setenv("CH_UNFUSED", mode)
+        G = ch.Grid(*w.shape, 3, w.gamma, w.bc)
+        G.set_state(w.u)
+        n0 = G.kernel_launches
+        G.step(dt)
+        res[mode] = (G.get_state(), G.kernel_launches - n0, G.compute_dt(w.cfl))
+        G.close()
+    assert res["1"][1] == res["0"][1] + 1                       # one more kernel when unfused
+    for mode in res:
+        assert max(max_rel_error(res[mode][0], ur, w.gamma)) <= ONE_STEP_TOL
+    assert max(max_rel_error(res["0"][0], res["1"][0], w.gamma)) <= ONE_STEP_TOL
+    assert abs(res["0"][2] - res["1"][2]) <= 4 * np.spacing(res["0"][2])
