@@ -106,7 +106,7 @@ __device__ __forceinline__ void copy5(double dst[5], const double src[5]) {
 #define CH_MARCH_MINB 3
 #endif
 #ifndef CH_X_MINB
-#define CH_X_MINB 3
+#define CH_X_MINB 6
 #endif
 #ifndef CH_P2_T
 #define CH_P2_T 128
@@ -185,7 +185,10 @@ __global__ void __launch_bounds__(CH_MARCH_T, CH_MARCH_MINB) k_pass1_march(const
 // left-face states).  A CTA of T threads yields T-5 interfaces; lanes on cells outside the needed
 // ranges are masked so garbage row-crossing stencils cost nothing.
 // ---------------------------------------------------------------------------------------------
-constexpr int kXT = 256;       // threads per CTA
+#ifndef CH_X_T
+#define CH_X_T 128
+#endif
+constexpr int kXT = CH_X_T;    // threads per CTA
 constexpr int kXOut = kXT - 5; // interfaces produced per CTA
 
 __global__ void __launch_bounds__(kXT, CH_X_MINB) k_pass1_x(const StepArgs A, long long q_begin, long long q_end) {

@@ -23,7 +23,7 @@ pytestmark = pytest.mark.gpu
 
 def subbox_origins(n, m, rng, extra=6):
     lo, hi, mid = 0, n - m, (n - m) // 2
-    seams = [251 - m // 2, 64 - m // 2, 128 - m // 2]     # x-tile seam, march-segment seam, column-block seam
+    seams = [123 - m // 2, 64 - m // 2, 128 - m // 2]     # x-tile seam, march-segment seam, column-block seam
     pts = [(lo, lo, lo), (hi, hi, hi), (lo, hi, mid), (hi, lo, mid), (mid, mid, lo), (mid, mid, hi),
            (min(seams[0], hi), min(seams[1], hi), min(seams[2], hi)),
            (min(30 - m // 2, hi), min(8 - m // 2, hi), min(64 - m // 2, hi)),      # k_final3d tile seams: 30 x 8 x 64

@@ -10,7 +10,7 @@ Every test drives the CUDA library (paper_1410_4194_b200.Grid -> libch_b200.so) 
   fed to both) and free-running.
 
 Sizes are chosen so the oracle finishes in seconds while the grid still spans several CTA tiles
-in every kernel (x tiles of 251 interfaces, 128-column march blocks, 64-interface march
+in every kernel (x tiles of 123 interfaces, 128-column march blocks, 64-interface march
 segments) and leaves a ragged tail in each.
 """
 import math
