@@ -137,8 +137,11 @@ def test_conservation_2d_and_positivity(ref):
     assert np.all(u1[3] == 0.0) and np.all(u1[0] > 0)
 
 
+@pytest.mark.parametrize("aniso", [False, True])
 @pytest.mark.parametrize("axis", [0, 1, 2])
-def test_1d_embedded_in_3d_is_bitwise(ref, axis):
+def test_1d_embedded_in_3d_is_bitwise(ref, axis, aniso):
+    """aniso: the two transverse cell widths differ from the sweep's — the result must not notice, which pins
+    that the sweep along `axis` uses dx_axis (and only it) in tracing, update and nothing else."""
     n, m = 32, 4
     one = wl.sod(n)
     G1 = ref.RefGrid(n, 1, 1, 3, one.gamma, one.bc)
@@ -155,8 +158,14 @@ def test_1d_embedded_in_3d_is_bitwise(ref, axis):
     bc = tuple(O if d == axis else P for d in range(3) for _ in range(2))
     G3 = ref.RefGrid(*shape, 3, one.gamma, bc)
     # keep the same cell width as the 1-D run (reading S8 ties dx to nx)
-    G3.set_spacing(1.0 / n, 1.0 / n, 1.0 / n)
+    sp = [1.0 / n, 1.0 / n, 1.0 / n]
+    if aniso:
+        sp = [0.37, 0.011, 2.3]; sp[axis] = 1.0 / n
+    G3.set_spacing(*sp)
     G3.set_state(u3)
+    if aniso:                                  # Eq. 22 picks each direction's own width
+        a = np.sqrt(one.gamma * 1.0 / 1.0)      # fastest signal at t = 0: sound speed of the left state, v = 0
+        assert G3.compute_dt(0.4) == pytest.approx(0.4 * min(sp) / a, rel=1e-14)
     for dt in dts:
         G3.step(dt)
     out = G3.get_state()
