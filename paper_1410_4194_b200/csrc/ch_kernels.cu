@@ -11,6 +11,7 @@
 // Data layout: struct-of-arrays fp64, x fastest, ghosts included; every kernel maps
 // consecutive lanes to consecutive x so loads and stores coalesce.  No operand is reshaped for
 // tensor cores: this is a stencil / ALU path.
+#include <cuda.h>
 #include <cuda_runtime.h>
 
 #include <cmath>
@@ -631,6 +632,250 @@ __global__ void __launch_bounds__(kFT, CH_F_MINB) k_final3d(const StepArgs A, in
 }
 
 // ---------------------------------------------------------------------------------------------
+// TMA-fed form of k_final3d (used when the padded strides meet TMA's 16-byte rules).  Same tile, same
+// arithmetic, same exchanges; what changes is how a plane's 50 doubles per cell reach the SM: a
+// producer warp streams them as ten 4-D boxes {32 x, kTY y, 1 z, 5 fields} per plane
+// (cp.async.bulk.tensor, mbarrier complete_tx) into four staging groups in shared memory, in the order
+// the consumers use them — F* (flux differences), z states, x states + u, y states — and refills a
+// group for the next plane as soon as all 320 consumer threads have released it (empty mbarrier), so
+// the loads of plane k+1 run under the solves of plane k.
+// ---------------------------------------------------------------------------------------------
+#ifndef CH_T_TY
+#define CH_T_TY 11
+#endif
+constexpr int kTY = CH_T_TY, kTT = kFX * kTY;      // consumer threads; one more warp produces
+struct TmaMaps { CUtensorMap m[10]; };              // Fs0 Fs1 Fs2 | UL2 UR2 | UL0 UR0 u | UL1 UR1
+__device__ __forceinline__ constexpr int group_first(int q) { return q == 0 ? 0 : q == 1 ? 3 : q == 2 ? 5 : q == 3 ? 8 : 10; }   // arrays of group q: [first(q), first(q+1))
+
+__device__ __forceinline__ void mbar_init(unsigned bar, unsigned count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
+}
+__device__ __forceinline__ void mbar_arrive(unsigned bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned bar, unsigned bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "WAIT_LOOP:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@!p bra WAIT_LOOP;\n"
+      "}\n" ::"r"(bar), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void tma_load_4d(unsigned dst, const CUtensorMap* map, unsigned bar, int c0, int c1, int c2, int c3) {
+  asm volatile(
+      "cp.async.bulk.tensor.4d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6}], [%2];"
+      ::"r"(dst), "l"(map), "r"(bar), "r"(c0), "r"(c1), "r"(c2), "r"(c3) : "memory");
+}
+
+__global__ void __launch_bounds__(kTT + 32, 1) k_final3d_tma(const StepArgs A, const __grid_constant__ TmaMaps M, int seg) {
+  extern __shared__ __align__(1024) double s_t[];
+  __shared__ unsigned long long s_full[4], s_empty[4];
+  typedef double (*Arr)[kTT];
+  // staging: array a (0..9) holds its 5 fields as [f][row][lane] = [f][tid]
+  Arr sX = reinterpret_cast<Arr>(s_t + 50 * kTT);
+  Arr sF = reinterpret_cast<Arr>(s_t + 55 * kTT);
+  const Geom& g = A.geo;
+  const Gas& G = A.gas;
+  const unsigned full = 0xffffffffu;
+  const int tid = threadIdx.x, lane = tid & 31, row = tid >> 5;
+  const int nx = g.n[0], ny = g.n[1], nz = g.n[2];
+  const int i0 = (int)blockIdx.x * (kFX - 2) - 1, j0 = (int)blockIdx.y * (kTY - 2) - 1;
+  const int k0 = (int)blockIdx.z * seg;
+  const int k1 = min(k0 + seg, nz);
+  unsigned bfull[4], bempty[4];
+#pragma unroll
+  for (int q = 0; q < 4; ++q) {
+    bfull[q] = (unsigned)__cvta_generic_to_shared(&s_full[q]);
+    bempty[q] = (unsigned)__cvta_generic_to_shared(&s_empty[q]);
+  }
+  if (tid == 0) {
+#pragma unroll
+    for (int q = 0; q < 4; ++q) { mbar_init(bfull[q], 1); mbar_init(bempty[q], kTT); }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+
+  if (row == kTY) {
+    // ===== producer warp: one lane streams the planes =====
+    if (lane == 0) {
+      const unsigned stage = (unsigned)__cvta_generic_to_shared(s_t);
+      int n = 0;
+      for (int k = k0 - 1; k <= k1; ++k, ++n) {
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+          if (n > 0) mbar_wait(bempty[q], (unsigned)((n - 1) & 1));      // all consumers released plane k-1's copy
+          const int a0 = group_first(q), a1 = group_first(q + 1);
+          mbar_expect_tx(bfull[q], (unsigned)((a1 - a0) * 5 * kTT * sizeof(double)));
+          for (int a = a0; a < a1; ++a)
+            tma_load_4d(stage + (unsigned)(a * 5 * kTT * sizeof(double)), &M.m[a], bfull[q], i0 + g.g[0], j0 + g.g[1], k + g.g[2], 0);
+        }
+      }
+    }
+    return;
+  }
+
+  // ===== consumer warps =====
+  Arr stg = reinterpret_cast<Arr>(s_t);
+  const int i = i0 + lane, j = j0 + row;
+  const bool valid = i <= nx && j <= ny;
+  const bool realI = i >= 0 && i < nx, realJ = j >= 0 && j < ny;
+  const bool updL = lane >= 1 && lane <= kFX - 2 && realI, updR = row >= 1 && row <= kTY - 2 && realJ;
+  const bool need0 = valid && updR, need1 = valid && updL, need2 = updL && updR;
+  const bool solve0 = need0 && lane >= 1 && i >= 0, solve1 = need1 && row >= 1 && j >= 0;
+  const long long np = g.np, s2 = g.st[2];
+  const long long qcol = (long long)(i + g.g[0]) + (long long)(j + g.g[1]) * g.st[1] + (long long)g.g[2] * s2;
+  const double hx = 0.5 * A.dtdx[0], hy = 0.5 * A.dtdx[1], hz = 0.5 * A.dtdx[2];
+  double tmin = 0.0;
+  bool bad = false;
+  // carried from the previous plane (registers: one CTA per SM leaves ~150 per thread)
+  double zU[5] = {1.0, 0.0, 0.0, 0.0, 1.0};    // U^{n+1/2}_R(., z) of cell k-1, primitive, z-local order
+  double zF[5] = {0.0, 0.0, 0.0, 0.0, 0.0};    // H^{n+1/2} on the low z face of cell k-1, z-local order
+  double zP[5] = {0.0, 0.0, 0.0, 0.0, 0.0};    // u + x and y flux differences of cell k-1, global order
+  double zS[5] = {0.0, 0.0, 0.0, 0.0, 0.0};    // F*_z of cell k-1 (global field order)
+  int n = 0;
+  for (int k = k0 - 1; k <= k1; ++k, ++n) {
+    const bool first = k == k0 - 1, tail = k == k1, mid = !first && !tail;
+    const unsigned ph = (unsigned)(n & 1);
+    const long long q = qcol + (long long)k * s2;
+    // ---- group 0: first-pass fluxes -> transverse flux differences of this cell
+    double dF[3][5];
+    mbar_wait(bfull[0], ph);
+    {
+      double fx[5];
+#pragma unroll
+      for (int f = 0; f < 5; ++f) {
+        fx[f] = stg[f][tid];
+        const double fy = stg[5 + f][tid];
+        const double fym = stg[5 + f][row > 0 ? tid - kFX : tid];      // row 0 never uses its y difference
+        const double fz = stg[10 + f][tid];
+        const double fzm = zS[f];                                   // garbage on the first plane: unused there
+        zS[f] = fz;
+        dF[1][f] = hy * (fym - fy);
+        dF[2][f] = hz * (fzm - fz);
+      }
+      mbar_arrive(bempty[0]);
+#pragma unroll
+      for (int f = 0; f < 5; ++f) {
+        const double t = __shfl_up_sync(full, fx[f], 1);                 // lane 0 never uses its x difference
+        dF[0][f] = hx * (t - fx[f]);
+      }
+    }
+    // ---- group 1: z states; the neighbour is this thread's previous plane
+    double wrz[5] = {1.0, 0.0, 0.0, 0.0, 1.0}, flz[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+    mbar_wait(bfull[1], ph);
+    {
+      double ul[5], ur[5];
+#pragma unroll
+      for (int m = 0; m < 5; ++m) { ul[m] = stg[15 + comp<2>(m)][tid]; ur[m] = stg[20 + comp<2>(m)][tid]; }
+      mbar_arrive(bempty[1]);
+      if (need2) {
+        double wl[5], nb[5];
+        correct_faces<2>(A, ul, ur, dF, wl, wrz);
+        if (!first) {
+#pragma unroll
+          for (int m = 0; m < 5; ++m) nb[m] = zU[m];
+          ch::riemann_exact(G, nb, wl, flz);
+        }
+        if (k > k0) {
+          // finish cell k-1 (Eq. 24): z-local order (rho, mz, mx, my, E)
+          const double dtd = A.dtdx[2];
+          const long long qm = q - s2;
+          const double v0 = zP[0] + dtd * (zF[0] - flz[0]);
+          const double v1 = zP[1] + dtd * (zF[2] - flz[2]);
+          const double v2 = zP[2] + dtd * (zF[3] - flz[3]);
+          const double v3 = zP[3] + dtd * (zF[1] - flz[1]);
+          const double v4 = zP[4] + dtd * (zF[4] - flz[4]);
+          A.u[qm] = v0; A.u[np + qm] = v1; A.u[2 * np + qm] = v2; A.u[3 * np + qm] = v3; A.u[4 * np + qm] = v4;
+          const double t = cell_rate(A, v0, v1, v2, v3, v4, bad);
+          tmin = t > tmin ? t : tmin;
+        }
+      }
+    }
+    // ---- group 2: x states and u; neighbours are lanes of the same warp
+    double part[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+    mbar_wait(bfull[2], ph);
+    {
+      double ul[5], ur[5];
+#pragma unroll
+      for (int m = 0; m < 5; ++m) { ul[m] = stg[25 + m][tid]; ur[m] = stg[30 + m][tid]; part[m] = stg[35 + m][tid]; }
+      mbar_arrive(bempty[2]);
+      if (mid) {
+        double wl[5] = {1.0, 0.0, 0.0, 0.0, 1.0}, wr[5] = {1.0, 0.0, 0.0, 0.0, 1.0}, nb[5], fl[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+        if (need0) correct_faces<0>(A, ul, ur, dF, wl, wr);
+#pragma unroll
+        for (int m = 0; m < 5; ++m) nb[m] = __shfl_up_sync(full, wr[m], 1);
+        if (solve0) ch::riemann_exact(G, nb, wl, fl);
+#pragma unroll
+        for (int m = 0; m < 5; ++m) {
+          const double hi = __shfl_down_sync(full, fl[m], 1);
+          part[m] += A.dtdx[0] * (fl[m] - hi);      // x-local order is the global order
+        }
+      }
+    }
+    // ---- group 3: y states; neighbours are rows of the CTA
+    mbar_wait(bfull[3], ph);
+    {
+      double ul[5], ur[5];
+#pragma unroll
+      for (int m = 0; m < 5; ++m) { ul[m] = stg[40 + comp<1>(m)][tid]; ur[m] = stg[45 + comp<1>(m)][tid]; }
+      mbar_arrive(bempty[3]);
+      if (mid) {
+        double wl[5] = {1.0, 0.0, 0.0, 0.0, 1.0}, wr[5] = {1.0, 0.0, 0.0, 0.0, 1.0}, nb[5], fl[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+        if (need1) correct_faces<1>(A, ul, ur, dF, wl, wr);
+#pragma unroll
+        for (int m = 0; m < 5; ++m) sX[m][tid] = wr[m];
+        asm volatile("bar.sync 1, %0;" ::"n"(kTT) : "memory");
+        const int src = tid >= kFX ? tid - kFX : tid;
+#pragma unroll
+        for (int m = 0; m < 5; ++m) nb[m] = sX[m][src];
+        if (solve1) ch::riemann_exact(G, nb, wl, fl);
+#pragma unroll
+        for (int m = 0; m < 5; ++m) sF[m][tid] = fl[m];
+        asm volatile("bar.sync 1, %0;" ::"n"(kTT) : "memory");
+        if (need2) {
+          const int dst = tid + kFX;
+          // y-local order (rho, my, mz, mx, E) -> global
+          part[0] += A.dtdx[1] * (fl[0] - sF[0][dst]);
+          part[2] += A.dtdx[1] * (fl[1] - sF[1][dst]);
+          part[3] += A.dtdx[1] * (fl[2] - sF[2][dst]);
+          part[1] += A.dtdx[1] * (fl[3] - sF[3][dst]);
+          part[4] += A.dtdx[1] * (fl[4] - sF[4][dst]);
+        }
+      }
+    }
+    if (need2) {
+#pragma unroll
+      for (int m = 0; m < 5; ++m) { zU[m] = wrz[m]; zF[m] = flz[m]; zP[m] = part[m]; }
+    }
+  }
+  // Eq. 22 reduction over the consumer warps (the producer warp has left)
+  {
+    __shared__ double s_max[32];
+    __shared__ int s_badflag;
+    if (tid == 0) s_badflag = 0;
+    asm volatile("bar.sync 1, %0;" ::"n"(kTT) : "memory");
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) tmin = fmax(tmin, __shfl_xor_sync(full, tmin, o));
+    if (__any_sync(full, bad) && lane == 0) s_badflag = 1;
+    if (lane == 0) s_max[row] = tmin;
+    asm volatile("bar.sync 1, %0;" ::"n"(kTT) : "memory");
+    if (tid < 32) {
+      double v = tid < kTY ? s_max[tid] : 0.0;
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(full, v, o));
+      if (tid == 0) {
+        atomicMax(A.red, (unsigned long long)__double_as_longlong(v));
+        if (s_badflag) atomicOr(A.red + 1, 1ULL);
+      }
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
 // Ghost fill (readings S6, S7).  Filling x, then y over the padded x extent, then z over
 // the padded x,y extent makes every ghost cell a copy of the real cell obtained by mapping
 // each coordinate on its own, with the sign of each reflected normal momentum flipped; so one
@@ -723,6 +968,9 @@ struct ch_ctx {
   long long launches = 0;
   int march_seg = 64;
   int final_seg = 64;
+  bool use_tma = true;       // CH_TMA=0: plain-load k_final3d even where the TMA form applies
+  bool tma_ok = false;       // tensor maps built for the bound buffers
+  TmaMaps maps;
   bool unfused = false;      // CH_UNFUSED=1: k_pass2 + k_update on 3-D grids too (A/B measurements, instruction counts)
   // optional per-kernel timing (ch_profile): one event pair per kernel kind
   bool profiling = false;
@@ -829,6 +1077,41 @@ int copy_real(ch_ctx* c, double* user, bool to_device) {
   return CH_OK;
 }
 
+// Tensor maps of the ten arrays k_final3d_tma streams: each is [5][pz][py][px] fp64, box {32, kTY, 1, 5}.
+// TMA wants 16-byte aligned base addresses and strides: px and np even.  Returns false (plain-load kernel is
+// used instead) when that does not hold or the driver entry point is missing.
+bool build_tma_maps(ch_ctx* c) {
+  const Geom& g = c->geo;
+  if (!(g.act[0] && g.act[1] && g.act[2])) return false;
+  if ((g.pd[0] & 1) || (g.np & 1)) return false;
+  typedef CUresult (*EncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                               const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                               CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+  void* fn = nullptr;
+  cudaDriverEntryPointQueryResult qres;
+  if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn ||
+      qres != cudaDriverEntryPointSuccess) {
+    cudaGetLastError();
+    return false;
+  }
+  EncodeFn encode = reinterpret_cast<EncodeFn>(fn);
+  const long long blk = 5 * g.np;
+  double* Fs[3]; double* UL[3]; double* UR[3];
+  for (int d = 0; d < 3; ++d) { Fs[d] = c->ws + (long long)d * blk; UL[d] = c->ws + (long long)(3 + d) * blk; UR[d] = c->ws + (long long)(6 + d) * blk; }
+  double* arr[10] = {Fs[0], Fs[1], Fs[2], UL[2], UR[2], UL[0], UR[0], c->state, UL[1], UR[1]};
+  const cuuint64_t dims[4] = {(cuuint64_t)g.pd[0], (cuuint64_t)g.pd[1], (cuuint64_t)g.pd[2], 5};
+  const cuuint64_t strides[3] = {(cuuint64_t)g.pd[0] * 8, (cuuint64_t)g.st[2] * 8, (cuuint64_t)g.np * 8};
+  const cuuint32_t box[4] = {(cuuint32_t)kFX, (cuuint32_t)kTY, 1, 5};
+  const cuuint32_t estr[4] = {1, 1, 1, 1};
+  for (int a = 0; a < 10; ++a) {
+    if ((uintptr_t)arr[a] & 15) return false;
+    if (encode(&c->maps.m[a], CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, arr[a], dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+               CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+      return false;
+  }
+  return true;
+}
+
 }  // namespace
 
 extern "C" {
@@ -847,6 +1130,7 @@ ch_ctx* ch_init(int nx, int ny, int nz, int nghost, double gamma, const int* bc)
   c->nghost = nghost;
   if (const char* e = std::getenv("CH_MARCH_SEG")) { const int v = std::atoi(e); if (v >= 4) c->march_seg = v; }   // tuning knob
   if (const char* e = std::getenv("CH_UNFUSED")) c->unfused = std::atoi(e) != 0;
+  if (const char* e = std::getenv("CH_TMA")) c->use_tma = std::atoi(e) != 0;
   if (const char* e = std::getenv("CH_FINAL_SEG")) { const int v = std::atoi(e); if (v >= 4) c->final_seg = v; }
   for (int s = 0; s < 6; ++s) {
     c->bc[s] = bc ? bc[s] : CH_BC_PERIODIC;
@@ -909,6 +1193,7 @@ int ch_bind(ch_ctx* c, const ch_buffers* b, void* stream) {
   c->stream = static_cast<cudaStream_t>(stream);
   if (!c->h_red) CH_CUDA(cudaHostAlloc((void**)&c->h_red, 16, cudaHostAllocDefault), "cudaHostAlloc");
   c->bound = true; c->have_state = false; c->dt_valid = false;
+  c->tma_ok = build_tma_maps(c);
   return CH_OK;
 }
 
@@ -1009,6 +1294,18 @@ int ch_step(ch_ctx* c, double dt) {
     const int seg = c->final_seg;
     dim3 grid((unsigned)((g.n[0] + kFX - 3) / (kFX - 2)), (unsigned)((g.n[1] + kFY - 3) / (kFY - 2)),
               (unsigned)((g.n[2] + seg - 1) / seg));
+    if (c->tma_ok && c->use_tma) {
+      const size_t tsmem = (size_t)60 * kTT * sizeof(double);
+      static bool tattr_set = false;
+      if (!tattr_set) {
+        CH_CUDA(cudaFuncSetAttribute(k_final3d_tma, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tsmem), "k_final3d_tma smem attribute");
+        tattr_set = true;
+      }
+      dim3 tgrid((unsigned)((g.n[0] + kFX - 3) / (kFX - 2)), (unsigned)((g.n[1] + kTY - 3) / (kTY - 2)),
+                 (unsigned)((g.n[2] + seg - 1) / seg));
+      Bracket b(c, CH_K_FINAL);
+      k_final3d_tma<<<tgrid, kTT + 32, tsmem, st>>>(A, c->maps, seg);
+    } else {
     const size_t smem = (size_t)30 * kFT * sizeof(double);
     static bool attr_set = false;
     if (!attr_set) {
@@ -1017,6 +1314,7 @@ int ch_step(ch_ctx* c, double dt) {
     }
     Bracket b(c, CH_K_FINAL);
     k_final3d<<<grid, kFT, smem, st>>>(A, seg);
+    }
   } else {
     {
       const long long cells = (long long)(g.act[0] ? g.n[0] + 1 : 1) * (g.act[1] ? g.n[1] + 1 : 1) * (g.act[2] ? g.n[2] + 1 : 1);
