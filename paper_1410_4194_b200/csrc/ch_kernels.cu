@@ -4,8 +4,10 @@
 //   k_reset            reset the dt reduction cells
 //   k_pass1_x          PPMC + tracing + exact Riemann along x   -> U*_L,U*_R(.,x), F*      (steps 1-2)
 //   k_pass1_march<1|2> same along y / z, marching in registers  -> U*_L,U*_R(.,d), G*, H*
-//   k_final3d          3-D grids: Eq. 23 transverse correction + second exact Riemann pass + Eq. 24
-//                      update + Eq. 22 reduction of the new state, fused (steps 3-5; F,G,H^{n+1/2} stay on chip)
+//   k_final3d_tma      3-D grids: Eq. 23 transverse correction + second exact Riemann pass + Eq. 24
+//   (k_final3d)        update + Eq. 22 reduction of the new state, fused (steps 3-5; F,G,H^{n+1/2} stay on
+//                      chip); planes staged by TMA from a producer warp (plain loads where TMA's
+//                      16-byte stride rules do not hold, or with CH_TMA=0)
 //   k_pass2, k_update  the same two halves unfused, for 1-D / 2-D grids
 //   k_ghost            ghost fill of the new state
 // Data layout: struct-of-arrays fp64, x fastest, ghosts included; every kernel maps
