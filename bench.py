@@ -7,7 +7,7 @@ A "step" is one pass of the whole hot path over the grid: `dt = ch_compute_dt(cf
 `ch_step(dt)` (PPMC + exact Riemann in x, y, z; transverse correction; second Riemann pass; update;
 ghost fill).  Workload: BASELINE.json's throughput-sweep configuration (periodic box, gamma = 5/3,
 seeded sum of 8 random-phase sinusoids) at `--size`^3 (default 512, the largest size the metric is
-quoted on; 256^3 is reported beside it under "other_sizes").  The state (5.6 GB at 512^3) is far
+quoted on; 128^3, 256^3 and 384^3 are reported beside it under "other_sizes").  The state (5.6 GB at 512^3) is far
 larger than the 126 MB L2, so no L2 flush is needed between steps.
 
 N > 1 (torchrun): the path does not shard in this build ("replicas only"): every rank
@@ -45,7 +45,7 @@ def parse():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--size", type=int, default=512)
-    ap.add_argument("--other-sizes", type=str, default="256")
+    ap.add_argument("--other-sizes", type=str, default="128,256,384")
     ap.add_argument("--impl", type=str, default="b200", choices=["b200", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
