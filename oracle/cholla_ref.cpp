@@ -36,6 +36,7 @@ constexpr double NEWTON_TOL = 1e-8;     // P:L1095 "e.g. 1e-6"; reading S2: 1e-8
 constexpr int NEWTON_CAP = 20;          // reading S2
 
 enum { BC_PERIODIC = 1, BC_REFLECTIVE = 2, BC_OUTFLOW = 3 };
+enum { SOLVER_EXACT = 0, SOLVER_ROE = 1 };   // the Riemann solver is selectable
 
 thread_local std::string g_err;
 
@@ -315,14 +316,106 @@ void riemann_exact(double gamma, const double WL[5], const double WR[5], double 
   if (diag) { diag->pm = pm; diag->um = um; diag->rho = rho; diag->u = u; diag->p = p; diag->iters = it; diag->region = region; }
 }
 
+// ---------------------------------------------------------------------------------------------
+// Roe solver with the HLLE failsafe (B.2), x-interface form in direction-local order
+// (rho, u, v, w, p).  Step by step as printed; B29 read as NEXT-1/G9 in DESIGN.md:
+// s1 = C0(u~ - a~) + C3 u~ + C4(u~ + a~), s3 = C0 w~ + C2 + C3 w~ + C4 w~,
+// s4 = C0(H~ - u~ a~) + C1 v~ + C2 w~ + 0.5 C3 V~^2 + C4(H~ + u~ a~)
+// (the printed "(u~ - u~)", "C3 2~" and "(H~ - u~ u~)" are the eigenvectors of B31-B32 garbled).
+// path: 0 = F_L (supersonic to the right), 1 = F_R, 2 = Roe flux, 3 = HLLE flux.
+// ---------------------------------------------------------------------------------------------
+void flux_eq11(double gamma, const double W[5], double U[5], double F[5]) {   // Eq. 9, 11
+  const double rho = W[0], u = W[1], v = W[2], w = W[3], p = W[4];
+  const double E = p / (gamma - 1.0) + 0.5 * rho * ((u * u + v * v) + w * w);
+  U[0] = rho; U[1] = rho * u; U[2] = rho * v; U[3] = rho * w; U[4] = E;
+  F[0] = rho * u;
+  F[1] = rho * u * u + p;
+  F[2] = rho * u * v;
+  F[3] = rho * u * w;
+  F[4] = (E + p) * u;
+}
+
+void riemann_roe(double gamma, const double WL[5], const double WR[5], double flux[5], int* path) {
+  double UL[5], UR[5], FL[5], FR[5];
+  flux_eq11(gamma, WL, UL, FL);
+  flux_eq11(gamma, WR, UR, FR);
+  // B23
+  const double sl = std::sqrt(WL[0]), sr = std::sqrt(WR[0]);
+  const double HL = (UL[4] + WL[4]) / WL[0], HR = (UR[4] + WR[4]) / WR[0];
+  const double ut = (sl * WL[1] + sr * WR[1]) / (sl + sr);
+  const double vt = (sl * WL[2] + sr * WR[2]) / (sl + sr);
+  const double wt = (sl * WL[3] + sr * WR[3]) / (sl + sr);
+  const double Ht = (sl * HL + sr * HR) / (sl + sr);
+  const double V2 = (ut * ut + vt * vt) + wt * wt;
+  const double at = std::sqrt((gamma - 1.0) * (Ht - 0.5 * V2));          // B24
+  const double lm = ut - at, l0 = ut, lp = ut + at;                        // B25
+  if (lm >= 0.0) { for (int m = 0; m < 5; ++m) flux[m] = FL[m]; if (path) *path = 0; return; }
+  if (lp <= 0.0) { for (int m = 0; m < 5; ++m) flux[m] = FR[m]; if (path) *path = 1; return; }
+  // B26
+  double dU[5];
+  for (int m = 0; m < 5; ++m) dU[m] = UR[m] - UL[m];
+  // B27
+  const double Na = 1.0 / (2.0 * at * at), gp = gamma - 1.0, ia2 = 1.0 / (at * at);
+  double xi[5];
+  xi[0] = dU[0] * Na * (0.5 * gp * V2 + ut * at) - dU[1] * Na * (gp * ut + at) - dU[2] * Na * gp * vt -
+          dU[3] * Na * gp * wt + dU[4] * Na * gp;
+  xi[1] = -dU[0] * vt + dU[2];
+  xi[2] = -dU[0] * wt + dU[3];
+  xi[3] = dU[0] * (1.0 - Na * gp * V2) + dU[1] * gp * ut * ia2 + dU[2] * gp * vt * ia2 + dU[3] * gp * wt * ia2 -
+          dU[4] * gp * ia2;
+  xi[4] = dU[0] * Na * (0.5 * gp * V2 - ut * at) - dU[1] * Na * (gp * ut - at) - dU[2] * Na * gp * vt -
+          dU[3] * Na * gp * wt + dU[4] * Na * gp;
+  // B28
+  const double C0 = xi[0] * std::fabs(lm), C1 = xi[1] * std::fabs(l0), C2 = xi[2] * std::fabs(l0),
+               C3 = xi[3] * std::fabs(l0), C4 = xi[4] * std::fabs(lp);
+  // B29
+  double sv[5];
+  sv[0] = C0 + C3 + C4;
+  sv[1] = C0 * (ut - at) + C3 * ut + C4 * (ut + at);
+  sv[2] = C0 * vt + C1 + C3 * vt + C4 * vt;
+  sv[3] = C0 * wt + C2 + C3 * wt + C4 * wt;
+  sv[4] = C0 * (Ht - ut * at) + C1 * vt + C2 * wt + 0.5 * C3 * V2 + C4 * (Ht + ut * at);
+  // B31, B32: intermediate states; negative density or pressure -> HLLE
+  bool hlle = false;
+  double Um[5];
+  Um[0] = UL[0] + xi[0];
+  Um[1] = UL[1] + xi[0] * (ut - at);
+  Um[2] = UL[2] + xi[0] * vt;
+  Um[3] = UL[3] + xi[0] * wt;
+  Um[4] = UL[4] + xi[0] * (Ht - ut * at);
+  auto pressure = [&](const double* U) { return (gamma - 1.0) * (U[4] - 0.5 * ((U[1] * U[1] + U[2] * U[2]) + U[3] * U[3]) / U[0]); };
+  if (l0 > lm) { if (!(Um[0] > 0.0) || !(pressure(Um) > 0.0)) hlle = true; }
+  Um[0] += xi[3];
+  Um[1] += xi[3] * ut;
+  Um[2] += xi[1] + xi[3] * vt;
+  Um[3] += xi[2] + xi[3] * wt;
+  Um[4] += xi[1] * vt + xi[2] * wt + 0.5 * xi[3] * V2;
+  if (lp > l0) { if (!(Um[0] > 0.0) || !(pressure(Um) > 0.0)) hlle = true; }
+  if (!hlle) {
+    for (int m = 0; m < 5; ++m) flux[m] = 0.5 * ((FL[m] + FR[m]) - sv[m]);   // B30
+    if (path) *path = 2;
+    return;
+  }
+  // HLLE (B33-B35)
+  const double aL = std::sqrt(gamma * WL[4] / WL[0]), aR = std::sqrt(gamma * WR[4] / WR[0]);
+  const double bm = std::min(std::min(lm, WL[1] - aL), 0.0), bp = std::max(std::max(lp, WR[1] + aR), 0.0);
+  const double t = (bp + bm) / (bp - bm);
+  for (int m = 0; m < 5; ++m) {
+    const double fl = FL[m] - bm * UL[m], fr = FR[m] - bp * UR[m];       // B34
+    flux[m] = 0.5 * ((fl + fr) + (fl - fr) * t);                          // B35
+  }
+  if (path) *path = 3;
+}
+
 // Riemann problem at an interface normal to d from two conserved states in GLOBAL order.
-void riemann_interface(double gamma, int d, const double UL[5], const double UR[5], double F[5]) {
+void riemann_interface(double gamma, int solver, int d, const double UL[5], const double UR[5], double F[5]) {
   double wl[5], wr[5], ll[5], lr[5], fl[5];
   cons_to_prim(gamma, UL, wl);
   cons_to_prim(gamma, UR, wr);
   to_local(d, wl, ll);
   to_local(d, wr, lr);
-  riemann_exact(gamma, ll, lr, fl, nullptr);
+  if (solver == SOLVER_ROE) riemann_roe(gamma, ll, lr, fl, nullptr);
+  else riemann_exact(gamma, ll, lr, fl, nullptr);
   to_global(d, fl, F);
 }
 
@@ -336,6 +429,7 @@ struct Ctx {
   int bc[6];
   bool active[3];
   bool have_state = false;
+  int solver = SOLVER_EXACT;
   std::vector<double> u;  // [5][np], x fastest
   inline long idx(int i, int j, int k) const {  // real-cell coordinates, ghosts negative / >= n
     return ((long)(k + gd[2]) * pd[1] + (j + gd[1])) * pd[0] + (i + gd[0]);
@@ -475,7 +569,7 @@ void ctu_step(Ctx& c, double dt) {
           const long q = c.idx(i, j, k), qp = q + stride[d];
           double UL[5], UR[5], F[5];
           for (int f = 0; f < 5; ++f) { UL[f] = UsR[d][f * np + q]; UR[f] = UsL[d][f * np + qp]; }
-          riemann_interface(gamma, d, UL, UR, F);
+          riemann_interface(gamma, c.solver, d, UL, UR, F);
           for (int f = 0; f < 5; ++f) Fs[d][f * np + q] = F[f];
         }
   }
@@ -517,7 +611,7 @@ void ctu_step(Ctx& c, double dt) {
           const long q = c.idx(i, j, k), qp = q + stride[d];
           double UL[5], UR[5], F[5];
           for (int f = 0; f < 5; ++f) { UL[f] = UhR[d][f * np + q]; UR[f] = UhL[d][f * np + qp]; }
-          riemann_interface(gamma, d, UL, UR, F);
+          riemann_interface(gamma, c.solver, d, UL, UR, F);
           for (int f = 0; f < 5; ++f) Fh[d][f * np + q] = F[f];
         }
   }
@@ -659,6 +753,16 @@ void ref_ppmc_cell(double gamma, double dtdx, const double* w, double* out) {
   ppmc_cell(gamma, dtdx, ws, out, out + 5, out + 10, out + 15);
 }
 // WL, WR primitive; flux[5]; diag[7] = pm, um, rho, u, p, iterations, region
+int ref_set_solver(void* h, int solver) {
+  if (!h || (solver != SOLVER_EXACT && solver != SOLVER_ROE)) return fail("ref_set_solver: bad argument");
+  static_cast<Ctx*>(h)->solver = solver;
+  return 0;
+}
+int ref_riemann_roe(double gamma, const double* WL, const double* WR, double* flux) {
+  int path = -1;
+  riemann_roe(gamma, WL, WR, flux, &path);
+  return path;
+}
 void ref_riemann_exact(double gamma, const double* WL, const double* WR, double* flux, double* diag) {
   RiemannDiag d;
   riemann_exact(gamma, WL, WR, flux, &d);

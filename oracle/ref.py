@@ -55,6 +55,9 @@ def lib() -> C.CDLL:
         L.ref_limited_slope.argtypes = [C.c_double, dp, dp, dp, dp]
         L.ref_ppmc_cell.argtypes = [C.c_double, C.c_double, dp, dp]
         L.ref_riemann_exact.argtypes = [C.c_double, dp, dp, dp, dp]
+        L.ref_riemann_roe.argtypes = [C.c_double, dp, dp, dp]
+        L.ref_riemann_roe.restype = C.c_int
+        L.ref_set_solver.argtypes = [C.c_void_p, C.c_int]
         _lib = L
     return _lib
 
@@ -114,6 +117,11 @@ class RefGrid:
     def compute_dt(self, cfl) -> float:
         return float(lib().ref_compute_dt(self._h, cfl))
 
+    def set_solver(self, solver):
+        """0 = exact (default), 1 = Roe with the HLLE failsafe (the solver is selectable)."""
+        if lib().ref_set_solver(self._h, int(solver)) != 0:
+            raise ValueError("ref_set_solver: " + lib().ref_last_error().decode())
+
     def step(self, dt):
         if lib().ref_step(self._h, dt) != 0:
             raise ValueError("ref_step: " + lib().ref_last_error().decode())
@@ -164,3 +172,14 @@ def riemann_exact(gamma, WL, WR):
     f = np.empty(5); d = np.empty(7)
     lib().ref_riemann_exact(gamma, _p(WL), _p(WR), _p(f), _p(d))
     return f, dict(pm=d[0], um=d[1], rho=d[2], u=d[3], p=d[4], iters=int(d[5]), region=int(d[6]))
+
+
+ROE_PATHS = ("F_L", "F_R", "roe", "hlle")
+
+
+def riemann_roe(gamma, WL, WR):
+    """Roe solver with the HLLE failsafe (B.2) -> (flux[5], path) with path in ROE_PATHS."""
+    WL, WR = _arr(WL), _arr(WR)
+    f = np.empty(5)
+    path = lib().ref_riemann_roe(gamma, _p(WL), _p(WR), _p(f))
+    return f, ROE_PATHS[path]
