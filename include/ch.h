@@ -123,6 +123,14 @@ double ch_compute_dt(ch_ctx* ctx, double cfl);
  * CH_ESTATE if no state is set; CH_EINVAL if dt <= 0 or non-finite; CH_ECUDA on launch failure. */
 int ch_step(ch_ctx* ctx, double dt);
 
+/* Riemann solver used at every interface by ch_step (the solver is selectable at compile time in the
+ * paper's code, at run time here).  CH_SOLVER_EXACT (default): the exact solver, B.1.  CH_SOLVER_ROE: the
+ * Roe solver with the HLLE failsafe, B.2; without the H correction of Appendix C. */
+enum { CH_SOLVER_EXACT = 0, CH_SOLVER_ROE = 1 };
+
+/* ch_set_solver — select the Riemann solver for later steps.  CH_EINVAL for an unknown code. */
+int ch_set_solver(ch_ctx* ctx, int solver);
+
 /* ch_sync — block until all work queued on the context's stream has finished. */
 int ch_sync(ch_ctx* ctx);
 

@@ -361,4 +361,85 @@ CH_D void riemann_exact(const Gas& G, const double WL[5], const double WR[5], do
   flux[4] = (E + p) * u;
 }
 
+// Roe solver with the HLLE failsafe (B.2): primitive L/R states (direction-local) -> flux.
+// B23-B30 with B29 read as in DESIGN.md (G9); the intermediate states B31-B32 are checked for negative
+// density or pressure and the HLLE flux B33-B35 substituted if either occurs.  Square roots and quotients
+// through the branch-free rsqrt / rcp above.
+CH_D void riemann_roe(const Gas& G, const double WL[5], const double WR[5], double flux[5]) {
+  const double rL = WL[0], uL = WL[1], vL = WL[2], wL = WL[3], pL = floor_p(WL[4]);
+  const double rR = WR[0], uR = WR[1], vR = WR[2], wR = WR[3], pR = floor_p(WR[4]);
+  const double EL = pL * G.inv_gm1 + 0.5 * rL * ((uL * uL + vL * vL) + wL * wL);
+  const double ER = pR * G.inv_gm1 + 0.5 * rR * ((uR * uR + vR * vR) + wR * wR);
+  const double UL[5] = {rL, rL * uL, rL * vL, rL * wL, EL}, UR[5] = {rR, rR * uR, rR * vR, rR * wR, ER};
+  const double FL[5] = {UL[1], UL[1] * uL + pL, UL[1] * vL, UL[1] * wL, (EL + pL) * uL};   // Eq. 11
+  const double FR[5] = {UR[1], UR[1] * uR + pR, UR[1] * vR, UR[1] * wR, (ER + pR) * uR};
+  // B23
+  const double isl = rsqrt_pos(rL), isr = rsqrt_pos(rR);
+  const double sl = rL * isl, sr = rR * isr;
+  const double inv = rcp(sl + sr);
+  const double HL = (EL + pL) * (isl * isl), HR = (ER + pR) * (isr * isr);
+  const double ut = (sl * uL + sr * uR) * inv, vt = (sl * vL + sr * vR) * inv, wt = (sl * wL + sr * wR) * inv;
+  const double Ht = (sl * HL + sr * HR) * inv;
+  const double V2 = (ut * ut + vt * vt) + wt * wt;
+  const double at2 = G.gm1 * (Ht - 0.5 * V2);                              // B24
+  const double iat = rsqrt_pos(at2), at = at2 * iat;
+  const double lm = ut - at, l0 = ut, lp = ut + at;                        // B25
+  if (lm >= 0.0) {
+#pragma unroll
+    for (int m = 0; m < 5; ++m) flux[m] = FL[m];
+    return;
+  }
+  if (lp <= 0.0) {
+#pragma unroll
+    for (int m = 0; m < 5; ++m) flux[m] = FR[m];
+    return;
+  }
+  double dU[5];
+#pragma unroll
+  for (int m = 0; m < 5; ++m) dU[m] = UR[m] - UL[m];                       // B26
+  // B27: acoustic strengths share  q = gamma' (0.5 V2 drho - u dmx - v dmy - w dmz + dE)
+  const double ia2 = iat * iat, Na = 0.5 * ia2, gp = G.gm1;
+  const double q = gp * ((0.5 * V2 * dU[0] - ut * dU[1]) - (vt * dU[2] + wt * dU[3]) + dU[4]);
+  const double r = at * (ut * dU[0] - dU[1]);
+  const double xi0 = Na * (q + r), xi4 = Na * (q - r);
+  const double xi1 = dU[2] - vt * dU[0], xi2 = dU[3] - wt * dU[0];
+  const double xi3 = dU[0] - q * ia2;
+  // B28, B29
+  const double C0 = xi0 * fabs(lm), C1 = xi1 * fabs(l0), C2 = xi2 * fabs(l0), C3 = xi3 * fabs(l0), C4 = xi4 * fabs(lp);
+  const double ua = ut * at, c04 = C0 + C4;
+  double sv[5];
+  sv[0] = c04 + C3;
+  sv[1] = (C0 * lm + C3 * ut) + C4 * lp;
+  sv[2] = (c04 + C3) * vt + C1;
+  sv[3] = (c04 + C3) * wt + C2;
+  sv[4] = (C0 * (Ht - ua) + C4 * (Ht + ua)) + ((C1 * vt + C2 * wt) + 0.5 * C3 * V2);
+  // B31, B32: intermediate states
+  double Um[5] = {UL[0] + xi0, UL[1] + xi0 * lm, UL[2] + xi0 * vt, UL[3] + xi0 * wt, UL[4] + xi0 * (Ht - ua)};
+  bool hlle = !(Um[0] > 0.0) || !(Um[4] * Um[0] - 0.5 * ((Um[1] * Um[1] + Um[2] * Um[2]) + Um[3] * Um[3]) > 0.0);
+  Um[0] += xi3; Um[1] += xi3 * ut; Um[2] += xi1 + xi3 * vt; Um[3] += xi2 + xi3 * wt;
+  Um[4] += (xi1 * vt + xi2 * wt) + 0.5 * xi3 * V2;
+  hlle = hlle || !(Um[0] > 0.0) || !(Um[4] * Um[0] - 0.5 * ((Um[1] * Um[1] + Um[2] * Um[2]) + Um[3] * Um[3]) > 0.0);
+  if (!hlle) {
+#pragma unroll
+    for (int m = 0; m < 5; ++m) flux[m] = 0.5 * ((FL[m] + FR[m]) - sv[m]);   // B30
+    return;
+  }
+  // HLLE (B33-B35)
+  const double aL = G.gamma * pL * inv_rho_a(G, rL, pL), aR = G.gamma * pR * inv_rho_a(G, rR, pR);
+  const double bm = sel_min(sel_min(lm, uL - aL), 0.0), bp = sel_max(sel_max(lp, uR + aR), 0.0);
+  const double t = (bp + bm) * rcp(bp - bm);
+#pragma unroll
+  for (int m = 0; m < 5; ++m) {
+    const double fl = FL[m] - bm * UL[m], fr = FR[m] - bp * UR[m];          // B34
+    flux[m] = 0.5 * ((fl + fr) + (fl - fr) * t);                             // B35
+  }
+}
+
+// Solver selection at compile time (reconstruction and solver are selectable): 0 exact, 1 Roe + HLLE.
+template <int S>
+CH_D void riemann(const Gas& G, const double WL[5], const double WR[5], double flux[5]) {
+  if (S == 0) riemann_exact(G, WL, WR, flux);
+  else riemann_roe(G, WL, WR, flux);
+}
+
 }  // namespace ch

@@ -118,7 +118,7 @@ __device__ __forceinline__ void copy5(double dst[5], const double src[5]) {
 #define CH_P2_MINB 1
 #endif
 
-template <int D>
+template <int D, int S>
 __global__ void __launch_bounds__(CH_MARCH_T, CH_MARCH_MINB) k_pass1_march(const StepArgs A, int seg) {
   constexpr int T = 3 - D;   // the other transverse dimension (x is the lane dimension)
   const Geom& g = A.geo;
@@ -172,7 +172,7 @@ __global__ void __launch_bounds__(CH_MARCH_T, CH_MARCH_MINB) k_pass1_march(const
     }
     if (c > c0) {
       double fl[5];
-      ch::riemann_exact(G, pr_prev, WLs, fl);      // the solver's first act would be conserved -> primitive
+      ch::riemann<S>(G, pr_prev, WLs, fl);      // the solver's first act would be conserved -> primitive
       store_local<D>(A.Fs[D], np, q - sD, fl);
     }
     copy5(pr_prev, WRs);
@@ -194,6 +194,7 @@ __global__ void __launch_bounds__(CH_MARCH_T, CH_MARCH_MINB) k_pass1_march(const
 constexpr int kXT = CH_X_T;    // threads per CTA
 constexpr int kXOut = kXT - 5; // interfaces produced per CTA
 
+template <int S>
 __global__ void __launch_bounds__(kXT, CH_X_MINB) k_pass1_x(const StepArgs A, long long q_begin, long long q_end) {
   __shared__ double sP[5][kXT];
   __shared__ double sS[5][kXT];
@@ -260,7 +261,7 @@ __global__ void __launch_bounds__(kXT, CH_X_MINB) k_pass1_x(const StepArgs A, lo
     double wr[5], fl[5];
 #pragma unroll
     for (int m = 0; m < 5; ++m) wr[m] = sL[m][tid + 1];
-    ch::riemann_exact(G, prR, wr, fl);
+    ch::riemann<S>(G, prR, wr, fl);
     store_local<0>(A.Fs[0], np, q, fl);
   }
 }
@@ -295,6 +296,7 @@ __device__ __forceinline__ void corrected_prim(const Gas& G, const DirSel& S, lo
   ch::cons2prim(G, c[0], c[1], c[2], c[3], c[4], w);
 }
 
+template <int SOLVER>
 __global__ void __launch_bounds__(CH_P2_T, CH_P2_MINB) k_pass2(const StepArgs A) {
   const Geom& g = A.geo;
   const int e0 = g.act[0] ? g.n[0] + 1 : 1, e1 = g.act[1] ? g.n[1] + 1 : 1, e2 = g.act[2] ? g.n[2] + 1 : 1;
@@ -322,7 +324,7 @@ __global__ void __launch_bounds__(CH_P2_T, CH_P2_MINB) k_pass2(const StepArgs A)
     double wl[5], wr[5], fl[5];
     corrected_prim(A.gas, S, np, A.UR[d], q, wl);           // U^{n+1/2}_R of cell c   -> left state
     corrected_prim(A.gas, S, np, A.UL[d], q + S.s0, wr);    // U^{n+1/2}_L of cell c+1 -> right state
-    ch::riemann_exact(A.gas, wl, wr, fl);
+    ch::riemann<SOLVER>(A.gas, wl, wr, fl);
     double* __restrict__ Fh = A.Fh[d];
     Fh[q] = fl[0]; Fh[S.f1 + q] = fl[1]; Fh[S.f2 + q] = fl[2]; Fh[S.f3 + q] = fl[3]; Fh[4 * np + q] = fl[4];
   }
@@ -505,6 +507,7 @@ __device__ __forceinline__ void face_states(const StepArgs& A, long long q, cons
   correct_faces<D>(A, ul, ur, dF, wl, wr);
 }
 
+template <int S>
 __global__ void __launch_bounds__(kFT, CH_F_MINB) k_final3d(const StepArgs A, int seg) {
   extern __shared__ double s_final[];
   typedef double (*Arr)[kFT];
@@ -574,7 +577,7 @@ __global__ void __launch_bounds__(kFT, CH_F_MINB) k_final3d(const StepArgs A, in
         if (need0) face_states<0>(A, q, dF, wl, wr);
 #pragma unroll
         for (int m = 0; m < 5; ++m) nb[m] = __shfl_up_sync(full, wr[m], 1);
-        if (solve0) ch::riemann_exact(G, nb, wl, fl);
+        if (solve0) ch::riemann<S>(G, nb, wl, fl);
 #pragma unroll
         for (int m = 0; m < 5; ++m) {
           const double hi = __shfl_down_sync(full, fl[m], 1);
@@ -590,7 +593,7 @@ __global__ void __launch_bounds__(kFT, CH_F_MINB) k_final3d(const StepArgs A, in
         const int src = tid >= kFX ? tid - kFX : tid;
 #pragma unroll
         for (int m = 0; m < 5; ++m) nb[m] = sX[m][src];
-        if (solve1) ch::riemann_exact(G, nb, wl, fl);
+        if (solve1) ch::riemann<S>(G, nb, wl, fl);
 #pragma unroll
         for (int m = 0; m < 5; ++m) sF[m][tid] = fl[m];
         __syncthreads();
@@ -611,7 +614,7 @@ __global__ void __launch_bounds__(kFT, CH_F_MINB) k_final3d(const StepArgs A, in
       if (!first) {
 #pragma unroll
         for (int m = 0; m < 5; ++m) nb[m] = zU[m][tid];
-        ch::riemann_exact(G, nb, wl, fl);
+        ch::riemann<S>(G, nb, wl, fl);
       }
       if (k > k0) {
         // finish cell k-1 (Eq. 24): z-local order (rho, mz, mx, my, E)
@@ -673,6 +676,7 @@ __device__ __forceinline__ void tma_load_4d(unsigned dst, const CUtensorMap* map
       ::"r"(dst), "l"(map), "r"(bar), "r"(c0), "r"(c1), "r"(c2), "r"(c3) : "memory");
 }
 
+template <int S>
 __global__ void __launch_bounds__(kTT + 32, 1) k_final3d_tma(const StepArgs A, const __grid_constant__ TmaMaps M, int seg) {
   extern __shared__ __align__(1024) double s_t[];
   __shared__ unsigned long long s_full[4], s_empty[4];
@@ -780,7 +784,7 @@ __global__ void __launch_bounds__(kTT + 32, 1) k_final3d_tma(const StepArgs A, c
         if (!first) {
 #pragma unroll
           for (int m = 0; m < 5; ++m) nb[m] = zU[m];
-          ch::riemann_exact(G, nb, wl, flz);
+          ch::riemann<S>(G, nb, wl, flz);
         }
         if (k > k0) {
           // finish cell k-1 (Eq. 24): z-local order (rho, mz, mx, my, E)
@@ -810,7 +814,7 @@ __global__ void __launch_bounds__(kTT + 32, 1) k_final3d_tma(const StepArgs A, c
         if (need0) correct_faces<0>(A, ul, ur, dF, wl, wr);
 #pragma unroll
         for (int m = 0; m < 5; ++m) nb[m] = __shfl_up_sync(full, wr[m], 1);
-        if (solve0) ch::riemann_exact(G, nb, wl, fl);
+        if (solve0) ch::riemann<S>(G, nb, wl, fl);
 #pragma unroll
         for (int m = 0; m < 5; ++m) {
           const double hi = __shfl_down_sync(full, fl[m], 1);
@@ -834,7 +838,7 @@ __global__ void __launch_bounds__(kTT + 32, 1) k_final3d_tma(const StepArgs A, c
         const int src = tid >= kFX ? tid - kFX : tid;
 #pragma unroll
         for (int m = 0; m < 5; ++m) nb[m] = sX[m][src];
-        if (solve1) ch::riemann_exact(G, nb, wl, fl);
+        if (solve1) ch::riemann<S>(G, nb, wl, fl);
 #pragma unroll
         for (int m = 0; m < 5; ++m) sF[m][tid] = fl[m];
         asm volatile("bar.sync 1, %0;" ::"n"(kTT) : "memory");
@@ -973,6 +977,7 @@ struct ch_ctx {
   bool use_tma = true;       // CH_TMA=0: plain-load k_final3d even where the TMA form applies
   bool tma_ok = false;       // tensor maps built for the bound buffers
   TmaMaps maps;
+  int solver = 0;            // CH_SOLVER_EXACT
   bool unfused = false;      // CH_UNFUSED=1: k_pass2 + k_update on 3-D grids too (A/B measurements, instruction counts)
   // optional per-kernel timing (ch_profile): one event pair per kernel kind
   bool profiling = false;
@@ -1262,7 +1267,13 @@ double ch_compute_dt(ch_ctx* c, double cfl) {
   return cfl * (1.0 / rate);
 }
 
-int ch_step(ch_ctx* c, double dt) {
+}  // extern "C"
+
+namespace {
+
+// One CTU step with Riemann solver S (0 exact, 1 Roe + HLLE) compiled into every kernel that solves.
+template <int S>
+int step_impl(ch_ctx* c, double dt) {
   if (!c) return fail(CH_EINVAL, "ch_step: null context");
   if (!c->have_state) return fail(CH_ESTATE, "ch_step: no state set");
   if (!(dt > 0.0) || !std::isfinite(dt)) return fail(CH_EINVAL, "ch_step: dt <= 0 or non-finite");
@@ -1279,7 +1290,7 @@ int ch_step(ch_ctx* c, double dt) {
     const long long qe = (long long)j1 * g.st[1] + (long long)k1 * g.st[2] + g.pd[0];
     const long long nb = (qe - qb + kXOut - 1) / kXOut;
     Bracket b(c, CH_K_PASS1_X);
-    k_pass1_x<<<(unsigned)nb, kXT, 0, st>>>(A, qb, qe);
+    k_pass1_x<S><<<(unsigned)nb, kXT, 0, st>>>(A, qb, qe);
   }
   for (int d = 1; d < 3; ++d) {
     if (!g.act[d]) continue;
@@ -1288,8 +1299,8 @@ int ch_step(ch_ctx* c, double dt) {
     const int seg = c->march_seg;
     dim3 grid((unsigned)((cols + CH_MARCH_T - 1) / CH_MARCH_T), (unsigned)((g.n[d] + 1 + seg - 1) / seg));
     Bracket b(c, d == 1 ? CH_K_PASS1_Y : CH_K_PASS1_Z);
-    if (d == 1) k_pass1_march<1><<<grid, CH_MARCH_T, 0, st>>>(A, seg);
-    else k_pass1_march<2><<<grid, CH_MARCH_T, 0, st>>>(A, seg);
+    if (d == 1) k_pass1_march<1, S><<<grid, CH_MARCH_T, 0, st>>>(A, seg);
+    else k_pass1_march<2, S><<<grid, CH_MARCH_T, 0, st>>>(A, seg);
   }
   CH_CUDA(cudaGetLastError(), "pass 1");
   if (g.act[0] && g.act[1] && g.act[2] && !c->unfused) {
@@ -1300,28 +1311,28 @@ int ch_step(ch_ctx* c, double dt) {
       const size_t tsmem = (size_t)60 * kTT * sizeof(double);
       static bool tattr_set = false;
       if (!tattr_set) {
-        CH_CUDA(cudaFuncSetAttribute(k_final3d_tma, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tsmem), "k_final3d_tma smem attribute");
+        CH_CUDA(cudaFuncSetAttribute(k_final3d_tma<S>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tsmem), "k_final3d_tma smem attribute");
         tattr_set = true;
       }
       dim3 tgrid((unsigned)((g.n[0] + kFX - 3) / (kFX - 2)), (unsigned)((g.n[1] + kTY - 3) / (kTY - 2)),
                  (unsigned)((g.n[2] + seg - 1) / seg));
       Bracket b(c, CH_K_FINAL);
-      k_final3d_tma<<<tgrid, kTT + 32, tsmem, st>>>(A, c->maps, seg);
+      k_final3d_tma<S><<<tgrid, kTT + 32, tsmem, st>>>(A, c->maps, seg);
     } else {
     const size_t smem = (size_t)30 * kFT * sizeof(double);
     static bool attr_set = false;
     if (!attr_set) {
-      CH_CUDA(cudaFuncSetAttribute(k_final3d, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem), "k_final3d smem attribute");
+      CH_CUDA(cudaFuncSetAttribute(k_final3d<S>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem), "k_final3d smem attribute");
       attr_set = true;
     }
     Bracket b(c, CH_K_FINAL);
-    k_final3d<<<grid, kFT, smem, st>>>(A, seg);
+    k_final3d<S><<<grid, kFT, smem, st>>>(A, seg);
     }
   } else {
     {
       const long long cells = (long long)(g.act[0] ? g.n[0] + 1 : 1) * (g.act[1] ? g.n[1] + 1 : 1) * (g.act[2] ? g.n[2] + 1 : 1);
       Bracket b(c, CH_K_PASS2);
-      k_pass2<<<(unsigned)((cells + CH_P2_T - 1) / CH_P2_T), CH_P2_T, 0, st>>>(A);
+      k_pass2<S><<<(unsigned)((cells + CH_P2_T - 1) / CH_P2_T), CH_P2_T, 0, st>>>(A);
     }
     {
       const long long N = (long long)g.n[0] * g.n[1] * g.n[2];
@@ -1334,6 +1345,22 @@ int ch_step(ch_ctx* c, double dt) {
   if (rc) return rc;
   c->dt_valid = true;
   return profile_collect(c);
+}
+
+}  // namespace
+
+extern "C" {
+
+int ch_step(ch_ctx* c, double dt) {
+  if (!c) return fail(CH_EINVAL, "ch_step: null context");
+  return c->solver == CH_SOLVER_ROE ? step_impl<1>(c, dt) : step_impl<0>(c, dt);
+}
+
+int ch_set_solver(ch_ctx* c, int solver) {
+  if (!c) return fail(CH_EINVAL, "ch_set_solver: null context");
+  if (solver != CH_SOLVER_EXACT && solver != CH_SOLVER_ROE) return fail(CH_EINVAL, "ch_set_solver: unknown solver");
+  c->solver = solver;
+  return CH_OK;
 }
 
 int ch_sync(ch_ctx* c) {

@@ -400,3 +400,79 @@ def test_tma_and_plain_load_forms_of_the_fused_kernel_are_bitwise_equal(ch, monk
             G.close()
         assert np.all(np.isfinite(res["0"][0]))
         assert np.array_equal(res["0"][0], res["1"][0]) and res["0"][1] == res["1"][1]
+
+
+# ---- NEXT-1: Roe solver with the HLLE failsafe (B.2) ------------------------------------------------
+ROE_CASES = {
+    "sod_1d_128": lambda: wl.sod(128),
+    "sod_along_z": lambda: wl.sod(96, axis=2, n_other=5),
+    "kh_2d_128": lambda: wl.kelvin_helmholtz(128),
+    "sedov_32": lambda: wl.sedov(32),
+    "shock_cloud_48": lambda: wl.shock_cloud(48),
+    "sweep_ragged_3d_tma": lambda: wl.sweep(shape=(270, 44, 36)),      # even padded strides: TMA form
+    "sweep_ragged_3d_plain": lambda: wl.sweep(shape=(135, 45, 37)),    # odd: plain-load form
+    "rough_3d_hlle": lambda: wl.rough_random(38, 21, 13, seed=11, decades=0.5),
+    "einfeldt_123": lambda: wl.riemann_tube(128, (1.0, -2.0, 0.4), (1.0, 2.0, 0.4), gamma=1.4, t_end=0.15),
+}
+
+
+@pytest.mark.parametrize("name", sorted(ROE_CASES))
+def test_roe_one_step_parity(ch, ref, name):
+    w = ROE_CASES[name]()
+    G, Rg = both(ch, ref, w)
+    for g in (G, Rg):
+        g.set_solver(1)
+        g.set_state(w.u)
+    dt = Rg.compute_dt(w.cfl)
+    G.step(dt); Rg.step(dt)
+    ur = Rg.get_state()
+    assert np.all(np.isfinite(ur))
+    assert max(max_rel_error(G.get_state(), ur, w.gamma)) <= ONE_STEP_TOL, name
+    G.close()
+
+
+def test_roe_differs_from_exact_and_switches_back(ch, ref):
+    """ch_set_solver really changes the path (the two solvers give different fluxes at a shock) and back."""
+    w = wl.sod(128)
+    G = ch.Grid(*w.shape, 3, w.gamma, w.bc)
+    outs = []
+    for solver in (0, 1, 0):
+        G.set_solver(solver)
+        G.set_state(w.u)
+        for _ in range(5):
+            G.step(G.compute_dt(w.cfl))
+        outs.append(G.get_state())
+    assert np.array_equal(outs[0], outs[2]) and not np.array_equal(outs[0], outs[1])
+    with pytest.raises(ValueError):
+        G.set_solver(7)
+    G.close()
+
+
+def test_roe_runs_match_oracle(ch, ref):
+    for w in (wl.sod(128), wl.sweep(shape=(72, 56, 40), steps=15),
+              wl.riemann_tube(128, (1.0, -2.0, 0.4), (1.0, 2.0, 0.4), gamma=1.4, t_end=0.15)):
+        G, Rg = both(ch, ref, w)
+        G.set_solver(1); Rg.set_solver(1)
+        dts = []
+        run(Rg, w, record_dts=dts)
+        run(G, w, dts=dts)
+        assert max(rel_l1_error(G.get_state(), Rg.get_state(), w.gamma)) <= RUN_L1_TOL
+        G.close()
+
+
+def test_roe_tma_and_plain_forms_agree(ch, monkeypatch):
+    """Same arithmetic in two kernels; with the Roe solver inlined the compiler contracts a few multiply-adds
+    differently in the two, so the comparison is to rounding level rather than bitwise."""
+    w = wl.sweep(shape=(64, 40, 70))
+    res = {}
+    for mode in ("1", "0"):
+        monkeypatch.setenv("CH_TMA", mode)
+        G = ch.Grid(*w.shape, 3, w.gamma, w.bc)
+        G.set_solver(1)
+        G.set_state(w.u)
+        for _ in range(2):
+            G.step(G.compute_dt(w.cfl))
+        res[mode] = G.get_state()
+        G.close()
+    assert np.all(np.isfinite(res["0"]))
+    assert max(max_rel_error(res["0"], res["1"], w.gamma)) <= 1e-14
