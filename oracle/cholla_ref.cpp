@@ -37,6 +37,7 @@ constexpr int NEWTON_CAP = 20;          // reading S2
 
 enum { BC_PERIODIC = 1, BC_REFLECTIVE = 2, BC_OUTFLOW = 3 };
 enum { SOLVER_EXACT = 0, SOLVER_ROE = 1 };   // the Riemann solver is selectable
+enum { RECON_PPMC = 0, RECON_PLMC = 1, RECON_PCM = 2 };   // so is the reconstruction
 
 thread_local std::string g_err;
 
@@ -206,6 +207,64 @@ void ppmc_cell(double gamma, double dtdx, const double w[5][5], double WL[5], do
     WLs[m] = WLm[m] + sL[m];
     WRs[m] = WRp[m] + sR[m];
   }
+}
+
+// ---------------------------------------------------------------------------------------------
+// PLMC for one cell (A.2): linear reconstruction with the slope limited in the characteristic
+// variables (A8-A11, the same limited_slope PPMC uses), faces A12, monotonised A13, slope A14,
+// characteristic tracing A15-A19.  A19's second vector lost its last row in the text: the contact term
+// has the same shape as A17's first vector, [x, 0, x, x, 0] (reading G10).  Same argument layout as
+// ppmc_cell; only w[1..3] (cells i-1, i, i+1) are used.
+// ---------------------------------------------------------------------------------------------
+void plmc_cell(double gamma, double dtdx, const double w[5][5], double WL[5], double WR[5],
+               double WLs[5], double WRs[5]) {
+  const double* wi = w[2];
+  const double* wim = w[1];
+  const double* wip = w[3];
+  double dw0[5], dwi[5];
+  limited_slope(gamma, wim, wi, wip, dw0);                       // A8-A11
+  for (int m = 0; m < 5; ++m) {
+    const double LA = wi[m] - 0.5 * dw0[m], RA = wi[m] + 0.5 * dw0[m];              // A12
+    const double LB = std::max(std::min(wi[m], wim[m]), LA);                        // A13
+    WL[m] = std::min(std::max(wi[m], wim[m]), LB);
+    const double RB = std::max(std::min(wi[m], wip[m]), RA);
+    WR[m] = std::min(std::max(wi[m], wip[m]), RB);
+    dwi[m] = WR[m] - WL[m];                                                         // A14
+  }
+  const double rho = wi[0], a = std::sqrt(gamma * wi[4] / wi[0]), a2 = a * a;
+  const double lm = wi[1] - a, l0 = wi[1], lp = wi[1] + a;                          // A8
+  double sL[5] = {0, 0, 0, 0, 0}, sR[5] = {0, 0, 0, 0, 0};
+  if (l0 < 0.0) {                                                                   // A17, contact term
+    sL[0] += (lm - l0) * (dwi[0] - dwi[4] / a2);
+    sL[2] += (lm - l0) * dwi[2];
+    sL[3] += (lm - l0) * dwi[3];
+  }
+  if (lp < 0.0) {                                                                   // A17, right acoustic term
+    sL[0] += 0.5 * (lm - lp) * (rho * dwi[1] / a + dwi[4] / a2);
+    sL[1] += 0.5 * (lm - lp) * (dwi[1] + dwi[4] / (a * rho));
+    sL[4] += 0.5 * (lm - lp) * (rho * dwi[1] * a + dwi[4]);
+  }
+  if (lm > 0.0) {                                                                   // A19, left acoustic term
+    sR[0] += 0.5 * (lp - lm) * (-(rho * dwi[1] / a) + dwi[4] / a2);
+    sR[1] += 0.5 * (lp - lm) * (dwi[1] - dwi[4] / (a * rho));
+    sR[4] += 0.5 * (lp - lm) * (-(rho * dwi[1] * a) + dwi[4]);
+  }
+  if (l0 > 0.0) {                                                                   // A19, contact term (G10)
+    sR[0] += (lp - l0) * (dwi[0] - dwi[4] / a2);
+    sR[2] += (lp - l0) * dwi[2];
+    sR[3] += (lp - l0) * dwi[3];
+  }
+  for (int m = 0; m < 5; ++m) {
+    const double WLt = WL[m] - 0.5 * dtdx * std::min(lm, 0.0) * dwi[m];             // A15
+    const double WRt = WR[m] - 0.5 * dtdx * std::max(lp, 0.0) * dwi[m];
+    WLs[m] = WLt + 0.5 * dtdx * sL[m];                                              // A16
+    WRs[m] = WRt + 0.5 * dtdx * sR[m];                                              // A18
+  }
+}
+
+// PCM (Eq. 25-26): the face values are the cell average; no time evolution.
+void pcm_cell(const double w[5][5], double WL[5], double WR[5], double WLs[5], double WRs[5]) {
+  for (int m = 0; m < 5; ++m) WL[m] = WR[m] = WLs[m] = WRs[m] = w[2][m];
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -430,6 +489,7 @@ struct Ctx {
   bool active[3];
   bool have_state = false;
   int solver = SOLVER_EXACT;
+  int recon = RECON_PPMC;
   std::vector<double> u;  // [5][np], x fastest
   inline long idx(int i, int j, int k) const {  // real-cell coordinates, ghosts negative / >= n
     return ((long)(k + gd[2]) * pd[1] + (j + gd[1])) * pd[0] + (i + gd[0]);
@@ -546,7 +606,9 @@ void ctu_step(Ctx& c, double dt) {
             to_local(d, wg, ws[s]);
           }
           double WL[5], WR[5], WLs[5], WRs[5], gl[5], gr[5], ul[5], ur[5];
-          ppmc_cell(gamma, dtdx, ws, WL, WR, WLs, WRs);
+          if (c.recon == RECON_PLMC) plmc_cell(gamma, dtdx, ws, WL, WR, WLs, WRs);
+          else if (c.recon == RECON_PCM) pcm_cell(ws, WL, WR, WLs, WRs);
+          else ppmc_cell(gamma, dtdx, ws, WL, WR, WLs, WRs);
           to_global(d, WLs, gl);
           to_global(d, WRs, gr);
           prim_to_cons(gamma, gl, ul);
@@ -757,6 +819,16 @@ int ref_set_solver(void* h, int solver) {
   if (!h || (solver != SOLVER_EXACT && solver != SOLVER_ROE)) return fail("ref_set_solver: bad argument");
   static_cast<Ctx*>(h)->solver = solver;
   return 0;
+}
+int ref_set_reconstruction(void* h, int recon) {
+  if (!h || recon < RECON_PPMC || recon > RECON_PCM) return fail("ref_set_reconstruction: bad argument");
+  static_cast<Ctx*>(h)->recon = recon;
+  return 0;
+}
+void ref_plmc_cell(double gamma, double dtdx, const double* w, double* out) {
+  double ws[5][5];
+  for (int s = 0; s < 5; ++s) for (int m = 0; m < 5; ++m) ws[s][m] = w[s * 5 + m];
+  plmc_cell(gamma, dtdx, ws, out, out + 5, out + 10, out + 15);
 }
 int ref_riemann_roe(double gamma, const double* WL, const double* WR, double* flux) {
   int path = -1;

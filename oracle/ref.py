@@ -58,6 +58,8 @@ def lib() -> C.CDLL:
         L.ref_riemann_roe.argtypes = [C.c_double, dp, dp, dp]
         L.ref_riemann_roe.restype = C.c_int
         L.ref_set_solver.argtypes = [C.c_void_p, C.c_int]
+        L.ref_set_reconstruction.argtypes = [C.c_void_p, C.c_int]
+        L.ref_plmc_cell.argtypes = [C.c_double, C.c_double, dp, dp]
         _lib = L
     return _lib
 
@@ -122,6 +124,11 @@ class RefGrid:
         if lib().ref_set_solver(self._h, int(solver)) != 0:
             raise ValueError("ref_set_solver: " + lib().ref_last_error().decode())
 
+    def set_reconstruction(self, recon):
+        """0 = PPMC (default), 1 = PLMC, 2 = PCM (P:L336)."""
+        if lib().ref_set_reconstruction(self._h, int(recon)) != 0:
+            raise ValueError("ref_set_reconstruction: " + lib().ref_last_error().decode())
+
     def step(self, dt):
         if lib().ref_step(self._h, dt) != 0:
             raise ValueError("ref_step: " + lib().ref_last_error().decode())
@@ -183,3 +190,11 @@ def riemann_roe(gamma, WL, WR):
     f = np.empty(5)
     path = lib().ref_riemann_roe(gamma, _p(WL), _p(WR), _p(f))
     return f, ROE_PATHS[path]
+
+
+def plmc_cell(gamma, dtdx, w):
+    """PLMC (A.2): w[5 cells i-2..i+2][5 comps] (only i-1..i+1 used) -> (WL, WR, WLstar, WRstar)."""
+    w = _arr(w); assert w.shape == (5, 5)
+    out = np.empty((4, 5))
+    lib().ref_plmc_cell(gamma, dtdx, _p(w), _p(out))
+    return out[0], out[1], out[2], out[3]
