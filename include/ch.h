@@ -131,6 +131,14 @@ enum { CH_SOLVER_EXACT = 0, CH_SOLVER_ROE = 1 };
 /* ch_set_solver — select the Riemann solver for later steps.  CH_EINVAL for an unknown code. */
 int ch_set_solver(ch_ctx* ctx, int solver);
 
+/* Interface reconstruction used by ch_step.  CH_RECON_PPMC (default): A.3.  CH_RECON_PLMC: piecewise
+ * linear, limited in the characteristic variables, with characteristic tracing, A.2.
+ * CH_RECON_PCM: piecewise constant, Eq. 25-26. */
+enum { CH_RECON_PPMC = 0, CH_RECON_PLMC = 1, CH_RECON_PCM = 2 };
+
+/* ch_set_reconstruction — select the reconstruction for later steps.  CH_EINVAL for an unknown code. */
+int ch_set_reconstruction(ch_ctx* ctx, int recon);
+
 /* ch_sync — block until all work queued on the context's stream has finished. */
 int ch_sync(ch_ctx* ctx);
 

@@ -21,12 +21,13 @@ _HEADERS = [os.path.join(_CSRC, "ch_hydro.cuh"), os.path.join(os.path.dirname(_H
 
 PERIODIC, REFLECTIVE, OUTFLOW = 1, 2, 3
 SOLVER_EXACT, SOLVER_ROE = 0, 1
+RECON_PPMC, RECON_PLMC, RECON_PCM = 0, 1, 2
 CH_OK, CH_EINVAL, CH_ESTATE, CH_ECUDA, CH_ENONPHYS = 0, -1, -2, -3, -4
 
 # every symbol include/ch.h declares
 SYMBOLS = ("ch_init", "ch_free", "ch_last_error", "ch_set_spacing", "ch_padded_cells", "ch_workspace_bytes",
            "ch_bind", "ch_set_state", "ch_get_state", "ch_set_padded", "ch_get_padded", "ch_compute_dt",
-           "ch_step", "ch_set_solver", "ch_sync", "ch_kernel_launches", "ch_profile", "ch_profile_read", "ch_kernel_name",
+           "ch_step", "ch_set_solver", "ch_set_reconstruction", "ch_sync", "ch_kernel_launches", "ch_profile", "ch_profile_read", "ch_kernel_name",
            "ch_fp64_peak_probe")
 K_COUNT = 9
 
@@ -81,6 +82,7 @@ def load_library() -> C.CDLL:
     L.ch_compute_dt.argtypes = [vp, C.c_double]
     L.ch_step.argtypes = [vp, C.c_double]
     L.ch_set_solver.argtypes = [vp, C.c_int]
+    L.ch_set_reconstruction.argtypes = [vp, C.c_int]
     L.ch_sync.argtypes = [vp]
     L.ch_kernel_launches.restype = C.c_longlong
     L.ch_kernel_launches.argtypes = [vp]
@@ -203,6 +205,10 @@ class Grid:
     def set_solver(self, solver):
         """0 = exact (default), 1 = Roe with the HLLE failsafe."""
         self._check(self._L.ch_set_solver(self._h, int(solver)), "ch_set_solver")
+
+    def set_reconstruction(self, recon):
+        """0 = PPMC (default), 1 = PLMC, 2 = PCM."""
+        self._check(self._L.ch_set_reconstruction(self._h, int(recon)), "ch_set_reconstruction")
 
     def sync(self):
         self._check(self._L.ch_sync(self._h), "ch_sync")

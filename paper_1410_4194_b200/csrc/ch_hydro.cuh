@@ -243,6 +243,72 @@ CH_D void ppmc_faces(const Gas& G, double dtdx, const double wm[5], const double
   WRs[0] = WRp[0] + sR0; WRs[1] = WRp[1] + sR1; WRs[2] = WRp[2] + sR2; WRs[3] = WRp[3] + sR3; WRs[4] = WRp[4] + sR4;
 }
 
+// PLMC for one cell (A.2): faces A12 from the limited slope dw0 of this cell, monotonised A13,
+// slope A14, characteristic tracing A15-A19 (A19's contact term restored, reading G10).
+CH_D void plmc_faces(const Gas& G, double dtdx, const double wm[5], const double w0[5], const double wp[5],
+                     const double dw0[5], double s, double WLs[5], double WRs[5]) {
+  double WL[5], WR[5], dwi[5];
+#pragma unroll
+  for (int m = 0; m < 5; ++m) {
+    const double wi = w0[m];
+    double L = wi - 0.5 * dw0[m], R = wi + 0.5 * dw0[m];               // A12
+    {                                                                  // A13
+      const bool up = wm[m] < wi;
+      const double lo = up ? wm[m] : wi, hi = up ? wi : wm[m];
+      L = sel_min(hi, sel_max(lo, L));
+    }
+    {
+      const bool up = wp[m] < wi;
+      const double lo = up ? wp[m] : wi, hi = up ? wi : wp[m];
+      R = sel_min(hi, sel_max(lo, R));
+    }
+    WL[m] = L; WR[m] = R; dwi[m] = R - L;                              // A14
+  }
+  const double rho = w0[0];
+  const double a = G.gamma * w0[4] * s;
+  const double ia = rho * s, ia2 = ia * ia, ra = rho * ia, rhoa = rho * a;
+  const double lm = w0[1] - a, l0 = w0[1], lp = w0[1] + a;            // A8
+  const double h = 0.5 * dtdx;
+  double sL0 = 0.0, sL1 = 0.0, sL2 = 0.0, sL3 = 0.0, sL4 = 0.0;
+  double sR0 = 0.0, sR1 = 0.0, sR2 = 0.0, sR3 = 0.0, sR4 = 0.0;
+  if (l0 < 0.0) {   // A17 contact term
+    const double c = lm - l0;
+    sL0 += c * (dwi[0] - dwi[4] * ia2); sL2 += c * dwi[2]; sL3 += c * dwi[3];
+  }
+  if (lp < 0.0) {   // A17 right acoustic term
+    const double c = 0.5 * (lm - lp);
+    sL0 += c * (ra * dwi[1] + dwi[4] * ia2); sL1 += c * (dwi[1] + dwi[4] * s); sL4 += c * (rhoa * dwi[1] + dwi[4]);
+  }
+  if (lm > 0.0) {   // A19 left acoustic term
+    const double c = 0.5 * (lp - lm);
+    sR0 += c * (dwi[4] * ia2 - ra * dwi[1]); sR1 += c * (dwi[1] - dwi[4] * s); sR4 += c * (dwi[4] - rhoa * dwi[1]);
+  }
+  if (l0 > 0.0) {   // A19 contact term
+    const double c = lp - l0;
+    sR0 += c * (dwi[0] - dwi[4] * ia2); sR2 += c * dwi[2]; sR3 += c * dwi[3];
+  }
+  const double cl = h * sel_min(lm, 0.0), cr = h * sel_max(lp, 0.0);   // A15
+  const double sLv[5] = {sL0, sL1, sL2, sL3, sL4}, sRv[5] = {sR0, sR1, sR2, sR3, sR4};
+#pragma unroll
+  for (int m = 0; m < 5; ++m) {
+    WLs[m] = (WL[m] - cl * dwi[m]) + h * sLv[m];                       // A16
+    WRs[m] = (WR[m] - cr * dwi[m]) + h * sRv[m];                       // A18
+  }
+}
+
+// Reconstruction selection at compile time: 0 PPMC, 1 PLMC, 2 PCM (Eq. 25-26: the cell average).
+template <int R>
+CH_D void recon_faces(const Gas& G, double dtdx, const double wm[5], const double w0[5], const double wp[5],
+                      const double dwm[5], const double dw0[5], const double dwp[5], double s, double WLs[5],
+                      double WRs[5]) {
+  if (R == 0) ppmc_faces(G, dtdx, wm, w0, wp, dwm, dw0, dwp, s, WLs, WRs);
+  else if (R == 1) plmc_faces(G, dtdx, wm, w0, wp, dw0, s, WLs, WRs);
+  else {
+#pragma unroll
+    for (int m = 0; m < 5; ++m) { WLs[m] = w0[m]; WRs[m] = w0[m]; }
+  }
+}
+
 // (1 + t)^z - 1 for |t| <= kPowRadius: 13-term binomial series in Horner form (truncation
 // C(z,14) 16^-14 < 1e-18).  Returns the value WITHOUT the leading 1 so that f_k = 2a/(gamma-1) (x-1)
 // (B5) does not cancel.

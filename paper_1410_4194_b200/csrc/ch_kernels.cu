@@ -118,7 +118,7 @@ __device__ __forceinline__ void copy5(double dst[5], const double src[5]) {
 #define CH_P2_MINB 1
 #endif
 
-template <int D, int S>
+template <int D, int S, int R>
 __global__ void __launch_bounds__(CH_MARCH_T, CH_MARCH_MINB) k_pass1_march(const StepArgs A, int seg) {
   constexpr int T = 3 - D;   // the other transverse dimension (x is the lane dimension)
   const Geom& g = A.geo;
@@ -163,7 +163,7 @@ __global__ void __launch_bounds__(CH_MARCH_T, CH_MARCH_MINB) k_pass1_march(const
     icc = ch::inv_rho_a(G, wc[0], wc[4]);
     ch::limited_slope(G, wb, wc, wd, icc, sc);
     double WLs[5], WRs[5], cl[5], cr[5];
-    ch::ppmc_faces(G, dtdx, wa, wb, wc, sa, sb, sc, icb, WLs, WRs);
+    ch::recon_faces<R>(G, dtdx, wa, wb, wc, sa, sb, sc, icb, WLs, WRs);
     ch::prim2cons(G, WLs, cl);     // states are kept conserved between stages
     ch::prim2cons(G, WRs, cr);
     if (c < c1 || last) {
@@ -194,7 +194,7 @@ __global__ void __launch_bounds__(CH_MARCH_T, CH_MARCH_MINB) k_pass1_march(const
 constexpr int kXT = CH_X_T;    // threads per CTA
 constexpr int kXOut = kXT - 5; // interfaces produced per CTA
 
-template <int S>
+template <int S, int R>
 __global__ void __launch_bounds__(kXT, CH_X_MINB) k_pass1_x(const StepArgs A, long long q_begin, long long q_end) {
   __shared__ double sP[5][kXT];
   __shared__ double sS[5][kXT];
@@ -243,7 +243,7 @@ __global__ void __launch_bounds__(kXT, CH_X_MINB) k_pass1_x(const StepArgs A, lo
     double sm[5], sp[5], WLs[5], WRs[5], cl[5], cr[5];
 #pragma unroll
     for (int m = 0; m < 5; ++m) { sm[m] = sS[m][tid - 1]; sp[m] = sS[m][tid + 1]; }
-    ch::ppmc_faces(G, A.dtdx[0], wm, w0, wp, sm, s0, sp, ic, WLs, WRs);
+    ch::recon_faces<R>(G, A.dtdx[0], wm, w0, wp, sm, s0, sp, ic, WLs, WRs);
     ch::prim2cons(G, WLs, cl);
     ch::prim2cons(G, WRs, cr);
     // a cell's faces are written by the CTA whose output window [2, kXT-4] holds it, plus the
@@ -978,6 +978,7 @@ struct ch_ctx {
   bool tma_ok = false;       // tensor maps built for the bound buffers
   TmaMaps maps;
   int solver = 0;            // CH_SOLVER_EXACT
+  int recon = 0;             // CH_RECON_PPMC
   bool unfused = false;      // CH_UNFUSED=1: k_pass2 + k_update on 3-D grids too (A/B measurements, instruction counts)
   // optional per-kernel timing (ch_profile): one event pair per kernel kind
   bool profiling = false;
@@ -1272,7 +1273,7 @@ double ch_compute_dt(ch_ctx* c, double cfl) {
 namespace {
 
 // One CTU step with Riemann solver S (0 exact, 1 Roe + HLLE) compiled into every kernel that solves.
-template <int S>
+template <int S, int R>
 int step_impl(ch_ctx* c, double dt) {
   if (!c) return fail(CH_EINVAL, "ch_step: null context");
   if (!c->have_state) return fail(CH_ESTATE, "ch_step: no state set");
@@ -1290,7 +1291,7 @@ int step_impl(ch_ctx* c, double dt) {
     const long long qe = (long long)j1 * g.st[1] + (long long)k1 * g.st[2] + g.pd[0];
     const long long nb = (qe - qb + kXOut - 1) / kXOut;
     Bracket b(c, CH_K_PASS1_X);
-    k_pass1_x<S><<<(unsigned)nb, kXT, 0, st>>>(A, qb, qe);
+    k_pass1_x<S, R><<<(unsigned)nb, kXT, 0, st>>>(A, qb, qe);
   }
   for (int d = 1; d < 3; ++d) {
     if (!g.act[d]) continue;
@@ -1299,8 +1300,8 @@ int step_impl(ch_ctx* c, double dt) {
     const int seg = c->march_seg;
     dim3 grid((unsigned)((cols + CH_MARCH_T - 1) / CH_MARCH_T), (unsigned)((g.n[d] + 1 + seg - 1) / seg));
     Bracket b(c, d == 1 ? CH_K_PASS1_Y : CH_K_PASS1_Z);
-    if (d == 1) k_pass1_march<1, S><<<grid, CH_MARCH_T, 0, st>>>(A, seg);
-    else k_pass1_march<2, S><<<grid, CH_MARCH_T, 0, st>>>(A, seg);
+    if (d == 1) k_pass1_march<1, S, R><<<grid, CH_MARCH_T, 0, st>>>(A, seg);
+    else k_pass1_march<2, S, R><<<grid, CH_MARCH_T, 0, st>>>(A, seg);
   }
   CH_CUDA(cudaGetLastError(), "pass 1");
   if (g.act[0] && g.act[1] && g.act[2] && !c->unfused) {
@@ -1353,7 +1354,20 @@ extern "C" {
 
 int ch_step(ch_ctx* c, double dt) {
   if (!c) return fail(CH_EINVAL, "ch_step: null context");
-  return c->solver == CH_SOLVER_ROE ? step_impl<1>(c, dt) : step_impl<0>(c, dt);
+  const bool roe = c->solver == CH_SOLVER_ROE;
+  switch (c->recon) {
+    case CH_RECON_PLMC: return roe ? step_impl<1, 1>(c, dt) : step_impl<0, 1>(c, dt);
+    case CH_RECON_PCM: return roe ? step_impl<1, 2>(c, dt) : step_impl<0, 2>(c, dt);
+    default: return roe ? step_impl<1, 0>(c, dt) : step_impl<0, 0>(c, dt);
+  }
+}
+
+int ch_set_reconstruction(ch_ctx* c, int recon) {
+  if (!c) return fail(CH_EINVAL, "ch_set_reconstruction: null context");
+  if (recon != CH_RECON_PPMC && recon != CH_RECON_PLMC && recon != CH_RECON_PCM)
+    return fail(CH_EINVAL, "ch_set_reconstruction: unknown reconstruction");
+  c->recon = recon;
+  return CH_OK;
 }
 
 int ch_set_solver(ch_ctx* c, int solver) {

@@ -476,3 +476,60 @@ def test_roe_tma_and_plain_forms_agree(ch, monkeypatch):
         G.close()
     assert np.all(np.isfinite(res["0"]))
     assert max(max_rel_error(res["0"], res["1"], w.gamma)) <= 1e-14
+
+
+# ---- NEXT-2: PLMC and PCM reconstructions (A.2, Eq. 25-26) --------------------------------------------
+RECON_CASES = {
+    "sod_1d_128": lambda: wl.sod(128),
+    "sod_along_y": lambda: wl.sod(128, axis=1, n_other=4),
+    "kh_2d_128": lambda: wl.kelvin_helmholtz(128),
+    "sedov_32": lambda: wl.sedov(32),
+    "sweep_ragged_3d_tma": lambda: wl.sweep(shape=(270, 44, 36)),
+    "sweep_ragged_3d_plain": lambda: wl.sweep(shape=(135, 45, 37)),
+    "rough_3d": lambda: wl.rough_random(38, 21, 13, seed=11, decades=0.5),
+    "smooth_mixed_bc": lambda: wl.smooth_random(41, 29, 23, seed=5, bc=(R, O, P, P, O, R)),
+}
+
+
+@pytest.mark.parametrize("solver", [0, 1])
+@pytest.mark.parametrize("recon", [1, 2])
+@pytest.mark.parametrize("name", sorted(RECON_CASES))
+def test_plmc_pcm_one_step_parity(ch, ref, name, recon, solver):
+    w = RECON_CASES[name]()
+    G, Rg = both(ch, ref, w)
+    for g in (G, Rg):
+        g.set_reconstruction(recon)
+        g.set_solver(solver)
+        g.set_state(w.u)
+    dt = Rg.compute_dt(w.cfl)
+    G.step(dt); Rg.step(dt)
+    ur = Rg.get_state()
+    assert np.all(np.isfinite(ur))
+    assert max(max_rel_error(G.get_state(), ur, w.gamma)) <= ONE_STEP_TOL, (name, recon, solver)
+    G.close()
+
+
+def test_plmc_pcm_runs_match_oracle_and_switch_back(ch, ref):
+    for recon in (1, 2):
+        for w in (wl.sod(128), wl.sweep(shape=(56, 40, 36), steps=12)):
+            G, Rg = both(ch, ref, w)
+            G.set_reconstruction(recon); Rg.set_reconstruction(recon)
+            dts = []
+            run(Rg, w, record_dts=dts)
+            run(G, w, dts=dts)
+            assert max(rel_l1_error(G.get_state(), Rg.get_state(), w.gamma)) <= RUN_L1_TOL
+            G.close()
+    w = wl.sod(128)
+    G = ch.Grid(*w.shape, 3, w.gamma, w.bc)
+    outs = []
+    for recon in (0, 1, 2, 0):
+        G.set_reconstruction(recon)
+        G.set_state(w.u)
+        for _ in range(5):
+            G.step(G.compute_dt(w.cfl))
+        outs.append(G.get_state())
+    assert np.array_equal(outs[0], outs[3])
+    assert not np.array_equal(outs[0], outs[1]) and not np.array_equal(outs[1], outs[2])
+    with pytest.raises(ValueError):
+        G.set_reconstruction(5)
+    G.close()
