@@ -10,6 +10,8 @@
 //                      16-byte stride rules do not hold, or with CH_TMA=0)
 //   k_pass2, k_update  the same two halves unfused, for 1-D / 2-D grids
 //   k_ghost            ghost fill of the new state
+// Every kernel that reconstructs or solves is a template on the reconstruction (PPMC / PLMC / PCM) and on the
+// Riemann solver (exact / Roe + HLLE); the defaults are the paper's PPMC + exact.
 // Data layout: struct-of-arrays fp64, x fastest, ghosts included; every kernel maps
 // consecutive lanes to consecutive x so loads and stores coalesce.  No operand is reshaped for
 // tensor cores: this is a stencil / ALU path.
