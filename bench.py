@@ -50,6 +50,10 @@ def parse():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-other-workloads", action="store_true")
+    ap.add_argument("--solver", type=str, default="exact", choices=["exact", "roe"],
+                    help="Riemann solver of the main measured workload (default: the metric's exact solver)")
+    ap.add_argument("--recon", type=str, default="ppmc", choices=["ppmc", "plmc", "pcm"],
+                    help="reconstruction of the main measured workload (default: the metric's PPM)")
     return ap.parse_args()
 
 
@@ -165,13 +169,15 @@ def timed_steps(G, cfl, steps, stream_events):
     return e0.elapsed_time(e1) * 1e-3
 
 
-def bench_size(pkg, wl, n, steps, warmup, device, dist=None, profile=True, e2e=True):
+def bench_size(pkg, wl, n, steps, warmup, device, dist=None, profile=True, e2e=True, solver=0, recon=0):
     import numpy as np
     import torch
     from paper_1410_4194_b200.driver import max_over_ranks
     w = wl.sweep(n)
     N = n ** 3
     G = pkg.Grid(n, n, n, 3, w.gamma, w.bc, device=device)
+    G.set_solver(solver)
+    G.set_reconstruction(recon)
     u_dev = torch.from_numpy(w.u).to(device)
     G.set_state(u_dev)
     ev = (torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
@@ -246,14 +252,18 @@ def main():
 
     sampler = ClockSampler(local) if rank == 0 else None
     peak_tf, _ = fp64_peak_probe(device=device)                 # measured DFMA rate, burst
+    solver = {"exact": 0, "roe": 1}[args.solver]
+    recon = {"ppmc": 0, "plmc": 1, "pcm": 2}[args.recon]
+    default_method = solver == 0 and recon == 0
     main_res, w = bench_size(pkg, wl, args.size, args.steps, args.warmup, device, dist,
-                             profile=True, e2e=not args.no_e2e)
+                             profile=True, e2e=not args.no_e2e, solver=solver, recon=recon)
     clocks = sampler.stop() if sampler else None
     others = {}
     if world == 1:
         for s in [int(x) for x in args.other_sizes.split(",") if x]:
             if s != args.size:
-                r, _ = bench_size(pkg, wl, s, args.steps, args.warmup, device, None, profile=False, e2e=False)
+                r, _ = bench_size(pkg, wl, s, args.steps, args.warmup, device, None, profile=False, e2e=False,
+                                  solver=solver, recon=recon)
                 others[str(s)] = {"value": r["cells"] * args.steps / r["seconds"], "unit": UNIT,
                                   "ms_per_step": r["seconds"] / args.steps * 1e3}
     other_wl = {}
@@ -309,8 +319,10 @@ def main():
             continue
         t = v["ms_avg"] * 1e-3
         gbs = rf.ALG_BYTES[k] * N / t / 1e9
-        tfs = rf.ALG_FLOPS[k] * N / t / 1e12
-        t_h, t_a = rf.ALG_BYTES[k] * N / (hbm_gbs * 1e9), rf.ALG_FLOPS[k] * N / (peak_tf * 1e12)
+        # the frozen flop counts belong to PPMC + exact; other method choices are charged bytes only
+        flops = rf.ALG_FLOPS[k] if default_method else 0.0
+        tfs = flops * N / t / 1e12
+        t_h, t_a = rf.ALG_BYTES[k] * N / (hbm_gbs * 1e9), flops * N / (peak_tf * 1e12)
         t_roof_step += max(t_h, t_a) * v["launches_per_step"]
         per_kernel[k] = {"ms": v["ms_avg"], "bound": "hbm" if t_h >= t_a else "alu",
                          "hbm_GBps": gbs, "hbm_frac": gbs / hbm_gbs, "fp64_TFLOPs": tfs, "fp64_frac": tfs / peak_tf,
@@ -325,7 +337,7 @@ def main():
                 f"{sm_mhz:.0f} MHz = {rf.nominal_fp64_tflops(sm_mhz):.1f}")
     step_ms = main_res["seconds"] / K * 1e3
     roofline = {"bound": pk["bound"], "kernel": top, "achieved": ach, "peak": peak, "unit": unit,
-                "frac": ach / peak, "traffic": TRAFFIC_NCU.get(top),
+                "frac": ach / peak, "traffic": TRAFFIC_NCU.get(top) if default_method else None,
                 "traffic_note": "dram__bytes_read.sum + dram__bytes_write.sum per launch from profiles/ (ncu --set full, 512^3)",
                 "peak_source": psrc,
                 "alg_bytes_per_cell": rf.ALG_BYTES[top], "alg_flops_per_cell": rf.ALG_FLOPS[top],
@@ -341,6 +353,7 @@ def main():
             "config": {"workload": f"throughput sweep (BASELINE.json config 5) {args.size}^3 periodic, "
                                    "sum of 8 seeded sinusoids, 1 replica per GPU",
                        "gamma": w.gamma, "cfl": w.cfl, "nghost": 3, "l2": "state (5 fields) larger than L2, no flush",
+                       "reconstruction": args.recon, "riemann_solver": args.solver,
                        "parallelism": "replicas only" if world > 1 else "single GPU"},
             "gpu_launches": main_res["launches"], "clocks": clocks, "roofline": roofline}
     if others:
