@@ -394,7 +394,7 @@ void flux_eq11(double gamma, const double W[5], double U[5], double F[5]) {   //
   F[4] = (E + p) * u;
 }
 
-void riemann_roe(double gamma, const double WL[5], const double WR[5], double flux[5], int* path) {
+void riemann_roe(double gamma, const double WL[5], const double WR[5], double flux[5], int* path, double etaH = 0.0) {
   double UL[5], UR[5], FL[5], FR[5];
   flux_eq11(gamma, WL, UL, FL);
   flux_eq11(gamma, WR, UR, FR);
@@ -425,8 +425,9 @@ void riemann_roe(double gamma, const double WL[5], const double WR[5], double fl
   xi[4] = dU[0] * Na * (0.5 * gp * V2 - ut * at) - dU[1] * Na * (gp * ut - at) - dU[2] * Na * gp * vt -
           dU[3] * Na * gp * wt + dU[4] * Na * gp;
   // B28
-  const double C0 = xi[0] * std::fabs(lm), C1 = xi[1] * std::fabs(l0), C2 = xi[2] * std::fabs(l0),
-               C3 = xi[3] * std::fabs(l0), C4 = xi[4] * std::fabs(lp);
+  // C3: with the H correction |lambda| -> max(|lambda|, eta^H) here and only here (reading S18)
+  const double alm = std::max(std::fabs(lm), etaH), al0 = std::max(std::fabs(l0), etaH), alp = std::max(std::fabs(lp), etaH);
+  const double C0 = xi[0] * alm, C1 = xi[1] * al0, C2 = xi[2] * al0, C3 = xi[3] * al0, C4 = xi[4] * alp;
   // B29
   double sv[5];
   sv[0] = C0 + C3 + C4;
@@ -467,13 +468,13 @@ void riemann_roe(double gamma, const double WL[5], const double WR[5], double fl
 }
 
 // Riemann problem at an interface normal to d from two conserved states in GLOBAL order.
-void riemann_interface(double gamma, int solver, int d, const double UL[5], const double UR[5], double F[5]) {
+void riemann_interface(double gamma, int solver, int d, const double UL[5], const double UR[5], double F[5], double etaH = 0.0) {
   double wl[5], wr[5], ll[5], lr[5], fl[5];
   cons_to_prim(gamma, UL, wl);
   cons_to_prim(gamma, UR, wr);
   to_local(d, wl, ll);
   to_local(d, wr, lr);
-  if (solver == SOLVER_ROE) riemann_roe(gamma, ll, lr, fl, nullptr);
+  if (solver == SOLVER_ROE) riemann_roe(gamma, ll, lr, fl, nullptr, etaH);
   else riemann_exact(gamma, ll, lr, fl, nullptr);
   to_global(d, fl, F);
 }
@@ -490,6 +491,7 @@ struct Ctx {
   bool have_state = false;
   int solver = SOLVER_EXACT;
   int recon = RECON_PPMC;
+  bool hcorr = false;   // H correction (Appendix C): Roe solver only, second Riemann pass only, needs g >= 4
   std::vector<double> u;  // [5][np], x fastest
   inline long idx(int i, int j, int k) const {  // real-cell coordinates, ghosts negative / >= n
     return ((long)(k + gd[2]) * pd[1] + (j + gd[1])) * pd[0] + (i + gd[0]);
@@ -584,14 +586,18 @@ void ctu_step(Ctx& c, double dt) {
   };
   const long stride[3] = {1, c.pd[0], (long)c.pd[0] * c.pd[1]};
 
+  // With the H correction the second-pass states are also needed one cell further out in the transverse
+  // directions (eta of the neighbouring interfaces, C2), hence F* one interface further out along its own
+  // direction, hence U* one cell further out: "an extra ghost cell on each side".
+  const int X = c.hcorr ? 2 : 1;
   // Step 1: U*_L, U*_R per direction (conserved, global order) — O2.
-  std::vector<double> UsL[3], UsR[3], Fs[3], UhL[3], UhR[3], Fh[3];
+  std::vector<double> UsL[3], UsR[3], Fs[3], UhL[3], UhR[3], Fh[3], eta[3];
   for (int d = 0; d < 3; ++d) {
     if (!c.active[d]) continue;
     UsL[d].assign(5 * np, 0.0);
     UsR[d].assign(5 * np, 0.0);
     int lo[3], hi[3];
-    for (int e = 0; e < 3; ++e) range(e, 1, lo[e], hi[e]);
+    for (int e = 0; e < 3; ++e) range(e, X, lo[e], hi[e]);
     const double dtdx = dt / c.dx[d];
 #pragma omp parallel for collapse(2)
     for (int k = lo[2]; k < hi[2]; ++k)
@@ -622,8 +628,8 @@ void ctu_step(Ctx& c, double dt) {
     if (!c.active[d]) continue;
     Fs[d].assign(5 * np, 0.0);
     int lo[3], hi[3];
-    for (int e = 0; e < 3; ++e) range(e, 1, lo[e], hi[e]);
-    hi[d] -= 1;  // interfaces c in [-1, n-1]
+    for (int e = 0; e < 3; ++e) range(e, X, lo[e], hi[e]);
+    hi[d] -= 1;  // interfaces c in [-X, n+X-2]
 #pragma omp parallel for collapse(2)
     for (int k = lo[2]; k < hi[2]; ++k)
       for (int j = lo[1]; j < hi[1]; ++j)
@@ -641,7 +647,7 @@ void ctu_step(Ctx& c, double dt) {
     UhL[d].assign(5 * np, 0.0);
     UhR[d].assign(5 * np, 0.0);
     int lo[3], hi[3];
-    for (int e = 0; e < 3; ++e) range(e, e == d ? 1 : 0, lo[e], hi[e]);
+    for (int e = 0; e < 3; ++e) range(e, (e == d || c.hcorr) ? 1 : 0, lo[e], hi[e]);
 #pragma omp parallel for collapse(2)
     for (int k = lo[2]; k < hi[2]; ++k)
       for (int j = lo[1]; j < hi[1]; ++j)
@@ -659,6 +665,29 @@ void ctu_step(Ctx& c, double dt) {
           }
         }
   }
+  // Step 3b (H correction, C1 P:L1281): eta = |(u_R + a_R) - (u_L + a_L)| / 2 at every interface from the
+  // second-pass input states, normal velocity and sound speed of each side.
+  if (c.hcorr) {
+    for (int d = 0; d < 3; ++d) {
+      if (!c.active[d]) continue;
+      eta[d].assign(np, 0.0);
+      int lo[3], hi[3];
+      for (int e = 0; e < 3; ++e) range(e, 1, lo[e], hi[e]);
+      hi[d] -= 1;
+#pragma omp parallel for collapse(2)
+      for (int k = lo[2]; k < hi[2]; ++k)
+        for (int j = lo[1]; j < hi[1]; ++j)
+          for (int i = lo[0]; i < hi[0]; ++i) {
+            const long q = c.idx(i, j, k), qp = q + stride[d];
+            double UL[5], UR[5], wl[5], wr[5];
+            for (int f = 0; f < 5; ++f) { UL[f] = UhR[d][f * np + q]; UR[f] = UhL[d][f * np + qp]; }
+            cons_to_prim(gamma, UL, wl);
+            cons_to_prim(gamma, UR, wr);
+            const double aL = std::sqrt(gamma * wl[4] / wl[0]), aR = std::sqrt(gamma * wr[4] / wr[0]);
+            eta[d][q] = 0.5 * std::fabs((wr[1 + d] + aR) - (wl[1 + d] + aL));
+          }
+    }
+  }
   // Step 4: CTU fluxes — O5.
   for (int d = 0; d < 3; ++d) {
     if (!c.active[d]) continue;
@@ -673,7 +702,18 @@ void ctu_step(Ctx& c, double dt) {
           const long q = c.idx(i, j, k), qp = q + stride[d];
           double UL[5], UR[5], F[5];
           for (int f = 0; f < 5; ++f) { UL[f] = UhR[d][f * np + q]; UR[f] = UhL[d][f * np + qp]; }
-          riemann_interface(gamma, c.solver, d, UL, UR, F);
+          double etaH = 0.0;
+          if (c.hcorr) {
+            // C2 read with the cells that share the interface (reading G11): the interface's own eta
+            // and, for each transverse direction, eta on the two faces of cell c and of cell c+1
+            etaH = eta[d][q];
+            for (int e = 0; e < 3; ++e) {
+              if (e == d || !c.active[e]) continue;
+              etaH = std::max(etaH, std::max(std::max(eta[e][q - stride[e]], eta[e][q]),
+                                             std::max(eta[e][qp - stride[e]], eta[e][qp])));
+            }
+          }
+          riemann_interface(gamma, c.solver, d, UL, UR, F, etaH);
           for (int f = 0; f < 5; ++f) Fh[d][f * np + q] = F[f];
         }
   }
@@ -796,6 +836,7 @@ int ref_step(void* h, double dt) {
   Ctx* c = static_cast<Ctx*>(h);
   if (!c->have_state) return fail("no state");
   if (!(dt > 0.0) || !std::isfinite(dt)) return fail("bad dt");
+  if (c->hcorr && c->solver != SOLVER_ROE) return fail("the H correction goes with the Roe solver (P:L1279)");
   ctu_step(*c, dt);
   return 0;
 }
@@ -829,6 +870,18 @@ void ref_plmc_cell(double gamma, double dtdx, const double* w, double* out) {
   double ws[5][5];
   for (int s = 0; s < 5; ++s) for (int m = 0; m < 5; ++m) ws[s][m] = w[s * 5 + m];
   plmc_cell(gamma, dtdx, ws, out, out + 5, out + 10, out + 15);
+}
+int ref_set_hcorrection(void* h, int on) {
+  if (!h) return fail("ref_set_hcorrection: null");
+  Ctx& c = *static_cast<Ctx*>(h);
+  if (on && c.g < 4) return fail("ref_set_hcorrection: needs nghost >= 4 (P:L1291)");
+  c.hcorr = on != 0;
+  return 0;
+}
+int ref_riemann_roe_eta(double gamma, const double* WL, const double* WR, double etaH, double* flux) {
+  int path = -1;
+  riemann_roe(gamma, WL, WR, flux, &path, etaH);
+  return path;
 }
 int ref_riemann_roe(double gamma, const double* WL, const double* WR, double* flux) {
   int path = -1;

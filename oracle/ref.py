@@ -59,6 +59,9 @@ def lib() -> C.CDLL:
         L.ref_riemann_roe.restype = C.c_int
         L.ref_set_solver.argtypes = [C.c_void_p, C.c_int]
         L.ref_set_reconstruction.argtypes = [C.c_void_p, C.c_int]
+        L.ref_set_hcorrection.argtypes = [C.c_void_p, C.c_int]
+        L.ref_riemann_roe_eta.argtypes = [C.c_double, dp, dp, C.c_double, dp]
+        L.ref_riemann_roe_eta.restype = C.c_int
         L.ref_plmc_cell.argtypes = [C.c_double, C.c_double, dp, dp]
         _lib = L
     return _lib
@@ -123,6 +126,11 @@ class RefGrid:
         """0 = exact (default), 1 = Roe with the HLLE failsafe (the solver is selectable)."""
         if lib().ref_set_solver(self._h, int(solver)) != 0:
             raise ValueError("ref_set_solver: " + lib().ref_last_error().decode())
+
+    def set_hcorrection(self, on):
+        """H correction (Appendix C): Roe solver only, nghost >= 4."""
+        if lib().ref_set_hcorrection(self._h, int(bool(on))) != 0:
+            raise ValueError("ref_set_hcorrection: " + lib().ref_last_error().decode())
 
     def set_reconstruction(self, recon):
         """0 = PPMC (default), 1 = PLMC, 2 = PCM (P:L336)."""
@@ -198,3 +206,11 @@ def plmc_cell(gamma, dtdx, w):
     out = np.empty((4, 5))
     lib().ref_plmc_cell(gamma, dtdx, _p(w), _p(out))
     return out[0], out[1], out[2], out[3]
+
+
+def riemann_roe_eta(gamma, WL, WR, eta_h):
+    """Roe solver with |lambda| -> max(|lambda|, eta_h) in B28 (H correction, C3) -> (flux[5], path)."""
+    WL, WR = _arr(WL), _arr(WR)
+    f = np.empty(5)
+    path = lib().ref_riemann_roe_eta(gamma, _p(WL), _p(WR), float(eta_h), _p(f))
+    return f, ROE_PATHS[path]

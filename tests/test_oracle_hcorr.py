@@ -1,0 +1,175 @@
+"""Pins of the oracle's H correction (oracle/cholla_ref.cpp; Appendix C):
+
+* C3 on one interface: with eta^H above every |lambda| the Roe dissipation sum_k xi_k |lambda_k| r_k becomes
+  eta^H (U_R - U_L) (the right eigenvectors resolve the jump), i.e. the flux is the local Lax-Friedrichs closed
+  form F = (F_L + F_R)/2 - eta^H (U_R - U_L)/2; eta^H = 0 is the plain Roe flux, bitwise;
+* a planar problem has eta = 0 on every transverse interface, so the 1-D run is reproduced bitwise inside a
+  3-D box, and differs from the uncorrected run only through the interface's own eta;
+* C2 gathers the transverse eta the same way for every direction: transposing / cyclically permuting the axes
+  of the data permutes the result (which cells it gathers from, reading G11, is NOT pinned: see DESIGN.md);
+* uniform states, conservation; the correction adds dissipation: a grid-aligned Mach-10 shock with odd-even
+  noise ends with smaller transverse density variation than without it (the carbuncle's seed).
+"""
+import math
+
+import numpy as np
+import pytest
+
+from paper_1410_4194_b200 import workloads as wl
+from paper_1410_4194_b200.driver import run
+
+G = 1.4
+P, R, O = wl.PERIODIC, wl.REFLECTIVE, wl.OUTFLOW
+
+
+def eq11_and_u(W, gamma=G):
+    rho, u, v, w, p = W
+    E = p / (gamma - 1) + 0.5 * rho * (u * u + v * v + w * w)
+    return np.array([rho * u, rho * u * u + p, rho * u * v, rho * u * w, (E + p) * u]), np.array([rho, rho * u, rho * v, rho * w, E])
+
+
+def test_c3_large_eta_is_local_lax_friedrichs_and_zero_eta_is_roe(ref):
+    rng = np.random.default_rng(4)
+    for _ in range(100):
+        WL = [rng.uniform(0.5, 2), rng.normal(0, 0.3), rng.normal(), rng.normal(), rng.uniform(0.5, 2)]
+        WR = [WL[0] * rng.uniform(0.8, 1.25), WL[1] + rng.normal(0, 0.1), rng.normal(), rng.normal(), WL[4] * rng.uniform(0.8, 1.25)]
+        f0, path0 = ref.riemann_roe(G, WL, WR)
+        fz, pathz = ref.riemann_roe_eta(G, WL, WR, 0.0)
+        assert np.array_equal(f0, fz) and path0 == pathz
+        if path0 != "roe":
+            continue
+        eta = 10.0
+        f, path = ref.riemann_roe_eta(G, WL, WR, eta)
+        FL, UL = eq11_and_u(WL); FR, UR = eq11_and_u(WR)
+        assert path == "roe"
+        assert np.allclose(f, 0.5 * (FL + FR) - 0.5 * eta * (UR - UL), rtol=0, atol=1e-12)
+
+
+def grid(ref, w, hc, g=4):
+    Gd = ref.RefGrid(*w.shape, g, w.gamma, w.bc)
+    Gd.set_solver(1)
+    Gd.set_hcorrection(hc)
+    return Gd
+
+
+def test_needs_four_ghosts_and_the_roe_solver(ref):
+    w = wl.sod(32)
+    Gd = ref.RefGrid(*w.shape, 3, w.gamma, w.bc)
+    with pytest.raises(ValueError):
+        Gd.set_hcorrection(True)
+    Gd = ref.RefGrid(*w.shape, 4, w.gamma, w.bc)
+    Gd.set_hcorrection(True)
+    Gd.set_state(w.u)
+    with pytest.raises(ValueError):
+        Gd.step(1e-4)                       # exact solver selected
+
+
+@pytest.mark.parametrize("axis", [0, 1, 2])
+def test_planar_problem_in_3d_equals_the_1d_run_bitwise(ref, axis):
+    n, m = 32, 5
+    one = wl.sod(n)
+    G1 = grid(ref, one, True)
+    dts = []
+    run(G1, one, max_steps=10, record_dts=dts)
+    u1 = G1.get_state()[:, 0, 0, :]
+    shape = [m, m, m]; shape[axis] = n
+    u3 = np.zeros((5, shape[2], shape[1], shape[0]))
+    idx = [None, None, None]; idx[2 - axis] = slice(None)
+    for f_src, f_dst in ((0, 0), (1, 1 + axis), (4, 4)):
+        u3[f_dst] = one.u[:, 0, 0, :][f_src][tuple(idx)]
+    bc = tuple(O if d == axis else P for d in range(3) for _ in range(2))
+    G3 = ref.RefGrid(*shape, 4, one.gamma, bc)
+    G3.set_solver(1); G3.set_hcorrection(True)
+    G3.set_spacing(1.0 / n, 1.0 / n, 1.0 / n)
+    G3.set_state(u3)
+    for dt in dts:
+        G3.step(dt)
+    out = G3.get_state()
+    for f_src, f_dst in ((0, 0), (1, 1 + axis), (4, 4)):
+        assert np.array_equal(out[f_dst], u1[f_src][tuple(idx)] * np.ones_like(out[0]))
+    # and the correction is not a no-op in 1-D: the interface's own eta enters
+    G0 = grid(ref, one, False)
+    run(G0, one, dts=dts)
+    assert not np.array_equal(G0.get_state()[:, 0, 0, :], u1)
+
+
+def test_transposition_symmetry_pins_the_per_direction_indexing_of_c2(ref):
+    """Swapping the x and y axes of the data (and the velocity components) swaps the result: eta of the
+    transverse interfaces is gathered the same way for x-, y- and z-interfaces.  (C1 as printed,
+    |(u_R + a_R) - (u_L + a_L)|/2, is not mirror symmetric, so mirror images are NOT a property of this
+    scheme; which cells C2 gathers from — reading G11 — is argued from the H shape.)"""
+    w = wl.rough_random(20, 20, 1, seed=8, decades=0.3, mach=0.8, bc=(P,) * 6)
+    Gd = grid(ref, w, True)
+    Gd.set_state(w.u)
+    dt = 0.5 * Gd.compute_dt(w.cfl)
+    Gd.step(dt)
+    a = Gd.get_state()
+    ut = np.ascontiguousarray(np.swapaxes(w.u, 2, 3))[[0, 2, 1, 3, 4]]       # transpose, swap rho*vx <-> rho*vy
+    Gt = grid(ref, w, True)
+    Gt.set_state(np.ascontiguousarray(ut))
+    Gt.step(dt)
+    b = np.swapaxes(Gt.get_state(), 2, 3)[[0, 2, 1, 3, 4]]
+    assert np.allclose(a, b, rtol=0, atol=1e-13 * np.abs(a).max())
+    G0 = grid(ref, w, False)
+    G0.set_state(w.u); G0.step(dt)
+    assert np.abs(G0.get_state() - a).max() > 1e-6                   # the correction acts on this problem
+    # 3-D: cyclic permutation x -> y -> z -> x
+    w3 = wl.rough_random(12, 12, 12, seed=9, decades=0.3, mach=0.8, bc=(P,) * 6)
+    G3 = grid(ref, w3, True); G3.set_state(w3.u)
+    dt = 0.5 * G3.compute_dt(w3.cfl)
+    G3.step(dt)
+    a = G3.get_state()
+    # new[x', y', z'] = old[z', x', y'] with (vx', vy', vz') = (vz, vx, vy): array axes (f, z, y, x)
+    up = np.ascontiguousarray(np.transpose(w3.u, (0, 2, 3, 1)))[[0, 3, 1, 2, 4]]
+    Gp = grid(ref, w3, True); Gp.set_state(np.ascontiguousarray(up)); Gp.step(dt)
+    b = np.transpose(Gp.get_state()[[0, 2, 3, 1, 4]], (0, 3, 1, 2))
+    assert np.allclose(a, b, rtol=0, atol=1e-13 * np.abs(a).max())
+
+
+def test_uniform_state_and_conservation(ref):
+    u = wl.conserved(0.7, 0.3, -0.45, 0.21, 1.9, 1.4).reshape(5, 1, 1, 1) * np.ones((5, 6, 7, 8))
+    Gd = ref.RefGrid(8, 7, 6, 4, 1.4, (P,) * 6)
+    Gd.set_solver(1); Gd.set_hcorrection(True)
+    Gd.set_state(u)
+    Gd.step(Gd.compute_dt(0.4))
+    assert np.array_equal(Gd.get_state(), u)
+    w = wl.sweep(shape=(16, 12, 10))
+    Gd = grid(ref, w, True)
+    Gd.set_state(w.u)
+    for _ in range(3):
+        Gd.step(Gd.compute_dt(w.cfl))
+    u1 = Gd.get_state()
+    for f in range(5):
+        assert abs(math.fsum(u1[f].ravel()) - math.fsum(w.u[f].ravel())) <= 1e-13 * (math.fsum(np.abs(w.u[f]).ravel()) + w.u[0].size)
+
+
+def test_adds_crossflow_dissipation_at_a_grid_aligned_shock(ref):
+    """Quirk-type odd-even test: a planar Mach-10 shock moving along x through a 2-D duct whose centre-line
+    density carries an odd-even perturbation.  The transverse (y) variation of the post-shock density is the
+    carbuncle's seed; with the H correction it must be smaller than without."""
+    nx, ny, gamma, M = 96, 12, 1.4, 10.0
+    rho0, p0 = 1.0, 1.0
+    a0 = math.sqrt(gamma * p0 / rho0)
+    r = (gamma + 1) * M * M / ((gamma - 1) * M * M + 2)              # Rankine-Hugoniot
+    p1 = p0 * (2 * gamma * M * M - (gamma - 1)) / (gamma + 1)
+    u1 = M * a0 * (1 - 1 / r)
+    x = (np.arange(nx) + 0.5) / nx
+    rho = np.where(x < 0.1, rho0 * r, rho0)[None, None, :] * np.ones((1, ny, nx))
+    vx = np.where(x < 0.1, u1, 0.0)[None, None, :] * np.ones((1, ny, nx))
+    p = np.where(x < 0.1, p1, p0)[None, None, :] * np.ones((1, ny, nx))
+    rho[0, ny // 2, :] *= 1.0 + 1e-3 * (-1.0) ** np.arange(nx)       # odd-even noise on the centre line
+    u = wl.conserved(rho, vx, 0.0, 0.0, p, gamma)
+    res = {}
+    for hc in (False, True):
+        Gd = ref.RefGrid(nx, ny, 1, 4, gamma, (O, O, P, P, P, P))
+        Gd.set_solver(1); Gd.set_hcorrection(hc)
+        Gd.set_state(u)
+        t = 0.0
+        while t < 0.04:
+            dt = Gd.compute_dt(0.4)
+            Gd.step(dt); t += dt
+        d = Gd.get_state()[0, 0]
+        assert np.all(np.isfinite(d))
+        behind = d[:, (x > 0.15) & (x < 0.1 + M * a0 * 0.04 - 0.05)]
+        res[hc] = float(np.mean(np.std(behind, axis=0)))
+    assert res[True] < res[False], res
