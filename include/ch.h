@@ -77,8 +77,8 @@ int ch_set_spacing(ch_ctx* ctx, double dx, double dy, double dz);
 long long ch_padded_cells(const ch_ctx* ctx);
 
 /* ch_workspace_bytes — bytes of scratch ch_bind needs for this grid: the first-pass fluxes F*,G*,H*
- * (P:L157), the traced interface states U*_L, U*_R per direction and the CTU fluxes
- * F,G,H^{n+1/2}, all padded SoA fp64.  Returns 0 on bad arguments. */
+ * (P:L157), the traced interface states U*_L, U*_R per direction, the CTU fluxes
+ * F,G,H^{n+1/2}, all padded SoA fp64, and the three eta fields of the H correction.  Returns 0 on bad arguments. */
 size_t ch_workspace_bytes(int nx, int ny, int nz, int nghost);
 
 /* ch_bind — attach caller-owned device buffers and the CUDA stream (a cudaStream_t passed as
@@ -136,6 +136,13 @@ int ch_set_solver(ch_ctx* ctx, int solver);
  * CH_RECON_PCM: piecewise constant, Eq. 25-26. */
 enum { CH_RECON_PPMC = 0, CH_RECON_PLMC = 1, CH_RECON_PCM = 2 };
 
+/* ch_set_hcorrection — switch the H correction of Appendix C on or off for later steps: in the
+ * second Riemann pass the Roe eigenvalues of B28 become max(|lambda|, eta^H), eta^H the largest
+ * eta = |(u_R + a_R) - (u_L + a_L)| / 2 over the interface and the transverse faces of the two cells that share
+ * it.  Needs nghost >= 4 (CH_EINVAL otherwise) and CH_SOLVER_ROE (ch_step returns CH_ESTATE otherwise); the
+ * second half of the step then runs unfused. */
+int ch_set_hcorrection(ch_ctx* ctx, int on);
+
 /* ch_set_reconstruction — select the reconstruction for later steps.  CH_EINVAL for an unknown code. */
 int ch_set_reconstruction(ch_ctx* ctx, int recon);
 
@@ -150,6 +157,7 @@ long long ch_kernel_launches(const ch_ctx* ctx);
 enum {
   CH_K_RESET = 0, CH_K_PASS1_X, CH_K_PASS1_Y, CH_K_PASS1_Z, CH_K_PASS2, CH_K_UPDATE, CH_K_GHOST, CH_K_DT,
   CH_K_FINAL, /* fused pass 2 + update of 3-D grids */
+  CH_K_ETA,   /* H correction: eta of every interface */
   CH_K_COUNT
 };
 

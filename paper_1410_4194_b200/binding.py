@@ -27,9 +27,9 @@ CH_OK, CH_EINVAL, CH_ESTATE, CH_ECUDA, CH_ENONPHYS = 0, -1, -2, -3, -4
 # every symbol include/ch.h declares
 SYMBOLS = ("ch_init", "ch_free", "ch_last_error", "ch_set_spacing", "ch_padded_cells", "ch_workspace_bytes",
            "ch_bind", "ch_set_state", "ch_get_state", "ch_set_padded", "ch_get_padded", "ch_compute_dt",
-           "ch_step", "ch_set_solver", "ch_set_reconstruction", "ch_sync", "ch_kernel_launches", "ch_profile", "ch_profile_read", "ch_kernel_name",
+           "ch_step", "ch_set_solver", "ch_set_reconstruction", "ch_set_hcorrection", "ch_sync", "ch_kernel_launches", "ch_profile", "ch_profile_read", "ch_kernel_name",
            "ch_fp64_peak_probe")
-K_COUNT = 9
+K_COUNT = 10
 
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-shared"]
@@ -83,6 +83,7 @@ def load_library() -> C.CDLL:
     L.ch_step.argtypes = [vp, C.c_double]
     L.ch_set_solver.argtypes = [vp, C.c_int]
     L.ch_set_reconstruction.argtypes = [vp, C.c_int]
+    L.ch_set_hcorrection.argtypes = [vp, C.c_int]
     L.ch_sync.argtypes = [vp]
     L.ch_kernel_launches.restype = C.c_longlong
     L.ch_kernel_launches.argtypes = [vp]
@@ -205,6 +206,10 @@ class Grid:
     def set_solver(self, solver):
         """0 = exact (default), 1 = Roe with the HLLE failsafe."""
         self._check(self._L.ch_set_solver(self._h, int(solver)), "ch_set_solver")
+
+    def set_hcorrection(self, on):
+        """H correction (Appendix C): Roe solver only, nghost >= 4."""
+        self._check(self._L.ch_set_hcorrection(self._h, int(bool(on))), "ch_set_hcorrection")
 
     def set_reconstruction(self, recon):
         """0 = PPMC (default), 1 = PLMC, 2 = PCM."""

@@ -431,7 +431,7 @@ CH_D void riemann_exact(const Gas& G, const double WL[5], const double WR[5], do
 // B23-B30 with B29 read as in DESIGN.md (G9); the intermediate states B31-B32 are checked for negative
 // density or pressure and the HLLE flux B33-B35 substituted if either occurs.  Square roots and quotients
 // through the branch-free rsqrt / rcp above.
-CH_D void riemann_roe(const Gas& G, const double WL[5], const double WR[5], double flux[5]) {
+CH_D void riemann_roe(const Gas& G, const double WL[5], const double WR[5], double flux[5], double etaH = 0.0) {
   const double rL = WL[0], uL = WL[1], vL = WL[2], wL = WL[3], pL = floor_p(WL[4]);
   const double rR = WR[0], uR = WR[1], vR = WR[2], wR = WR[3], pR = floor_p(WR[4]);
   const double EL = pL * G.inv_gm1 + 0.5 * rL * ((uL * uL + vL * vL) + wL * wL);
@@ -471,7 +471,9 @@ CH_D void riemann_roe(const Gas& G, const double WL[5], const double WR[5], doub
   const double xi1 = dU[2] - vt * dU[0], xi2 = dU[3] - wt * dU[0];
   const double xi3 = dU[0] - q * ia2;
   // B28, B29
-  const double C0 = xi0 * fabs(lm), C1 = xi1 * fabs(l0), C2 = xi2 * fabs(l0), C3 = xi3 * fabs(l0), C4 = xi4 * fabs(lp);
+  // C3: with the H correction |lambda| -> max(|lambda|, eta^H), here and only here (reading S18)
+  const double alm = sel_max(fabs(lm), etaH), al0 = sel_max(fabs(l0), etaH), alp = sel_max(fabs(lp), etaH);
+  const double C0 = xi0 * alm, C1 = xi1 * al0, C2 = xi2 * al0, C3 = xi3 * al0, C4 = xi4 * alp;
   const double ua = ut * at, c04 = C0 + C4;
   double sv[5];
   sv[0] = c04 + C3;

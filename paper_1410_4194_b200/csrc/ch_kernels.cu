@@ -54,6 +54,8 @@ struct StepArgs {
   double* UL[3];     // U*_L(c,d): traced state at the left face of cell c     [5][np]
   double* UR[3];     // U*_R(c,d)
   double* Fh[3];     // CTU fluxes F^{n+1/2}_d                                 [5][np]
+  double* eta[3];    // H correction: eta of interface c+1/2 along d stored at c      [np]
+  int ext;           // pass-1 reach along the sweep: cells [-ext, n+ext-1]; 1, or 2 with the H correction
   unsigned long long* red;  // [0] = bits of max cell rate (|v_d|+a)/dx_d, [1] = non-physical flag
 };
 
@@ -131,11 +133,12 @@ __global__ void __launch_bounds__(CH_MARCH_T, CH_MARCH_MINB) k_pass1_march(const
   if (col >= (long long)ext0 * extT) return;
   const int i = lo0 + (int)(col % ext0);
   const int t = loT + (int)(col / ext0);
-  const int c0 = -1 + (int)blockIdx.y * seg;          // first interface of this segment
+  const int c0 = -A.ext + (int)blockIdx.y * seg;      // first interface of this segment
   const int nD = g.n[D];
   int c1 = c0 + seg;                                   // one past the last interface
-  const bool last = c1 >= nD;
-  if (last) c1 = nD;
+  const int cend = nD + A.ext - 1;                     // last cell whose faces are needed
+  const bool last = c1 >= cend;
+  if (last) c1 = cend;
   const long long sD = g.st[D];
   const long long np = g.np;
   const long long base = (long long)(i + g.g[0]) + (long long)(t + g.g[T]) * g.st[T] + (long long)g.g[D] * sD;
@@ -226,7 +229,7 @@ __global__ void __launch_bounds__(kXT, CH_X_MINB) k_pass1_x(const StepArgs A, lo
   __syncthreads();
   // stage 2: slopes for i in [-2, nx+1]
   double wm[5], wp[5], s0[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
-  const bool slope_ok = row_ok && tid >= 1 && tid <= kXT - 2 && i >= -2 && i <= nx + 1;
+  const bool slope_ok = row_ok && tid >= 1 && tid <= kXT - 2 && i >= -1 - A.ext && i <= nx + A.ext;
   const int tl = tid > 0 ? tid - 1 : 0, tr = tid < kXT - 1 ? tid + 1 : kXT - 1;
 #pragma unroll
   for (int m = 0; m < 5; ++m) { wm[m] = sP[m][tl]; wp[m] = sP[m][tr]; }
@@ -239,7 +242,7 @@ __global__ void __launch_bounds__(kXT, CH_X_MINB) k_pass1_x(const StepArgs A, lo
   for (int m = 0; m < 5; ++m) sS[m][tid] = s0[m];
   __syncthreads();
   // stage 3: parabola + tracing for i in [-1, nx]
-  const bool face_ok = slope_ok && tid >= 2 && tid <= kXT - 3 && i >= -1 && i <= nx;
+  const bool face_ok = slope_ok && tid >= 2 && tid <= kXT - 3 && i >= -A.ext && i <= nx + A.ext - 1;
   double prR[5] = {1.0, 0.0, 0.0, 0.0, 1.0}, prL[5] = {1.0, 0.0, 0.0, 0.0, 1.0};
   if (face_ok) {
     double sm[5], sp[5], WLs[5], WRs[5], cl[5], cr[5];
@@ -259,7 +262,7 @@ __global__ void __launch_bounds__(kXT, CH_X_MINB) k_pass1_x(const StepArgs A, lo
   for (int m = 0; m < 5; ++m) sL[m][tid] = prL[m];
   __syncthreads();
   // stage 4: Riemann problem at i+1/2 for i in [-1, nx-1]
-  if (face_ok && tid <= kXT - 4 && i <= nx - 1 && q < q_end) {
+  if (face_ok && tid <= kXT - 4 && i <= nx + A.ext - 2 && q < q_end) {
     double wr[5], fl[5];
 #pragma unroll
     for (int m = 0; m < 5; ++m) wr[m] = sL[m][tid + 1];
@@ -298,7 +301,37 @@ __device__ __forceinline__ void corrected_prim(const Gas& G, const DirSel& S, lo
   ch::cons2prim(G, c[0], c[1], c[2], c[3], c[4], w);
 }
 
-template <int SOLVER>
+// H correction, C1: eta = |(u_R + a_R) - (u_L + a_L)| / 2 at every interface c+1/2, c in [-1, n-1],
+// from the transverse-corrected states, over the transverse range [-1, n] that C2's stencil reaches.
+__global__ void __launch_bounds__(CH_P2_T) k_eta(const StepArgs A) {
+  const Geom& g = A.geo;
+  const int e0 = g.act[0] ? g.n[0] + 2 : 1, e1 = g.act[1] ? g.n[1] + 2 : 1, e2 = g.act[2] ? g.n[2] + 2 : 1;
+  const long long id = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (id >= (long long)e0 * e1 * e2) return;
+  const int c[3] = {(int)(id % e0) - (g.act[0] ? 1 : 0), (int)((id / e0) % e1) - (g.act[1] ? 1 : 0),
+                    (int)(id / ((long long)e0 * e1)) - (g.act[2] ? 1 : 0)};
+  const long long np = g.np;
+  const long long q = (long long)(c[0] + g.g[0]) + (long long)(c[1] + g.g[1]) * g.st[1] + (long long)(c[2] + g.g[2]) * g.st[2];
+#pragma unroll 1
+  for (int d = 0; d < 3; ++d) {
+    if (!g.act[d] || c[d] > g.n[d] - 1) continue;
+    const int d1 = d == 2 ? 0 : d + 1, d2 = d == 0 ? 2 : d - 1;
+    DirSel S;
+    S.F1 = A.Fs[d1]; S.F2 = A.Fs[d2];
+    S.s0 = g.st[d]; S.s1 = g.st[d1]; S.s2 = g.st[d2];
+    S.h1 = 0.5 * A.dtdx[d1]; S.h2 = 0.5 * A.dtdx[d2];
+    S.a1 = g.act[d1] != 0; S.a2 = g.act[d2] != 0;
+    S.f1 = (long long)(1 + d) * np; S.f2 = (long long)(1 + d1) * np; S.f3 = (long long)(1 + d2) * np;
+    double wl[5], wr[5];
+    corrected_prim(A.gas, S, np, A.UR[d], q, wl);
+    corrected_prim(A.gas, S, np, A.UL[d], q + S.s0, wr);
+    const double aL = A.gas.gamma * wl[4] * ch::inv_rho_a(A.gas, wl[0], wl[4]);
+    const double aR = A.gas.gamma * wr[4] * ch::inv_rho_a(A.gas, wr[0], wr[4]);
+    A.eta[d][q] = 0.5 * fabs((wr[1] + aR) - (wl[1] + aL));
+  }
+}
+
+template <int SOLVER, bool HC>
 __global__ void __launch_bounds__(CH_P2_T, CH_P2_MINB) k_pass2(const StepArgs A) {
   const Geom& g = A.geo;
   const int e0 = g.act[0] ? g.n[0] + 1 : 1, e1 = g.act[1] ? g.n[1] + 1 : 1, e2 = g.act[2] ? g.n[2] + 1 : 1;
@@ -326,7 +359,18 @@ __global__ void __launch_bounds__(CH_P2_T, CH_P2_MINB) k_pass2(const StepArgs A)
     double wl[5], wr[5], fl[5];
     corrected_prim(A.gas, S, np, A.UR[d], q, wl);           // U^{n+1/2}_R of cell c   -> left state
     corrected_prim(A.gas, S, np, A.UL[d], q + S.s0, wr);    // U^{n+1/2}_L of cell c+1 -> right state
-    ch::riemann<SOLVER>(A.gas, wl, wr, fl);
+    if (HC) {
+      // C2 (reading G11): the interface's own eta and eta on the transverse faces of cells c and c+1
+      const long long qp = q + S.s0;
+      double etaH = A.eta[d][q];
+      if (S.a1) etaH = ch::sel_max(etaH, ch::sel_max(ch::sel_max(A.eta[d1][q - S.s1], A.eta[d1][q]),
+                                                     ch::sel_max(A.eta[d1][qp - S.s1], A.eta[d1][qp])));
+      if (S.a2) etaH = ch::sel_max(etaH, ch::sel_max(ch::sel_max(A.eta[d2][q - S.s2], A.eta[d2][q]),
+                                                     ch::sel_max(A.eta[d2][qp - S.s2], A.eta[d2][qp])));
+      ch::riemann_roe(A.gas, wl, wr, fl, etaH);
+    } else {
+      ch::riemann<SOLVER>(A.gas, wl, wr, fl);
+    }
     double* __restrict__ Fh = A.Fh[d];
     Fh[q] = fl[0]; Fh[S.f1 + q] = fl[1]; Fh[S.f2 + q] = fl[2]; Fh[S.f3 + q] = fl[3]; Fh[4 * np + q] = fl[4];
   }
@@ -981,6 +1025,7 @@ struct ch_ctx {
   TmaMaps maps;
   int solver = 0;            // CH_SOLVER_EXACT
   int recon = 0;             // CH_RECON_PPMC
+  bool hcorr = false;        // H correction (Appendix C): Roe solver, nghost >= 4, unfused second half
   bool unfused = false;      // CH_UNFUSED=1: k_pass2 + k_update on 3-D grids too (A/B measurements, instruction counts)
   // optional per-kernel timing (ch_profile): one event pair per kernel kind
   bool profiling = false;
@@ -1026,12 +1071,14 @@ StepArgs make_args(const ch_ctx* c, double dt) {
     A.UR[d] = c->ws + (long long)(6 + d) * blk;
     A.Fh[d] = c->ws + (long long)(9 + d) * blk;
   }
+  for (int d = 0; d < 3; ++d) A.eta[d] = c->ws + (long long)12 * blk + (long long)d * c->geo.np;
+  A.ext = c->hcorr ? 2 : 1;
   A.red = c->red;
   return A;
 }
 
 const char* const kKernelNames[CH_K_COUNT] = {"k_reset", "k_pass1_x", "k_pass1_march<y>", "k_pass1_march<z>",
-                                              "k_pass2", "k_update", "k_ghost", "k_dt", "k_final3d"};
+                                              "k_pass2", "k_update", "k_ghost", "k_dt", "k_final3d", "k_eta"};
 
 // event brackets around one launch when profiling is on (no-ops otherwise)
 struct Bracket {
@@ -1187,13 +1234,13 @@ long long ch_padded_cells(const ch_ctx* c) { return c ? c->geo.np : 0; }
 size_t ch_workspace_bytes(int nx, int ny, int nz, int nghost) {
   Geom g;
   if (!geometry(nx, ny, nz, nghost, g)) return 0;
-  return (size_t)12 * 5 * (size_t)g.np * sizeof(double);
+  return ((size_t)12 * 5 + 3) * (size_t)g.np * sizeof(double);
 }
 
 int ch_bind(ch_ctx* c, const ch_buffers* b, void* stream) {
   if (!c || !b) return fail(CH_EINVAL, "ch_bind: null argument");
   if (!b->state || !b->workspace || !b->reduce) return fail(CH_EINVAL, "ch_bind: null buffer");
-  if (b->workspace_bytes < (size_t)12 * 5 * (size_t)c->geo.np * sizeof(double))
+  if (b->workspace_bytes < ((size_t)12 * 5 + 3) * (size_t)c->geo.np * sizeof(double))
     return fail(CH_EINVAL, "ch_bind: workspace too small");
   if (((uintptr_t)b->state & 7) || ((uintptr_t)b->workspace & 7) || ((uintptr_t)b->reduce & 7))
     return fail(CH_EINVAL, "ch_bind: misaligned buffer");
@@ -1300,13 +1347,13 @@ int step_impl(ch_ctx* c, double dt) {
     const int T = 3 - d;
     const long long cols = (long long)(g.act[0] ? g.n[0] + 2 : 1) * (g.act[T] ? g.n[T] + 2 : 1);
     const int seg = c->march_seg;
-    dim3 grid((unsigned)((cols + CH_MARCH_T - 1) / CH_MARCH_T), (unsigned)((g.n[d] + 1 + seg - 1) / seg));
+    dim3 grid((unsigned)((cols + CH_MARCH_T - 1) / CH_MARCH_T), (unsigned)((g.n[d] + 2 * A.ext - 1 + seg - 1) / seg));
     Bracket b(c, d == 1 ? CH_K_PASS1_Y : CH_K_PASS1_Z);
     if (d == 1) k_pass1_march<1, S, R><<<grid, CH_MARCH_T, 0, st>>>(A, seg);
     else k_pass1_march<2, S, R><<<grid, CH_MARCH_T, 0, st>>>(A, seg);
   }
   CH_CUDA(cudaGetLastError(), "pass 1");
-  if (g.act[0] && g.act[1] && g.act[2] && !c->unfused) {
+  if (g.act[0] && g.act[1] && g.act[2] && !c->unfused && !c->hcorr) {
     const int seg = c->final_seg;
     dim3 grid((unsigned)((g.n[0] + kFX - 3) / (kFX - 2)), (unsigned)((g.n[1] + kFY - 3) / (kFY - 2)),
               (unsigned)((g.n[2] + seg - 1) / seg));
@@ -1334,8 +1381,14 @@ int step_impl(ch_ctx* c, double dt) {
   } else {
     {
       const long long cells = (long long)(g.act[0] ? g.n[0] + 1 : 1) * (g.act[1] ? g.n[1] + 1 : 1) * (g.act[2] ? g.n[2] + 1 : 1);
+      if (c->hcorr) {
+        const long long ecells = (long long)(g.act[0] ? g.n[0] + 2 : 1) * (g.act[1] ? g.n[1] + 2 : 1) * (g.act[2] ? g.n[2] + 2 : 1);
+        Bracket b(c, CH_K_ETA);
+        k_eta<<<(unsigned)((ecells + CH_P2_T - 1) / CH_P2_T), CH_P2_T, 0, st>>>(A);
+      }
       Bracket b(c, CH_K_PASS2);
-      k_pass2<S><<<(unsigned)((cells + CH_P2_T - 1) / CH_P2_T), CH_P2_T, 0, st>>>(A);
+      if (c->hcorr) k_pass2<1, true><<<(unsigned)((cells + CH_P2_T - 1) / CH_P2_T), CH_P2_T, 0, st>>>(A);
+      else k_pass2<S, false><<<(unsigned)((cells + CH_P2_T - 1) / CH_P2_T), CH_P2_T, 0, st>>>(A);
     }
     {
       const long long N = (long long)g.n[0] * g.n[1] * g.n[2];
@@ -1357,11 +1410,19 @@ extern "C" {
 int ch_step(ch_ctx* c, double dt) {
   if (!c) return fail(CH_EINVAL, "ch_step: null context");
   const bool roe = c->solver == CH_SOLVER_ROE;
+  if (c->hcorr && !roe) return fail(CH_ESTATE, "ch_step: the H correction goes with the Roe solver (ch_set_solver)");
   switch (c->recon) {
     case CH_RECON_PLMC: return roe ? step_impl<1, 1>(c, dt) : step_impl<0, 1>(c, dt);
     case CH_RECON_PCM: return roe ? step_impl<1, 2>(c, dt) : step_impl<0, 2>(c, dt);
     default: return roe ? step_impl<1, 0>(c, dt) : step_impl<0, 0>(c, dt);
   }
+}
+
+int ch_set_hcorrection(ch_ctx* c, int on) {
+  if (!c) return fail(CH_EINVAL, "ch_set_hcorrection: null context");
+  if (on && c->nghost < 4) return fail(CH_EINVAL, "ch_set_hcorrection: needs nghost >= 4 (P:L1291)");
+  c->hcorr = on != 0;
+  return CH_OK;
 }
 
 int ch_set_reconstruction(ch_ctx* c, int recon) {

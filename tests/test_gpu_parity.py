@@ -533,3 +533,58 @@ def test_plmc_pcm_runs_match_oracle_and_switch_back(ch, ref):
     with pytest.raises(ValueError):
         G.set_reconstruction(5)
     G.close()
+
+
+# ---- NEXT-1 completed: the H correction (Appendix C) ----------------------------------------------------
+HC_CASES = {
+    "sod_1d_128": lambda: wl.sod(128),
+    "sod_along_z": lambda: wl.sod(96, axis=2, n_other=5),
+    "rough_2d": lambda: wl.rough_random(40, 33, 1, seed=8, decades=0.3, mach=0.8, bc=(P,) * 6),
+    "rough_3d": lambda: wl.rough_random(38, 21, 13, seed=11, decades=0.3, mach=0.8),
+    "sweep_ragged_3d": lambda: wl.sweep(shape=(135, 45, 37)),
+    "sedov_24": lambda: wl.sedov(24),
+    "smooth_mixed_bc": lambda: wl.smooth_random(41, 29, 23, seed=5, bc=(R, O, P, P, O, R)),
+}
+
+
+@pytest.mark.parametrize("recon", [0, 1])
+@pytest.mark.parametrize("name", sorted(HC_CASES))
+def test_hcorrection_one_step_parity(ch, ref, name, recon):
+    w = HC_CASES[name]()
+    G, Rg = both(ch, ref, w, nghost=4)
+    for g in (G, Rg):
+        g.set_solver(1)
+        g.set_reconstruction(recon)
+        g.set_hcorrection(True)
+        g.set_state(w.u)
+    dt = Rg.compute_dt(w.cfl)
+    G.step(dt); Rg.step(dt)
+    ur = Rg.get_state()
+    assert np.all(np.isfinite(ur))
+    assert max(max_rel_error(G.get_state(), ur, w.gamma)) <= ONE_STEP_TOL, (name, recon)
+    G.close()
+
+
+def test_hcorrection_run_switches_and_errors(ch, ref):
+    w = wl.rough_random(48, 40, 1, seed=3, decades=0.3, mach=0.8, bc=(P,) * 6, steps=10)
+    G, Rg = both(ch, ref, w, nghost=4)
+    for g in (G, Rg):
+        g.set_solver(1); g.set_hcorrection(True)
+    dts = []
+    run(Rg, w, record_dts=dts)
+    run(G, w, dts=dts)
+    with_hc = G.get_state()
+    assert max(rel_l1_error(with_hc, Rg.get_state(), w.gamma)) <= RUN_L1_TOL
+    G.set_hcorrection(False)
+    run(G, w, dts=dts)
+    assert not np.array_equal(G.get_state(), with_hc)          # the correction acts, and can be switched off
+    G.set_hcorrection(True)
+    G.set_solver(0)
+    G.set_state(w.u)
+    with pytest.raises(RuntimeError):
+        G.step(1e-4)                                           # exact solver + H correction: refused
+    G.close()
+    G3 = ch.Grid(16, 16, 16, 3, 1.4)
+    with pytest.raises(ValueError):
+        G3.set_hcorrection(True)                               # three ghost layers are not enough
+    G3.close()
