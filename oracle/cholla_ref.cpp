@@ -16,8 +16,8 @@
 // step contains no floating-point reduction; min is exact).
 //
 // Parity pins: every function below is pinned by tests/test_oracle_*.py (closed forms,
-// invariants, special cases); see DESIGN.md §"Oracle pins".  No function here is "parity
-// unpinned".
+// invariants, special cases); see DESIGN.md §5.  One reading is "parity unpinned": which cells the H
+// correction's C2 gathers eta from (reading G11); everything else is pinned.
 
 #include <algorithm>
 #include <cmath>
