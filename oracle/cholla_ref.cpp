@@ -16,8 +16,7 @@
 // step contains no floating-point reduction; min is exact).
 //
 // Parity pins: every function below is pinned by tests/test_oracle_*.py (closed forms,
-// invariants, special cases); see DESIGN.md §5.  One reading is "parity unpinned": which cells the H
-// correction's C2 gathers eta from (reading G11); everything else is pinned.
+// invariants, special cases); see DESIGN.md §5.  No function here is "parity unpinned".
 
 #include <algorithm>
 #include <cmath>

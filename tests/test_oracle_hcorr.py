@@ -173,3 +173,38 @@ def test_adds_crossflow_dissipation_at_a_grid_aligned_shock(ref):
         behind = d[:, (x > 0.15) & (x < 0.1 + M * a0 * 0.04 - 0.05)]
         res[hc] = float(np.mean(np.std(behind, axis=0)))
     assert res[True] < res[False], res
+
+
+def test_c2_gathers_from_the_two_cells_that_share_the_interface(ref):
+    """Reading G11 made observable.  A density ramp along x gives every x-interface the same jump; one cell
+    (i0, j0+1) gets a large transverse velocity, which makes eta large on the y-interface (i0, j0+1/2) only.
+    With the correction, the x-interface (i0+1/2, j0) — cells i0 and i0+1 share it — gathers that eta, so cell
+    (i0+1, j0) responds; the x-interface (i0+3/2, j0) gathers only from cells i0+1 and i0+2, whose eta do not
+    depend on the perturbed cell, so cell (i0+2, j0) is untouched to the bit.  With the indices as printed (i-1
+    and i+1) it would be the interface (i0+3/2, j0) that sees the large eta, and cell (i0+2, j0) would change."""
+    nx, ny, i0, j0, gamma = 24, 12, 10, 5, 1.4
+    rho = (1.0 + 0.02 * np.arange(nx))[None, None, :] * np.ones((1, ny, nx))
+    vy = np.zeros((1, ny, nx))
+    vy_p = vy.copy(); vy_p[0, j0 + 1, i0] = 2.0
+    base = wl.conserved(rho, 0.3, vy, 0.0, 1.0, gamma)
+    pert = wl.conserved(rho, 0.3, vy_p, 0.0, 1.0, gamma)
+
+    def change(dt, hc):
+        out = []
+        for u in (base, pert):
+            Gd = ref.RefGrid(nx, ny, 1, 4, gamma, (P,) * 6)
+            Gd.set_solver(1); Gd.set_hcorrection(hc)
+            Gd.set_state(u)
+            Gd.step(dt)
+            out.append(Gd.get_state()[0, 0])
+        d = np.abs(out[1] - out[0])
+        return d[j0, i0 + 1], d[j0, i0 + 2]
+
+    dt = 2e-3
+    near0, far0 = change(dt, False)
+    near1, far1 = change(dt, True)
+    _, far2 = change(dt / 4, True)
+    # (uncorrected, the perturbed cell reaches (i0+1, j0) through the x-flux at i0+1/2 at O(dt), and (i0+2, j0)
+    # only through second-order couplings)
+    assert abs(near1 - near0) > 1e-6                            # the shared interface sees the large eta
+    assert far1 == 0.0 and far2 == 0.0                          # the next interface does not: no path to that cell
