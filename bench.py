@@ -270,7 +270,8 @@ def main():
     if world == 1 and not args.no_other_workloads:
         # strong shocks change Newton iteration counts and warp divergence: the smooth sweep alone flatters the
         # solver, so configs 3 and 4 are timed beside it (state after `pre` steps)
-        for name, make, pre, k in (("sedov_128 (config 3)", lambda: wl.sedov(128), 20, 20),
+        for name, make, pre, k in (("kelvin_helmholtz_256x256 (config 2)", lambda: wl.kelvin_helmholtz(256), 20, 50),
+                                   ("sedov_128 (config 3)", lambda: wl.sedov(128), 20, 20),
                                    ("shock_cloud_256 (config 4)", lambda: wl.shock_cloud(256), 10, 10)):
             ww = make()
             G = pkg.Grid(*ww.shape, 3, ww.gamma, ww.bc, device=device)
@@ -287,10 +288,13 @@ def main():
     if world == 1 and not args.no_other_workloads:
         # the paper's other method choices on the same workload and size: the Roe + HLLE solver (B.2)
         # with PPMC, and the second-order pair PLMC + Roe the paper quotes its 2-D figure for
-        for label, solver, recon in ((f"sweep_{args.size} PPMC + Roe/HLLE", 1, 0), (f"sweep_{args.size} PLMC + Roe/HLLE", 1, 1)):
-            G = pkg.Grid(args.size, args.size, args.size, 3, w.gamma, w.bc, device=device)
+        for label, solver, recon, hc in ((f"sweep_{args.size} PPMC + Roe/HLLE", 1, 0, False),
+                                         (f"sweep_{args.size} PLMC + Roe/HLLE", 1, 1, False),
+                                         (f"sweep_{args.size} PPMC + Roe/HLLE + H correction (4 ghost layers, unfused second half)", 1, 0, True)):
+            G = pkg.Grid(args.size, args.size, args.size, 4 if hc else 3, w.gamma, w.bc, device=device)
             G.set_solver(solver)
             G.set_reconstruction(recon)
+            G.set_hcorrection(hc)
             G.set_state(torch.from_numpy(w.u).to(device))
             for _ in range(3):
                 G.step(G.compute_dt(w.cfl))
