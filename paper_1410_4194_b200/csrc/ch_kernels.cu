@@ -1018,8 +1018,8 @@ struct ch_ctx {
   cudaStream_t stream = nullptr;
   unsigned long long* h_red = nullptr;   // pinned, 16 bytes
   long long launches = 0;
-  int march_seg = 64;
-  int final_seg = 64;
+  int march_seg = 0;         // cells a marching thread sweeps; 0 = chosen per launch from the grid size
+  int final_seg = 0;         // planes a k_final3d CTA marches; 0 = chosen per launch
   bool use_tma = true;       // CH_TMA=0: plain-load k_final3d even where the TMA form applies
   bool tma_ok = false;       // tensor maps built for the bound buffers
   TmaMaps maps;
@@ -1346,7 +1346,13 @@ int step_impl(ch_ctx* c, double dt) {
     if (!g.act[d]) continue;
     const int T = 3 - d;
     const long long cols = (long long)(g.act[0] ? g.n[0] + 2 : 1) * (g.act[T] ? g.n[T] + 2 : 1);
-    const int seg = c->march_seg;
+    // enough segments to fill the chip on small grids (a segment costs ~1.5 cells of warm-up), 64 on large ones
+    int seg = c->march_seg;
+    if (seg == 0) {
+      const long long want = cols * (g.n[d] + 1) / (148LL * 1024);
+      seg = 4;
+      while (seg < 64 && seg * 2 <= want) seg *= 2;
+    }
     dim3 grid((unsigned)((cols + CH_MARCH_T - 1) / CH_MARCH_T), (unsigned)((g.n[d] + 2 * A.ext - 1 + seg - 1) / seg));
     Bracket b(c, d == 1 ? CH_K_PASS1_Y : CH_K_PASS1_Z);
     if (d == 1) k_pass1_march<1, S, R><<<grid, CH_MARCH_T, 0, st>>>(A, seg);
@@ -1354,7 +1360,15 @@ int step_impl(ch_ctx* c, double dt) {
   }
   CH_CUDA(cudaGetLastError(), "pass 1");
   if (g.act[0] && g.act[1] && g.act[2] && !c->unfused && !c->hcorr) {
-    const int seg = c->final_seg;
+    // at least four waves of CTAs on small grids (a segment costs two light planes), 64 planes on large ones
+    int seg = c->final_seg;
+    if (seg == 0) {
+      const bool tma = c->tma_ok && c->use_tma;
+      const long long tiles = (long long)((g.n[0] + kFX - 3) / (kFX - 2)) * ((g.n[1] + (tma ? kTY : kFY) - 3) / ((tma ? kTY : kFY) - 2));
+      const long long want = tiles * g.n[2] / (148LL * 4);
+      seg = 8;
+      while (seg < 64 && seg * 2 <= want) seg *= 2;
+    }
     dim3 grid((unsigned)((g.n[0] + kFX - 3) / (kFX - 2)), (unsigned)((g.n[1] + kFY - 3) / (kFY - 2)),
               (unsigned)((g.n[2] + seg - 1) / seg));
     if (c->tma_ok && c->use_tma) {
