@@ -58,7 +58,7 @@ def sampled_one_step(ref, w, m=12, extra=6, seed=0):
     return worst, post, dt
 
 
-@pytest.mark.parametrize("n", [256, 512])
+@pytest.mark.parametrize("n", [128, 256, 384, 512])
 def test_sweep_full_size_sampled_parity_and_conservation(ref, n):
     """Throughput-sweep workload (BASELINE.json config 5) at the sizes the metric is quoted on."""
     w = wl.sweep(n)
