@@ -116,3 +116,60 @@ def test_kelvin_helmholtz_256_200_steps(ref):
     G.close()
     assert max(e_lock) <= RUN_L1_TOL, e_lock
     assert max(e_free) <= RUN_L1_TOL, e_free
+
+
+def test_sedov_128_full_run_reaches_the_sedov_taylor_radius():
+    """BASELINE.json config 3 in full on the GPU (the oracle cannot run ~2000 steps of 128^3): ambient rho = 1,
+    E = 1 in the 160 central cells, run until the closed form R = 1.15 (E t^2 / rho)^(1/5) says 0.4
+    (t = 0.071352).  The shell-averaged density's outer half-rise radius must sit within 1.5 cells of it, the
+    blast must stay octant-symmetric, and total energy is conserved while the shock is inside the box."""
+    import paper_1410_4194_b200 as ch
+    n = 128
+    w = wl.sedov(n)
+    dx = 1.0 / n
+    G = ch.Grid(n, n, n, 3, w.gamma, w.bc)
+    steps, t = run(G, w)
+    u = G.get_state()
+    G.close()
+    assert abs(t - w.t_end) < 1e-12 and steps > 500
+    rho = u[0]
+    c = (np.arange(n) + 0.5) * dx - 0.5
+    r = np.sqrt(c[None, None, :] ** 2 + c[None, :, None] ** 2 + c[:, None, None] ** 2)
+    bins = np.arange(0, 0.5, dx)
+    which = np.digitize(r.ravel(), bins)
+    prof = np.array([rho.ravel()[which == b].mean() for b in range(1, len(bins))])
+    rc = 0.5 * (bins[1:] + bins[:-1])
+    half = 0.5 * (prof.max() + 1.0)
+    i = np.max(np.nonzero(prof > half)[0])
+    r_half = rc[i] + (prof[i] - half) / (prof[i] - prof[i + 1]) * dx
+    want = 1.15 * (t * t) ** 0.2
+    assert abs(want - 0.4) < 1e-4
+    assert abs(r_half - want) <= 1.5 * dx, (r_half, want, steps)
+    assert prof.max() > 2.5                                           # compression toward (g+1)/(g-1) = 4
+    assert np.allclose(rho, rho[::-1, :, :], rtol=1e-8) and np.allclose(rho, rho.transpose(2, 1, 0), rtol=1e-8)
+    e_tot = math.fsum(u[4].ravel()) * dx ** 3
+    assert abs(e_tot - (1.0 + 1e-5 / (w.gamma - 1) * (1 - 160 * dx ** 3))) < 1e-8
+
+
+def test_shock_cloud_256_500_steps_stays_physical():
+    """BASELINE.json config 4 in full on the GPU: 500 steps at CFL 0.3.  The Mach-50 shock must have advanced
+    at the Rankine-Hugoniot speed (204.124 in code units) through the part of the box it has not yet reached
+    the cloud in, density and pressure stay positive everywhere, no non-physical cell is reported."""
+    import paper_1410_4194_b200 as ch
+    w = wl.shock_cloud(256)
+    G = ch.Grid(*w.shape, 3, w.gamma, w.bc)
+    steps, t = run(G, w)
+    assert steps == 500
+    dt_next = G.compute_dt(w.cfl)
+    u = G.get_state()
+    G.close()
+    assert math.isfinite(dt_next) and dt_next > 0
+    rho = u[0]
+    p = (w.gamma - 1) * (u[4] - 0.5 * (u[1] ** 2 + u[2] ** 2 + u[3] ** 2) / rho)
+    assert np.all(np.isfinite(u)) and rho.min() > 0 and p.min() > 0
+    # shock position along a line far from the cloud (y = z = 8 cells from the corner): first cell from the +x
+    # side whose density exceeds twice the ambient value
+    line = rho[8, 8, :]
+    front = np.max(np.nonzero(line > 0.2)[0]) + 1
+    want = 16 + 204.12414523 * t * 256
+    assert abs(front - want) <= 2.5, (front, want, t)
