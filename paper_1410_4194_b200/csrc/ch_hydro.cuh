@@ -153,15 +153,34 @@ CH_D void limited_slope(const Gas& G, const double wm[5], const double w0[5], co
 // PPMC for one cell (A.3): parabola edges A20-A23, A24/A26(=A50, G2), characteristic
 // tracing A25-A33 (A30/A32 read as G3).  wm,w0,wp = cells i-1,i,i+1; dwm,dw0,dwp their limited
 // slopes; s = inv_rho_a(i); dtdx = dt/dx_d.  Outputs W*_L, W*_R (primitive).
+// A20: the interpolated value on the interface between a cell (w_lo, slope d_lo) and its upper
+// neighbour (w_hi, d_hi).  It is cell lo's W_{R,A} and cell hi's W_{L,A}: the marching kernels compute it once.
+CH_D void ppm_interface(const double w_lo[5], const double w_hi[5], const double d_lo[5], const double d_hi[5],
+                        double e[5]) {
+#pragma unroll
+  for (int m = 0; m < 5; ++m) e[m] = 0.5 * (w_hi[m] + w_lo[m]) - (d_hi[m] - d_lo[m]) * (1.0 / 6.0);
+}
+
+CH_D void ppmc_from_interfaces(const Gas& G, double dtdx, const double wm[5], const double w0[5], const double wp[5],
+                               const double LA[5], const double RA[5], double s, double WLs[5], double WRs[5]);
+
 CH_D void ppmc_faces(const Gas& G, double dtdx, const double wm[5], const double w0[5], const double wp[5],
                       const double dwm[5], const double dw0[5], const double dwp[5], double s, double WLs[5],
                       double WRs[5]) {
+  double LA[5], RA[5];
+  ppm_interface(wm, w0, dwm, dw0, LA);
+  ppm_interface(w0, wp, dw0, dwp, RA);
+  ppmc_from_interfaces(G, dtdx, wm, w0, wp, LA, RA, s, WLs, WRs);
+}
+
+CH_D void ppmc_from_interfaces(const Gas& G, double dtdx, const double wm[5], const double w0[5], const double wp[5],
+                               const double LA[5], const double RA[5], double s, double WLs[5], double WRs[5]) {
   double WL[5], WR[5], dwi[5], w6[5];
 #pragma unroll
   for (int m = 0; m < 5; ++m) {
     const double wi = w0[m];
-    double L = 0.5 * (wi + wm[m]) - (dw0[m] - dwm[m]) * (1.0 / 6.0);   // A20
-    double R = 0.5 * (wp[m] + wi) - (dwp[m] - dw0[m]) * (1.0 / 6.0);
+    double L = LA[m];                                                  // A20
+    double R = RA[m];
     if ((R - wi) * (wi - L) <= 0.0) { L = wi; R = wi; }                // A21
     const double t3 = 3.0 * wi;
     const double cl = t3 - 2.0 * R, cr = t3 - 2.0 * L;                 // A22, G8
@@ -293,6 +312,26 @@ CH_D void plmc_faces(const Gas& G, double dtdx, const double wm[5], const double
   for (int m = 0; m < 5; ++m) {
     WLs[m] = (WL[m] - cl * dwi[m]) + h * sLv[m];                       // A16
     WRs[m] = (WR[m] - cr * dwi[m]) + h * sRv[m];                       // A18
+  }
+}
+
+// The same for a thread that marches along the sweep: `ifc` carries the A20 value of the cell's lower interface
+// in and of its upper interface out (PPMC only; the other reconstructions do not use it).
+template <int R>
+CH_D void recon_faces_march(const Gas& G, double dtdx, const double wm[5], const double w0[5], const double wp[5],
+                            const double dw0[5], const double dwp[5], double s, double ifc[5], double WLs[5],
+                            double WRs[5]) {
+  if (R == 0) {
+    double RA[5];
+    ppm_interface(w0, wp, dw0, dwp, RA);
+    ppmc_from_interfaces(G, dtdx, wm, w0, wp, ifc, RA, s, WLs, WRs);
+#pragma unroll
+    for (int m = 0; m < 5; ++m) ifc[m] = RA[m];
+  } else if (R == 1) {
+    plmc_faces(G, dtdx, wm, w0, wp, dw0, s, WLs, WRs);
+  } else {
+#pragma unroll
+    for (int m = 0; m < 5; ++m) { WLs[m] = w0[m]; WRs[m] = w0[m]; }
   }
 }
 

@@ -146,7 +146,8 @@ __global__ void __launch_bounds__(CH_MARCH_T, CH_MARCH_MINB) k_pass1_march(const
   const double* __restrict__ u = A.u;
 
   double wa[5], wb[5], wc[5], wd[5];   // cells c-1, c, c+1, c+2 (rotating)
-  double sa[5], sb[5], sc[5];          // slopes of c-1, c, c+1
+  double sb[5], sc[5];                 // slopes of c, c+1
+  double ifc[5];                       // A20 value on the lower interface of cell c (PPMC)
   double icb, icc;                     // 1/(rho a) of c, c+1
   double pr_prev[5];                   // previous cell's right-face primitive state W*_R
   double raw[5];                       // conserved values of the next cell to enter the stencil (loaded one step ahead)
@@ -157,9 +158,11 @@ __global__ void __launch_bounds__(CH_MARCH_T, CH_MARCH_MINB) k_pass1_march(const
     load_prim<D>(G, u, np, base + (long long)(c0)*sD, wb);
     load_prim<D>(G, u, np, base + (long long)(c0 + 1) * sD, wc);
     load_raw<D>(u, np, base + (long long)(c0 + 2) * sD, raw);
+    double sa[5];
     ch::limited_slope(G, wz, wa, wb, ch::inv_rho_a(G, wa[0], wa[4]), sa);
     icb = ch::inv_rho_a(G, wb[0], wb[4]);
     ch::limited_slope(G, wa, wb, wc, icb, sb);
+    ch::ppm_interface(wa, wb, sa, sb, ifc);
   }
   for (int c = c0; c <= c1; ++c) {
     const long long q = base + (long long)c * sD;
@@ -168,7 +171,7 @@ __global__ void __launch_bounds__(CH_MARCH_T, CH_MARCH_MINB) k_pass1_march(const
     icc = ch::inv_rho_a(G, wc[0], wc[4]);
     ch::limited_slope(G, wb, wc, wd, icc, sc);
     double WLs[5], WRs[5], cl[5], cr[5];
-    ch::recon_faces<R>(G, dtdx, wa, wb, wc, sa, sb, sc, icb, WLs, WRs);
+    ch::recon_faces_march<R>(G, dtdx, wa, wb, wc, sb, sc, icb, ifc, WLs, WRs);
     ch::prim2cons(G, WLs, cl);     // states are kept conserved between stages
     ch::prim2cons(G, WRs, cr);
     if (c < c1 || last) {
@@ -182,7 +185,7 @@ __global__ void __launch_bounds__(CH_MARCH_T, CH_MARCH_MINB) k_pass1_march(const
     }
     copy5(pr_prev, WRs);
     copy5(wa, wb); copy5(wb, wc); copy5(wc, wd);
-    copy5(sa, sb); copy5(sb, sc);
+    copy5(sb, sc);
     icb = icc;
   }
 }

@@ -31,16 +31,16 @@ ALG_BYTES = {
 # (DADD + DMUL + 2*DFMA) per real cell-update at 512^3, throughput-sweep workload.
 ALG_FLOPS = {
     "k_pass1_x": 580.4,
-    "k_pass1_march<y>": 586.4,
-    "k_pass1_march<z>": 586.5,
+    "k_pass1_march<y>": 561.4,   # r01f count 586.4 minus the A20 interface value now computed once per interface
+    "k_pass1_march<z>": 561.5,   # (5 components x 5 flops), not re-profiled
     "k_final3d": 1030.0,      # k_pass2 (929.0) + k_update (101.0) of the unfused path
 }
 
 # FP64-pipe arithmetic instructions (DADD + DMUL + DFMA) per real cell-update, same provenance.
 ALG_INST = {
     "k_pass1_x": 442.3,
-    "k_pass1_march<y>": 446.9,
-    "k_pass1_march<z>": 446.9,
+    "k_pass1_march<y>": 426.9,
+    "k_pass1_march<z>": 426.9,
     "k_final3d": 731.4,
 }
 
