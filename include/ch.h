@@ -146,6 +146,20 @@ int ch_set_hcorrection(ch_ctx* ctx, int on);
 /* ch_set_reconstruction — select the reconstruction for later steps.  CH_EINVAL for an unknown code. */
 int ch_set_reconstruction(ch_ctx* ctx, int recon);
 
+/* ch_step_cfl — one step whose size never visits the host: dt = cfl * min dx_d/(|v_d| + a) (Eq. 22, from the
+ * reduction the previous step left on the device, or a fresh pass after ch_set_state), clipped to t_left when
+ * 0 < t_left < dt, then the same kernels as ch_step read it from device memory and form dt/dx_d with the same
+ * correctly rounded division.  Fully asynchronous: steps can be queued back to back without the 16-byte
+ * read-back ch_compute_dt needs.  A sequence of ch_step_cfl calls gives bitwise the states the
+ * ch_compute_dt + ch_step loop gives.  A non-physical cell makes dt NaN (visible through ch_last_dt).
+ * CH_EINVAL if cfl is not in (0,1] or t_left is NaN; t_left <= 0 means "no clipping". */
+int ch_step_cfl(ch_ctx* ctx, double cfl, double t_left);
+
+/* ch_last_dt — the dt the most recent ch_step_cfl used (synchronises; NaN + CH_ENONPHYS if it met a non-physical
+ * cell).  ch_elapsed — the sum of the dt of all ch_step_cfl calls since ch_bind (synchronises). */
+double ch_last_dt(ch_ctx* ctx);
+double ch_elapsed(ch_ctx* ctx);
+
 /* ch_sync — block until all work queued on the context's stream has finished. */
 int ch_sync(ch_ctx* ctx);
 

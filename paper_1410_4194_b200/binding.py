@@ -27,7 +27,7 @@ CH_OK, CH_EINVAL, CH_ESTATE, CH_ECUDA, CH_ENONPHYS = 0, -1, -2, -3, -4
 # every symbol include/ch.h declares
 SYMBOLS = ("ch_init", "ch_free", "ch_last_error", "ch_set_spacing", "ch_padded_cells", "ch_workspace_bytes",
            "ch_bind", "ch_set_state", "ch_get_state", "ch_set_padded", "ch_get_padded", "ch_compute_dt",
-           "ch_step", "ch_set_solver", "ch_set_reconstruction", "ch_set_hcorrection", "ch_sync", "ch_kernel_launches", "ch_profile", "ch_profile_read", "ch_kernel_name",
+           "ch_step", "ch_step_cfl", "ch_last_dt", "ch_elapsed", "ch_set_solver", "ch_set_reconstruction", "ch_set_hcorrection", "ch_sync", "ch_kernel_launches", "ch_profile", "ch_profile_read", "ch_kernel_name",
            "ch_fp64_peak_probe")
 K_COUNT = 10
 
@@ -81,6 +81,11 @@ def load_library() -> C.CDLL:
     L.ch_compute_dt.restype = C.c_double
     L.ch_compute_dt.argtypes = [vp, C.c_double]
     L.ch_step.argtypes = [vp, C.c_double]
+    L.ch_step_cfl.argtypes = [vp, C.c_double, C.c_double]
+    L.ch_last_dt.restype = C.c_double
+    L.ch_last_dt.argtypes = [vp]
+    L.ch_elapsed.restype = C.c_double
+    L.ch_elapsed.argtypes = [vp]
     L.ch_set_solver.argtypes = [vp, C.c_int]
     L.ch_set_reconstruction.argtypes = [vp, C.c_int]
     L.ch_set_hcorrection.argtypes = [vp, C.c_int]
@@ -202,6 +207,16 @@ class Grid:
 
     def step(self, dt):
         self._check(self._L.ch_step(self._h, dt), "ch_step")
+
+    def step_cfl(self, cfl, t_left=0.0):
+        """One step with the device-resident Eq. 22 time step (no host round trip); t_left > 0 clips it."""
+        self._check(self._L.ch_step_cfl(self._h, cfl, t_left), "ch_step_cfl")
+
+    def last_dt(self) -> float:
+        return float(self._L.ch_last_dt(self._h))
+
+    def elapsed(self) -> float:
+        return float(self._L.ch_elapsed(self._h))
 
     def set_solver(self, solver):
         """0 = exact (default), 1 = Roe with the HLLE failsafe."""

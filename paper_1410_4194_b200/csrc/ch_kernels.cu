@@ -55,9 +55,23 @@ struct StepArgs {
   double* UR[3];     // U*_R(c,d)
   double* Fh[3];     // CTU fluxes F^{n+1/2}_d                                 [5][np]
   double* eta[3];    // H correction: eta of interface c+1/2 along d stored at c      [np]
+  const double* dt_dev;   // ch_step_cfl: the time step lives on the device (written by k_pick_dt); else nullptr
   int ext;           // pass-1 reach along the sweep: cells [-ext, n+ext-1]; 1, or 2 with the H correction
   unsigned long long* red;  // [0] = bits of max cell rate (|v_d|+a)/dx_d, [1] = non-physical flag
 };
+
+// dt / dx_d of this step: from the kernel arguments (ch_step) or from the device-resident dt (ch_step_cfl), with
+// the same correctly rounded division the host does, so the two ways of stepping agree bitwise
+__device__ __forceinline__ void step_dtdx(const StepArgs& A, double out[3]) {
+  if (A.dt_dev) {
+    const double dt = *A.dt_dev;
+#pragma unroll
+    for (int d = 0; d < 3; ++d) out[d] = __ddiv_rn(dt, A.dx[d]);
+  } else {
+#pragma unroll
+    for (int d = 0; d < 3; ++d) out[d] = A.dtdx[d];
+  }
+}
 
 // global component index of direction-local component m for a sweep along D (cyclic)
 template <int D>
@@ -126,6 +140,8 @@ template <int D, int S, int R>
 __global__ void __launch_bounds__(CH_MARCH_T, CH_MARCH_MINB) k_pass1_march(const StepArgs A, int seg) {
   constexpr int T = 3 - D;   // the other transverse dimension (x is the lane dimension)
   const Geom& g = A.geo;
+  double dtx[3];
+  step_dtdx(A, dtx);
   const Gas& G = A.gas;
   const int ext0 = g.act[0] ? g.n[0] + 2 : 1, lo0 = g.act[0] ? -1 : 0;
   const int extT = g.act[T] ? g.n[T] + 2 : 1, loT = g.act[T] ? -1 : 0;
@@ -142,7 +158,7 @@ __global__ void __launch_bounds__(CH_MARCH_T, CH_MARCH_MINB) k_pass1_march(const
   const long long sD = g.st[D];
   const long long np = g.np;
   const long long base = (long long)(i + g.g[0]) + (long long)(t + g.g[T]) * g.st[T] + (long long)g.g[D] * sD;
-  const double dtdx = A.dtdx[D];
+  const double dtdx = dtx[D];
   const double* __restrict__ u = A.u;
 
   double wa[5], wb[5], wc[5], wd[5];   // cells c-1, c, c+1, c+2 (rotating)
@@ -208,6 +224,8 @@ __global__ void __launch_bounds__(kXT, CH_X_MINB) k_pass1_x(const StepArgs A, lo
   __shared__ double sS[5][kXT];
   __shared__ double sL[5][kXT];
   const Geom& g = A.geo;
+  double dtx[3];
+  step_dtdx(A, dtx);
   const Gas& G = A.gas;
   const long long np = g.np;
   const int tid = threadIdx.x;
@@ -251,7 +269,7 @@ __global__ void __launch_bounds__(kXT, CH_X_MINB) k_pass1_x(const StepArgs A, lo
     double sm[5], sp[5], WLs[5], WRs[5], cl[5], cr[5];
 #pragma unroll
     for (int m = 0; m < 5; ++m) { sm[m] = sS[m][tid - 1]; sp[m] = sS[m][tid + 1]; }
-    ch::recon_faces<R>(G, A.dtdx[0], wm, w0, wp, sm, s0, sp, ic, WLs, WRs);
+    ch::recon_faces<R>(G, dtx[0], wm, w0, wp, sm, s0, sp, ic, WLs, WRs);
     ch::prim2cons(G, WLs, cl);
     ch::prim2cons(G, WRs, cr);
     // a cell's faces are written by the CTA whose output window [2, kXT-4] holds it, plus the
@@ -308,6 +326,8 @@ __device__ __forceinline__ void corrected_prim(const Gas& G, const DirSel& S, lo
 // from the transverse-corrected states, over the transverse range [-1, n] that C2's stencil reaches.
 __global__ void __launch_bounds__(CH_P2_T) k_eta(const StepArgs A) {
   const Geom& g = A.geo;
+  double dtx[3];
+  step_dtdx(A, dtx);
   const int e0 = g.act[0] ? g.n[0] + 2 : 1, e1 = g.act[1] ? g.n[1] + 2 : 1, e2 = g.act[2] ? g.n[2] + 2 : 1;
   const long long id = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (id >= (long long)e0 * e1 * e2) return;
@@ -322,7 +342,7 @@ __global__ void __launch_bounds__(CH_P2_T) k_eta(const StepArgs A) {
     DirSel S;
     S.F1 = A.Fs[d1]; S.F2 = A.Fs[d2];
     S.s0 = g.st[d]; S.s1 = g.st[d1]; S.s2 = g.st[d2];
-    S.h1 = 0.5 * A.dtdx[d1]; S.h2 = 0.5 * A.dtdx[d2];
+    S.h1 = 0.5 * (d1 == 0 ? dtx[0] : d1 == 1 ? dtx[1] : dtx[2]); S.h2 = 0.5 * (d2 == 0 ? dtx[0] : d2 == 1 ? dtx[1] : dtx[2]);
     S.a1 = g.act[d1] != 0; S.a2 = g.act[d2] != 0;
     S.f1 = (long long)(1 + d) * np; S.f2 = (long long)(1 + d1) * np; S.f3 = (long long)(1 + d2) * np;
     double wl[5], wr[5];
@@ -337,6 +357,8 @@ __global__ void __launch_bounds__(CH_P2_T) k_eta(const StepArgs A) {
 template <int SOLVER, bool HC>
 __global__ void __launch_bounds__(CH_P2_T, CH_P2_MINB) k_pass2(const StepArgs A) {
   const Geom& g = A.geo;
+  double dtx[3];
+  step_dtdx(A, dtx);
   const int e0 = g.act[0] ? g.n[0] + 1 : 1, e1 = g.act[1] ? g.n[1] + 1 : 1, e2 = g.act[2] ? g.n[2] + 1 : 1;
   const long long id = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (id >= (long long)e0 * e1 * e2) return;
@@ -356,7 +378,7 @@ __global__ void __launch_bounds__(CH_P2_T, CH_P2_MINB) k_pass2(const StepArgs A)
     DirSel S;
     S.F1 = A.Fs[d1]; S.F2 = A.Fs[d2];
     S.s0 = g.st[d]; S.s1 = g.st[d1]; S.s2 = g.st[d2];
-    S.h1 = 0.5 * A.dtdx[d1]; S.h2 = 0.5 * A.dtdx[d2];
+    S.h1 = 0.5 * (d1 == 0 ? dtx[0] : d1 == 1 ? dtx[1] : dtx[2]); S.h2 = 0.5 * (d2 == 0 ? dtx[0] : d2 == 1 ? dtx[1] : dtx[2]);
     S.a1 = g.act[d1] != 0; S.a2 = g.act[d2] != 0;
     S.f1 = (long long)(1 + d) * np; S.f2 = (long long)(1 + d1) * np; S.f3 = (long long)(1 + d2) * np;
     double wl[5], wr[5], fl[5];
@@ -444,6 +466,19 @@ __device__ __forceinline__ void block_max_reduce(double t, bool bad, unsigned lo
   }
 }
 
+// ch_step_cfl: Eq. 22 finished on the device.  red[0] holds the grid maximum of (|v_d| + a)/dx_d of the current
+// state; dt = cfl * (1 / rate) exactly as ch_compute_dt forms it on the host, clipped to t_left if that is
+// positive and smaller.  red[2] <- dt (NaN if a non-physical cell was met), red[3] += dt.
+__global__ void k_pick_dt(unsigned long long* red, double cfl, double t_left) {
+  if (threadIdx.x != 0) return;
+  double dt = __dmul_rn(cfl, __ddiv_rn(1.0, __longlong_as_double((long long)red[0])));
+  if (t_left > 0.0 && dt > t_left) dt = t_left;
+  if (red[1] != 0ULL) dt = __longlong_as_double(0x7FF8000000000000LL);
+  double* r = reinterpret_cast<double*>(red);
+  r[2] = dt;
+  r[3] += dt;
+}
+
 __global__ void __launch_bounds__(256) k_reset(unsigned long long* red) {
   if (threadIdx.x == 0) { red[0] = 0ULL; red[1] = 0ULL; }
 }
@@ -469,6 +504,8 @@ __global__ void __launch_bounds__(256) k_dt(const StepArgs A) {
 // Eq. 24 on real cells, fused with the Eq. 22 reduction of the updated state.
 __global__ void __launch_bounds__(256) k_update(const StepArgs A) {
   const Geom& g = A.geo;
+  double dtx[3];
+  step_dtdx(A, dtx);
   const long long N = (long long)g.n[0] * g.n[1] * g.n[2];
   const long long id = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   double t = 0.0;
@@ -485,7 +522,7 @@ __global__ void __launch_bounds__(256) k_update(const StepArgs A) {
       double x = A.u[f * g.np + q];
 #pragma unroll
       for (int d = 0; d < 3; ++d)
-        if (g.act[d]) x += A.dtdx[d] * (A.Fh[d][f * g.np + q - g.st[d]] - A.Fh[d][f * g.np + q]);
+        if (g.act[d]) x += dtx[d] * (A.Fh[d][f * g.np + q - g.st[d]] - A.Fh[d][f * g.np + q]);
       v[f] = x;
       A.u[f * g.np + q] = x;
     }
@@ -567,6 +604,8 @@ __global__ void __launch_bounds__(kFT, CH_F_MINB) k_final3d(const StepArgs A, in
   Arr zP = reinterpret_cast<Arr>(s_final + 20 * kFT);   // carried: u + x and y flux differences of cell k-1, global order
   Arr zS = reinterpret_cast<Arr>(s_final + 25 * kFT);   // carried: F*_z of cell k-1 (global field order)
   const Geom& g = A.geo;
+  double dtx[3];
+  step_dtdx(A, dtx);
   const Gas& G = A.gas;
   const unsigned full = 0xffffffffu;
   const int tid = threadIdx.x, lane = tid & 31, row = tid >> 5;
@@ -583,7 +622,7 @@ __global__ void __launch_bounds__(kFT, CH_F_MINB) k_final3d(const StepArgs A, in
   const long long np = g.np;
   const long long s1 = g.st[1], s2 = g.st[2];
   const long long qcol = (long long)(i + g.g[0]) + (long long)(j + g.g[1]) * s1 + (long long)g.g[2] * s2;
-  const double hx = 0.5 * A.dtdx[0], hy = 0.5 * A.dtdx[1], hz = 0.5 * A.dtdx[2];
+  const double hx = 0.5 * dtx[0], hy = 0.5 * dtx[1], hz = 0.5 * dtx[2];
   double tmin = 0.0;   // running maximum of the cell rates (Eq. 22 inverted)
   bool bad = false;
 
@@ -630,7 +669,7 @@ __global__ void __launch_bounds__(kFT, CH_F_MINB) k_final3d(const StepArgs A, in
 #pragma unroll
         for (int m = 0; m < 5; ++m) {
           const double hi = __shfl_down_sync(full, fl[m], 1);
-          part[m] += A.dtdx[0] * (fl[m] - hi);      // x-local order is the global order
+          part[m] += dtx[0] * (fl[m] - hi);      // x-local order is the global order
         }
       }
       {   // ---- y: neighbours are rows of the CTA
@@ -649,11 +688,11 @@ __global__ void __launch_bounds__(kFT, CH_F_MINB) k_final3d(const StepArgs A, in
         if (need2) {
           const int dst = tid + kFX;
           // y-local order (rho, my, mz, mx, E) -> global
-          part[0] += A.dtdx[1] * (fl[0] - sF[0][dst]);
-          part[2] += A.dtdx[1] * (fl[1] - sF[1][dst]);
-          part[3] += A.dtdx[1] * (fl[2] - sF[2][dst]);
-          part[1] += A.dtdx[1] * (fl[3] - sF[3][dst]);
-          part[4] += A.dtdx[1] * (fl[4] - sF[4][dst]);
+          part[0] += dtx[1] * (fl[0] - sF[0][dst]);
+          part[2] += dtx[1] * (fl[1] - sF[1][dst]);
+          part[3] += dtx[1] * (fl[2] - sF[2][dst]);
+          part[1] += dtx[1] * (fl[3] - sF[3][dst]);
+          part[4] += dtx[1] * (fl[4] - sF[4][dst]);
         }
       }
     }
@@ -667,7 +706,7 @@ __global__ void __launch_bounds__(kFT, CH_F_MINB) k_final3d(const StepArgs A, in
       }
       if (k > k0) {
         // finish cell k-1 (Eq. 24): z-local order (rho, mz, mx, my, E)
-        const double dtd = A.dtdx[2];
+        const double dtd = dtx[2];
         const long long qm = q - s2;
         const double v0 = zP[0][tid] + dtd * (zF[0][tid] - fl[0]);
         const double v1 = zP[1][tid] + dtd * (zF[2][tid] - fl[2]);
@@ -740,6 +779,8 @@ __global__ void __launch_bounds__(kTT + 32, 1) k_final3d_tma(const StepArgs A, c
   Arr sX = reinterpret_cast<Arr>(s_t + 50 * kTT);
   Arr sF = reinterpret_cast<Arr>(s_t + 55 * kTT);
   const Geom& g = A.geo;
+  double dtx[3];
+  step_dtdx(A, dtx);
   const Gas& G = A.gas;
   const unsigned full = 0xffffffffu;
   const int tid = threadIdx.x, lane = tid & 31, row = tid >> 5;
@@ -789,7 +830,7 @@ __global__ void __launch_bounds__(kTT + 32, 1) k_final3d_tma(const StepArgs A, c
   const bool solve0 = need0 && lane >= 1 && i >= 0, solve1 = need1 && row >= 1 && j >= 0;
   const long long np = g.np, s2 = g.st[2];
   const long long qcol = (long long)(i + g.g[0]) + (long long)(j + g.g[1]) * g.st[1] + (long long)g.g[2] * s2;
-  const double hx = 0.5 * A.dtdx[0], hy = 0.5 * A.dtdx[1], hz = 0.5 * A.dtdx[2];
+  const double hx = 0.5 * dtx[0], hy = 0.5 * dtx[1], hz = 0.5 * dtx[2];
   double tmin = 0.0;
   bool bad = false;
   // carried from the previous plane (registers: one CTA per SM leaves ~150 per thread)
@@ -843,7 +884,7 @@ __global__ void __launch_bounds__(kTT + 32, 1) k_final3d_tma(const StepArgs A, c
         }
         if (k > k0) {
           // finish cell k-1 (Eq. 24): z-local order (rho, mz, mx, my, E)
-          const double dtd = A.dtdx[2];
+          const double dtd = dtx[2];
           const long long qm = q - s2;
           const double v0 = zP[0] + dtd * (zF[0] - flz[0]);
           const double v1 = zP[1] + dtd * (zF[2] - flz[2]);
@@ -873,7 +914,7 @@ __global__ void __launch_bounds__(kTT + 32, 1) k_final3d_tma(const StepArgs A, c
 #pragma unroll
         for (int m = 0; m < 5; ++m) {
           const double hi = __shfl_down_sync(full, fl[m], 1);
-          part[m] += A.dtdx[0] * (fl[m] - hi);      // x-local order is the global order
+          part[m] += dtx[0] * (fl[m] - hi);      // x-local order is the global order
         }
       }
     }
@@ -900,11 +941,11 @@ __global__ void __launch_bounds__(kTT + 32, 1) k_final3d_tma(const StepArgs A, c
         if (need2) {
           const int dst = tid + kFX;
           // y-local order (rho, my, mz, mx, E) -> global
-          part[0] += A.dtdx[1] * (fl[0] - sF[0][dst]);
-          part[2] += A.dtdx[1] * (fl[1] - sF[1][dst]);
-          part[3] += A.dtdx[1] * (fl[2] - sF[2][dst]);
-          part[1] += A.dtdx[1] * (fl[3] - sF[3][dst]);
-          part[4] += A.dtdx[1] * (fl[4] - sF[4][dst]);
+          part[0] += dtx[1] * (fl[0] - sF[0][dst]);
+          part[2] += dtx[1] * (fl[1] - sF[1][dst]);
+          part[3] += dtx[1] * (fl[2] - sF[2][dst]);
+          part[1] += dtx[1] * (fl[3] - sF[3][dst]);
+          part[4] += dtx[1] * (fl[4] - sF[4][dst]);
         }
       }
     }
@@ -1082,6 +1123,7 @@ StepArgs make_args(const ch_ctx* c, double dt) {
   }
   for (int d = 0; d < 3; ++d) A.eta[d] = c->ws + (long long)12 * blk + (long long)d * c->geo.np;
   A.ext = c->hcorr ? 2 : 1;
+  A.dt_dev = nullptr;
   A.red = c->red;
   return A;
 }
@@ -1259,6 +1301,7 @@ int ch_bind(ch_ctx* c, const ch_buffers* b, void* stream) {
   c->stream = static_cast<cudaStream_t>(stream);
   if (!c->h_red) CH_CUDA(cudaHostAlloc((void**)&c->h_red, 16, cudaHostAllocDefault), "cudaHostAlloc");
   c->bound = true; c->have_state = false; c->dt_valid = false;
+  CH_CUDA(cudaMemsetAsync(c->red, 0, 64, c->stream), "ch_bind: clearing the reduction cells");
   c->tma_ok = build_tma_maps(c);
   return CH_OK;
 }
@@ -1332,12 +1375,13 @@ namespace {
 
 // One CTU step with Riemann solver S (0 exact, 1 Roe + HLLE) compiled into every kernel that solves.
 template <int S, int R>
-int step_impl(ch_ctx* c, double dt) {
+int step_impl(ch_ctx* c, double dt, bool devdt) {
   if (!c) return fail(CH_EINVAL, "ch_step: null context");
   if (!c->have_state) return fail(CH_ESTATE, "ch_step: no state set");
-  if (!(dt > 0.0) || !std::isfinite(dt)) return fail(CH_EINVAL, "ch_step: dt <= 0 or non-finite");
+  if (!devdt && (!(dt > 0.0) || !std::isfinite(dt))) return fail(CH_EINVAL, "ch_step: dt <= 0 or non-finite");
   const Geom& g = c->geo;
-  StepArgs A = make_args(c, dt);
+  StepArgs A = make_args(c, devdt ? 1.0 : dt);
+  if (devdt) A.dt_dev = reinterpret_cast<const double*>(c->red) + 2;     // written by k_pick_dt just before
   cudaStream_t st = c->stream;
   { Bracket b(c, CH_K_RESET); k_reset<<<1, 32, 0, st>>>(c->red); }
   // pass 1
@@ -1430,15 +1474,61 @@ int step_impl(ch_ctx* c, double dt) {
 
 extern "C" {
 
-int ch_step(ch_ctx* c, double dt) {
-  if (!c) return fail(CH_EINVAL, "ch_step: null context");
+static int step_dispatch(ch_ctx* c, double dt, bool devdt) {
   const bool roe = c->solver == CH_SOLVER_ROE;
   if (c->hcorr && !roe) return fail(CH_ESTATE, "ch_step: the H correction goes with the Roe solver (ch_set_solver)");
   switch (c->recon) {
-    case CH_RECON_PLMC: return roe ? step_impl<1, 1>(c, dt) : step_impl<0, 1>(c, dt);
-    case CH_RECON_PCM: return roe ? step_impl<1, 2>(c, dt) : step_impl<0, 2>(c, dt);
-    default: return roe ? step_impl<1, 0>(c, dt) : step_impl<0, 0>(c, dt);
+    case CH_RECON_PLMC: return roe ? step_impl<1, 1>(c, dt, devdt) : step_impl<0, 1>(c, dt, devdt);
+    case CH_RECON_PCM: return roe ? step_impl<1, 2>(c, dt, devdt) : step_impl<0, 2>(c, dt, devdt);
+    default: return roe ? step_impl<1, 0>(c, dt, devdt) : step_impl<0, 0>(c, dt, devdt);
   }
+}
+
+int ch_step(ch_ctx* c, double dt) {
+  if (!c) return fail(CH_EINVAL, "ch_step: null context");
+  return step_dispatch(c, dt, false);
+}
+
+int ch_step_cfl(ch_ctx* c, double cfl, double t_left) {
+  if (!c) return fail(CH_EINVAL, "ch_step_cfl: null context");
+  if (!c->have_state) return fail(CH_ESTATE, "ch_step_cfl: no state set");
+  if (!(cfl > 0.0) || !(cfl <= 1.0)) return fail(CH_EINVAL, "ch_step_cfl: cfl not in (0,1]");
+  if (t_left != t_left) return fail(CH_EINVAL, "ch_step_cfl: t_left is NaN");
+  if (!c->dt_valid) {
+    StepArgs A = make_args(c, 1.0);
+    { Bracket b(c, CH_K_RESET); k_reset<<<1, 32, 0, c->stream>>>(c->red); }
+    const long long N = (long long)c->geo.n[0] * c->geo.n[1] * c->geo.n[2];
+    long long blocks = (N + 255) / 256;
+    if (blocks > 148 * 8) blocks = 148 * 8;
+    { Bracket b(c, CH_K_DT); k_dt<<<(unsigned)blocks, 256, 0, c->stream>>>(A); }
+    c->dt_valid = true;
+  }
+  { Bracket b(c, CH_K_RESET); k_pick_dt<<<1, 32, 0, c->stream>>>(c->red, cfl, t_left); }
+  CH_CUDA(cudaGetLastError(), "k_pick_dt");
+  return step_dispatch(c, 0.0, true);
+}
+
+double ch_last_dt(ch_ctx* c) {
+  const double nan = std::numeric_limits<double>::quiet_NaN();
+  if (!c || !c->bound) { fail(CH_ESTATE, "ch_last_dt: no buffers bound"); return nan; }
+  cudaError_t e = cudaMemcpyAsync(c->h_red, c->red + 2, 16, cudaMemcpyDeviceToHost, c->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+  if (e != cudaSuccess) { cuda_fail(e, "ch_last_dt read-back"); return nan; }
+  double dt;
+  std::memcpy(&dt, &c->h_red[0], 8);
+  if (dt != dt) fail(CH_ENONPHYS, "ch_last_dt: non-physical cell (rho <= 0 or non-finite) met by ch_step_cfl");
+  return dt;
+}
+
+double ch_elapsed(ch_ctx* c) {
+  const double nan = std::numeric_limits<double>::quiet_NaN();
+  if (!c || !c->bound) { fail(CH_ESTATE, "ch_elapsed: no buffers bound"); return nan; }
+  cudaError_t e = cudaMemcpyAsync(c->h_red, c->red + 2, 16, cudaMemcpyDeviceToHost, c->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+  if (e != cudaSuccess) { cuda_fail(e, "ch_elapsed read-back"); return nan; }
+  double t;
+  std::memcpy(&t, &c->h_red[1], 8);
+  return t;
 }
 
 int ch_set_hcorrection(ch_ctx* c, int on) {

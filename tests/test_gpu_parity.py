@@ -588,3 +588,51 @@ def test_hcorrection_run_switches_and_errors(ch, ref):
     with pytest.raises(ValueError):
         G3.set_hcorrection(True)                               # three ghost layers are not enough
     G3.close()
+
+
+# ---- ch_step_cfl: Eq. 22 finished on the device, no host round trip per step --------------------------
+@pytest.mark.parametrize("maker", [lambda: wl.sod(128), lambda: wl.kelvin_helmholtz(64), lambda: wl.sweep(shape=(64, 40, 36)),
+                                   lambda: wl.sweep(shape=(45, 37, 33)), lambda: wl.sedov(24)])
+def test_step_cfl_equals_the_compute_dt_step_loop_bitwise(ch, maker):
+    w = maker()
+    G = ch.Grid(*w.shape, 3, w.gamma, w.bc)
+    G.set_state(w.u)
+    dts = []
+    for _ in range(6):
+        dt = G.compute_dt(w.cfl)
+        dts.append(dt)
+        G.step(dt)
+    a = G.get_padded()
+    G.set_state(w.u)
+    for n in range(6):
+        G.step_cfl(w.cfl)
+        if n == 2:
+            assert G.last_dt() == dts[2]
+    assert np.array_equal(G.get_padded(), a)
+    assert G.last_dt() == dts[-1]
+    G.close()
+
+
+def test_step_cfl_clips_to_the_time_left_and_accumulates(ch, ref):
+    w = wl.sod(128)
+    G, Rg = both(ch, ref, w)
+    t_ref = run(Rg, w)[1]
+    G.set_state(w.u)
+    t0 = G.elapsed()
+    steps = 0
+    while True:
+        left = w.t_end - (G.elapsed() - t0)
+        if left <= w.t_end * 1e-14:
+            break
+        G.step_cfl(w.cfl, left)
+        steps += 1
+        assert steps < 1000
+    assert abs((G.elapsed() - t0) - w.t_end) <= 1e-15 and abs(t_ref - w.t_end) <= 1e-15
+    assert max(rel_l1_error(G.get_state(), Rg.get_state(), w.gamma)) <= RUN_L1_TOL
+    with pytest.raises(ValueError):
+        G.step_cfl(1.5)
+    u = w.u.copy(); u[0, 0, 0, 5] = -1.0
+    G.set_state(u)
+    G.step_cfl(w.cfl)
+    assert math.isnan(G.last_dt())
+    G.close()
