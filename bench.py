@@ -282,6 +282,15 @@ def main():
             sec = timed_steps(G, ww.cfl, k, ev)
             other_wl[name] = {"value": ww.u[0].size * k / sec, "unit": UNIT, "ms_per_step": sec / k * 1e3,
                               "steps": k, "after_steps": pre}
+            # the same steps queued through ch_step_cfl (dt stays on the device: no per-step read-back)
+            torch.cuda.synchronize()
+            ev[0].record(G.cuda_stream)
+            for _ in range(k):
+                G.step_cfl(ww.cfl)
+            ev[1].record(G.cuda_stream)
+            torch.cuda.synchronize()
+            sec2 = ev[0].elapsed_time(ev[1]) * 1e-3
+            other_wl[name]["ch_step_cfl"] = {"value": ww.u[0].size * k / sec2, "unit": UNIT, "ms_per_step": sec2 / k * 1e3}
             G.close()
             del G
             torch.cuda.empty_cache()
