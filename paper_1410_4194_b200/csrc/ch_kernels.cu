@@ -73,6 +73,10 @@ __device__ __forceinline__ void step_dtdx(const StepArgs& A, double out[3]) {
   }
 }
 
+__device__ __forceinline__ double step_dtdx1(const StepArgs& A, int d) {   // one direction only (pass 1)
+  return A.dt_dev ? __ddiv_rn(*A.dt_dev, A.dx[d]) : A.dtdx[d];
+}
+
 // global component index of direction-local component m for a sweep along D (cyclic)
 template <int D>
 __device__ __forceinline__ constexpr int comp(int m) {
@@ -140,8 +144,6 @@ template <int D, int S, int R>
 __global__ void __launch_bounds__(CH_MARCH_T, CH_MARCH_MINB) k_pass1_march(const StepArgs A, int seg) {
   constexpr int T = 3 - D;   // the other transverse dimension (x is the lane dimension)
   const Geom& g = A.geo;
-  double dtx[3];
-  step_dtdx(A, dtx);
   const Gas& G = A.gas;
   const int ext0 = g.act[0] ? g.n[0] + 2 : 1, lo0 = g.act[0] ? -1 : 0;
   const int extT = g.act[T] ? g.n[T] + 2 : 1, loT = g.act[T] ? -1 : 0;
@@ -158,7 +160,7 @@ __global__ void __launch_bounds__(CH_MARCH_T, CH_MARCH_MINB) k_pass1_march(const
   const long long sD = g.st[D];
   const long long np = g.np;
   const long long base = (long long)(i + g.g[0]) + (long long)(t + g.g[T]) * g.st[T] + (long long)g.g[D] * sD;
-  const double dtdx = dtx[D];
+  const double dtdx = step_dtdx1(A, D);
   const double* __restrict__ u = A.u;
 
   double wa[5], wb[5], wc[5], wd[5];   // cells c-1, c, c+1, c+2 (rotating)
@@ -224,8 +226,7 @@ __global__ void __launch_bounds__(kXT, CH_X_MINB) k_pass1_x(const StepArgs A, lo
   __shared__ double sS[5][kXT];
   __shared__ double sL[5][kXT];
   const Geom& g = A.geo;
-  double dtx[3];
-  step_dtdx(A, dtx);
+  const double dtdx0 = step_dtdx1(A, 0);
   const Gas& G = A.gas;
   const long long np = g.np;
   const int tid = threadIdx.x;
@@ -269,7 +270,7 @@ __global__ void __launch_bounds__(kXT, CH_X_MINB) k_pass1_x(const StepArgs A, lo
     double sm[5], sp[5], WLs[5], WRs[5], cl[5], cr[5];
 #pragma unroll
     for (int m = 0; m < 5; ++m) { sm[m] = sS[m][tid - 1]; sp[m] = sS[m][tid + 1]; }
-    ch::recon_faces<R>(G, dtx[0], wm, w0, wp, sm, s0, sp, ic, WLs, WRs);
+    ch::recon_faces<R>(G, dtdx0, wm, w0, wp, sm, s0, sp, ic, WLs, WRs);
     ch::prim2cons(G, WLs, cl);
     ch::prim2cons(G, WRs, cr);
     // a cell's faces are written by the CTA whose output window [2, kXT-4] holds it, plus the
