@@ -73,3 +73,12 @@ def test_product_does_not_import_the_oracle():
             if f.endswith((".py", ".cu", ".cuh", ".h")):
                 src = open(os.path.join(root, f)).read()
                 assert "import oracle" not in src and "from oracle" not in src and "cholla_ref" not in src, f
+
+
+def test_sass_holds_the_tma_pipeline():
+    """The fused second half streams its planes with TMA: the built library must contain bulk tensor loads
+    (UTMALDG.4D, the SASS of cp.async.bulk.tensor.4d) and mbarrier phase checks (SYNCS...TRYWAIT)."""
+    import subprocess
+    out = subprocess.run(["cuobjdump", "-sass", binding._LIB], capture_output=True, text=True).stdout
+    assert "UTMALDG.4D" in out and "SYNCS.PHASECHK.TRANS64.TRYWAIT" in out
+    assert "MUFU.RSQ64H" in out and "MUFU.RCP64H" in out          # the branch-free rsqrt / rcp seeds
