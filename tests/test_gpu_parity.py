@@ -133,6 +133,9 @@ ONE_STEP_CASES = {
     "sweep_xz_2d": lambda: wl.sweep(shape=(64, 1, 48)),           # inactive y
     "sweep_yz_2d": lambda: wl.sweep(shape=(1, 40, 48)),           # inactive x
     "sweep_min_size": lambda: wl.sweep(shape=(3, 3, 3)),
+    "sweep_tiny_even_tma": lambda: wl.sweep(shape=(4, 4, 4)),          # even padded strides: the TMA form on one partial tile
+    "sweep_flat_even_tma": lambda: wl.sweep(shape=(8, 6, 4)),
+    "sweep_two_z_segments_tma": lambda: wl.sweep(shape=(34, 20, 20)),
     "smooth_mixed_bc": lambda: wl.smooth_random(41, 29, 23, seed=5, bc=(R, O, P, P, O, R)),
     "rough_3d": lambda: wl.rough_random(37, 21, 13, seed=11, decades=0.5),
     "rough_1d": lambda: wl.rough_random(1000, seed=12, mach=3.0),
