@@ -737,6 +737,9 @@ __global__ void __launch_bounds__(kFT, CH_F_MINB) k_final3d(const StepArgs A, in
 #ifndef CH_T_TY
 #define CH_T_TY 11
 #endif
+#ifndef CH_T_SLEEP
+#define CH_T_SLEEP 200      // ns between the producer's polls of an empty barrier
+#endif
 constexpr int kTY = CH_T_TY, kTT = kFX * kTY;      // consumer threads; one more warp produces
 struct TmaMaps { CUtensorMap m[10]; };              // Fs0 Fs1 Fs2 | UL2 UR2 | UL0 UR0 u | UL1 UR1
 __device__ __forceinline__ constexpr int group_first(int q) { return q == 0 ? 0 : q == 1 ? 3 : q == 2 ? 5 : q == 3 ? 8 : 10; }   // arrays of group q: [first(q), first(q+1))
@@ -763,6 +766,22 @@ __device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
         "}\n" : "=r"(done) : "r"(bar), "r"(parity) : "memory");
     if (done) return;
     if (spin > (1u << 26)) __trap();
+  }
+}
+// The producer's waits: it has a whole plane of slack, so it sleeps between polls instead of spending the
+// issue slots of the scheduler it shares with three consumer warps.
+__device__ __forceinline__ void mbar_wait_relaxed(unsigned bar, unsigned parity) {
+  for (unsigned spin = 0;; ++spin) {
+    unsigned done;
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+        "selp.u32 %0, 1, 0, p;\n"
+        "}\n" : "=r"(done) : "r"(bar), "r"(parity) : "memory");
+    if (done) return;
+    __nanosleep(CH_T_SLEEP);
+    if (spin > (1u << 24)) __trap();
   }
 }
 __device__ __forceinline__ void tma_load_4d(unsigned dst, const CUtensorMap* map, unsigned bar, int c0, int c1, int c2, int c3) {
@@ -810,7 +829,7 @@ __global__ void __launch_bounds__(kTT + 32, 1) k_final3d_tma(const StepArgs A, c
       for (int k = k0 - 1; k <= k1; ++k, ++n) {
 #pragma unroll
         for (int q = 0; q < 4; ++q) {
-          if (n > 0) mbar_wait(bempty[q], (unsigned)((n - 1) & 1));      // all consumers released plane k-1's copy
+          if (n > 0) mbar_wait_relaxed(bempty[q], (unsigned)((n - 1) & 1));      // all consumers released plane k-1's copy
           const int a0 = group_first(q), a1 = group_first(q + 1);
           mbar_expect_tx(bfull[q], (unsigned)((a1 - a0) * 5 * kTT * sizeof(double)));
           for (int a = a0; a < a1; ++a)
