@@ -578,9 +578,9 @@ __device__ __forceinline__ void correct_faces(const StepArgs& A, const double ul
 #pragma unroll
   for (int m = 0; m < 5; ++m) {
     const int f = comp<D>(m);
-    const double corr = dF[D1][f] + dF[D2][f];
-    cl[m] = ul[m] + corr;
-    cr[m] = ur[m] + corr;
+    const double corr = __dadd_rn(dF[D1][f], dF[D2][f]);     // explicitly rounded: every form of the kernel gets the same bits
+    cl[m] = __dadd_rn(ul[m], corr);
+    cr[m] = __dadd_rn(ur[m], corr);
   }
   ch::cons2prim(A.gas, cl[0], cl[1], cl[2], cl[3], cl[4], wl);
   ch::cons2prim(A.gas, cr[0], cr[1], cr[2], cr[3], cr[4], wr);
@@ -645,14 +645,14 @@ __global__ void __launch_bounds__(kFT, CH_F_MINB) k_final3d(const StepArgs A, in
           const double fz = A.Fs[2][a];
           const double fzm = first ? A.Fs[2][a - s2] : zS[f][tid];
           zS[f][tid] = fz;
-          dF[1][f] = hy * (A.Fs[1][a - s1] - A.Fs[1][a]);
-          dF[2][f] = hz * (fzm - fz);
+          dF[1][f] = __dmul_rn(hy, A.Fs[1][a - s1] - A.Fs[1][a]);
+          dF[2][f] = __dmul_rn(hz, fzm - fz);
         }
       }
 #pragma unroll
       for (int f = 0; f < 5; ++f) {
         const double t = __shfl_up_sync(full, fx[f], 1);
-        dF[0][f] = hx * ((lane == 0 ? fxm[f] : t) - fx[f]);
+        dF[0][f] = __dmul_rn(hx, (lane == 0 ? fxm[f] : t) - fx[f]);
       }
     }
     double part[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
@@ -735,12 +735,12 @@ __global__ void __launch_bounds__(kFT, CH_F_MINB) k_final3d(const StepArgs A, in
 // the loads of plane k+1 run under the solves of plane k.
 // ---------------------------------------------------------------------------------------------
 #ifndef CH_T_TY
-#define CH_T_TY 11
+#define CH_T_TY 12
 #endif
 #ifndef CH_T_SLEEP
 #define CH_T_SLEEP 200      // ns between the producer's polls of an empty barrier
 #endif
-constexpr int kTY = CH_T_TY, kTT = kFX * kTY;      // consumer threads; one more warp produces
+constexpr int kTY = CH_T_TY, kTT = kFX * kTY, kTC = kTT - kFX;   // staged rows; threads = staged slots; consumer threads
 struct TmaMaps { CUtensorMap m[10]; };              // Fs0 Fs1 Fs2 | UL2 UR2 | UL0 UR0 u | UL1 UR1
 __device__ __forceinline__ constexpr int group_first(int q) { return q == 0 ? 0 : q == 1 ? 3 : q == 2 ? 5 : q == 3 ? 8 : 10; }   // arrays of group q: [first(q), first(q+1))
 
@@ -791,7 +791,7 @@ __device__ __forceinline__ void tma_load_4d(unsigned dst, const CUtensorMap* map
 }
 
 template <int S>
-__global__ void __launch_bounds__(kTT + 32, 1) k_final3d_tma(const StepArgs A, const __grid_constant__ TmaMaps M, int seg) {
+__global__ void __launch_bounds__(kTT, 1) k_final3d_tma(const StepArgs A, const __grid_constant__ TmaMaps M, int seg) {
   extern __shared__ __align__(1024) double s_t[];
   __shared__ unsigned long long s_full[4], s_empty[4];
   typedef double (*Arr)[kTT];
@@ -803,7 +803,10 @@ __global__ void __launch_bounds__(kTT + 32, 1) k_final3d_tma(const StepArgs A, c
   step_dtdx(A, dtx);
   const Gas& G = A.gas;
   const unsigned full = 0xffffffffu;
-  const int tid = threadIdx.x, lane = tid & 31, row = tid >> 5;
+  // kTY rows are staged.  Warps 0..kTY-3 update rows 1..kTY-2; warp kTY-2 serves both halo rows (row 0 supplies its
+  // right-face y state, row kTY-1 its low-face y flux: a third of an updating warp's work); warp kTY-1 produces.
+  const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5, row = wid + 1;
+  const int sidx = row * kFX + lane;                   // this thread's slot in the staged and exchanged arrays
   const int nx = g.n[0], ny = g.n[1], nz = g.n[2];
   const int i0 = (int)blockIdx.x * (kFX - 2) - 1, j0 = (int)blockIdx.y * (kTY - 2) - 1;
   const int k0 = (int)blockIdx.z * seg;
@@ -816,12 +819,12 @@ __global__ void __launch_bounds__(kTT + 32, 1) k_final3d_tma(const StepArgs A, c
   }
   if (tid == 0) {
 #pragma unroll
-    for (int q = 0; q < 4; ++q) { mbar_init(bfull[q], 1); mbar_init(bempty[q], kTT); }
+    for (int q = 0; q < 4; ++q) { mbar_init(bfull[q], 1); mbar_init(bempty[q], kTC); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncthreads();
 
-  if (row == kTY) {
+  if (wid == kTY - 1) {
     // ===== producer warp: one lane streams the planes =====
     if (lane == 0) {
       const unsigned stage = (unsigned)__cvta_generic_to_shared(s_t);
@@ -841,18 +844,69 @@ __global__ void __launch_bounds__(kTT + 32, 1) k_final3d_tma(const StepArgs A, c
   }
 
   // ===== consumer warps =====
+  Arr stg0 = reinterpret_cast<Arr>(s_t);
+  double tmin = 0.0;
+  bool bad = false;
+  if (wid == kTY - 2) {
+    // ----- halo warp: rows 0 and kTY-1 of the tile -----
+    const int ih = i0 + lane, jt = j0 + kTY - 1, st_ = (kTY - 1) * kFX + lane;
+    const bool laneok = lane >= 1 && lane <= kFX - 2 && ih >= 0 && ih < nx;
+    const bool topok = laneok && jt <= ny && jt >= 0;
+    const double hxh = 0.5 * dtx[0], hzh = 0.5 * dtx[2];
+    double zSb[5] = {0.0, 0.0, 0.0, 0.0, 0.0}, zSt[5] = {0.0, 0.0, 0.0, 0.0, 0.0};   // F*_z of the previous plane, both rows
+    int n = 0;
+    for (int k = k0 - 1; k <= k1; ++k, ++n) {
+      const bool mid = k != k0 - 1 && k != k1;
+      const unsigned ph = (unsigned)(n & 1);
+      double dxb[5], dzb[5], dxt[5], dzt[5];
+      mbar_wait(bfull[0], ph);
+#pragma unroll
+      for (int f = 0; f < 5; ++f) {
+        const double fxb = stg0[f][lane], fzb = stg0[10 + f][lane];
+        const double fxt = stg0[f][st_], fzt = stg0[10 + f][st_];
+        dzb[f] = __dmul_rn(hzh, zSb[f] - fzb); zSb[f] = fzb;
+        dzt[f] = __dmul_rn(hzh, zSt[f] - fzt); zSt[f] = fzt;
+        dxb[f] = __dmul_rn(hxh, __shfl_up_sync(full, fxb, 1) - fxb);
+        dxt[f] = __dmul_rn(hxh, __shfl_up_sync(full, fxt, 1) - fxt);
+      }
+      mbar_arrive(bempty[0]);
+      mbar_wait(bfull[1], ph); mbar_arrive(bempty[1]);
+      mbar_wait(bfull[2], ph); mbar_arrive(bempty[2]);
+      mbar_wait(bfull[3], ph);
+      double cb[5], ct[5];
+#pragma unroll
+      for (int m = 0; m < 5; ++m) {
+        // exactly what correct_faces<1> forms: U* + (dF_z + dF_x), y-local order
+        cb[m] = __dadd_rn(stg0[45 + comp<1>(m)][lane], __dadd_rn(dzb[comp<1>(m)], dxb[comp<1>(m)]));     // U^{n+1/2}_R(., y), row 0
+        ct[m] = __dadd_rn(stg0[40 + comp<1>(m)][st_], __dadd_rn(dzt[comp<1>(m)], dxt[comp<1>(m)]));      // U^{n+1/2}_L(., y), row kTY-1
+      }
+      mbar_arrive(bempty[3]);
+      if (mid) {
+        double wr0[5] = {1.0, 0.0, 0.0, 0.0, 1.0}, wlt[5] = {1.0, 0.0, 0.0, 0.0, 1.0}, nb[5], fl[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+        if (laneok) ch::cons2prim(A.gas, cb[0], cb[1], cb[2], cb[3], cb[4], wr0);
+        if (topok) ch::cons2prim(A.gas, ct[0], ct[1], ct[2], ct[3], ct[4], wlt);
+#pragma unroll
+        for (int m = 0; m < 5; ++m) sX[m][lane] = wr0[m];
+        asm volatile("bar.sync 1, %0;" ::"n"(kTC) : "memory");
+#pragma unroll
+        for (int m = 0; m < 5; ++m) nb[m] = sX[m][st_ - kFX];
+        if (topok) ch::riemann<S>(G, nb, wlt, fl);
+#pragma unroll
+        for (int m = 0; m < 5; ++m) sF[m][st_] = fl[m];
+        asm volatile("bar.sync 1, %0;" ::"n"(kTC) : "memory");
+      }
+    }
+  } else {
   Arr stg = reinterpret_cast<Arr>(s_t);
   const int i = i0 + lane, j = j0 + row;
   const bool valid = i <= nx && j <= ny;
   const bool realI = i >= 0 && i < nx, realJ = j >= 0 && j < ny;
-  const bool updL = lane >= 1 && lane <= kFX - 2 && realI, updR = row >= 1 && row <= kTY - 2 && realJ;
+  const bool updL = lane >= 1 && lane <= kFX - 2 && realI, updR = realJ;
   const bool need0 = valid && updR, need1 = valid && updL, need2 = updL && updR;
   const bool solve0 = need0 && lane >= 1 && i >= 0, solve1 = need1 && row >= 1 && j >= 0;
   const long long np = g.np, s2 = g.st[2];
   const long long qcol = (long long)(i + g.g[0]) + (long long)(j + g.g[1]) * g.st[1] + (long long)g.g[2] * s2;
   const double hx = 0.5 * dtx[0], hy = 0.5 * dtx[1], hz = 0.5 * dtx[2];
-  double tmin = 0.0;
-  bool bad = false;
   // carried from the previous plane (registers: one CTA per SM leaves ~150 per thread)
   double zU[5] = {1.0, 0.0, 0.0, 0.0, 1.0};    // U^{n+1/2}_R(., z) of cell k-1, primitive, z-local order
   double zF[5] = {0.0, 0.0, 0.0, 0.0, 0.0};    // H^{n+1/2} on the low z face of cell k-1, z-local order
@@ -870,20 +924,20 @@ __global__ void __launch_bounds__(kTT + 32, 1) k_final3d_tma(const StepArgs A, c
       double fx[5];
 #pragma unroll
       for (int f = 0; f < 5; ++f) {
-        fx[f] = stg[f][tid];
-        const double fy = stg[5 + f][tid];
-        const double fym = stg[5 + f][row > 0 ? tid - kFX : tid];      // row 0 never uses its y difference
-        const double fz = stg[10 + f][tid];
+        fx[f] = stg[f][sidx];
+        const double fy = stg[5 + f][sidx];
+        const double fym = stg[5 + f][sidx - kFX];
+        const double fz = stg[10 + f][sidx];
         const double fzm = zS[f];                                   // garbage on the first plane: unused there
         zS[f] = fz;
-        dF[1][f] = hy * (fym - fy);
-        dF[2][f] = hz * (fzm - fz);
+        dF[1][f] = __dmul_rn(hy, fym - fy);
+        dF[2][f] = __dmul_rn(hz, fzm - fz);
       }
       mbar_arrive(bempty[0]);
 #pragma unroll
       for (int f = 0; f < 5; ++f) {
         const double t = __shfl_up_sync(full, fx[f], 1);                 // lane 0 never uses its x difference
-        dF[0][f] = hx * (t - fx[f]);
+        dF[0][f] = __dmul_rn(hx, t - fx[f]);
       }
     }
     // ---- group 1: z states; the neighbour is this thread's previous plane
@@ -892,7 +946,7 @@ __global__ void __launch_bounds__(kTT + 32, 1) k_final3d_tma(const StepArgs A, c
     {
       double ul[5], ur[5];
 #pragma unroll
-      for (int m = 0; m < 5; ++m) { ul[m] = stg[15 + comp<2>(m)][tid]; ur[m] = stg[20 + comp<2>(m)][tid]; }
+      for (int m = 0; m < 5; ++m) { ul[m] = stg[15 + comp<2>(m)][sidx]; ur[m] = stg[20 + comp<2>(m)][sidx]; }
       mbar_arrive(bempty[1]);
       if (need2) {
         double wl[5], nb[5];
@@ -923,7 +977,7 @@ __global__ void __launch_bounds__(kTT + 32, 1) k_final3d_tma(const StepArgs A, c
     {
       double ul[5], ur[5];
 #pragma unroll
-      for (int m = 0; m < 5; ++m) { ul[m] = stg[25 + m][tid]; ur[m] = stg[30 + m][tid]; part[m] = stg[35 + m][tid]; }
+      for (int m = 0; m < 5; ++m) { ul[m] = stg[25 + m][sidx]; ur[m] = stg[30 + m][sidx]; part[m] = stg[35 + m][sidx]; }
       mbar_arrive(bempty[2]);
       if (mid) {
         double wl[5] = {1.0, 0.0, 0.0, 0.0, 1.0}, wr[5] = {1.0, 0.0, 0.0, 0.0, 1.0}, nb[5], fl[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
@@ -943,23 +997,22 @@ __global__ void __launch_bounds__(kTT + 32, 1) k_final3d_tma(const StepArgs A, c
     {
       double ul[5], ur[5];
 #pragma unroll
-      for (int m = 0; m < 5; ++m) { ul[m] = stg[40 + comp<1>(m)][tid]; ur[m] = stg[45 + comp<1>(m)][tid]; }
+      for (int m = 0; m < 5; ++m) { ul[m] = stg[40 + comp<1>(m)][sidx]; ur[m] = stg[45 + comp<1>(m)][sidx]; }
       mbar_arrive(bempty[3]);
       if (mid) {
         double wl[5] = {1.0, 0.0, 0.0, 0.0, 1.0}, wr[5] = {1.0, 0.0, 0.0, 0.0, 1.0}, nb[5], fl[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
         if (need1) correct_faces<1>(A, ul, ur, dF, wl, wr);
 #pragma unroll
-        for (int m = 0; m < 5; ++m) sX[m][tid] = wr[m];
-        asm volatile("bar.sync 1, %0;" ::"n"(kTT) : "memory");
-        const int src = tid >= kFX ? tid - kFX : tid;
+        for (int m = 0; m < 5; ++m) sX[m][sidx] = wr[m];
+        asm volatile("bar.sync 1, %0;" ::"n"(kTC) : "memory");
 #pragma unroll
-        for (int m = 0; m < 5; ++m) nb[m] = sX[m][src];
+        for (int m = 0; m < 5; ++m) nb[m] = sX[m][sidx - kFX];
         if (solve1) ch::riemann<S>(G, nb, wl, fl);
 #pragma unroll
-        for (int m = 0; m < 5; ++m) sF[m][tid] = fl[m];
-        asm volatile("bar.sync 1, %0;" ::"n"(kTT) : "memory");
+        for (int m = 0; m < 5; ++m) sF[m][sidx] = fl[m];
+        asm volatile("bar.sync 1, %0;" ::"n"(kTC) : "memory");
         if (need2) {
-          const int dst = tid + kFX;
+          const int dst = sidx + kFX;
           // y-local order (rho, my, mz, mx, E) -> global
           part[0] += dtx[1] * (fl[0] - sF[0][dst]);
           part[2] += dtx[1] * (fl[1] - sF[1][dst]);
@@ -974,19 +1027,20 @@ __global__ void __launch_bounds__(kTT + 32, 1) k_final3d_tma(const StepArgs A, c
       for (int m = 0; m < 5; ++m) { zU[m] = wrz[m]; zF[m] = flz[m]; zP[m] = part[m]; }
     }
   }
+  }
   // Eq. 22 reduction over the consumer warps (the producer warp has left)
   {
     __shared__ double s_max[32];
     __shared__ int s_badflag;
     if (tid == 0) s_badflag = 0;
-    asm volatile("bar.sync 1, %0;" ::"n"(kTT) : "memory");
+    asm volatile("bar.sync 1, %0;" ::"n"(kTC) : "memory");
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) tmin = fmax(tmin, __shfl_xor_sync(full, tmin, o));
     if (__any_sync(full, bad) && lane == 0) s_badflag = 1;
-    if (lane == 0) s_max[row] = tmin;
-    asm volatile("bar.sync 1, %0;" ::"n"(kTT) : "memory");
+    if (lane == 0) s_max[wid] = tmin;
+    asm volatile("bar.sync 1, %0;" ::"n"(kTC) : "memory");
     if (tid < 32) {
-      double v = tid < kTY ? s_max[tid] : 0.0;
+      double v = tid < kTY - 1 ? s_max[tid] : 0.0;
 #pragma unroll
       for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(full, v, o));
       if (tid == 0) {
@@ -1454,7 +1508,7 @@ int step_impl(ch_ctx* c, double dt, bool devdt) {
       dim3 tgrid((unsigned)((g.n[0] + kFX - 3) / (kFX - 2)), (unsigned)((g.n[1] + kTY - 3) / (kTY - 2)),
                  (unsigned)((g.n[2] + seg - 1) / seg));
       Bracket b(c, CH_K_FINAL);
-      k_final3d_tma<S><<<tgrid, kTT + 32, tsmem, st>>>(A, c->maps, seg);
+      k_final3d_tma<S><<<tgrid, kTT, tsmem, st>>>(A, c->maps, seg);
     } else {
     const size_t smem = (size_t)30 * kFT * sizeof(double);
     static bool attr_set = false;

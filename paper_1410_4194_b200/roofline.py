@@ -16,7 +16,7 @@ ALG_FLOPS / ALG_INST were frozen from the ncu thread-level counts
 piece once with the present arithmetic, divided by 512^3: k_pass1_* from
 profiles/r01f_full_512_summary.txt, and the unfused k_pass2 + k_update (CH_UNFUSED=1,
 profiles/r01f_unfused_counts.csv) for the second half.  k_final3d recomputes halo lanes / rows
-(32/30 x 10/8) and is still charged only the unfused count.  Re-freeze whenever ch_hydro.cuh changes.
+(32/30 x 12/10) and is still charged only the unfused count.  Re-freeze whenever ch_hydro.cuh changes.
 """
 
 # bytes per real cell-update (fp64 = 8 B): pass 1 reads u (5) and writes U*_L, U*_R, F* (15);
