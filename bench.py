@@ -35,8 +35,8 @@ if ROOT not in sys.path:
 METRIC = "cell-updates/sec (fp64 CTU+PPM+exact Riemann)"
 UNIT = "cell-updates/s"
 CPU_SAMPLE_N = 128          # the oracle is timed on a 128^3 corner of the workload
-# DRAM bytes per launch at 512^3 from the committed ncu --set full capture (profiles/r01i_*); None = not captured
-TRAFFIC_NCU = {"k_pass1_x": 21.98e9, "k_pass1_march<y>": 22.73e9, "k_pass1_march<z>": 22.96e9, "k_final3d": 72.97e9}
+# DRAM bytes per launch at 512^3 from the committed ncu --set full capture (profiles/r01k_*); None = not captured
+TRAFFIC_NCU = {"k_pass1_x": 22.04e9, "k_pass1_march<y>": 22.71e9, "k_pass1_march<z>": 22.94e9, "k_final3d": 75.91e9}
 
 
 def parse():
