@@ -34,9 +34,8 @@ if ROOT not in sys.path:
 
 METRIC = "cell-updates/sec (fp64 CTU+PPM+exact Riemann)"
 UNIT = "cell-updates/s"
-CPU_SAMPLE_N = 128          # the oracle is timed on a 128^3 corner of the workload
-# DRAM bytes per launch at 512^3 from the committed ncu --set full capture (profiles/r01k_*); None = not captured
-TRAFFIC_NCU = {"k_pass1_x": 22.04e9, "k_pass1_march<y>": 22.71e9, "k_pass1_march<z>": 22.94e9, "k_final3d": 75.91e9}
+CPU_SAMPLE_N = 128          # the oracle is timed on a 128^3 corner of the workload (and on a 256^3 one, all cores)
+ORACLE_FLAGS = "g++ -std=c++17 -O2 -ffp-contract=off -fopenmp (oracle/ref.py)"
 
 
 def parse():
@@ -112,12 +111,47 @@ def corner_sample(w, m):
     return np.ascontiguousarray(w.u[:, :m, :m, :m])
 
 
-def time_oracle(w, steps, warmup, m=CPU_SAMPLE_N):
+def host_cores():
+    return len(os.sched_getaffinity(0)) if hasattr(os, "sched_getaffinity") else (os.cpu_count() or 1)
+
+
+def cpu_model():
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
+def set_oracle_threads(n):
+    """Thread count of the oracle's OpenMP loops, set through the OpenMP runtime the oracle library links (the
+    oracle itself is untouched).  Returns the count in force."""
+    import ctypes
+    from oracle import ref
+    ref.lib()                                   # make sure libgomp is loaded by the oracle first
+    try:
+        gomp = ctypes.CDLL("libgomp.so.1")
+        gomp.omp_set_num_threads(int(n))
+        return int(gomp.omp_get_max_threads())
+    except OSError:
+        return None
+
+
+def time_oracle(w, steps, warmup, m=CPU_SAMPLE_N, threads=None):
     from oracle import ref
     from paper_1410_4194_b200 import workloads as wl
     nx = w.shape[0]
     m = min(m, nx)
     u = corner_sample(w, m)
+    cores = host_cores()
+    omp = os.environ.get("OMP_NUM_THREADS")
+    if omp:
+        cores = min(cores, int(omp))
+    if threads is not None:
+        got = set_oracle_threads(threads)
+        cores = got if got is not None else cores
     G = ref.RefGrid(m, m, m, 3, w.gamma, (wl.OUTFLOW,) * 6)
     G.set_spacing(1.0 / nx, 1.0 / nx, 1.0 / nx)
     G.set_state(u)
@@ -127,14 +161,29 @@ def time_oracle(w, steps, warmup, m=CPU_SAMPLE_N):
     for _ in range(steps):
         G.step(G.compute_dt(w.cfl))
     el = time.perf_counter() - t0
-    cores = len(os.sched_getaffinity(0)) if hasattr(os, "sched_getaffinity") else os.cpu_count()
-    omp = os.environ.get("OMP_NUM_THREADS")
-    if omp:
-        cores = min(cores, int(omp))
+    del G
     return dict(value=m ** 3 * steps / el, unit=UNIT, cores=cores, kind="oracle",
                 sample=f"{m}^3 corner of the {nx}^3 sweep initial state (outflow faces, dx=1/{nx}), "
-                       f"{steps} steps of compute_dt+step after {warmup} warm-up, OpenMP over the outer loops",
-                ms_per_step=el / steps * 1e3)
+                       f"{steps} steps of compute_dt+step after {warmup} warm-up, OpenMP over the outer loops, "
+                       f"{cores} thread(s)",
+                ms_per_step=el / steps * 1e3, per_core=m ** 3 * steps / el / max(cores, 1))
+
+
+def oracle_legs(w):
+    """SURVEY.md section 8(d) "Oracle timing": (i) one thread, 128^3, 3 steps; (ii) all host cores, 128^3 x 10 steps and
+    256^3 x 2 steps.  The oracle as it stands; bit-identical at any thread count (no floating-point reduction)."""
+    n_all = host_cores()
+    legs = []
+    for label, m, steps, warm, thr in (("single thread 128^3 x 3", 128, 3, 0, 1),
+                                       ("all cores 128^3 x 10", 128, 10, 1, n_all),
+                                       ("all cores 256^3 x 2", 256, 2, 0, n_all)):
+        if m > w.shape[0]:
+            continue
+        r = time_oracle(w, steps, warm, m=m, threads=thr)
+        legs.append({"leg": label, "value": r["value"], "unit": UNIT, "per_core": r["per_core"], "cores": r["cores"],
+                     "ms_per_step": r["ms_per_step"], "sample": r["sample"]})
+    set_oracle_threads(n_all)
+    return legs
 
 
 def run_reference(args):
@@ -149,7 +198,8 @@ def run_reference(args):
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": f"throughput sweep (BASELINE.json config 5), {CPU_SAMPLE_N}^3 corner sample per step",
                        "gamma": w.gamma, "cfl": w.cfl, "bc": "outflow (sample faces)"},
-            "cpu_baseline": {k: r[k] for k in ("value", "unit", "cores", "kind", "sample")},
+            "cpu_baseline": dict({k: r[k] for k in ("value", "unit", "cores", "kind", "sample")},
+                                 cpu_model=cpu_model(), nproc=host_cores(), build=ORACLE_FLAGS),
             "e2e": {"value": r["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line))
@@ -321,44 +371,73 @@ def main():
 
     N, K = main_res["cells"], args.steps
     value = world * N * K / main_res["seconds"]
-    # per-kernel rooflines: the slower of HBM (algorithmic bytes / measured copy bandwidth) and FP64 ALU
-    # (algorithmic flops / DFMA rate measured above); DESIGN.md section 6
+    # Rooflines as SURVEY.md section 8(d) defines them (paper_1410_4194_b200/roofline.py): the slower of the METHOD's
+    # bytes (80 B x ghost factor per cell-update) over the measured copy bandwidth and the FP64 arithmetic
+    # instructions (from the committed ncu capture) over the DFMA instruction rate measured in this run.
     kern = main_res["kernels"]
     hbm_gbs, hbm_src = rf.hbm_peak_gbs(ROOT)
     sm_mhz = (clocks or {}).get("sm_mhz") or 1965.0
-    per_kernel, t_roof_step = {}, 0.0
+    cap = rf.per_cell_counts(rf.load_capture(ROOT)) if default_method else {}
+    ghost = (args.size + 6) ** 3 / args.size ** 3
+    dfma_rate = peak_tf * 1e12 / 2.0                                    # FP64 instructions / s
+    method_bytes = rf.METHOD_BYTES_PER_CELL * ghost
+    capture_applies = default_method and args.size == 512 and bool(cap)
+    per_kernel, inst_step = {}, 0.0
     for k, v in kern.items():
-        if k not in rf.ALG_BYTES:
+        if k not in rf.DECOMPOSITION_BYTES:
             continue
         t = v["ms_avg"] * 1e-3
-        gbs = rf.ALG_BYTES[k] * N / t / 1e9
-        # the frozen flop counts belong to PPMC + exact; other method choices are charged bytes only
-        flops = rf.ALG_FLOPS[k] if default_method else 0.0
-        tfs = flops * N / t / 1e12
-        t_h, t_a = rf.ALG_BYTES[k] * N / (hbm_gbs * 1e9), flops * N / (peak_tf * 1e12)
-        t_roof_step += max(t_h, t_a) * v["launches_per_step"]
+        c = cap.get(k)
+        # bytes of the method this kernel touches: pass 1 reads u^n; the last kernel reads u^n and writes u^{n+1}
+        mb = method_bytes if k == "k_final3d" else 0.5 * method_bytes
+        t_h = mb * N / (hbm_gbs * 1e9)
+        t_a = c["inst"] * N / dfma_rate if c else 0.0
+        inst_step += (c["inst"] if c else 0.0) * v["launches_per_step"]
+        dec = rf.DECOMPOSITION_BYTES[k]
         per_kernel[k] = {"ms": v["ms_avg"], "bound": "hbm" if t_h >= t_a else "alu",
-                         "hbm_GBps": gbs, "hbm_frac": gbs / hbm_gbs, "fp64_TFLOPs": tfs, "fp64_frac": tfs / peak_tf,
-                         "roofline_ms": max(t_h, t_a) * 1e3, "frac": max(t_h, t_a) / t}
+                         "roofline_ms": max(t_h, t_a) * 1e3, "frac": max(t_h, t_a) / t,
+                         "method_bytes_per_cell": mb, "fp64_inst_per_cell": c["inst"] if c else None,
+                         "fp64_flops_per_cell": c["flops"] if c else None,
+                         "fp64_TFLOPs": c["flops"] * N / t / 1e12 if c else None,
+                         "fp64_pipe_inst_per_cell_incl_compares": c["fp64_pipe_inst"] if c else None,
+                         "ncu_sm__pipe_fp64_cycles_active_pct": c["pipe_pct"] if c else None,
+                         "ncu_ms": c["ncu_ms"] if c else None,
+                         "decomposition_bytes_per_cell": dec,
+                         "hbm_utilisation_of_decomposition": dec * N / t / 1e9 / hbm_gbs,
+                         "traffic": c["dram_bytes"] if (c and capture_applies) else None}
     top = max(per_kernel, key=lambda k: kern[k]["ms_avg"] * kern[k]["launches_per_step"])
     pk = per_kernel[top]
+    step_ms = main_res["seconds"] / K * 1e3
+    t_h_step, t_a_step = method_bytes * N / (hbm_gbs * 1e9), inst_step * N / dfma_rate
     if pk["bound"] == "hbm":
-        ach, peak, unit, psrc = pk["hbm_GBps"], hbm_gbs, "GB/s", hbm_src
+        ach, peak, unit, psrc = pk["method_bytes_per_cell"] * N / (pk["ms"] * 1e-3) / 1e9, hbm_gbs, "GB/s", hbm_src
     else:
-        ach, peak, unit = pk["fp64_TFLOPs"], peak_tf, "TFLOP/s"
+        # every FP64 instruction counted as one FMA slot (2 flop), exactly as the DFMA peak counts its own
+        ach, peak, unit = 2.0 * pk["fp64_inst_per_cell"] * N / (pk["ms"] * 1e-3) / 1e12, peak_tf, "TFLOP/s"
         psrc = ("measured: ch_fp64_peak_probe DFMA chains in this run (burst); nominal 148 SM x 64 lanes x 2 x "
                 f"{sm_mhz:.0f} MHz = {rf.nominal_fp64_tflops(sm_mhz):.1f}")
-    step_ms = main_res["seconds"] / K * 1e3
     roofline = {"bound": pk["bound"], "kernel": top, "achieved": ach, "peak": peak, "unit": unit,
-                "frac": ach / peak, "traffic": TRAFFIC_NCU.get(top) if default_method else None,
-                "traffic_note": "dram__bytes_read.sum + dram__bytes_write.sum per launch from profiles/ (ncu --set full, 512^3)",
+                "frac": ach / peak, "traffic": pk["traffic"],
+                "definition": "SURVEY.md 8(d): max(80 B x Np/N per cell-update / hbm_gbs, FP64 arithmetic instructions per "
+                              "cell-update / measured DFMA instruction rate) / measured kernel time; 'achieved' counts "
+                              "every FP64 instruction as one FMA slot (2 flop) as the DFMA peak does",
+                "capture": rf.CAPTURE if cap else None,
+                "capture_note": "per-cell instruction counts, DRAM traffic and pipe utilisation are read from this ncu "
+                                "--set full capture (512^3, kernels of this commit); traffic only when this run is the "
+                                "captured configuration",
                 "peak_source": psrc,
-                "alg_bytes_per_cell": rf.ALG_BYTES[top], "alg_flops_per_cell": rf.ALG_FLOPS[top],
                 "kernel_ms": kern[top]["ms_avg"],
                 "kernel_share_of_step": kern[top]["ms_avg"] * kern[top]["launches_per_step"] / main_res["kernel_ms_per_step"],
-                "fp64_peak_TFLOPs_measured": peak_tf, "hbm_peak_GBps": hbm_gbs,
-                "step": {"alg_bytes_per_cell": sum(rf.ALG_BYTES.values()), "alg_flops_per_cell": sum(rf.ALG_FLOPS.values()),
-                         "roofline_ms": t_roof_step * 1e3, "measured_ms": step_ms, "frac": t_roof_step * 1e3 / step_ms},
+                "fp64_peak_TFLOPs_measured": peak_tf, "fp64_inst_rate_measured": dfma_rate, "hbm_peak_GBps": hbm_gbs,
+                "ghost_factor": ghost,
+                "step": {"method_bytes_per_cell": method_bytes, "fp64_inst_per_cell": inst_step or None,
+                         "hbm_ms": t_h_step * 1e3, "fp64_ms": t_a_step * 1e3,
+                         "bound": "hbm" if t_h_step >= t_a_step else "alu",
+                         "roofline_ms": max(t_h_step, t_a_step) * 1e3, "measured_ms": step_ms,
+                         "frac": max(t_h_step, t_a_step) * 1e3 / step_ms,
+                         "decomposition_bytes_per_cell": sum(rf.DECOMPOSITION_BYTES[k] for k in per_kernel),
+                         "hbm_utilisation_of_decomposition":
+                             sum(rf.DECOMPOSITION_BYTES[k] for k in per_kernel) * N / (step_ms * 1e-3) / 1e9 / hbm_gbs},
                 "kernels": per_kernel, "kernel_times": kern}
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": args.warmup,
             "ms_per_step": main_res["seconds"] / K * 1e3, "higher_is_better": True, "scaling": "weak",
@@ -379,8 +458,11 @@ def main():
                        "h2d_bytes_per_step": e["h2d"], "d2h_bytes_per_step": e["d2h"], "steps": e["steps"],
                        "how": "ch_set_state(pinned host) + ch_compute_dt + ch_step + ch_get_state(pinned host) per step"}
     if world == 1 and not args.no_cpu_baseline:
-        r = time_oracle(w, steps=3, warmup=1)
-        line["cpu_baseline"] = {k: r[k] for k in ("value", "unit", "cores", "kind", "sample")}
+        legs = oracle_legs(w)
+        head = next(l for l in legs if l["leg"].startswith("all cores 128"))
+        line["cpu_baseline"] = {"value": head["value"], "unit": UNIT, "cores": head["cores"], "kind": "oracle",
+                                "sample": head["sample"], "cpu_model": cpu_model(), "nproc": host_cores(),
+                                "build": ORACLE_FLAGS, "legs": legs}
     print(json.dumps(line))
     if dist is not None:
         dist.destroy_process_group()

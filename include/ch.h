@@ -22,6 +22,8 @@
  *     ch_bind and stays owned by the caller.  It does own a few bytes of pinned HOST memory (the
  *     dt read-back cell) per context.
  *   - A context is not thread-safe; use one per host thread / stream.
+ *   - ch_bind records the device its buffers live on; every later call runs there whatever device is current
+ *     in the calling thread, and restores the caller's current device before returning.
  *   - There is no CPU fallback: every call that touches data launches CUDA work on the bound
  *     stream and returns CH_ECUDA if that fails.
  */
@@ -146,12 +148,26 @@ int ch_set_hcorrection(ch_ctx* ctx, int on);
 /* ch_set_reconstruction — select the reconstruction for later steps.  CH_EINVAL for an unknown code. */
 int ch_set_reconstruction(ch_ctx* ctx, int recon);
 
+/* ch_set_option — launch-configuration choices that change HOW a step is computed, never WHAT (every setting
+ * gives results within the one-step gate of every other; the tests compare them).  Defaults are what bench.py
+ * times.  Nothing here is read from the environment.
+ *   CH_OPT_MARCH_SEG  cells a thread of the marching pass-1 kernels sweeps (0 = chosen from the grid size; >= 4)
+ *   CH_OPT_FINAL_SEG  planes a CTA of the fused second half marches (0 = chosen from the grid size; >= 4)
+ *   CH_OPT_TMA        1 (default): the TMA-fed fused second half where the padded strides allow it; 0: plain loads
+ *   CH_OPT_UNFUSED    1: run the second half as k_pass2 + k_update on 3-D grids too (A/B measurements); default 0
+ * CH_EINVAL for an unknown option or an out-of-range value. */
+enum { CH_OPT_MARCH_SEG = 0, CH_OPT_FINAL_SEG = 1, CH_OPT_TMA = 2, CH_OPT_UNFUSED = 3 };
+int ch_set_option(ch_ctx* ctx, int option, int value);
+
 /* ch_step_cfl — one step whose size never visits the host: dt = cfl * min dx_d/(|v_d| + a) (Eq. 22, from the
  * reduction the previous step left on the device, or a fresh pass after ch_set_state), clipped to t_left when
  * 0 < t_left < dt, then the same kernels as ch_step read it from device memory and form dt/dx_d with the same
  * correctly rounded division.  Fully asynchronous: steps can be queued back to back without the 16-byte
  * read-back ch_compute_dt needs.  A sequence of ch_step_cfl calls gives bitwise the states the
- * ch_compute_dt + ch_step loop gives.  A non-physical cell makes dt NaN (visible through ch_last_dt).
+ * ch_compute_dt + ch_step loop gives.  A non-physical cell (rho <= 0 or non-finite) makes dt NaN and the step
+ * is REFUSED on the device: no kernel writes, the state, its reduction cells and ch_elapsed stay as they were, so
+ * ch_last_dt returns NaN + CH_ENONPHYS and ch_compute_dt reports CH_ENONPHYS, exactly as the ch_compute_dt +
+ * ch_step loop stops before touching the state.
  * CH_EINVAL if cfl is not in (0,1] or t_left is NaN; t_left <= 0 means "no clipping". */
 int ch_step_cfl(ch_ctx* ctx, double cfl, double t_left);
 
@@ -163,6 +179,13 @@ double ch_elapsed(ch_ctx* ctx);
 /* ch_sync — block until all work queued on the context's stream has finished. */
 int ch_sync(ch_ctx* ctx);
 
+/* ch_tiling — how the bound grid is cut into CTAs, for tests that place samples across tile seams: out[8] (HOST)
+ * = { interfaces per CTA of the x pass (over the flat run of padded cells), columns per CTA of the marching
+ * passes, interfaces per marching thread along y, along z, updated columns per tile of the fused second half
+ * along x, along y, planes per CTA of the fused second half, 1 if the TMA-fed form runs }.  Zeros where a kernel
+ * does not run on this grid.  Call after ch_bind. */
+int ch_tiling(const ch_ctx* ctx, int* out);
+
 /* ch_kernel_launches — number of kernels this context has launched since ch_init (for bench.py's
  * gpu_launches claim). */
 long long ch_kernel_launches(const ch_ctx* ctx);
@@ -172,6 +195,7 @@ enum {
   CH_K_RESET = 0, CH_K_PASS1_X, CH_K_PASS1_Y, CH_K_PASS1_Z, CH_K_PASS2, CH_K_UPDATE, CH_K_GHOST, CH_K_DT,
   CH_K_FINAL, /* fused pass 2 + update of 3-D grids */
   CH_K_ETA,   /* H correction: eta of every interface */
+  CH_K_PICK_DT, /* ch_step_cfl: Eq. 22 finished on the device */
   CH_K_COUNT
 };
 

@@ -27,9 +27,10 @@ CH_OK, CH_EINVAL, CH_ESTATE, CH_ECUDA, CH_ENONPHYS = 0, -1, -2, -3, -4
 # every symbol include/ch.h declares
 SYMBOLS = ("ch_init", "ch_free", "ch_last_error", "ch_set_spacing", "ch_padded_cells", "ch_workspace_bytes",
            "ch_bind", "ch_set_state", "ch_get_state", "ch_set_padded", "ch_get_padded", "ch_compute_dt",
-           "ch_step", "ch_step_cfl", "ch_last_dt", "ch_elapsed", "ch_set_solver", "ch_set_reconstruction", "ch_set_hcorrection", "ch_sync", "ch_kernel_launches", "ch_profile", "ch_profile_read", "ch_kernel_name",
+           "ch_step", "ch_step_cfl", "ch_last_dt", "ch_elapsed", "ch_set_solver", "ch_set_reconstruction", "ch_set_hcorrection", "ch_set_option", "ch_tiling", "ch_sync", "ch_kernel_launches", "ch_profile", "ch_profile_read", "ch_kernel_name",
            "ch_fp64_peak_probe")
-K_COUNT = 10
+K_COUNT = 11
+OPT_MARCH_SEG, OPT_FINAL_SEG, OPT_TMA, OPT_UNFUSED = 0, 1, 2, 3
 
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-shared"]
@@ -89,6 +90,8 @@ def load_library() -> C.CDLL:
     L.ch_set_solver.argtypes = [vp, C.c_int]
     L.ch_set_reconstruction.argtypes = [vp, C.c_int]
     L.ch_set_hcorrection.argtypes = [vp, C.c_int]
+    L.ch_set_option.argtypes = [vp, C.c_int, C.c_int]
+    L.ch_tiling.argtypes = [vp, C.POINTER(C.c_int)]
     L.ch_sync.argtypes = [vp]
     L.ch_kernel_launches.restype = C.c_longlong
     L.ch_kernel_launches.argtypes = [vp]
@@ -229,6 +232,18 @@ class Grid:
     def set_reconstruction(self, recon):
         """0 = PPMC (default), 1 = PLMC, 2 = PCM."""
         self._check(self._L.ch_set_reconstruction(self._h, int(recon)), "ch_set_reconstruction")
+
+    def set_option(self, option, value):
+        """Launch-configuration choice (OPT_MARCH_SEG, OPT_FINAL_SEG, OPT_TMA, OPT_UNFUSED); see ch_set_option."""
+        self._check(self._L.ch_set_option(self._h, int(option), int(value)), "ch_set_option")
+
+    def tiling(self) -> dict:
+        """How the grid is cut into CTAs (ch_tiling)."""
+        out = (C.c_int * 8)()
+        self._check(self._L.ch_tiling(self._h, out), "ch_tiling")
+        keys = ("x_interfaces_per_cta", "march_columns_per_cta", "march_seg_y", "march_seg_z", "final_tile_x",
+                "final_tile_y", "final_seg", "tma")
+        return dict(zip(keys, [int(v) for v in out]))
 
     def sync(self):
         self._check(self._L.ch_sync(self._h), "ch_sync")

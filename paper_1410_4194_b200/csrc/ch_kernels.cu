@@ -77,6 +77,11 @@ __device__ __forceinline__ double step_dtdx1(const StepArgs& A, int d) {   // on
   return A.dt_dev ? __ddiv_rn(*A.dt_dev, A.dx[d]) : A.dtdx[d];
 }
 
+// ch_step_cfl on a non-physical state: k_pick_dt leaves dt = NaN; every kernel of the step then returns at once,
+// so the last state and its reduction cells (rate, flag) survive and the failure stays visible (ch_last_dt,
+// ch_compute_dt) instead of turning the whole grid into NaN.
+__device__ __forceinline__ bool step_refused(const StepArgs& A) { return A.dt_dev && !(*A.dt_dev > 0.0); }
+
 // global component index of direction-local component m for a sweep along D (cyclic)
 template <int D>
 __device__ __forceinline__ constexpr int comp(int m) {
@@ -142,6 +147,7 @@ __device__ __forceinline__ void copy5(double dst[5], const double src[5]) {
 
 template <int D, int S, int R>
 __global__ void __launch_bounds__(CH_MARCH_T, CH_MARCH_MINB) k_pass1_march(const StepArgs A, int seg) {
+  if (step_refused(A)) return;
   constexpr int T = 3 - D;   // the other transverse dimension (x is the lane dimension)
   const Geom& g = A.geo;
   const Gas& G = A.gas;
@@ -225,6 +231,7 @@ __global__ void __launch_bounds__(kXT, CH_X_MINB) k_pass1_x(const StepArgs A, lo
   __shared__ double sP[5][kXT];
   __shared__ double sS[5][kXT];
   __shared__ double sL[5][kXT];
+  if (step_refused(A)) return;
   const Geom& g = A.geo;
   const double dtdx0 = step_dtdx1(A, 0);
   const Gas& G = A.gas;
@@ -326,6 +333,7 @@ __device__ __forceinline__ void corrected_prim(const Gas& G, const DirSel& S, lo
 // H correction, C1: eta = |(u_R + a_R) - (u_L + a_L)| / 2 at every interface c+1/2, c in [-1, n-1],
 // from the transverse-corrected states, over the transverse range [-1, n] that C2's stencil reaches.
 __global__ void __launch_bounds__(CH_P2_T) k_eta(const StepArgs A) {
+  if (step_refused(A)) return;
   const Geom& g = A.geo;
   double dtx[3];
   step_dtdx(A, dtx);
@@ -357,6 +365,7 @@ __global__ void __launch_bounds__(CH_P2_T) k_eta(const StepArgs A) {
 
 template <int SOLVER, bool HC>
 __global__ void __launch_bounds__(CH_P2_T, CH_P2_MINB) k_pass2(const StepArgs A) {
+  if (step_refused(A)) return;
   const Geom& g = A.geo;
   double dtx[3];
   step_dtdx(A, dtx);
@@ -474,13 +483,17 @@ __global__ void k_pick_dt(unsigned long long* red, double cfl, double t_left) {
   if (threadIdx.x != 0) return;
   double dt = __dmul_rn(cfl, __ddiv_rn(1.0, __longlong_as_double((long long)red[0])));
   if (t_left > 0.0 && dt > t_left) dt = t_left;
-  if (red[1] != 0ULL) dt = __longlong_as_double(0x7FF8000000000000LL);
   double* r = reinterpret_cast<double*>(red);
+  if (red[1] != 0ULL) {           // non-physical cell: dt = NaN refuses the step (step_refused); elapsed time untouched
+    r[2] = __longlong_as_double(0x7FF8000000000000LL);
+    return;
+  }
   r[2] = dt;
   r[3] += dt;
 }
 
-__global__ void __launch_bounds__(256) k_reset(unsigned long long* red) {
+__global__ void __launch_bounds__(256) k_reset(unsigned long long* red, const double* dt_dev) {
+  if (dt_dev && !(*dt_dev > 0.0)) return;      // a refused step keeps the reduction of the state it refused
   if (threadIdx.x == 0) { red[0] = 0ULL; red[1] = 0ULL; }
 }
 
@@ -504,6 +517,7 @@ __global__ void __launch_bounds__(256) k_dt(const StepArgs A) {
 
 // Eq. 24 on real cells, fused with the Eq. 22 reduction of the updated state.
 __global__ void __launch_bounds__(256) k_update(const StepArgs A) {
+  if (step_refused(A)) return;
   const Geom& g = A.geo;
   double dtx[3];
   step_dtdx(A, dtx);
@@ -604,6 +618,7 @@ __global__ void __launch_bounds__(kFT, CH_F_MINB) k_final3d(const StepArgs A, in
   Arr zF = reinterpret_cast<Arr>(s_final + 15 * kFT);   // carried: H^{n+1/2} on the low z face of cell k-1, z-local order
   Arr zP = reinterpret_cast<Arr>(s_final + 20 * kFT);   // carried: u + x and y flux differences of cell k-1, global order
   Arr zS = reinterpret_cast<Arr>(s_final + 25 * kFT);   // carried: F*_z of cell k-1 (global field order)
+  if (step_refused(A)) return;
   const Geom& g = A.geo;
   double dtx[3];
   step_dtdx(A, dtx);
@@ -798,6 +813,7 @@ __global__ void __launch_bounds__(kTT, 1) k_final3d_tma(const StepArgs A, const 
   // staging: array a (0..9) holds its 5 fields as [f][row][lane] = [f][tid]
   Arr sX = reinterpret_cast<Arr>(s_t + 50 * kTT);
   Arr sF = reinterpret_cast<Arr>(s_t + 55 * kTT);
+  if (step_refused(A)) return;
   const Geom& g = A.geo;
   double dtx[3];
   step_dtdx(A, dtx);
@@ -1074,6 +1090,7 @@ __device__ __forceinline__ int bc_source(int c, int n, int lo, int hi, bool& fli
 }
 
 __global__ void __launch_bounds__(256) k_ghost(const StepArgs A, const BcArgs B) {
+  if (step_refused(A)) return;
   const Geom& g = A.geo;
   // shell = z slabs (all padded x,y) + y slabs (real z, padded x) + x slabs (real z, real y)
   const long long nzs = (long long)2 * g.g[2] * g.pd[1] * g.pd[0];
@@ -1136,6 +1153,8 @@ struct ch_ctx {
   double dx[3];
   int bc[6];
   bool bound = false, have_state = false, dt_valid = false;
+  int device = -1;           // the device the bound buffers live on (ch_bind)
+  bool smem_attr[2][2] = {{false, false}, {false, false}};   // [tma form][solver]: dynamic shared memory limit raised on `device`
   double* state = nullptr;
   double* ws = nullptr;
   unsigned long long* red = nullptr;
@@ -1162,6 +1181,17 @@ struct ch_ctx {
 namespace {
 
 int fail(int code, const char* msg) { g_err = msg; return code; }
+
+// Every entry point that touches CUDA runs on the device the bound buffers live on (recorded by ch_bind), whatever
+// device is current in the calling thread, and restores the caller's device on return.
+struct DeviceGuard {
+  int prev = -1; bool switched = false;
+  explicit DeviceGuard(int dev) {
+    if (dev < 0) return;
+    if (cudaGetDevice(&prev) == cudaSuccess && prev != dev) switched = cudaSetDevice(dev) == cudaSuccess;
+  }
+  ~DeviceGuard() { if (switched) cudaSetDevice(prev); }
+};
 int cuda_fail(cudaError_t e, const char* where) {
   g_err = std::string(where) + ": " + cudaGetErrorString(e);
   return CH_ECUDA;
@@ -1203,7 +1233,7 @@ StepArgs make_args(const ch_ctx* c, double dt) {
 }
 
 const char* const kKernelNames[CH_K_COUNT] = {"k_reset", "k_pass1_x", "k_pass1_march<y>", "k_pass1_march<z>",
-                                              "k_pass2", "k_update", "k_ghost", "k_dt", "k_final3d", "k_eta"};
+                                              "k_pass2", "k_update", "k_ghost", "k_dt", "k_final3d", "k_eta", "k_pick_dt"};
 
 // event brackets around one launch when profiling is on (no-ops otherwise)
 struct Bracket {
@@ -1294,6 +1324,32 @@ bool build_tma_maps(ch_ctx* c) {
   return true;
 }
 
+// Interfaces a thread of the marching pass-1 kernel sweeps along d: enough segments to fill the chip on small grids
+// (a segment costs ~1.5 cells of warm-up), 64 on large ones; CH_OPT_MARCH_SEG overrides.
+int march_segment(const ch_ctx* c, int d) {
+  const Geom& g = c->geo;
+  if (c->march_seg) return c->march_seg;
+  const int T = 3 - d;
+  const long long cols = (long long)(g.act[0] ? g.n[0] + 2 : 1) * (g.act[T] ? g.n[T] + 2 : 1);
+  const long long want = cols * (g.n[d] + 1) / (148LL * 1024);
+  int seg = 4;
+  while (seg < 64 && seg * 2 <= want) seg *= 2;
+  return seg;
+}
+
+// Planes a CTA of the fused second half marches: at least four waves of CTAs on small grids (a segment costs two
+// light planes), 64 planes on large ones; CH_OPT_FINAL_SEG overrides.
+int final_segment(const ch_ctx* c) {
+  const Geom& g = c->geo;
+  if (c->final_seg) return c->final_seg;
+  const bool tma = c->tma_ok && c->use_tma;
+  const long long tiles = (long long)((g.n[0] + kFX - 3) / (kFX - 2)) * ((g.n[1] + (tma ? kTY : kFY) - 3) / ((tma ? kTY : kFY) - 2));
+  const long long want = tiles * g.n[2] / (148LL * 4);
+  int seg = 8;
+  while (seg < 64 && seg * 2 <= want) seg *= 2;
+  return seg;
+}
+
 }  // namespace
 
 extern "C" {
@@ -1310,10 +1366,6 @@ ch_ctx* ch_init(int nx, int ny, int nz, int nghost, double gamma, const int* bc)
   if (!c) { fail(CH_EINVAL, "ch_init: out of host memory"); return nullptr; }
   c->geo = g;
   c->nghost = nghost;
-  if (const char* e = std::getenv("CH_MARCH_SEG")) { const int v = std::atoi(e); if (v >= 4) c->march_seg = v; }   // tuning knob
-  if (const char* e = std::getenv("CH_UNFUSED")) c->unfused = std::atoi(e) != 0;
-  if (const char* e = std::getenv("CH_TMA")) c->use_tma = std::atoi(e) != 0;
-  if (const char* e = std::getenv("CH_FINAL_SEG")) { const int v = std::atoi(e); if (v >= 4) c->final_seg = v; }
   for (int s = 0; s < 6; ++s) {
     c->bc[s] = bc ? bc[s] : CH_BC_PERIODIC;
     if (g.act[s / 2] && (c->bc[s] < 1 || c->bc[s] > 3)) { delete c; fail(CH_EINVAL, "ch_init: bad boundary code"); return nullptr; }
@@ -1339,6 +1391,7 @@ ch_ctx* ch_init(int nx, int ny, int nz, int nghost, double gamma, const int* bc)
 
 int ch_free(ch_ctx* c) {
   if (!c) return CH_OK;
+  DeviceGuard guard(c->device);
   if (c->h_red) cudaFreeHost(c->h_red);
   for (int k = 0; k < 2 * CH_K_COUNT; ++k) if (c->ev[k]) cudaEventDestroy(c->ev[k]);
   delete c;
@@ -1369,6 +1422,16 @@ int ch_bind(ch_ctx* c, const ch_buffers* b, void* stream) {
     return fail(CH_EINVAL, "ch_bind: workspace too small");
   if (((uintptr_t)b->state & 7) || ((uintptr_t)b->workspace & 7) || ((uintptr_t)b->reduce & 7))
     return fail(CH_EINVAL, "ch_bind: misaligned buffer");
+  {
+    cudaPointerAttributes pa;
+    if (cudaPointerGetAttributes(&pa, b->state) != cudaSuccess || pa.type != cudaMemoryTypeDevice) {
+      cudaGetLastError();
+      return fail(CH_EINVAL, "ch_bind: state is not a device pointer");
+    }
+    if (pa.device != c->device) { c->smem_attr[0][0] = c->smem_attr[0][1] = c->smem_attr[1][0] = c->smem_attr[1][1] = false; }
+    c->device = pa.device;
+  }
+  DeviceGuard guard(c->device);
   c->state = b->state;
   c->ws = static_cast<double*>(b->workspace);
   c->red = static_cast<unsigned long long*>(b->reduce);
@@ -1383,6 +1446,7 @@ int ch_bind(ch_ctx* c, const ch_buffers* b, void* stream) {
 int ch_set_state(ch_ctx* c, const double* u) {
   if (!c || !u) return fail(CH_EINVAL, "ch_set_state: null argument");
   if (!c->bound) return fail(CH_ESTATE, "ch_set_state: no buffers bound");
+  DeviceGuard guard(c->device);
   int rc = copy_real(c, const_cast<double*>(u), true);
   if (rc) return rc;
   StepArgs A = make_args(c, 1.0);
@@ -1395,6 +1459,7 @@ int ch_set_state(ch_ctx* c, const double* u) {
 int ch_get_state(ch_ctx* c, double* u) {
   if (!c || !u) return fail(CH_EINVAL, "ch_get_state: null argument");
   if (!c->have_state) return fail(CH_ESTATE, "ch_get_state: no state set");
+  DeviceGuard guard(c->device);
   int rc = copy_real(c, u, false);
   if (rc) return rc;
   CH_CUDA(cudaStreamSynchronize(c->stream), "ch_get_state sync");
@@ -1404,6 +1469,7 @@ int ch_get_state(ch_ctx* c, double* u) {
 int ch_set_padded(ch_ctx* c, const double* up) {
   if (!c || !up) return fail(CH_EINVAL, "ch_set_padded: null argument");
   if (!c->bound) return fail(CH_ESTATE, "ch_set_padded: no buffers bound");
+  DeviceGuard guard(c->device);
   CH_CUDA(cudaMemcpyAsync(c->state, up, (size_t)5 * c->geo.np * 8, cudaMemcpyDefault, c->stream), "ch_set_padded");
   c->have_state = true; c->dt_valid = false;
   return CH_OK;
@@ -1412,6 +1478,7 @@ int ch_set_padded(ch_ctx* c, const double* up) {
 int ch_get_padded(ch_ctx* c, double* up) {
   if (!c || !up) return fail(CH_EINVAL, "ch_get_padded: null argument");
   if (!c->have_state) return fail(CH_ESTATE, "ch_get_padded: no state set");
+  DeviceGuard guard(c->device);
   CH_CUDA(cudaMemcpyAsync(up, c->state, (size_t)5 * c->geo.np * 8, cudaMemcpyDefault, c->stream), "ch_get_padded");
   CH_CUDA(cudaStreamSynchronize(c->stream), "ch_get_padded sync");
   return CH_OK;
@@ -1422,9 +1489,10 @@ double ch_compute_dt(ch_ctx* c, double cfl) {
   if (!c) { fail(CH_EINVAL, "ch_compute_dt: null context"); return nan; }
   if (!c->have_state) { fail(CH_ESTATE, "ch_compute_dt: no state set"); return nan; }
   if (!(cfl > 0.0) || !(cfl <= 1.0)) { fail(CH_EINVAL, "ch_compute_dt: cfl not in (0,1]"); return nan; }
+  DeviceGuard guard(c->device);
   if (!c->dt_valid) {
     StepArgs A = make_args(c, 1.0);
-    { Bracket b(c, CH_K_RESET); k_reset<<<1, 32, 0, c->stream>>>(c->red); }
+    { Bracket b(c, CH_K_RESET); k_reset<<<1, 32, 0, c->stream>>>(c->red, nullptr); }
     const long long N = (long long)c->geo.n[0] * c->geo.n[1] * c->geo.n[2];
     long long blocks = (N + 255) / 256;
     if (blocks > 148 * 8) blocks = 148 * 8;
@@ -1457,7 +1525,7 @@ int step_impl(ch_ctx* c, double dt, bool devdt) {
   StepArgs A = make_args(c, devdt ? 1.0 : dt);
   if (devdt) A.dt_dev = reinterpret_cast<const double*>(c->red) + 2;     // written by k_pick_dt just before
   cudaStream_t st = c->stream;
-  { Bracket b(c, CH_K_RESET); k_reset<<<1, 32, 0, st>>>(c->red); }
+  { Bracket b(c, CH_K_RESET); k_reset<<<1, 32, 0, st>>>(c->red, A.dt_dev); }
   // pass 1
   if (g.act[0]) {
     // flat run of padded cells from the first needed row to the last: rows j,k in [-1, n]
@@ -1474,12 +1542,7 @@ int step_impl(ch_ctx* c, double dt, bool devdt) {
     const int T = 3 - d;
     const long long cols = (long long)(g.act[0] ? g.n[0] + 2 : 1) * (g.act[T] ? g.n[T] + 2 : 1);
     // enough segments to fill the chip on small grids (a segment costs ~1.5 cells of warm-up), 64 on large ones
-    int seg = c->march_seg;
-    if (seg == 0) {
-      const long long want = cols * (g.n[d] + 1) / (148LL * 1024);
-      seg = 4;
-      while (seg < 64 && seg * 2 <= want) seg *= 2;
-    }
+    const int seg = march_segment(c, d);
     dim3 grid((unsigned)((cols + CH_MARCH_T - 1) / CH_MARCH_T), (unsigned)((g.n[d] + 2 * A.ext - 1 + seg - 1) / seg));
     Bracket b(c, d == 1 ? CH_K_PASS1_Y : CH_K_PASS1_Z);
     if (d == 1) k_pass1_march<1, S, R><<<grid, CH_MARCH_T, 0, st>>>(A, seg);
@@ -1488,22 +1551,14 @@ int step_impl(ch_ctx* c, double dt, bool devdt) {
   CH_CUDA(cudaGetLastError(), "pass 1");
   if (g.act[0] && g.act[1] && g.act[2] && !c->unfused && !c->hcorr) {
     // at least four waves of CTAs on small grids (a segment costs two light planes), 64 planes on large ones
-    int seg = c->final_seg;
-    if (seg == 0) {
-      const bool tma = c->tma_ok && c->use_tma;
-      const long long tiles = (long long)((g.n[0] + kFX - 3) / (kFX - 2)) * ((g.n[1] + (tma ? kTY : kFY) - 3) / ((tma ? kTY : kFY) - 2));
-      const long long want = tiles * g.n[2] / (148LL * 4);
-      seg = 8;
-      while (seg < 64 && seg * 2 <= want) seg *= 2;
-    }
+    const int seg = final_segment(c);
     dim3 grid((unsigned)((g.n[0] + kFX - 3) / (kFX - 2)), (unsigned)((g.n[1] + kFY - 3) / (kFY - 2)),
               (unsigned)((g.n[2] + seg - 1) / seg));
     if (c->tma_ok && c->use_tma) {
       const size_t tsmem = (size_t)60 * kTT * sizeof(double);
-      static bool tattr_set = false;
-      if (!tattr_set) {
+      if (!c->smem_attr[1][S]) {
         CH_CUDA(cudaFuncSetAttribute(k_final3d_tma<S>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tsmem), "k_final3d_tma smem attribute");
-        tattr_set = true;
+        c->smem_attr[1][S] = true;
       }
       dim3 tgrid((unsigned)((g.n[0] + kFX - 3) / (kFX - 2)), (unsigned)((g.n[1] + kTY - 3) / (kTY - 2)),
                  (unsigned)((g.n[2] + seg - 1) / seg));
@@ -1511,10 +1566,9 @@ int step_impl(ch_ctx* c, double dt, bool devdt) {
       k_final3d_tma<S><<<tgrid, kTT, tsmem, st>>>(A, c->maps, seg);
     } else {
     const size_t smem = (size_t)30 * kFT * sizeof(double);
-    static bool attr_set = false;
-    if (!attr_set) {
+    if (!c->smem_attr[0][S]) {
       CH_CUDA(cudaFuncSetAttribute(k_final3d<S>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem), "k_final3d smem attribute");
-      attr_set = true;
+      c->smem_attr[0][S] = true;
     }
     Bracket b(c, CH_K_FINAL);
     k_final3d<S><<<grid, kFT, smem, st>>>(A, seg);
@@ -1549,6 +1603,7 @@ int step_impl(ch_ctx* c, double dt, bool devdt) {
 extern "C" {
 
 static int step_dispatch(ch_ctx* c, double dt, bool devdt) {
+  DeviceGuard guard(c->device);
   const bool roe = c->solver == CH_SOLVER_ROE;
   if (c->hcorr && !roe) return fail(CH_ESTATE, "ch_step: the H correction goes with the Roe solver (ch_set_solver)");
   switch (c->recon) {
@@ -1568,16 +1623,17 @@ int ch_step_cfl(ch_ctx* c, double cfl, double t_left) {
   if (!c->have_state) return fail(CH_ESTATE, "ch_step_cfl: no state set");
   if (!(cfl > 0.0) || !(cfl <= 1.0)) return fail(CH_EINVAL, "ch_step_cfl: cfl not in (0,1]");
   if (t_left != t_left) return fail(CH_EINVAL, "ch_step_cfl: t_left is NaN");
+  DeviceGuard guard(c->device);
   if (!c->dt_valid) {
     StepArgs A = make_args(c, 1.0);
-    { Bracket b(c, CH_K_RESET); k_reset<<<1, 32, 0, c->stream>>>(c->red); }
+    { Bracket b(c, CH_K_RESET); k_reset<<<1, 32, 0, c->stream>>>(c->red, nullptr); }
     const long long N = (long long)c->geo.n[0] * c->geo.n[1] * c->geo.n[2];
     long long blocks = (N + 255) / 256;
     if (blocks > 148 * 8) blocks = 148 * 8;
     { Bracket b(c, CH_K_DT); k_dt<<<(unsigned)blocks, 256, 0, c->stream>>>(A); }
     c->dt_valid = true;
   }
-  { Bracket b(c, CH_K_RESET); k_pick_dt<<<1, 32, 0, c->stream>>>(c->red, cfl, t_left); }
+  { Bracket b(c, CH_K_PICK_DT); k_pick_dt<<<1, 32, 0, c->stream>>>(c->red, cfl, t_left); }
   CH_CUDA(cudaGetLastError(), "k_pick_dt");
   return step_dispatch(c, 0.0, true);
 }
@@ -1585,6 +1641,7 @@ int ch_step_cfl(ch_ctx* c, double cfl, double t_left) {
 double ch_last_dt(ch_ctx* c) {
   const double nan = std::numeric_limits<double>::quiet_NaN();
   if (!c || !c->bound) { fail(CH_ESTATE, "ch_last_dt: no buffers bound"); return nan; }
+  DeviceGuard guard(c->device);
   cudaError_t e = cudaMemcpyAsync(c->h_red, c->red + 2, 16, cudaMemcpyDeviceToHost, c->stream);
   if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
   if (e != cudaSuccess) { cuda_fail(e, "ch_last_dt read-back"); return nan; }
@@ -1597,6 +1654,7 @@ double ch_last_dt(ch_ctx* c) {
 double ch_elapsed(ch_ctx* c) {
   const double nan = std::numeric_limits<double>::quiet_NaN();
   if (!c || !c->bound) { fail(CH_ESTATE, "ch_elapsed: no buffers bound"); return nan; }
+  DeviceGuard guard(c->device);
   cudaError_t e = cudaMemcpyAsync(c->h_red, c->red + 2, 16, cudaMemcpyDeviceToHost, c->stream);
   if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
   if (e != cudaSuccess) { cuda_fail(e, "ch_elapsed read-back"); return nan; }
@@ -1620,6 +1678,37 @@ int ch_set_reconstruction(ch_ctx* c, int recon) {
   return CH_OK;
 }
 
+int ch_tiling(const ch_ctx* c, int* out) {
+  if (!c || !out) return fail(CH_EINVAL, "ch_tiling: null argument");
+  const Geom& g = c->geo;
+  const bool three_d = g.act[0] && g.act[1] && g.act[2];
+  const bool tma = three_d && c->tma_ok && c->use_tma && !c->unfused && !c->hcorr;
+  out[0] = kXOut;                          // interfaces per CTA of k_pass1_x (flat run of padded cells)
+  out[1] = CH_MARCH_T;                     // columns per CTA of the marching kernels
+  out[2] = march_segment(c, 1);            // interfaces a marching thread sweeps along y
+  out[3] = march_segment(c, 2);            // ... along z
+  out[4] = three_d ? kFX - 2 : 0;          // updated columns per tile of the fused second half along x
+  out[5] = three_d ? (tma ? kTY : kFY) - 2 : 0;   // ... along y
+  out[6] = three_d ? final_segment(c) : 0; // planes a CTA of the fused second half marches
+  out[7] = tma ? 1 : 0;
+  return CH_OK;
+}
+
+int ch_set_option(ch_ctx* c, int option, int value) {
+  if (!c) return fail(CH_EINVAL, "ch_set_option: null context");
+  switch (option) {
+    case CH_OPT_MARCH_SEG:
+      if (value != 0 && value < 4) return fail(CH_EINVAL, "ch_set_option: march segment < 4");
+      c->march_seg = value; return CH_OK;
+    case CH_OPT_FINAL_SEG:
+      if (value != 0 && value < 4) return fail(CH_EINVAL, "ch_set_option: final segment < 4");
+      c->final_seg = value; return CH_OK;
+    case CH_OPT_TMA: c->use_tma = value != 0; return CH_OK;
+    case CH_OPT_UNFUSED: c->unfused = value != 0; return CH_OK;
+    default: return fail(CH_EINVAL, "ch_set_option: unknown option");
+  }
+}
+
 int ch_set_solver(ch_ctx* c, int solver) {
   if (!c) return fail(CH_EINVAL, "ch_set_solver: null context");
   if (solver != CH_SOLVER_EXACT && solver != CH_SOLVER_ROE) return fail(CH_EINVAL, "ch_set_solver: unknown solver");
@@ -1629,6 +1718,7 @@ int ch_set_solver(ch_ctx* c, int solver) {
 
 int ch_sync(ch_ctx* c) {
   if (!c) return fail(CH_EINVAL, "ch_sync: null context");
+  DeviceGuard guard(c->device);
   CH_CUDA(cudaStreamSynchronize(c->stream), "ch_sync");
   return CH_OK;
 }
@@ -1637,6 +1727,7 @@ long long ch_kernel_launches(const ch_ctx* c) { return c ? c->launches : 0; }
 
 int ch_profile(ch_ctx* c, int enable) {
   if (!c) return fail(CH_EINVAL, "ch_profile: null context");
+  DeviceGuard guard(c->device);
   if (enable && !c->ev[0]) {
     for (int k = 0; k < 2 * CH_K_COUNT; ++k) CH_CUDA(cudaEventCreate(&c->ev[k]), "cudaEventCreate");
   }
@@ -1656,6 +1747,13 @@ const char* ch_kernel_name(int kind) { return (kind >= 0 && kind < CH_K_COUNT) ?
 double ch_fp64_peak_probe(double* sink, int blocks, int threads, int iters, void* stream) {
   if (!sink || blocks < 1 || threads < 1 || threads > 1024 || iters < 1) { fail(CH_EINVAL, "ch_fp64_peak_probe: bad argument"); return -1.0; }
   cudaStream_t st = static_cast<cudaStream_t>(stream);
+  int dev = -1;
+  {
+    cudaPointerAttributes pa;
+    if (cudaPointerGetAttributes(&pa, sink) == cudaSuccess && pa.type == cudaMemoryTypeDevice) dev = pa.device;
+    else cudaGetLastError();
+  }
+  DeviceGuard guard(dev);
   cudaEvent_t e0, e1;
   if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) { fail(CH_ECUDA, "event create"); return -1.0; }
   k_dfma_probe<<<blocks, threads, 0, st>>>(sink, iters);   // warm-up
