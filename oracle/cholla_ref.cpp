@@ -34,9 +34,9 @@ constexpr double P_GUESS_FLOOR = 1e-6;
 constexpr double NEWTON_TOL = 1e-8;     // P:L1095 "e.g. 1e-6"; reading S2: 1e-8
 constexpr int NEWTON_CAP = 20;          // reading S2
 
-enum { BC_PERIODIC = 1, BC_REFLECTIVE = 2, BC_OUTFLOW = 3 };
+enum { BC_PERIODIC = 1, BC_REFLECTIVE = 2, BC_OUTFLOW = 3, BC_NOH = 4 };   // 4: analytic inflow of the Noh test
 enum { SOLVER_EXACT = 0, SOLVER_ROE = 1 };   // the Riemann solver is selectable
-enum { RECON_PPMC = 0, RECON_PLMC = 1, RECON_PCM = 2 };   // so is the reconstruction
+enum { RECON_PPMC = 0, RECON_PLMC = 1, RECON_PCM = 2, RECON_PPMP = 3, RECON_PLMP = 4 };   // so is the reconstruction
 
 thread_local std::string g_err;
 
@@ -267,6 +267,155 @@ void pcm_cell(const double w[5][5], double WL[5], double WR[5], double WLs[5], d
 }
 
 // ---------------------------------------------------------------------------------------------
+// PPMP for one cell (A.4): parabolic reconstruction in the PRIMITIVE variables with contact
+// steepening, shock flattening, monotonisation and characteristic tracing in Colella & Woodward's form.
+// w[s] = primitive cell averages of cells i-3..i+3 (s = 0..6; cell i is w[3]), local order (rho, u_n, v, w, p).
+// Readings: G12 A38 requires OPPOSITE curvature on the two sides of a contact; G13 A41's rho_R uses
+// rho_{i+1}; G14 A48's third line assigns W_R; G15 A54's chi_L^p is the mirror image of chi_R^m; S19 the
+// order in which A43-A45 are evaluated when p_{i+2} = p_{i-2}.
+// ---------------------------------------------------------------------------------------------
+// A2-A4 per primitive variable.
+void prim_limited_slope(const double wm[5], const double w0[5], const double wp[5], double dw[5]) {
+  for (int m = 0; m < 5; ++m) dw[m] = limit(w0[m] - wm[m], wp[m] - w0[m], 0.5 * (wp[m] - wm[m]));
+}
+
+// A42-A45: the flattening coefficient F~_j of cell j from p_{j-2..j+2} and u_{j-1}, u_{j+1}.
+// A44 / A45 are tested first, so the quotient A42 is only formed where its numerator does not vanish (S19).
+double flatten_tilde(const double pm2, const double pm1, const double pp1, const double pp2, const double um1,
+                     const double up1) {
+  if (std::fabs(pp1 - pm1) / std::min(pp1, pm1) < 1.0 / 3.0) return 0.0;   // A44
+  if (up1 - um1 > 0.0) return 0.0;                                         // A45
+  const double S = (pp1 - pm1) / (pp2 - pm2);                              // A42
+  return std::max(0.0, std::min(1.0, 10.0 * (S - 0.75)));                  // A43
+}
+
+void ppmp_cell(double gamma, double dtdx, const double w[7][5], double WL[5], double WR[5], double WLs[5],
+               double WRs[5]) {
+  const double* wim = w[2];
+  const double* wi = w[3];
+  const double* wip = w[4];
+  double dwm[5], dw0[5], dwp[5];
+  prim_limited_slope(w[1], w[2], w[3], dwm);   // cell i-1
+  prim_limited_slope(w[2], w[3], w[4], dw0);   // cell i
+  prim_limited_slope(w[3], w[4], w[5], dwp);   // cell i+1
+  // A34
+  double L[5], R[5];
+  for (int m = 0; m < 5; ++m) {
+    L[m] = 0.5 * (wi[m] + wim[m]) - (dw0[m] - dwm[m]) / 6.0;
+    R[m] = 0.5 * (wip[m] + wi[m]) - (dwp[m] - dw0[m]) / 6.0;
+  }
+  // A.4.2 contact steepening of the density faces
+  {
+    const double rm = wim[0], rp = wip[0], pm = wim[4], pp = wip[4];
+    const double jump = std::fabs(rp - rm) / std::min(rp, rm);
+    if (jump > 0.01 &&                                                         // A35
+        std::fabs(pp - pm) / std::min(pp, pm) < 0.1 * gamma * jump) {          // A36
+      // A37 with dx = 1 (dx^2 cancels in A39)
+      const double d2m = (w[3][0] - 2.0 * w[2][0] + w[1][0]) / 6.0;            // delta^2 rho_{i-1}
+      const double d2p = (w[5][0] - 2.0 * w[4][0] + w[3][0]) / 6.0;            // delta^2 rho_{i+1}
+      if (d2m * d2p < 0.0) {                                                   // A38, reading G12
+        const double eta_t = -(d2p - d2m) / (rp - rm);                         // A39
+        const double eta = std::max(0.0, std::min(20.0 * eta_t - 1.0, 1.0));   // A40
+        L[0] = L[0] * (1.0 - eta) + (rm + 0.5 * dwm[0]) * eta;                 // A41
+        R[0] = R[0] * (1.0 - eta) + (rp - 0.5 * dwp[0]) * eta;                 // A41, reading G13
+      }
+    }
+  }
+  // A.4.3 shock flattening: F~ of cells i-1, i, i+1 along the sweep (normal velocity)
+  {
+    const double Fm = flatten_tilde(w[0][4], w[1][4], w[3][4], w[4][4], w[1][1], w[3][1]);   // cell i-1
+    const double F0 = flatten_tilde(w[1][4], w[2][4], w[4][4], w[5][4], w[2][1], w[4][1]);   // cell i
+    const double Fp = flatten_tilde(w[2][4], w[3][4], w[5][4], w[6][4], w[3][1], w[5][1]);   // cell i+1
+    const double F = (wip[4] - wim[4] < 0.0) ? std::max(F0, Fp) : std::max(F0, Fm);          // A46
+    for (int m = 0; m < 5; ++m) {                                                            // A47
+      L[m] = F * wi[m] + (1.0 - F) * L[m];
+      R[m] = F * wi[m] + (1.0 - F) * R[m];
+    }
+  }
+  // A.4.4 monotonicity, A48 = A21 + A22 (third line read as W_R, G14; tests on the pair after A21, G8)
+  double dwi[5], w6[5];
+  for (int m = 0; m < 5; ++m) {
+    double l = L[m], r = R[m];
+    if ((r - wi[m]) * (wi[m] - l) <= 0.0) { l = wi[m]; r = wi[m]; }
+    const bool fixL = (r - l) * (l - (3.0 * wi[m] - 2.0 * r)) < 0.0;
+    const bool fixR = (r - l) * ((3.0 * wi[m] - 2.0 * l) - r) < 0.0;
+    const double l0 = l, r0 = r;
+    if (fixL) l = 3.0 * wi[m] - 2.0 * r0;
+    if (fixR) r = 3.0 * wi[m] - 2.0 * l0;
+    WL[m] = l; WR[m] = r;
+    dwi[m] = r - l;                              // A50
+    w6[m] = 6.0 * (wi[m] - 0.5 * (l + r));
+  }
+  // A49, A51
+  const double a = std::sqrt(gamma * wi[4] / wi[0]);
+  const double lm = wi[1] - a, l0c = wi[1], lp = wi[1] + a;
+  const double am = dtdx * std::min(lm, 0.0), bm = dtdx * std::max(lm, 0.0);
+  const double a0 = dtdx * std::min(l0c, 0.0), b0 = dtdx * std::max(l0c, 0.0);
+  const double ap = dtdx * std::min(lp, 0.0), bp = dtdx * std::max(lp, 0.0);
+  // A52
+  double WLm[5], WL0[5], WLp[5], WRm[5], WR0[5], WRp[5];
+  for (int m = 0; m < 5; ++m) {
+    WLm[m] = WL[m] - 0.5 * am * (dwi[m] + w6[m] * (1.0 + (2.0 / 3.0) * am));
+    WL0[m] = WL[m] - 0.5 * a0 * (dwi[m] + w6[m] * (1.0 + (2.0 / 3.0) * a0));
+    WLp[m] = WL[m] - 0.5 * ap * (dwi[m] + w6[m] * (1.0 + (2.0 / 3.0) * ap));
+    WRm[m] = WR[m] - 0.5 * bm * (dwi[m] - w6[m] * (1.0 - (2.0 / 3.0) * bm));
+    WR0[m] = WR[m] - 0.5 * b0 * (dwi[m] - w6[m] * (1.0 - (2.0 / 3.0) * b0));
+    WRp[m] = WR[m] - 0.5 * bp * (dwi[m] - w6[m] * (1.0 - (2.0 / 3.0) * bp));
+  }
+  // A53: sound speeds of the reference states; C = rho a of the reference state
+  const double aL = std::sqrt(gamma * WLm[4] / WLm[0]), aR = std::sqrt(gamma * WRp[4] / WRp[0]);
+  const double CL = WLm[0] * aL, CR = WRp[0] * aR;
+  // A54, chi_L^p read as the mirror image of chi_R^m (G15); A55
+  double chiLp = -1.0 / (2.0 * CL) * ((WLm[1] - WLp[1]) - (WLp[4] - WLm[4]) / CL);
+  double chiRm = 1.0 / (2.0 * CR) * ((WRp[1] - WRm[1]) - (WRp[4] - WRm[4]) / CR);
+  double chiL0 = (WLm[4] - WL0[4]) / (CL * CL) + 1.0 / WLm[0] - 1.0 / WL0[0];
+  double chiR0 = (WRp[4] - WR0[4]) / (CR * CR) + 1.0 / WRp[0] - 1.0 / WR0[0];
+  if (l0c > 0.0) chiL0 = 0.0;
+  if (lp > 0.0) chiLp = 0.0;
+  if (lm < 0.0) chiRm = 0.0;
+  if (l0c < 0.0) chiR0 = 0.0;
+  // A56
+  WLs[0] = 1.0 / (1.0 / WLm[0] - chiL0 - chiLp);
+  WRs[0] = 1.0 / (1.0 / WRp[0] - chiRm - chiR0);
+  WLs[1] = WLm[1] + CL * chiLp;
+  WRs[1] = WRp[1] - CR * chiRm;
+  WLs[4] = WLm[4] + (CL * CL) * chiLp;
+  WRs[4] = WRp[4] + (CR * CR) * chiRm;
+  WLs[2] = WL0[2]; WRs[2] = WR0[2];
+  WLs[3] = WL0[3]; WRs[3] = WR0[3];
+}
+
+// ---------------------------------------------------------------------------------------------
+// PLMP for one cell (A.1): linear reconstruction with the slope limited in the primitive variables
+// (A1-A4), evolved half a step with the fluxes of its own two face states in conserved form (A6, A7; Eq. 11).
+// Uses cells i-1, i, i+1 of the 7-cell argument (w[2..4]).  WLs, WRs come back PRIMITIVE like the others.
+// ---------------------------------------------------------------------------------------------
+void euler_flux_local(double gamma, const double wv[5], double U[5], double F[5]) {   // Eq. 9, 11 in local order
+  prim_to_cons(gamma, wv, U);
+  F[0] = U[1];
+  F[1] = U[1] * wv[1] + wv[4];
+  F[2] = U[1] * wv[2];
+  F[3] = U[1] * wv[3];
+  F[4] = (U[4] + wv[4]) * wv[1];
+}
+
+void plmp_cell(double gamma, double dtdx, const double w[7][5], double WL[5], double WR[5], double WLs[5],
+               double WRs[5]) {
+  double dw[5];
+  prim_limited_slope(w[2], w[3], w[4], dw);
+  for (int m = 0; m < 5; ++m) { WL[m] = w[3][m] - 0.5 * dw[m]; WR[m] = w[3][m] + 0.5 * dw[m]; }   // A1
+  double UL[5], UR[5], FL[5], FR[5], ULs[5], URs[5];
+  euler_flux_local(gamma, WL, UL, FL);
+  euler_flux_local(gamma, WR, UR, FR);
+  for (int m = 0; m < 5; ++m) {
+    ULs[m] = UL[m] + 0.5 * dtdx * (FL[m] - FR[m]);   // A6
+    URs[m] = UR[m] + 0.5 * dtdx * (FL[m] - FR[m]);   // A7
+  }
+  cons_to_prim(gamma, ULs, WLs);
+  cons_to_prim(gamma, URs, WRs);
+}
+
+// ---------------------------------------------------------------------------------------------
 // Exact Riemann solver (B.1).  Inputs: primitive L/R states in local order
 // (rho, u_n, v_t1, v_t2, p).  Output: flux in local order (B22) and diagnostics.
 // ---------------------------------------------------------------------------------------------
@@ -491,6 +640,8 @@ struct Ctx {
   int solver = SOLVER_EXACT;
   int recon = RECON_PPMC;
   bool hcorr = false;   // H correction (Appendix C): Roe solver only, second Riemann pass only, needs g >= 4
+  double time = 0.0;    // sum of the dt of all steps since set_state / ref_set_time: the t of the Noh boundary
+  double noh_rho0 = 1.0, noh_p0 = 1e-6;
   std::vector<double> u;  // [5][np], x fastest
   inline long idx(int i, int j, int k) const {  // real-cell coordinates, ghosts negative / >= n
     return ((long)(k + gd[2]) * pd[1] + (j + gd[1])) * pd[0] + (i + gd[0]);
@@ -519,6 +670,34 @@ void ghost_fill(Ctx& c) {
         } else {
           gi = n - 1 + l;
           si = bc == BC_PERIODIC ? l - 1 : bc == BC_REFLECTIVE ? n - l : n - 1;
+        }
+        if (bc == BC_NOH) {
+          // Analytic boundary of the Noh test: rho = rho0 (1 + t/r)^(n-1), |V| = 1 toward the
+          // origin, E = p0/(gamma-1) + rho/2, at the centre of the ghost cell; box origin at x = y = z = 0,
+          // n = number of active dimensions, r over the active dimensions.
+          int nact = 0;
+          for (int e = 0; e < 3; ++e) nact += c.active[e] ? 1 : 0;
+          int a[3];
+          for (a[2] = lo[2]; a[2] < hi[2]; ++a[2])
+            for (a[1] = lo[1]; a[1] < hi[1]; ++a[1])
+              for (a[0] = lo[0]; a[0] < hi[0]; ++a[0]) {
+                int gq[3] = {a[0], a[1], a[2]};
+                gq[d] = gi;
+                double x[3], r2 = 0.0;
+                for (int e = 0; e < 3; ++e) {
+                  x[e] = c.active[e] ? (gq[e] + 0.5) * c.dx[e] : 0.0;
+                  r2 += x[e] * x[e];
+                }
+                const double r = std::sqrt(r2);
+                const double q1 = 1.0 + c.time / r;
+                double rho = c.noh_rho0;
+                for (int e = 1; e < nact; ++e) rho *= q1;
+                const long ig = c.idx(gq[0], gq[1], gq[2]);
+                c.u[0 * c.np + ig] = rho;
+                for (int e = 0; e < 3; ++e) c.u[(1 + e) * c.np + ig] = rho * (-(x[e] / r));
+                c.u[4 * c.np + ig] = c.noh_p0 / (c.gamma - 1.0) + 0.5 * rho;
+              }
+          continue;
         }
         int a[3];
         for (a[2] = lo[2]; a[2] < hi[2]; ++a[2])
@@ -603,15 +782,29 @@ void ctu_step(Ctx& c, double dt) {
       for (int j = lo[1]; j < hi[1]; ++j)
         for (int i = lo[0]; i < hi[0]; ++i) {
           const long q = c.idx(i, j, k);
-          double ws[5][5];
+          double ws[5][5], w7[7][5];
           for (int s = 0; s < 5; ++s) {
             const long qs = q + (s - 2) * stride[d];
             double wg[5];
             for (int f = 0; f < 5; ++f) wg[f] = w[f * np + qs];
             to_local(d, wg, ws[s]);
           }
+          const bool wide = c.recon == RECON_PPMP || c.recon == RECON_PLMP;   // 7-cell stencil: g >= 4
+          if (wide)
+            for (int s = 0; s < 7; ++s) {
+              if (c.recon == RECON_PLMP && (s < 2 || s > 4)) {   // PLMP reads cells i-1..i+1 only (g = 3 suffices)
+                for (int f = 0; f < 5; ++f) w7[s][f] = 0.0;
+                continue;
+              }
+              const long qs = q + (s - 3) * stride[d];
+              double wg[5];
+              for (int f = 0; f < 5; ++f) wg[f] = w[f * np + qs];
+              to_local(d, wg, w7[s]);
+            }
           double WL[5], WR[5], WLs[5], WRs[5], gl[5], gr[5], ul[5], ur[5];
-          if (c.recon == RECON_PLMC) plmc_cell(gamma, dtdx, ws, WL, WR, WLs, WRs);
+          if (c.recon == RECON_PPMP) ppmp_cell(gamma, dtdx, w7, WL, WR, WLs, WRs);
+          else if (c.recon == RECON_PLMP) plmp_cell(gamma, dtdx, w7, WL, WR, WLs, WRs);
+          else if (c.recon == RECON_PLMC) plmc_cell(gamma, dtdx, ws, WL, WR, WLs, WRs);
           else if (c.recon == RECON_PCM) pcm_cell(ws, WL, WR, WLs, WRs);
           else ppmc_cell(gamma, dtdx, ws, WL, WR, WLs, WRs);
           to_global(d, WLs, gl);
@@ -731,6 +924,7 @@ void ctu_step(Ctx& c, double dt) {
           c.u[f * np + q] = v;
         }
       }
+  c.time += dt;   // the analytic (Noh) boundary is evaluated at t^{n+1}
   ghost_fill(c);  // O7
 }
 
@@ -763,7 +957,7 @@ void* ref_init(int nx, int ny, int nz, int nghost, double gamma, const int* bc) 
   }
   for (int s = 0; s < 6; ++s) {
     c->bc[s] = bc ? bc[s] : BC_PERIODIC;
-    if (c->active[s / 2] && (c->bc[s] < 1 || c->bc[s] > 3)) { delete c; fail("bad bc"); return nullptr; }
+    if (c->active[s / 2] && (c->bc[s] < 1 || c->bc[s] > 4)) { delete c; fail("bad bc"); return nullptr; }
   }
   for (int d = 0; d < 3; ++d)
     if (c->active[d] && ((c->bc[2 * d] == BC_PERIODIC) != (c->bc[2 * d + 1] == BC_PERIODIC))) {
@@ -794,10 +988,23 @@ int ref_set_state(void* h, const double* u) {
       for (int j = 0; j < c->n[1]; ++j)
         for (int i = 0; i < c->n[0]; ++i)
           c->u[f * c->np + c->idx(i, j, k)] = u[f * n + ((long)k * c->n[1] + j) * c->n[0] + i];
+  c->time = 0.0;
   ghost_fill(*c);
   c->have_state = true;
   return 0;
 }
+
+// Noh test boundary: ambient density and pressure of the analytic inflow; ref_set_time sets the t it
+// is evaluated at (set_state resets it to 0, every step adds its dt).
+int ref_set_noh(void* h, double rho0, double p0) {
+  Ctx* c = static_cast<Ctx*>(h);
+  if (!(rho0 > 0.0) || !(p0 > 0.0)) return fail("ref_set_noh: rho0, p0 must be positive");
+  c->noh_rho0 = rho0; c->noh_p0 = p0;
+  return 0;
+}
+int ref_set_time(void* h, double t) { static_cast<Ctx*>(h)->time = t; return 0; }
+double ref_get_time(void* h) { return static_cast<Ctx*>(h)->time; }
+int ref_fill_ghosts(void* h) { ghost_fill(*static_cast<Ctx*>(h)); return 0; }
 
 int ref_get_state(void* h, double* u) {
   Ctx* c = static_cast<Ctx*>(h);
@@ -861,9 +1068,22 @@ int ref_set_solver(void* h, int solver) {
   return 0;
 }
 int ref_set_reconstruction(void* h, int recon) {
-  if (!h || recon < RECON_PPMC || recon > RECON_PCM) return fail("ref_set_reconstruction: bad argument");
+  if (!h || recon < RECON_PPMC || recon > RECON_PLMP) return fail("ref_set_reconstruction: bad argument");
+  if (recon == RECON_PPMP && static_cast<Ctx*>(h)->g < 4) return fail("ref_set_reconstruction: PPMP needs nghost >= 4 (P:L962)");
+  if (recon == RECON_PPMP && static_cast<Ctx*>(h)->hcorr) return fail("ref_set_reconstruction: the H correction goes with PPMC or lower order (P:L565)");
   static_cast<Ctx*>(h)->recon = recon;
   return 0;
+}
+// w = [7 cells][5 comps] (cells i-3..i+3); out = [4][5] = WL, WR, W*_L, W*_R
+void ref_ppmp_cell(double gamma, double dtdx, const double* w, double* out) {
+  double ws[7][5];
+  std::memcpy(ws, w, sizeof(ws));
+  ppmp_cell(gamma, dtdx, ws, out, out + 5, out + 10, out + 15);
+}
+void ref_plmp_cell(double gamma, double dtdx, const double* w, double* out) {
+  double ws[7][5];
+  std::memcpy(ws, w, sizeof(ws));
+  plmp_cell(gamma, dtdx, ws, out, out + 5, out + 10, out + 15);
 }
 void ref_plmc_cell(double gamma, double dtdx, const double* w, double* out) {
   double ws[5][5];
@@ -874,6 +1094,7 @@ int ref_set_hcorrection(void* h, int on) {
   if (!h) return fail("ref_set_hcorrection: null");
   Ctx& c = *static_cast<Ctx*>(h);
   if (on && c.g < 4) return fail("ref_set_hcorrection: needs nghost >= 4 (P:L1291)");
+  if (on && c.recon == RECON_PPMP) return fail("ref_set_hcorrection: only with PPMC or lower-order reconstructions (P:L565)");
   c.hcorr = on != 0;
   return 0;
 }

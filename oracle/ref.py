@@ -15,7 +15,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "cholla_ref.cpp")
 _LIB = os.path.join(_HERE, "libcholla_ref.so")
 
-PERIODIC, REFLECTIVE, OUTFLOW = 1, 2, 3
+PERIODIC, REFLECTIVE, OUTFLOW, NOH = 1, 2, 3, 4
+PPMC, PLMC, PCM, PPMP, PLMP = 0, 1, 2, 3, 4
 
 
 def build(force: bool = False) -> str:
@@ -63,6 +64,13 @@ def lib() -> C.CDLL:
         L.ref_riemann_roe_eta.argtypes = [C.c_double, dp, dp, C.c_double, dp]
         L.ref_riemann_roe_eta.restype = C.c_int
         L.ref_plmc_cell.argtypes = [C.c_double, C.c_double, dp, dp]
+        L.ref_ppmp_cell.argtypes = [C.c_double, C.c_double, dp, dp]
+        L.ref_plmp_cell.argtypes = [C.c_double, C.c_double, dp, dp]
+        L.ref_set_noh.argtypes = [C.c_void_p, C.c_double, C.c_double]
+        L.ref_set_time.argtypes = [C.c_void_p, C.c_double]
+        L.ref_get_time.argtypes = [C.c_void_p]
+        L.ref_get_time.restype = C.c_double
+        L.ref_fill_ghosts.argtypes = [C.c_void_p]
         _lib = L
     return _lib
 
@@ -133,9 +141,23 @@ class RefGrid:
             raise ValueError("ref_set_hcorrection: " + lib().ref_last_error().decode())
 
     def set_reconstruction(self, recon):
-        """0 = PPMC (default), 1 = PLMC, 2 = PCM (P:L336)."""
+        """0 = PPMC (default), 1 = PLMC, 2 = PCM, 3 = PPMP (nghost >= 4), 4 = PLMP (P:L336)."""
         if lib().ref_set_reconstruction(self._h, int(recon)) != 0:
             raise ValueError("ref_set_reconstruction: " + lib().ref_last_error().decode())
+
+    def set_noh(self, rho0=1.0, p0=1e-6):
+        """Ambient state of the analytic Noh boundary (faces with bc code NOH)."""
+        if lib().ref_set_noh(self._h, rho0, p0) != 0:
+            raise ValueError("ref_set_noh: " + lib().ref_last_error().decode())
+
+    def set_time(self, t):
+        lib().ref_set_time(self._h, float(t))
+
+    def get_time(self) -> float:
+        return float(lib().ref_get_time(self._h))
+
+    def fill_ghosts(self):
+        lib().ref_fill_ghosts(self._h)
 
     def step(self, dt):
         if lib().ref_step(self._h, dt) != 0:
@@ -178,6 +200,22 @@ def ppmc_cell(gamma, dtdx, w):
     w = _arr(w); assert w.shape == (5, 5)
     out = np.empty((4, 5))
     lib().ref_ppmc_cell(gamma, dtdx, _p(w), _p(out))
+    return out[0], out[1], out[2], out[3]
+
+
+def ppmp_cell(gamma, dtdx, w):
+    """w[7 cells i-3..i+3][5 comps] -> (WL, WR, WLstar, WRstar), A.4."""
+    w = _arr(w); assert w.shape == (7, 5)
+    out = np.empty((4, 5))
+    lib().ref_ppmp_cell(gamma, dtdx, _p(w), _p(out))
+    return out[0], out[1], out[2], out[3]
+
+
+def plmp_cell(gamma, dtdx, w):
+    """w[7 cells][5 comps] (only i-1..i+1 are read) -> (WL, WR, WLstar, WRstar), A.1."""
+    w = _arr(w); assert w.shape == (7, 5)
+    out = np.empty((4, 5))
+    lib().ref_plmp_cell(gamma, dtdx, _p(w), _p(out))
     return out[0], out[1], out[2], out[3]
 
 

@@ -14,7 +14,7 @@ from dataclasses import dataclass, field
 
 import numpy as np
 
-PERIODIC, REFLECTIVE, OUTFLOW = 1, 2, 3
+PERIODIC, REFLECTIVE, OUTFLOW, NOH = 1, 2, 3, 4      # 4: the analytic inflow boundary of the Noh test
 
 
 @dataclass
@@ -69,6 +69,28 @@ def sod(nx=128, axis=0, n_other=1) -> Workload:
     zero = np.zeros(shape)
     bc = (OUTFLOW,) * 6 if n_other == 1 else tuple(OUTFLOW if d == axis else PERIODIC for d in range(3) for _ in range(2))
     return Workload("sod", conserved(rho, zero, zero, zero, p, gamma), gamma, bc, 0.4, t_end=0.2)
+
+
+# ---- Noh's strong shock (section 4.3.1; the consumer of the custom boundary and the H correction) ----
+def noh(n=64, dims=3, t_end=2.0, shape=None, rho0=1.0, p0=1e-6, cfl=0.4) -> Workload:
+    """Octant [0,1]^dims: rho = rho0, p = p0, unit velocity toward the origin; reflecting inner faces, analytic
+    (NOH) outer faces; gamma = 5/3.  `shape` overrides (n, dims) with an explicit (nx, ny, nz); dimensions of
+    size 1 are inactive."""
+    gamma = 5.0 / 3.0
+    if shape is None:
+        shape = tuple(n if d < dims else 1 for d in range(3))
+    nx, ny, nz = shape
+    x, y, z = centres(nx, ny, nz)
+    x = x if nx > 1 else np.zeros((1, 1, 1))
+    y = y if ny > 1 else np.zeros((1, 1, 1))
+    z = z if nz > 1 else np.zeros((1, 1, 1))
+    X, Y, Z = np.broadcast_arrays(x, y, z)
+    X, Y, Z = (np.broadcast_to(a, (nz, ny, nx)) for a in (X, Y, Z))
+    r = np.sqrt(X * X + Y * Y + Z * Z)
+    rho = np.full((nz, ny, nx), rho0)
+    u = conserved(rho, -X / r, -Y / r, -Z / r, np.full((nz, ny, nx), p0), gamma)
+    bc = (REFLECTIVE, NOH) * 3
+    return Workload("noh", u, gamma, bc, cfl, t_end=t_end, meta={"rho0": rho0, "p0": p0})
 
 
 # ---- config 2: Kelvin-Helmholtz (stands for P:L535-541) --------------------------------------
