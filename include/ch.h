@@ -47,7 +47,13 @@ enum {
 };
 
 /* Boundary-condition codes per face: any mix per face, periodic faces must be paired. */
-enum { CH_BC_PERIODIC = 1, CH_BC_REFLECTIVE = 2, CH_BC_OUTFLOW = 3 };
+enum {
+  CH_BC_PERIODIC = 1, CH_BC_REFLECTIVE = 2, CH_BC_OUTFLOW = 3,
+  CH_BC_NOH = 4 /* custom (analytic) boundary, "custom boundaries": the inflow of the Noh strong-shock test,
+                   P:L549-557: rho = rho0 (1 + t/r)^(n-1), unit velocity toward the origin of the box,
+                   E = p0/(gamma-1) + rho/2 at the centre of every ghost cell behind the face, n = number of active
+                   dimensions, t = ch_get_time (the state AFTER a step is filled at t^{n+1}); see ch_set_noh */
+};
 
 /* Device buffers handed to ch_bind.  All pointers are DEVICE pointers owned by the caller and must
  * stay valid until ch_free or the next ch_bind. */
@@ -62,7 +68,7 @@ typedef struct ch_buffers {
  * side of every active dimension, ratio of specific heats `gamma` (Eq. 8), and boundary
  * codes bc[6] = {x-,x+,y-,y+,z-,z+} (host pointer; NULL = all periodic).  Host-only: makes no CUDA
  * call.  Returns NULL on error (n < 1; nghost < 3 — PPMC inside six-solve CTU needs 3; gamma <= 1;
- * a bc code outside 1..3 on an active dimension; unpaired periodic faces; an active dimension
+ * a bc code outside 1..4 on an active dimension; unpaired periodic faces; an active dimension
  * smaller than nghost). */
 ch_ctx* ch_init(int nx, int ny, int nz, int nghost, double gamma, const int* bc);
 
@@ -136,7 +142,12 @@ int ch_set_solver(ch_ctx* ctx, int solver);
 /* Interface reconstruction used by ch_step.  CH_RECON_PPMC (default): A.3.  CH_RECON_PLMC: piecewise
  * linear, limited in the characteristic variables, with characteristic tracing, A.2.
  * CH_RECON_PCM: piecewise constant, Eq. 25-26. */
-enum { CH_RECON_PPMC = 0, CH_RECON_PLMC = 1, CH_RECON_PCM = 2 };
+enum {
+  CH_RECON_PPMC = 0, CH_RECON_PLMC = 1, CH_RECON_PCM = 2,
+  CH_RECON_PPMP = 3, /* A.4: parabolic in the primitive variables, contact steepening, shock flattening,
+                        Colella-Woodward tracing; 7-cell stencil: nghost >= 4; not with the H correction */
+  CH_RECON_PLMP = 4  /* A.1: linear in the primitive variables, evolved with its own face fluxes */
+};
 
 /* ch_set_hcorrection — switch the H correction of Appendix C on or off for later steps: in the
  * second Riemann pass the Roe eigenvalues of B28 become max(|lambda|, eta^H), eta^H the largest
@@ -147,6 +158,15 @@ int ch_set_hcorrection(ch_ctx* ctx, int on);
 
 /* ch_set_reconstruction — select the reconstruction for later steps.  CH_EINVAL for an unknown code. */
 int ch_set_reconstruction(ch_ctx* ctx, int recon);
+
+/* ch_set_noh — ambient density and pressure of the analytic CH_BC_NOH faces (defaults 1 and 1e-6).
+ * ch_set_time / ch_get_time — the time the analytic faces are evaluated at: ch_set_state resets it to 0, every ch_step
+ * adds its dt before the ghost fill.  ch_step_cfl refuses (CH_ESTATE) on a grid with an analytic face, because the
+ * time then lives on the device only.  ch_fill_ghosts — redo the ghost fill of the current state (after ch_set_time). */
+int ch_set_noh(ch_ctx* ctx, double rho0, double p0);
+int ch_set_time(ch_ctx* ctx, double t);
+double ch_get_time(const ch_ctx* ctx);
+int ch_fill_ghosts(ch_ctx* ctx);
 
 /* ch_set_option — launch-configuration choices that change HOW a step is computed, never WHAT (every setting
  * gives results within the one-step gate of every other; the tests compare them).  Defaults are what bench.py

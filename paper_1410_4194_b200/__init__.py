@@ -11,7 +11,7 @@ __all__ = ["workloads", "Grid", "load_library", "build"]
 
 
 def __getattr__(name):
-    if name in ("Grid", "load_library", "build", "PERIODIC", "REFLECTIVE", "OUTFLOW"):
+    if name in ("Grid", "load_library", "build", "PERIODIC", "REFLECTIVE", "OUTFLOW", "NOH"):
         from . import binding
         return getattr(binding, name)
     raise AttributeError(name)

@@ -19,15 +19,15 @@ _LIB = os.path.join(_HERE, "libch_b200.so")
 _SOURCES = [os.path.join(_CSRC, "ch_kernels.cu")]
 _HEADERS = [os.path.join(_CSRC, "ch_hydro.cuh"), os.path.join(os.path.dirname(_HERE), "include", "ch.h")]
 
-PERIODIC, REFLECTIVE, OUTFLOW = 1, 2, 3
+PERIODIC, REFLECTIVE, OUTFLOW, NOH = 1, 2, 3, 4
 SOLVER_EXACT, SOLVER_ROE = 0, 1
-RECON_PPMC, RECON_PLMC, RECON_PCM = 0, 1, 2
+RECON_PPMC, RECON_PLMC, RECON_PCM, RECON_PPMP, RECON_PLMP = 0, 1, 2, 3, 4
 CH_OK, CH_EINVAL, CH_ESTATE, CH_ECUDA, CH_ENONPHYS = 0, -1, -2, -3, -4
 
 # every symbol include/ch.h declares
 SYMBOLS = ("ch_init", "ch_free", "ch_last_error", "ch_set_spacing", "ch_padded_cells", "ch_workspace_bytes",
            "ch_bind", "ch_set_state", "ch_get_state", "ch_set_padded", "ch_get_padded", "ch_compute_dt",
-           "ch_step", "ch_step_cfl", "ch_last_dt", "ch_elapsed", "ch_set_solver", "ch_set_reconstruction", "ch_set_hcorrection", "ch_set_option", "ch_tiling", "ch_sync", "ch_kernel_launches", "ch_profile", "ch_profile_read", "ch_kernel_name",
+           "ch_step", "ch_step_cfl", "ch_last_dt", "ch_elapsed", "ch_set_solver", "ch_set_reconstruction", "ch_set_hcorrection", "ch_set_option", "ch_tiling", "ch_set_noh", "ch_set_time", "ch_get_time", "ch_fill_ghosts", "ch_sync", "ch_kernel_launches", "ch_profile", "ch_profile_read", "ch_kernel_name",
            "ch_fp64_peak_probe")
 K_COUNT = 11
 OPT_MARCH_SEG, OPT_FINAL_SEG, OPT_TMA, OPT_UNFUSED = 0, 1, 2, 3
@@ -92,6 +92,11 @@ def load_library() -> C.CDLL:
     L.ch_set_hcorrection.argtypes = [vp, C.c_int]
     L.ch_set_option.argtypes = [vp, C.c_int, C.c_int]
     L.ch_tiling.argtypes = [vp, C.POINTER(C.c_int)]
+    L.ch_set_noh.argtypes = [vp, C.c_double, C.c_double]
+    L.ch_set_time.argtypes = [vp, C.c_double]
+    L.ch_get_time.argtypes = [vp]
+    L.ch_get_time.restype = C.c_double
+    L.ch_fill_ghosts.argtypes = [vp]
     L.ch_sync.argtypes = [vp]
     L.ch_kernel_launches.restype = C.c_longlong
     L.ch_kernel_launches.argtypes = [vp]
@@ -230,8 +235,21 @@ class Grid:
         self._check(self._L.ch_set_hcorrection(self._h, int(bool(on))), "ch_set_hcorrection")
 
     def set_reconstruction(self, recon):
-        """0 = PPMC (default), 1 = PLMC, 2 = PCM."""
+        """0 = PPMC (default), 1 = PLMC, 2 = PCM, 3 = PPMP (nghost >= 4), 4 = PLMP."""
         self._check(self._L.ch_set_reconstruction(self._h, int(recon)), "ch_set_reconstruction")
+
+    def set_noh(self, rho0=1.0, p0=1e-6):
+        """Ambient state of the analytic (NOH) faces."""
+        self._check(self._L.ch_set_noh(self._h, rho0, p0), "ch_set_noh")
+
+    def set_time(self, t):
+        self._check(self._L.ch_set_time(self._h, float(t)), "ch_set_time")
+
+    def get_time(self) -> float:
+        return float(self._L.ch_get_time(self._h))
+
+    def fill_ghosts(self):
+        self._check(self._L.ch_fill_ghosts(self._h), "ch_fill_ghosts")
 
     def set_option(self, option, value):
         """Launch-configuration choice (OPT_MARCH_SEG, OPT_FINAL_SEG, OPT_TMA, OPT_UNFUSED); see ch_set_option."""

@@ -321,6 +321,162 @@ CH_D void plmc_faces(const Gas& G, double dtdx, const double wm[5], const double
   }
 }
 
+// ---- PPMP and PLMP (A.4 P:L886-1049, A.1 P:L679-717): reconstructions in the primitive variables ----------------
+// PPMP switches corrections on at thresholds (A35, A36, A38, A44, A45): a threshold decided differently on two
+// machines changes a face by a finite amount, so every quantity a threshold looks at is formed with explicitly
+// rounded IEEE operations from primitives that are themselves formed with IEEE division (cons2prim_ieee): the
+// decisions are then functions of the conserved state alone.  Everything downstream of a decision is continuous
+// and free to contract.
+CH_D void cons2prim_ieee(const Gas& G, double d, double mn, double mt1, double mt2, double E, double w[5]) {
+  const double u = __ddiv_rn(mn, d), v = __ddiv_rn(mt1, d), ww = __ddiv_rn(mt2, d);
+  const double ke = __dmul_rn(__dmul_rn(0.5, d), __dadd_rn(__dadd_rn(__dmul_rn(u, u), __dmul_rn(v, v)), __dmul_rn(ww, ww)));
+  w[0] = d; w[1] = u; w[2] = v; w[3] = ww;
+  w[4] = floor_p(__dmul_rn(G.gm1, __dadd_rn(E, -ke)));
+}
+
+// A2-A4: monotonised-central slope of one primitive variable
+CH_D double mc_slope(double wm, double w0, double wp) {
+  return mc_limit(w0 - wm, wp - w0, 0.5 * (wp - wm));
+}
+
+// A42-A45: F~ of cell j from p_{j-2}, p_{j-1}, p_{j+1}, p_{j+2}, u_{j-1}, u_{j+1}
+CH_D double ppmp_flatten_tilde(double pm2, double pm1, double pp1, double pp2, double um1, double up1) {
+  const double num = __dadd_rn(pp1, -pm1);
+  const double lo = (pp1 < pm1) ? pp1 : pm1;
+  if (__ddiv_rn(fabs(num), lo) < (1.0 / 3.0)) return 0.0;     // A44
+  if (__dadd_rn(up1, -um1) > 0.0) return 0.0;                 // A45
+  const double S = __ddiv_rn(num, __dadd_rn(pp2, -pm2));      // A42 (IEEE: a vanishing denominator gives +-inf)
+  const double t = __dmul_rn(10.0, __dadd_rn(S, -0.75));      // A43
+  const double c = (t < 1.0) ? t : 1.0;
+  return (c > 0.0) ? c : 0.0;
+}
+
+// w[s], s = 0..6 = cells i-3..i+3, direction-local order.  Outputs W*_L, W*_R (primitive).
+CH_D void ppmp_faces(const Gas& G, double dtdx, const double (&w)[7][5], double WLs[5], double WRs[5]) {
+  const double* wim = w[2];
+  const double* wi = w[3];
+  const double* wip = w[4];
+  double L[5], R[5], dm0 = 0.0, dp0 = 0.0;
+#pragma unroll
+  for (int m = 0; m < 5; ++m) {
+    const double dm = mc_slope(w[1][m], w[2][m], w[3][m]);
+    const double d0 = mc_slope(w[2][m], w[3][m], w[4][m]);
+    const double dp = mc_slope(w[3][m], w[4][m], w[5][m]);
+    L[m] = 0.5 * (wi[m] + wim[m]) - (d0 - dm) * (1.0 / 6.0);        // A34
+    R[m] = 0.5 * (wip[m] + wi[m]) - (dp - d0) * (1.0 / 6.0);
+    if (m == 0) { dm0 = dm; dp0 = dp; }
+  }
+  {   // A35-A41: contact steepening of the density faces (A38 read as G12, A41 as G13)
+    const double rm = wim[0], rp = wip[0], pm = wim[4], pp = wip[4];
+    const double drho = __dadd_rn(rp, -rm);
+    const double jump = __ddiv_rn(fabs(drho), (rp < rm) ? rp : rm);
+    const double pj = __ddiv_rn(fabs(__dadd_rn(pp, -pm)), (pp < pm) ? pp : pm);
+    if (jump > 0.01 && pj < __dmul_rn(__dmul_rn(0.1, G.gamma), jump)) {
+      const double d2m = __ddiv_rn(__dadd_rn(__dadd_rn(w[3][0], -__dmul_rn(2.0, w[2][0])), w[1][0]), 6.0);
+      const double d2p = __ddiv_rn(__dadd_rn(__dadd_rn(w[5][0], -__dmul_rn(2.0, w[4][0])), w[3][0]), 6.0);
+      if (__dmul_rn(d2m, d2p) < 0.0) {
+        const double et = __ddiv_rn(-__dadd_rn(d2p, -d2m), drho);                 // A39
+        double eta = __dadd_rn(__dmul_rn(20.0, et), -1.0);                         // A40
+        eta = (eta < 1.0) ? eta : 1.0;
+        eta = (eta > 0.0) ? eta : 0.0;
+        L[0] = __dadd_rn(__dmul_rn(L[0], __dadd_rn(1.0, -eta)), __dmul_rn(__dadd_rn(rm, __dmul_rn(0.5, dm0)), eta));   // A41
+        R[0] = __dadd_rn(__dmul_rn(R[0], __dadd_rn(1.0, -eta)), __dmul_rn(__dadd_rn(rp, -__dmul_rn(0.5, dp0)), eta));
+      }
+    }
+  }
+  {   // A42-A47: shock flattening of every variable
+    const double Fm = ppmp_flatten_tilde(w[0][4], w[1][4], w[3][4], w[4][4], w[1][1], w[3][1]);
+    const double F0 = ppmp_flatten_tilde(w[1][4], w[2][4], w[4][4], w[5][4], w[2][1], w[4][1]);
+    const double Fp = ppmp_flatten_tilde(w[2][4], w[3][4], w[5][4], w[6][4], w[3][1], w[5][1]);
+    const double Fn = (__dadd_rn(wip[4], -wim[4]) < 0.0) ? Fp : Fm;               // A46
+    const double F = (F0 > Fn) ? F0 : Fn;
+    const double oneF = __dadd_rn(1.0, -F);
+#pragma unroll
+    for (int m = 0; m < 5; ++m) {                                                  // A47
+      L[m] = __dadd_rn(__dmul_rn(F, wi[m]), __dmul_rn(oneF, L[m]));
+      R[m] = __dadd_rn(__dmul_rn(F, wi[m]), __dmul_rn(oneF, R[m]));
+    }
+  }
+  // A48 (= A21 + A22; G8, G14), A50
+  double WL[5], WR[5], dwi[5], w6[5];
+#pragma unroll
+  for (int m = 0; m < 5; ++m) {
+    const double c = wi[m];
+    double l = L[m], r = R[m];
+    double dR = r - c, dL = c - l;
+    if (dR * dL <= 0.0) { l = c; r = c; dR = 0.0; dL = 0.0; }
+    const double dR2 = dR + dR, dL2 = dL + dL;
+    const bool fixL = fabs(dL) > fabs(dR2), fixR = fabs(dR) > fabs(dL2);     // see ppmc_from_interfaces
+    if (fixL) l = c - dR2;
+    if (fixR) r = c + dL2;
+    WL[m] = l; WR[m] = r;
+    dwi[m] = r - l;
+    w6[m] = 6.0 * (c - 0.5 * (l + r));
+  }
+  // A49, A51, A52
+  const double a = sqrt_pos(G.gamma * wi[4] * rcp(wi[0]));
+  const double lm = wi[1] - a, l0 = wi[1], lp = wi[1] + a;
+  const double am = dtdx * sel_min(lm, 0.0), a0 = dtdx * sel_min(l0, 0.0), ap = dtdx * sel_min(lp, 0.0);
+  const double bm = dtdx * sel_max(lm, 0.0), b0 = dtdx * sel_max(l0, 0.0), bp = dtdx * sel_max(lp, 0.0);
+  const double k23 = 2.0 / 3.0;
+  double Lm[5], L0[5], Lp[5], Rm[5], R0[5], Rp[5];
+#pragma unroll
+  for (int m = 0; m < 5; ++m) {
+    Lm[m] = WL[m] - 0.5 * am * (dwi[m] + w6[m] * (1.0 + k23 * am));
+    L0[m] = WL[m] - 0.5 * a0 * (dwi[m] + w6[m] * (1.0 + k23 * a0));
+    Lp[m] = WL[m] - 0.5 * ap * (dwi[m] + w6[m] * (1.0 + k23 * ap));
+    Rm[m] = WR[m] - 0.5 * bm * (dwi[m] - w6[m] * (1.0 - k23 * bm));
+    R0[m] = WR[m] - 0.5 * b0 * (dwi[m] - w6[m] * (1.0 - k23 * b0));
+    Rp[m] = WR[m] - 0.5 * bp * (dwi[m] - w6[m] * (1.0 - k23 * bp));
+  }
+  // A53-A56 with C = rho a of the reference state; chi_L^p read as G15; 1/C through one rsqrt: 1/(rho a) = rsqrt(gamma p rho)
+  const double iCL = inv_rho_a(G, Lm[0], Lm[4]), iCR = inv_rho_a(G, Rp[0], Rp[4]);
+  const double CL = G.gamma * Lm[4] * Lm[0] * iCL, CR = G.gamma * Rp[4] * Rp[0] * iCR;      // rho a = gamma p rho / (rho a)
+  double chiLp = -0.5 * iCL * ((Lm[1] - Lp[1]) - (Lp[4] - Lm[4]) * iCL);
+  double chiRm = 0.5 * iCR * ((Rp[1] - Rm[1]) - (Rp[4] - Rm[4]) * iCR);
+  const double tLm = rcp(Lm[0]), tRp = rcp(Rp[0]);
+  double chiL0 = (Lm[4] - L0[4]) * (iCL * iCL) + (tLm - rcp(L0[0]));
+  double chiR0 = (Rp[4] - R0[4]) * (iCR * iCR) + (tRp - rcp(R0[0]));
+  if (l0 > 0.0) chiL0 = 0.0;                       // A55
+  if (lp > 0.0) chiLp = 0.0;
+  if (lm < 0.0) chiRm = 0.0;
+  if (l0 < 0.0) chiR0 = 0.0;
+  WLs[0] = rcp((tLm - chiL0) - chiLp);             // A56
+  WRs[0] = rcp((tRp - chiRm) - chiR0);
+  WLs[1] = Lm[1] + CL * chiLp;
+  WRs[1] = Rp[1] - CR * chiRm;
+  WLs[4] = Lm[4] + (CL * CL) * chiLp;
+  WRs[4] = Rp[4] + (CR * CR) * chiRm;
+  WLs[2] = L0[2]; WRs[2] = R0[2];
+  WLs[3] = L0[3]; WRs[3] = R0[3];
+}
+
+// PLMP (A1-A7): slope limited in the primitive variables, half-step by the cell's own two face fluxes (Eq. 11).
+CH_D void plmp_faces(const Gas& G, double dtdx, const double wm[5], const double w0[5], const double wp[5], double WLs[5],
+                     double WRs[5]) {
+  double WL[5], WR[5];
+#pragma unroll
+  for (int m = 0; m < 5; ++m) {
+    const double h = 0.5 * mc_slope(wm[m], w0[m], wp[m]);
+    WL[m] = w0[m] - h; WR[m] = w0[m] + h;                                         // A1
+  }
+  double UL[5], UR[5];
+  prim2cons(G, WL, UL);
+  prim2cons(G, WR, UR);
+  const double FL[5] = {UL[1], UL[1] * WL[1] + WL[4], UL[1] * WL[2], UL[1] * WL[3], (UL[4] + WL[4]) * WL[1]};
+  const double FR[5] = {UR[1], UR[1] * WR[1] + WR[4], UR[1] * WR[2], UR[1] * WR[3], (UR[4] + WR[4]) * WR[1]};
+  const double h = 0.5 * dtdx;
+  double cl[5], cr[5];
+#pragma unroll
+  for (int m = 0; m < 5; ++m) {
+    const double dF = FL[m] - FR[m];
+    cl[m] = UL[m] + h * dF;                                                        // A6
+    cr[m] = UR[m] + h * dF;                                                        // A7
+  }
+  cons2prim(G, cl[0], cl[1], cl[2], cl[3], cl[4], WLs);
+  cons2prim(G, cr[0], cr[1], cr[2], cr[3], cr[4], WRs);
+}
+
 // The same for a thread that marches along the sweep: `ifc` carries the A20 value of the cell's lower interface
 // in and of its upper interface out (PPMC only; the other reconstructions do not use it).
 template <int R>

@@ -301,6 +301,75 @@ __global__ void __launch_bounds__(kXT, CH_X_MINB) k_pass1_x(const StepArgs A, lo
 }
 
 // ---------------------------------------------------------------------------------------------
+// Pass 1 for the reconstructions in the primitive variables (PPMP: 7-cell stencil, g >= 4; PLMP: 3 cells),
+// a "next" row of SURVEY.md section 8(f): one thread per cell of [-1, n]^3 gathers its stencil along D (consecutive
+// lanes = consecutive x, so every load of the gather is a coalesced row segment and the re-reads of neighbouring
+// cells come from L1/L2), forms W*_L, W*_R and stores them conserved; k_riemann1 then solves the
+// interfaces.  Not marched: these kernels exist for completeness of the paper's method set, the headline path is
+// PPMC through k_pass1_x / k_pass1_march.
+// ---------------------------------------------------------------------------------------------
+template <int D, int R>     // R: 3 PPMP, 4 PLMP
+__global__ void __launch_bounds__(128) k_faces_wide(const StepArgs A) {
+  if (step_refused(A)) return;
+  const Geom& g = A.geo;
+  const int e0 = g.act[0] ? g.n[0] + 2 : 1, e1 = g.act[1] ? g.n[1] + 2 : 1, e2 = g.act[2] ? g.n[2] + 2 : 1;
+  const long long id = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (id >= (long long)e0 * e1 * e2) return;
+  const int i = (int)(id % e0) - (g.act[0] ? 1 : 0);
+  const long long r = id / e0;
+  const int j = (int)(r % e1) - (g.act[1] ? 1 : 0), k = (int)(r / e1) - (g.act[2] ? 1 : 0);
+  const long long np = g.np, sD = g.st[D];
+  const long long q = (long long)(i + g.g[0]) + (long long)(j + g.g[1]) * g.st[1] + (long long)(k + g.g[2]) * g.st[2];
+  const double dtdx = step_dtdx1(A, D);
+  constexpr int H = R == 3 ? 3 : 1;     // half width of the stencil
+  double w[7][5];
+#pragma unroll
+  for (int s = 0; s < 7; ++s) {
+    if (s < 3 - H || s > 3 + H) {
+#pragma unroll
+      for (int m = 0; m < 5; ++m) w[s][m] = 0.0;
+      continue;
+    }
+    const long long qs = q + (long long)(s - 3) * sD;
+    // primitives exactly as Eq. 6-8 read in the global component order (IEEE operations): PPMP's thresholds see them
+    double wg[5];
+    ch::cons2prim_ieee(A.gas, A.u[qs], A.u[np + qs], A.u[2 * np + qs], A.u[3 * np + qs], A.u[4 * np + qs], wg);
+#pragma unroll
+    for (int m = 0; m < 5; ++m) w[s][m] = wg[comp<D>(m)];
+  }
+  double WLs[5], WRs[5], cl[5], cr[5];
+  if (R == 3) ch::ppmp_faces(A.gas, dtdx, w, WLs, WRs);
+  else ch::plmp_faces(A.gas, dtdx, w[2], w[3], w[4], WLs, WRs);
+  ch::prim2cons(A.gas, WLs, cl);
+  ch::prim2cons(A.gas, WRs, cr);
+  store_local<D>(A.UL[D], np, q, cl);
+  store_local<D>(A.UR[D], np, q, cr);
+}
+
+// First Riemann pass over stored face states: F*_D at interface c+1/2, c in [-1, n_D - 1], transverse range [-1, n].
+template <int D, int S>
+__global__ void __launch_bounds__(128) k_riemann1(const StepArgs A) {
+  if (step_refused(A)) return;
+  const Geom& g = A.geo;
+  int e[3] = {g.act[0] ? g.n[0] + 2 : 1, g.act[1] ? g.n[1] + 2 : 1, g.act[2] ? g.n[2] + 2 : 1};
+  e[D] -= 1;
+  const long long id = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (id >= (long long)e[0] * e[1] * e[2]) return;
+  const int i = (int)(id % e[0]) - (g.act[0] ? 1 : 0);
+  const long long r = id / e[0];
+  const int j = (int)(r % e[1]) - (g.act[1] ? 1 : 0), k = (int)(r / e[1]) - (g.act[2] ? 1 : 0);
+  const long long np = g.np;
+  const long long q = (long long)(i + g.g[0]) + (long long)(j + g.g[1]) * g.st[1] + (long long)(k + g.g[2]) * g.st[2];
+  double ul[5], ur[5], wl[5], wr[5], fl[5];
+  load_raw<D>(A.UR[D], np, q, ul);
+  load_raw<D>(A.UL[D], np, q + g.st[D], ur);
+  ch::cons2prim(A.gas, ul[0], ul[1], ul[2], ul[3], ul[4], wl);
+  ch::cons2prim(A.gas, ur[0], ur[1], ur[2], ur[3], ur[4], wr);
+  ch::riemann<S>(A.gas, wl, wr, fl);
+  store_local<D>(A.Fs[D], np, q, fl);
+}
+
+// ---------------------------------------------------------------------------------------------
 // Pass 2: transverse correction (Eq. 23) of the two states meeting at interface c+1/2
 // along each active direction, then the second exact Riemann solve.  One thread per cell
 // of [-1, n)^3.  The three directions run through ONE copy of the solver (a rolled loop over d with
@@ -1073,7 +1142,32 @@ __global__ void __launch_bounds__(kTT, 1) k_final3d_tma(const StepArgs A, const 
 // each coordinate on its own, with the sign of each reflected normal momentum flipped; so one
 // launch over the ghost shell reads real cells only and writes ghost cells only.
 // ---------------------------------------------------------------------------------------------
-struct BcArgs { int bc[6]; };
+struct BcArgs {
+  int bc[6];
+  double noh_rho0, noh_p0, time;   // CH_BC_NOH: ambient state of the analytic inflow and the time it is evaluated at
+  int nact;                        // number of active dimensions (the n of rho0 (1 + t/r)^(n-1))
+};
+
+// Analytic boundary of the Noh test at the centre of cell (ci, cj, ck) (real-cell coordinates, box origin
+// at 0): rho = rho0 (1 + t/r)^(n-1), unit velocity toward the origin, E = p0/(gamma-1) + rho/2.  Explicitly rounded
+// operations in a fixed order: the ghost fill is index and copy work everywhere else, and stays bit-exact here too.
+__device__ __forceinline__ void noh_state(const StepArgs& A, const BcArgs& B, int ci, int cj, int ck, double v[5]) {
+  const int cc[3] = {ci, cj, ck};
+  double x[3], r2 = 0.0;
+#pragma unroll
+  for (int e = 0; e < 3; ++e) {
+    x[e] = A.geo.act[e] ? __dmul_rn((double)cc[e] + 0.5, A.dx[e]) : 0.0;
+    r2 = __dadd_rn(r2, __dmul_rn(x[e], x[e]));
+  }
+  const double r = __dsqrt_rn(r2);
+  const double q1 = __dadd_rn(1.0, __ddiv_rn(B.time, r));
+  double rho = B.noh_rho0;
+  for (int e = 1; e < B.nact; ++e) rho = __dmul_rn(rho, q1);
+  v[0] = rho;
+#pragma unroll
+  for (int e = 0; e < 3; ++e) v[1 + e] = __dmul_rn(rho, -__ddiv_rn(x[e], r));
+  v[4] = __dadd_rn(__ddiv_rn(B.noh_p0, A.gas.gm1), __dmul_rn(0.5, rho));
+}
 
 __device__ __forceinline__ int bc_source(int c, int n, int lo, int hi, bool& flip) {
   if (c < 0) {
@@ -1115,10 +1209,35 @@ __global__ void __launch_bounds__(256) k_ghost(const StepArgs A, const BcArgs B)
     pi = s < g.g[0] ? s : s + g.n[0];
   }
   bool fx = false, fy = false, fz = false;
+  const long long qd = (long long)pi + (long long)pj * g.st[1] + (long long)pk * g.st[2];
+  {
+    // Analytic faces.  The fill order x, y, z means the LAST direction in which a ghost lies outside
+    // decides where its value comes from: walk z, y, x; a reflective / periodic / outflow face maps that coordinate
+    // and the walk goes on, an analytic face ends it with the analytic state at the coordinates reached so far.
+    int cc[3] = {pi - g.g[0], pj - g.g[1], pk - g.g[2]};
+    bool fl[3] = {false, false, false};
+    bool analytic = false;
+#pragma unroll
+    for (int d = 2; d >= 0; --d) {
+      if (analytic || !g.act[d]) continue;
+      const int lo = B.bc[2 * d], hi = B.bc[2 * d + 1];
+      if ((cc[d] < 0 && lo == CH_BC_NOH) || (cc[d] >= g.n[d] && hi == CH_BC_NOH)) { analytic = true; continue; }
+      cc[d] = bc_source(cc[d], g.n[d], lo, hi, fl[d]);
+    }
+    if (analytic) {
+      double v[5];
+      noh_state(A, B, cc[0], cc[1], cc[2], v);
+      A.u[qd] = v[0];
+      A.u[g.np + qd] = fl[0] ? -v[1] : v[1];
+      A.u[2 * g.np + qd] = fl[1] ? -v[2] : v[2];
+      A.u[3 * g.np + qd] = fl[2] ? -v[3] : v[3];
+      A.u[4 * g.np + qd] = v[4];
+      return;
+    }
+  }
   const int si = bc_source(pi - g.g[0], g.n[0], B.bc[0], B.bc[1], fx);
   const int sj = bc_source(pj - g.g[1], g.n[1], B.bc[2], B.bc[3], fy);
   const int sk = bc_source(pk - g.g[2], g.n[2], B.bc[4], B.bc[5], fz);
-  const long long qd = (long long)pi + (long long)pj * g.st[1] + (long long)pk * g.st[2];
   const long long qs = (long long)(si + g.g[0]) + (long long)(sj + g.g[1]) * g.st[1] + (long long)(sk + g.g[2]) * g.st[2];
   double* u = A.u;
   u[qd] = u[qs];
@@ -1153,6 +1272,9 @@ struct ch_ctx {
   double dx[3];
   int bc[6];
   bool bound = false, have_state = false, dt_valid = false;
+  double time = 0.0;                       // sum of the dt of ch_step calls since ch_set_state / ch_set_time
+  double noh_rho0 = 1.0, noh_p0 = 1e-6;    // ambient state of the analytic (CH_BC_NOH) faces
+  bool has_noh = false;
   int device = -1;           // the device the bound buffers live on (ch_bind)
   bool smem_attr[2][2] = {{false, false}, {false, false}};   // [tma form][solver]: dynamic shared memory limit raised on `device`
   double* state = nullptr;
@@ -1265,6 +1387,8 @@ int launch_ghost(ch_ctx* c, const StepArgs& A) {
                           (long long)g.n[2] * g.n[1] * 2 * g.g[0];
   if (shell == 0) return CH_OK;
   BcArgs B; for (int s = 0; s < 6; ++s) B.bc[s] = c->bc[s];
+  B.noh_rho0 = c->noh_rho0; B.noh_p0 = c->noh_p0; B.time = c->time;
+  B.nact = g.act[0] + g.act[1] + g.act[2];
   { Bracket b(c, CH_K_GHOST); k_ghost<<<(unsigned)((shell + 255) / 256), 256, 0, c->stream>>>(A, B); }
   CH_CUDA(cudaGetLastError(), "k_ghost");
   return CH_OK;
@@ -1296,6 +1420,9 @@ bool build_tma_maps(ch_ctx* c) {
   const Geom& g = c->geo;
   if (!(g.act[0] && g.act[1] && g.act[2])) return false;
   if ((g.pd[0] & 1) || (g.np & 1)) return false;
+  // a tile's box starts at padded x = 30 b - 1 + nghost: with an even nghost that is an odd number of doubles, a
+  // start address that is not 16-byte aligned, which the bulk tensor copy faults on (observed: nghost = 4)
+  if (!(g.g[0] & 1)) return false;
   typedef CUresult (*EncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
                                const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
                                CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
@@ -1368,7 +1495,8 @@ ch_ctx* ch_init(int nx, int ny, int nz, int nghost, double gamma, const int* bc)
   c->nghost = nghost;
   for (int s = 0; s < 6; ++s) {
     c->bc[s] = bc ? bc[s] : CH_BC_PERIODIC;
-    if (g.act[s / 2] && (c->bc[s] < 1 || c->bc[s] > 3)) { delete c; fail(CH_EINVAL, "ch_init: bad boundary code"); return nullptr; }
+    if (g.act[s / 2] && (c->bc[s] < 1 || c->bc[s] > 4)) { delete c; fail(CH_EINVAL, "ch_init: bad boundary code"); return nullptr; }
+    if (g.act[s / 2] && c->bc[s] == CH_BC_NOH) c->has_noh = true;
   }
   for (int d = 0; d < 3; ++d) {
     if (g.act[d] && ((c->bc[2 * d] == CH_BC_PERIODIC) != (c->bc[2 * d + 1] == CH_BC_PERIODIC))) {
@@ -1449,6 +1577,7 @@ int ch_set_state(ch_ctx* c, const double* u) {
   DeviceGuard guard(c->device);
   int rc = copy_real(c, const_cast<double*>(u), true);
   if (rc) return rc;
+  c->time = 0.0;
   StepArgs A = make_args(c, 1.0);
   rc = launch_ghost(c, A);
   if (rc) return rc;
@@ -1527,6 +1656,19 @@ int step_impl(ch_ctx* c, double dt, bool devdt) {
   cudaStream_t st = c->stream;
   { Bracket b(c, CH_K_RESET); k_reset<<<1, 32, 0, st>>>(c->red, A.dt_dev); }
   // pass 1
+  if constexpr (R >= 3) {
+    // PPMP / PLMP: faces from the gathered stencil, then the interfaces (two launches per direction)
+    const long long cells = (long long)(g.act[0] ? g.n[0] + 2 : 1) * (g.act[1] ? g.n[1] + 2 : 1) * (g.act[2] ? g.n[2] + 2 : 1);
+    const unsigned nb = (unsigned)((cells + 127) / 128);
+    for (int d = 0; d < 3; ++d) {
+      if (!g.act[d]) continue;
+      Bracket b(c, d == 0 ? CH_K_PASS1_X : d == 1 ? CH_K_PASS1_Y : CH_K_PASS1_Z);
+      if (d == 0) { k_faces_wide<0, R><<<nb, 128, 0, st>>>(A); k_riemann1<0, S><<<nb, 128, 0, st>>>(A); }
+      else if (d == 1) { k_faces_wide<1, R><<<nb, 128, 0, st>>>(A); k_riemann1<1, S><<<nb, 128, 0, st>>>(A); }
+      else { k_faces_wide<2, R><<<nb, 128, 0, st>>>(A); k_riemann1<2, S><<<nb, 128, 0, st>>>(A); }
+      ++c->launches;     // two launches under one bracket
+    }
+  } else {
   if (g.act[0]) {
     // flat run of padded cells from the first needed row to the last: rows j,k in [-1, n]
     const int j0 = g.act[1] ? g.g[1] - 1 : 0, k0 = g.act[2] ? g.g[2] - 1 : 0;
@@ -1547,6 +1689,7 @@ int step_impl(ch_ctx* c, double dt, bool devdt) {
     Bracket b(c, d == 1 ? CH_K_PASS1_Y : CH_K_PASS1_Z);
     if (d == 1) k_pass1_march<1, S, R><<<grid, CH_MARCH_T, 0, st>>>(A, seg);
     else k_pass1_march<2, S, R><<<grid, CH_MARCH_T, 0, st>>>(A, seg);
+  }
   }
   CH_CUDA(cudaGetLastError(), "pass 1");
   if (g.act[0] && g.act[1] && g.act[2] && !c->unfused && !c->hcorr) {
@@ -1592,6 +1735,7 @@ int step_impl(ch_ctx* c, double dt, bool devdt) {
     }
 }
   CH_CUDA(cudaGetLastError(), "pass 2 / update");
+  if (!devdt) c->time += dt;     // analytic faces are evaluated at t^{n+1}
   int rc = launch_ghost(c, A);
   if (rc) return rc;
   c->dt_valid = true;
@@ -1609,6 +1753,8 @@ static int step_dispatch(ch_ctx* c, double dt, bool devdt) {
   switch (c->recon) {
     case CH_RECON_PLMC: return roe ? step_impl<1, 1>(c, dt, devdt) : step_impl<0, 1>(c, dt, devdt);
     case CH_RECON_PCM: return roe ? step_impl<1, 2>(c, dt, devdt) : step_impl<0, 2>(c, dt, devdt);
+    case CH_RECON_PPMP: return roe ? step_impl<1, 3>(c, dt, devdt) : step_impl<0, 3>(c, dt, devdt);
+    case CH_RECON_PLMP: return roe ? step_impl<1, 4>(c, dt, devdt) : step_impl<0, 4>(c, dt, devdt);
     default: return roe ? step_impl<1, 0>(c, dt, devdt) : step_impl<0, 0>(c, dt, devdt);
   }
 }
@@ -1623,6 +1769,7 @@ int ch_step_cfl(ch_ctx* c, double cfl, double t_left) {
   if (!c->have_state) return fail(CH_ESTATE, "ch_step_cfl: no state set");
   if (!(cfl > 0.0) || !(cfl <= 1.0)) return fail(CH_EINVAL, "ch_step_cfl: cfl not in (0,1]");
   if (t_left != t_left) return fail(CH_EINVAL, "ch_step_cfl: t_left is NaN");
+  if (c->has_noh) return fail(CH_ESTATE, "ch_step_cfl: an analytic (CH_BC_NOH) face needs the time on the host: use ch_compute_dt + ch_step");
   DeviceGuard guard(c->device);
   if (!c->dt_valid) {
     StepArgs A = make_args(c, 1.0);
@@ -1666,14 +1813,16 @@ double ch_elapsed(ch_ctx* c) {
 int ch_set_hcorrection(ch_ctx* c, int on) {
   if (!c) return fail(CH_EINVAL, "ch_set_hcorrection: null context");
   if (on && c->nghost < 4) return fail(CH_EINVAL, "ch_set_hcorrection: needs nghost >= 4 (P:L1291)");
+  if (on && c->recon >= CH_RECON_PPMP) return fail(CH_EINVAL, "ch_set_hcorrection: only with PPMC, PLMC or PCM (P:L565)");
   c->hcorr = on != 0;
   return CH_OK;
 }
 
 int ch_set_reconstruction(ch_ctx* c, int recon) {
   if (!c) return fail(CH_EINVAL, "ch_set_reconstruction: null context");
-  if (recon != CH_RECON_PPMC && recon != CH_RECON_PLMC && recon != CH_RECON_PCM)
-    return fail(CH_EINVAL, "ch_set_reconstruction: unknown reconstruction");
+  if (recon < CH_RECON_PPMC || recon > CH_RECON_PLMP) return fail(CH_EINVAL, "ch_set_reconstruction: unknown reconstruction");
+  if (recon == CH_RECON_PPMP && c->nghost < 4) return fail(CH_EINVAL, "ch_set_reconstruction: PPMP needs nghost >= 4 (P:L962)");
+  if (recon >= CH_RECON_PPMP && c->hcorr) return fail(CH_EINVAL, "ch_set_reconstruction: the H correction goes with PPMC, PLMC or PCM (P:L565)");
   c->recon = recon;
   return CH_OK;
 }
@@ -1692,6 +1841,30 @@ int ch_tiling(const ch_ctx* c, int* out) {
   out[6] = three_d ? final_segment(c) : 0; // planes a CTA of the fused second half marches
   out[7] = tma ? 1 : 0;
   return CH_OK;
+}
+
+int ch_set_noh(ch_ctx* c, double rho0, double p0) {
+  if (!c) return fail(CH_EINVAL, "ch_set_noh: null context");
+  if (!(rho0 > 0.0) || !(p0 > 0.0) || !std::isfinite(rho0) || !std::isfinite(p0)) return fail(CH_EINVAL, "ch_set_noh: rho0, p0 must be positive");
+  c->noh_rho0 = rho0; c->noh_p0 = p0;
+  return CH_OK;
+}
+
+int ch_set_time(ch_ctx* c, double t) {
+  if (!c) return fail(CH_EINVAL, "ch_set_time: null context");
+  if (!std::isfinite(t)) return fail(CH_EINVAL, "ch_set_time: t is not finite");
+  c->time = t;
+  return CH_OK;
+}
+
+double ch_get_time(const ch_ctx* c) { return c ? c->time : std::numeric_limits<double>::quiet_NaN(); }
+
+int ch_fill_ghosts(ch_ctx* c) {
+  if (!c) return fail(CH_EINVAL, "ch_fill_ghosts: null context");
+  if (!c->have_state) return fail(CH_ESTATE, "ch_fill_ghosts: no state set");
+  DeviceGuard guard(c->device);
+  StepArgs A = make_args(c, 1.0);
+  return launch_ghost(c, A);
 }
 
 int ch_set_option(ch_ctx* c, int option, int value) {
