@@ -364,6 +364,32 @@ def main():
             G.close()
             del G
             torch.cuda.empty_cache()
+    if world == 1 and not args.no_other_workloads:
+        # the same box cut into 2 x 2 x 2 blocks, all on this GPU: eight contexts, halo slabs through
+        # ch_halo_pack / ch_halo_unpack in x -> y -> z order, dt = min over the blocks; what the decomposition costs
+        # before any link is involved (results bitwise equal to the undivided grid: tests/test_gpu_decomp.py)
+        from paper_1410_4194_b200 import decomp
+        B = decomp.BlockGrid((args.size,) * 3, (2, 2, 2), 3, w.gamma, w.bc,
+                             lambda nx, ny, nz, g, gamma, bc, dev: pkg.Grid(nx, ny, nz, g, gamma, bc, device=dev), devices=device)
+        B.set_spacing(1.0 / args.size, 1.0 / args.size, 1.0 / args.size)
+        B.set_state(w.u)
+        for _ in range(3):
+            B.step(B.compute_dt(w.cfl))
+        k = max(1, min(args.steps, 10))
+        ev = (torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+        torch.cuda.synchronize()
+        ev[0].record(B.grids[0].cuda_stream)
+        for _ in range(k):
+            B.step(B.compute_dt(w.cfl))
+        ev[1].record(B.grids[0].cuda_stream)
+        torch.cuda.synchronize()
+        sec = ev[0].elapsed_time(ev[1]) * 1e-3
+        other_wl[f"sweep_{args.size} as 2x2x2 blocks on one GPU (block decomposition, halo exchange on the device)"] = {
+            "value": args.size ** 3 * k / sec, "unit": UNIT, "ms_per_step": sec / k * 1e3, "steps": k,
+            "halo_messages_per_step": 48}
+        B.close()
+        del B
+        torch.cuda.empty_cache()
     if rank != 0:
         if dist is not None:
             dist.destroy_process_group()

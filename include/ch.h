@@ -49,10 +49,15 @@ enum {
 /* Boundary-condition codes per face: any mix per face, periodic faces must be paired. */
 enum {
   CH_BC_PERIODIC = 1, CH_BC_REFLECTIVE = 2, CH_BC_OUTFLOW = 3,
-  CH_BC_NOH = 4 /* custom (analytic) boundary, "custom boundaries": the inflow of the Noh strong-shock test,
+  CH_BC_NOH = 4, /* custom (analytic) boundary, "custom boundaries": the inflow of the Noh strong-shock test,
                    P:L549-557: rho = rho0 (1 + t/r)^(n-1), unit velocity toward the origin of the box,
                    E = p0/(gamma-1) + rho/2 at the centre of every ghost cell behind the face, n = number of active
                    dimensions, t = ch_get_time (the state AFTER a step is filled at t^{n+1}); see ch_set_noh */
+  CH_BC_EXCHANGE = 5 /* the face borders another block of a decomposed domain (section 3.7): its ghost
+                   layers are written by ch_halo_unpack with what the neighbour's ch_halo_pack read.  A context with
+                   such a face never fills ghosts by itself: after ch_set_state and after every ch_step the caller
+                   runs, for d = x, y, z in this order: ch_halo_pack on the EXCHANGE faces of d, the
+                   transfer, ch_halo_unpack, and ch_fill_dim(d) for the faces of d with a local rule */
 };
 
 /* Device buffers handed to ch_bind.  All pointers are DEVICE pointers owned by the caller and must
@@ -68,7 +73,7 @@ typedef struct ch_buffers {
  * side of every active dimension, ratio of specific heats `gamma` (Eq. 8), and boundary
  * codes bc[6] = {x-,x+,y-,y+,z-,z+} (host pointer; NULL = all periodic).  Host-only: makes no CUDA
  * call.  Returns NULL on error (n < 1; nghost < 3 — PPMC inside six-solve CTU needs 3; gamma <= 1;
- * a bc code outside 1..4 on an active dimension; unpaired periodic faces; an active dimension
+ * a bc code outside 1..5 on an active dimension; unpaired periodic faces; an active dimension
  * smaller than nghost). */
 ch_ctx* ch_init(int nx, int ny, int nz, int nghost, double gamma, const int* bc);
 
@@ -167,6 +172,23 @@ int ch_set_noh(ch_ctx* ctx, double rho0, double p0);
 int ch_set_time(ch_ctx* ctx, double t);
 double ch_get_time(const ch_ctx* ctx);
 int ch_fill_ghosts(ch_ctx* ctx);
+
+/* Block decomposition.  Slab of direction d = nghost layers x (the other two directions: padded extent
+ * for a direction before d in the order x, y, z, real cells for a direction after d), so that edges and corners are
+ * carried by at most six messages per block.
+ * ch_halo_cells(d)   cells of one slab of direction d; a packed slab is 5 * ch_halo_cells(d) doubles, [5][nghost][.][.]
+ * ch_halo_pack       copy the nghost REAL layers next to `face` (0..5 = x-,x+,y-,y+,z-,z+) into the DEVICE buffer buf
+ * ch_halo_unpack     write buf into the nghost GHOST layers beyond `face` (pack of the neighbour's opposite face)
+ * ch_fill_dim(d)     fill the ghost layers of direction d behind faces with a local rule (periodic, reflective,
+ *                    outflow, analytic); EXCHANGE faces are left alone
+ * ch_set_origin      global index of this block's first real cell (the analytic boundary needs global coordinates)
+ * All asynchronous on the bound stream.  The time step of a decomposed domain is the minimum of the blocks'
+ * ch_compute_dt, handed to every block's ch_step; ch_step_cfl refuses (CH_ESTATE) on such a context. */
+long long ch_halo_cells(const ch_ctx* ctx, int d);
+int ch_halo_pack(ch_ctx* ctx, int face, double* buf);
+int ch_halo_unpack(ch_ctx* ctx, int face, const double* buf);
+int ch_fill_dim(ch_ctx* ctx, int d);
+int ch_set_origin(ch_ctx* ctx, int i0, int j0, int k0);
 
 /* ch_set_option — launch-configuration choices that change HOW a step is computed, never WHAT (every setting
  * gives results within the one-step gate of every other; the tests compare them).  Defaults are what bench.py

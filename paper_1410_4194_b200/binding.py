@@ -19,7 +19,7 @@ _LIB = os.path.join(_HERE, "libch_b200.so")
 _SOURCES = [os.path.join(_CSRC, "ch_kernels.cu")]
 _HEADERS = [os.path.join(_CSRC, "ch_hydro.cuh"), os.path.join(os.path.dirname(_HERE), "include", "ch.h")]
 
-PERIODIC, REFLECTIVE, OUTFLOW, NOH = 1, 2, 3, 4
+PERIODIC, REFLECTIVE, OUTFLOW, NOH, EXCHANGE = 1, 2, 3, 4, 5
 SOLVER_EXACT, SOLVER_ROE = 0, 1
 RECON_PPMC, RECON_PLMC, RECON_PCM, RECON_PPMP, RECON_PLMP = 0, 1, 2, 3, 4
 CH_OK, CH_EINVAL, CH_ESTATE, CH_ECUDA, CH_ENONPHYS = 0, -1, -2, -3, -4
@@ -27,7 +27,8 @@ CH_OK, CH_EINVAL, CH_ESTATE, CH_ECUDA, CH_ENONPHYS = 0, -1, -2, -3, -4
 # every symbol include/ch.h declares
 SYMBOLS = ("ch_init", "ch_free", "ch_last_error", "ch_set_spacing", "ch_padded_cells", "ch_workspace_bytes",
            "ch_bind", "ch_set_state", "ch_get_state", "ch_set_padded", "ch_get_padded", "ch_compute_dt",
-           "ch_step", "ch_step_cfl", "ch_last_dt", "ch_elapsed", "ch_set_solver", "ch_set_reconstruction", "ch_set_hcorrection", "ch_set_option", "ch_tiling", "ch_set_noh", "ch_set_time", "ch_get_time", "ch_fill_ghosts", "ch_sync", "ch_kernel_launches", "ch_profile", "ch_profile_read", "ch_kernel_name",
+           "ch_step", "ch_step_cfl", "ch_last_dt", "ch_elapsed", "ch_set_solver", "ch_set_reconstruction", "ch_set_hcorrection", "ch_set_option", "ch_tiling", "ch_set_noh", "ch_set_time", "ch_get_time", "ch_fill_ghosts",
+           "ch_halo_cells", "ch_halo_pack", "ch_halo_unpack", "ch_fill_dim", "ch_set_origin", "ch_sync", "ch_kernel_launches", "ch_profile", "ch_profile_read", "ch_kernel_name",
            "ch_fp64_peak_probe")
 K_COUNT = 11
 OPT_MARCH_SEG, OPT_FINAL_SEG, OPT_TMA, OPT_UNFUSED = 0, 1, 2, 3
@@ -97,6 +98,12 @@ def load_library() -> C.CDLL:
     L.ch_get_time.argtypes = [vp]
     L.ch_get_time.restype = C.c_double
     L.ch_fill_ghosts.argtypes = [vp]
+    L.ch_halo_cells.argtypes = [vp, C.c_int]
+    L.ch_halo_cells.restype = C.c_longlong
+    L.ch_halo_pack.argtypes = [vp, C.c_int, dp]
+    L.ch_halo_unpack.argtypes = [vp, C.c_int, dp]
+    L.ch_fill_dim.argtypes = [vp, C.c_int]
+    L.ch_set_origin.argtypes = [vp, C.c_int, C.c_int, C.c_int]
     L.ch_sync.argtypes = [vp]
     L.ch_kernel_launches.restype = C.c_longlong
     L.ch_kernel_launches.argtypes = [vp]
@@ -250,6 +257,22 @@ class Grid:
 
     def fill_ghosts(self):
         self._check(self._L.ch_fill_ghosts(self._h), "ch_fill_ghosts")
+
+    def halo_cells(self, d) -> int:
+        return int(self._L.ch_halo_cells(self._h, int(d)))
+
+    def halo_pack(self, face, buf):
+        """buf: device tensor of 5 * halo_cells(face // 2) doubles."""
+        self._check(self._L.ch_halo_pack(self._h, int(face), _addr(buf)), "ch_halo_pack")
+
+    def halo_unpack(self, face, buf):
+        self._check(self._L.ch_halo_unpack(self._h, int(face), _addr(buf)), "ch_halo_unpack")
+
+    def fill_dim(self, d):
+        self._check(self._L.ch_fill_dim(self._h, int(d)), "ch_fill_dim")
+
+    def set_origin(self, i0, j0, k0):
+        self._check(self._L.ch_set_origin(self._h, int(i0), int(j0), int(k0)), "ch_set_origin")
 
     def set_option(self, option, value):
         """Launch-configuration choice (OPT_MARCH_SEG, OPT_FINAL_SEG, OPT_TMA, OPT_UNFUSED); see ch_set_option."""

@@ -86,9 +86,12 @@ CH_D double floor_p(double p) { return (p < kPFloor) ? kPFloor : p; }  // keeps 
 CH_D void cons2prim(const Gas& G, double d, double mn, double mt1, double mt2, double E, double w[5]) {
   const double r = rcp(d);
   const double u = mn * r, v = mt1 * r, ww = mt2 * r;
-  const double ke = 0.5 * d * ((u * u + v * v) + ww * ww);
+  // every multiply-add spelled out: the same cell must get the same bits wherever the compiler inlines this
+  // (the warm-up of a marching segment and its loop body contract freely otherwise), so that a result does not
+  // depend on where a cell sits in a segment, a tile or a sub-domain
+  const double ke = __dmul_rn(0.5 * d, fma(ww, ww, fma(v, v, __dmul_rn(u, u))));
   w[0] = d; w[1] = u; w[2] = v; w[3] = ww;
-  w[4] = floor_p(G.gm1 * (E - ke));
+  w[4] = floor_p(__dmul_rn(G.gm1, E - ke));
 }
 
 // Eq. 6-8 inverted: primitive -> conserved (direction-local momenta).
@@ -107,49 +110,49 @@ CH_D double inv_rho_a(const Gas& G, double rho, double p) { return rsqrt_pos(G.g
 
 // Monotonised-central limiter A10 (reading G7: the formula governs).
 CH_D double mc_limit(double dL, double dR, double dC) {
-  const double m = sel_min(fabs(dC), 2.0 * sel_min(fabs(dL), fabs(dR)));
-  return (dL * dR > 0.0) ? copysign(m, dC) : 0.0;
+  const double m = sel_min(fabs(dC), __dmul_rn(2.0, sel_min(fabs(dL), fabs(dR))));
+  return (__dmul_rn(dL, dR) > 0.0) ? copysign(m, dC) : 0.0;
 }
 
 // Limited slope of cell q in primitive variables via characteristic variables (A2 P:L690, A9 P:L730
-// with row 0 read as G1, A10, A11 P:L741), projected with cell q's own rho, a.
-// s = inv_rho_a(q).
+// with row 0 read as G1, A10, A11 P:L741), projected with cell q's own rho, a.  s = inv_rho_a(q).
+// Every operation is an explicitly rounded intrinsic: this function is inlined both into the warm-up of a marching
+// segment and into its loop body, and a cell's slope must not depend on which of the two computed it (the result of
+// a step is then independent of how the sweeps are cut into segments, tiles or sub-domains — tested bitwise).
+CH_D void char_project(double ra, double ia2, double d0, double d1, double d2, double d3, double d4, double x[5]) {
+  const double t1 = __dmul_rn(ra, d1), t2 = __dmul_rn(d4, ia2);
+  x[0] = __dmul_rn(0.5, __dadd_rn(t2, -t1));
+  x[1] = __dadd_rn(d0, -t2);
+  x[2] = d2;
+  x[3] = d3;
+  x[4] = __dmul_rn(0.5, __dadd_rn(t1, t2));
+}
+
 CH_D void limited_slope(const Gas& G, const double wm[5], const double w0[5], const double wp[5], double s,
                         double dw[5]) {
   const double rho = w0[0];
-  const double a = G.gamma * w0[4] * s;
-  const double ia = rho * s;
-  const double ra = rho * ia;     // rho / a
-  const double ia2 = ia * ia;     // 1 / a^2
-  double xL[5], xR[5], x[5];
-  {
-    const double d0 = w0[0] - wm[0], d1 = w0[1] - wm[1], d4 = w0[4] - wm[4];
-    const double t1 = ra * d1, t2 = d4 * ia2;
-    xL[0] = 0.5 * (t2 - t1); xL[1] = d0 - t2; xL[2] = w0[2] - wm[2]; xL[3] = w0[3] - wm[3]; xL[4] = 0.5 * (t1 + t2);
-  }
-  {
-    const double d0 = wp[0] - w0[0], d1 = wp[1] - w0[1], d4 = wp[4] - w0[4];
-    const double t1 = ra * d1, t2 = d4 * ia2;
-    xR[0] = 0.5 * (t2 - t1); xR[1] = d0 - t2; xR[2] = wp[2] - w0[2]; xR[3] = wp[3] - w0[3]; xR[4] = 0.5 * (t1 + t2);
-  }
-  {
-    // centred difference (A2) projected the same way
-    const double d0 = 0.5 * (wp[0] - wm[0]), d1 = 0.5 * (wp[1] - wm[1]), d4 = 0.5 * (wp[4] - wm[4]);
-    const double t1 = ra * d1, t2 = d4 * ia2;
-    const double c0 = 0.5 * (t2 - t1), c1 = d0 - t2, c2 = 0.5 * (wp[2] - wm[2]), c3 = 0.5 * (wp[3] - wm[3]),
-                 c4 = 0.5 * (t1 + t2);
-    x[0] = mc_limit(xL[0], xR[0], c0);
-    x[1] = mc_limit(xL[1], xR[1], c1);
-    x[2] = mc_limit(xL[2], xR[2], c2);
-    x[3] = mc_limit(xL[3], xR[3], c3);
-    x[4] = mc_limit(xL[4], xR[4], c4);
-  }
-  const double s04 = x[0] + x[4];
-  dw[0] = x[1] + s04;
-  dw[1] = (a * a * s) * (x[4] - x[0]);   // a / rho
+  const double a = __dmul_rn(__dmul_rn(G.gamma, w0[4]), s);
+  const double ia = __dmul_rn(rho, s);
+  const double ra = __dmul_rn(rho, ia);     // rho / a
+  const double ia2 = __dmul_rn(ia, ia);     // 1 / a^2
+  double dl[5], dr[5], xL[5], xR[5], xC[5], x[5];
+#pragma unroll
+  for (int m = 0; m < 5; ++m) { dl[m] = __dadd_rn(w0[m], -wm[m]); dr[m] = __dadd_rn(wp[m], -w0[m]); }
+  char_project(ra, ia2, dl[0], dl[1], dl[2], dl[3], dl[4], xL);
+  char_project(ra, ia2, dr[0], dr[1], dr[2], dr[3], dr[4], xR);
+  // centred difference (A2) projected the same way
+  char_project(ra, ia2, __dmul_rn(0.5, __dadd_rn(wp[0], -wm[0])), __dmul_rn(0.5, __dadd_rn(wp[1], -wm[1])),
+               __dmul_rn(0.5, __dadd_rn(wp[2], -wm[2])), __dmul_rn(0.5, __dadd_rn(wp[3], -wm[3])),
+               __dmul_rn(0.5, __dadd_rn(wp[4], -wm[4])), xC);
+#pragma unroll
+  for (int m = 0; m < 5; ++m) x[m] = mc_limit(xL[m], xR[m], xC[m]);
+  const double s04 = __dadd_rn(x[0], x[4]);
+  const double a2 = __dmul_rn(a, a);
+  dw[0] = __dadd_rn(x[1], s04);
+  dw[1] = __dmul_rn(__dmul_rn(a2, s), __dadd_rn(x[4], -x[0]));   // a / rho
   dw[2] = x[2];
   dw[3] = x[3];
-  dw[4] = (a * a) * s04;
+  dw[4] = __dmul_rn(a2, s04);
 }
 
 // PPMC for one cell (A.3): parabola edges A20-A23, A24/A26(=A50, G2), characteristic
@@ -160,7 +163,7 @@ CH_D void limited_slope(const Gas& G, const double wm[5], const double w0[5], co
 CH_D void ppm_interface(const double w_lo[5], const double w_hi[5], const double d_lo[5], const double d_hi[5],
                         double e[5]) {
 #pragma unroll
-  for (int m = 0; m < 5; ++m) e[m] = 0.5 * (w_hi[m] + w_lo[m]) - (d_hi[m] - d_lo[m]) * (1.0 / 6.0);
+  for (int m = 0; m < 5; ++m) e[m] = fma(d_lo[m] - d_hi[m], 1.0 / 6.0, 0.5 * (w_hi[m] + w_lo[m]));
 }
 
 CH_D void ppmc_from_interfaces(const Gas& G, double dtdx, const double wm[5], const double w0[5], const double wp[5],
@@ -715,6 +718,19 @@ template <int S>
 CH_D void riemann(const Gas& G, const double WL[5], const double WR[5], double flux[5]) {
   if (S == 0) riemann_exact(G, WL, WR, flux);
   else riemann_roe(G, WL, WR, flux);
+}
+
+// The fused second half solves the same kind of interface in two places (the updating warps and the warp that serves
+// the two halo rows of a tile).  An interface on a tile seam is solved once by each, and both must return the same
+// bits (conservation to the bit, results independent of the tiling).  The exact solver's copies agree as inlined
+// (tested); the Roe solver's long sums contract differently from one inlining to the next, so it is called, not inlined.
+__device__ __noinline__ void riemann_roe_call(const Gas& G, const double WL[5], const double WR[5], double flux[5]) {
+  riemann_roe(G, WL, WR, flux);
+}
+template <int S>
+CH_D void riemann_tile(const Gas& G, const double WL[5], const double WR[5], double flux[5]) {
+  if (S == 0) riemann_exact(G, WL, WR, flux);
+  else riemann_roe_call(G, WL, WR, flux);
 }
 
 }  // namespace ch

@@ -975,7 +975,7 @@ __global__ void __launch_bounds__(kTT, 1) k_final3d_tma(const StepArgs A, const 
         asm volatile("bar.sync 1, %0;" ::"n"(kTC) : "memory");
 #pragma unroll
         for (int m = 0; m < 5; ++m) nb[m] = sX[m][st_ - kFX];
-        if (topok) ch::riemann<S>(G, nb, wlt, fl);
+        if (topok) ch::riemann_tile<S>(G, nb, wlt, fl);
 #pragma unroll
         for (int m = 0; m < 5; ++m) sF[m][st_] = fl[m];
         asm volatile("bar.sync 1, %0;" ::"n"(kTC) : "memory");
@@ -1039,7 +1039,7 @@ __global__ void __launch_bounds__(kTT, 1) k_final3d_tma(const StepArgs A, const 
         if (!first) {
 #pragma unroll
           for (int m = 0; m < 5; ++m) nb[m] = zU[m];
-          ch::riemann<S>(G, nb, wl, flz);
+          ch::riemann_tile<S>(G, nb, wl, flz);
         }
         if (k > k0) {
           // finish cell k-1 (Eq. 24): z-local order (rho, mz, mx, my, E)
@@ -1069,7 +1069,7 @@ __global__ void __launch_bounds__(kTT, 1) k_final3d_tma(const StepArgs A, const 
         if (need0) correct_faces<0>(A, ul, ur, dF, wl, wr);
 #pragma unroll
         for (int m = 0; m < 5; ++m) nb[m] = __shfl_up_sync(full, wr[m], 1);
-        if (solve0) ch::riemann<S>(G, nb, wl, fl);
+        if (solve0) ch::riemann_tile<S>(G, nb, wl, fl);
 #pragma unroll
         for (int m = 0; m < 5; ++m) {
           const double hi = __shfl_down_sync(full, fl[m], 1);
@@ -1092,7 +1092,7 @@ __global__ void __launch_bounds__(kTT, 1) k_final3d_tma(const StepArgs A, const 
         asm volatile("bar.sync 1, %0;" ::"n"(kTC) : "memory");
 #pragma unroll
         for (int m = 0; m < 5; ++m) nb[m] = sX[m][sidx - kFX];
-        if (solve1) ch::riemann<S>(G, nb, wl, fl);
+        if (solve1) ch::riemann_tile<S>(G, nb, wl, fl);
 #pragma unroll
         for (int m = 0; m < 5; ++m) sF[m][sidx] = fl[m];
         asm volatile("bar.sync 1, %0;" ::"n"(kTC) : "memory");
@@ -1146,6 +1146,7 @@ struct BcArgs {
   int bc[6];
   double noh_rho0, noh_p0, time;   // CH_BC_NOH: ambient state of the analytic inflow and the time it is evaluated at
   int nact;                        // number of active dimensions (the n of rho0 (1 + t/r)^(n-1))
+  int org[3];                      // global index of this block's first real cell (block decomposition; 0 otherwise)
 };
 
 // Analytic boundary of the Noh test at the centre of cell (ci, cj, ck) (real-cell coordinates, box origin
@@ -1156,7 +1157,7 @@ __device__ __forceinline__ void noh_state(const StepArgs& A, const BcArgs& B, in
   double x[3], r2 = 0.0;
 #pragma unroll
   for (int e = 0; e < 3; ++e) {
-    x[e] = A.geo.act[e] ? __dmul_rn((double)cc[e] + 0.5, A.dx[e]) : 0.0;
+    x[e] = A.geo.act[e] ? __dmul_rn((double)(cc[e] + B.org[e]) + 0.5, A.dx[e]) : 0.0;
     r2 = __dadd_rn(r2, __dmul_rn(x[e], x[e]));
   }
   const double r = __dsqrt_rn(r2);
@@ -1247,6 +1248,82 @@ __global__ void __launch_bounds__(256) k_ghost(const StepArgs A, const BcArgs B)
   u[4 * g.np + qd] = u[4 * g.np + qs];
 }
 
+// ---------------------------------------------------------------------------------------------
+// Block decomposition (section 3.7): a domain cut into blocks, each a grid of its own.  Ghost cells are
+// filled direction by direction, x then y then z, each direction over the padded extent of the directions before
+// it, so edges and corners ride along and at most six messages per block are needed.  Per direction:
+// k_halo packs the nghost real layers next to an EXCHANGE face into a contiguous buffer [5][nghost][b][a] (the
+// neighbour's unpack writes them into its ghost layers), k_fill_dim fills the faces with a local rule.
+// ---------------------------------------------------------------------------------------------
+struct SlabGeom { int d, e1, e2, lo1, lo2, n1, n2; };   // slab of direction d: n1 x n2 cells in the other two dims (e1 < e2)
+
+__device__ __host__ inline SlabGeom slab_geom(const Geom& g, int d) {
+  SlabGeom S;
+  S.d = d; S.e1 = d == 0 ? 1 : 0; S.e2 = d == 2 ? 1 : 2;
+  // directions before d: padded extent; after d: real cells only
+  S.lo1 = S.e1 < d ? -g.g[S.e1] : 0; S.n1 = S.e1 < d ? g.pd[S.e1] : g.n[S.e1];
+  S.lo2 = S.e2 < d ? -g.g[S.e2] : 0; S.n2 = S.e2 < d ? g.pd[S.e2] : g.n[S.e2];
+  return S;
+}
+
+// mode 0: pack the real layers next to face `side` of direction d into buf; mode 1: unpack buf into the ghost layers
+// beyond that face.  Layer l = 0..g-1 counts in the direction of increasing coordinate on both sides.
+__global__ void __launch_bounds__(256) k_halo(const StepArgs A, int d, int side, int mode, double* buf) {
+  const Geom& g = A.geo;
+  const SlabGeom S = slab_geom(g, d);
+  const int gl = g.g[d];
+  const long long per = (long long)gl * S.n1 * S.n2;
+  const long long id = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (id >= per) return;
+  const int a1 = (int)(id % S.n1);
+  const long long r = id / S.n1;
+  const int a2 = (int)(r % S.n2), l = (int)(r / S.n2);
+  int c[3];
+  c[S.e1] = S.lo1 + a1; c[S.e2] = S.lo2 + a2;
+  c[d] = mode == 0 ? (side == 0 ? l : g.n[d] - gl + l) : (side == 0 ? l - gl : g.n[d] + l);
+  const long long q = (long long)(c[0] + g.g[0]) + (long long)(c[1] + g.g[1]) * g.st[1] + (long long)(c[2] + g.g[2]) * g.st[2];
+#pragma unroll
+  for (int f = 0; f < 5; ++f) {
+    if (mode == 0) buf[f * per + id] = A.u[f * g.np + q];
+    else A.u[f * g.np + q] = buf[f * per + id];
+  }
+}
+
+// Local ghost fill of direction d alone (both faces; EXCHANGE faces are left to k_halo): the oracle's order.
+__global__ void __launch_bounds__(256) k_fill_dim(const StepArgs A, const BcArgs B, int d) {
+  const Geom& g = A.geo;
+  const SlabGeom S = slab_geom(g, d);
+  const int gl = g.g[d];
+  const long long per = (long long)gl * S.n1 * S.n2;
+  long long id = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (id >= 2 * per) return;
+  const int side = id >= per ? 1 : 0;
+  if (side) id -= per;
+  const int bc = B.bc[2 * d + side];
+  if (bc == CH_BC_EXCHANGE) return;
+  const int a1 = (int)(id % S.n1);
+  const long long r = id / S.n1;
+  const int a2 = (int)(r % S.n2), l = (int)(r / S.n2);
+  int c[3];
+  c[S.e1] = S.lo1 + a1; c[S.e2] = S.lo2 + a2;
+  c[d] = side == 0 ? l - gl : g.n[d] + l;
+  const long long qd = (long long)(c[0] + g.g[0]) + (long long)(c[1] + g.g[1]) * g.st[1] + (long long)(c[2] + g.g[2]) * g.st[2];
+  double v[5];
+  if (bc == CH_BC_NOH) {
+    noh_state(A, B, c[0], c[1], c[2], v);
+  } else {
+    bool flip = false;
+    int s[3] = {c[0], c[1], c[2]};
+    s[d] = bc_source(c[d], g.n[d], B.bc[2 * d], B.bc[2 * d + 1], flip);
+    const long long qs = (long long)(s[0] + g.g[0]) + (long long)(s[1] + g.g[1]) * g.st[1] + (long long)(s[2] + g.g[2]) * g.st[2];
+#pragma unroll
+    for (int f = 0; f < 5; ++f) v[f] = A.u[f * g.np + qs];
+    if (flip) v[1 + d] = -v[1 + d];
+  }
+#pragma unroll
+  for (int f = 0; f < 5; ++f) A.u[f * g.np + qd] = v[f];
+}
+
 // FP64 peak probe: 8 independent DFMA chains per thread.
 __global__ void k_dfma_probe(double* sink, int iters) {
   double a0 = threadIdx.x * 1e-9, a1 = a0 + 1, a2 = a0 + 2, a3 = a0 + 3, a4 = a0 + 4, a5 = a0 + 5, a6 = a0 + 6, a7 = a0 + 7;
@@ -1275,6 +1352,8 @@ struct ch_ctx {
   double time = 0.0;                       // sum of the dt of ch_step calls since ch_set_state / ch_set_time
   double noh_rho0 = 1.0, noh_p0 = 1e-6;    // ambient state of the analytic (CH_BC_NOH) faces
   bool has_noh = false;
+  bool has_exchange = false;               // a CH_BC_EXCHANGE face: ghost fill is driven by the caller (ch_fill_dim, ch_halo_*)
+  int org[3] = {0, 0, 0};                  // global index of the first real cell (ch_set_origin)
   int device = -1;           // the device the bound buffers live on (ch_bind)
   bool smem_attr[2][2] = {{false, false}, {false, false}};   // [tma form][solver]: dynamic shared memory limit raised on `device`
   double* state = nullptr;
@@ -1389,6 +1468,7 @@ int launch_ghost(ch_ctx* c, const StepArgs& A) {
   BcArgs B; for (int s = 0; s < 6; ++s) B.bc[s] = c->bc[s];
   B.noh_rho0 = c->noh_rho0; B.noh_p0 = c->noh_p0; B.time = c->time;
   B.nact = g.act[0] + g.act[1] + g.act[2];
+  for (int d = 0; d < 3; ++d) B.org[d] = c->org[d];
   { Bracket b(c, CH_K_GHOST); k_ghost<<<(unsigned)((shell + 255) / 256), 256, 0, c->stream>>>(A, B); }
   CH_CUDA(cudaGetLastError(), "k_ghost");
   return CH_OK;
@@ -1495,8 +1575,9 @@ ch_ctx* ch_init(int nx, int ny, int nz, int nghost, double gamma, const int* bc)
   c->nghost = nghost;
   for (int s = 0; s < 6; ++s) {
     c->bc[s] = bc ? bc[s] : CH_BC_PERIODIC;
-    if (g.act[s / 2] && (c->bc[s] < 1 || c->bc[s] > 4)) { delete c; fail(CH_EINVAL, "ch_init: bad boundary code"); return nullptr; }
+    if (g.act[s / 2] && (c->bc[s] < 1 || c->bc[s] > 5)) { delete c; fail(CH_EINVAL, "ch_init: bad boundary code"); return nullptr; }
     if (g.act[s / 2] && c->bc[s] == CH_BC_NOH) c->has_noh = true;
+    if (g.act[s / 2] && c->bc[s] == CH_BC_EXCHANGE) c->has_exchange = true;
   }
   for (int d = 0; d < 3; ++d) {
     if (g.act[d] && ((c->bc[2 * d] == CH_BC_PERIODIC) != (c->bc[2 * d + 1] == CH_BC_PERIODIC))) {
@@ -1579,7 +1660,7 @@ int ch_set_state(ch_ctx* c, const double* u) {
   if (rc) return rc;
   c->time = 0.0;
   StepArgs A = make_args(c, 1.0);
-  rc = launch_ghost(c, A);
+  rc = c->has_exchange ? CH_OK : launch_ghost(c, A);
   if (rc) return rc;
   c->have_state = true; c->dt_valid = false;
   return CH_OK;
@@ -1736,7 +1817,8 @@ int step_impl(ch_ctx* c, double dt, bool devdt) {
 }
   CH_CUDA(cudaGetLastError(), "pass 2 / update");
   if (!devdt) c->time += dt;     // analytic faces are evaluated at t^{n+1}
-  int rc = launch_ghost(c, A);
+  // a block of a decomposed domain: its ghosts are filled by the caller, direction by direction
+  int rc = c->has_exchange ? CH_OK : launch_ghost(c, A);
   if (rc) return rc;
   c->dt_valid = true;
   return profile_collect(c);
@@ -1769,6 +1851,7 @@ int ch_step_cfl(ch_ctx* c, double cfl, double t_left) {
   if (!c->have_state) return fail(CH_ESTATE, "ch_step_cfl: no state set");
   if (!(cfl > 0.0) || !(cfl <= 1.0)) return fail(CH_EINVAL, "ch_step_cfl: cfl not in (0,1]");
   if (t_left != t_left) return fail(CH_EINVAL, "ch_step_cfl: t_left is NaN");
+  if (c->has_exchange) return fail(CH_ESTATE, "ch_step_cfl: a block of a decomposed domain needs the global minimum of dt: use ch_compute_dt + ch_step");
   if (c->has_noh) return fail(CH_ESTATE, "ch_step_cfl: an analytic (CH_BC_NOH) face needs the time on the host: use ch_compute_dt + ch_step");
   DeviceGuard guard(c->device);
   if (!c->dt_valid) {
@@ -1865,6 +1948,51 @@ int ch_fill_ghosts(ch_ctx* c) {
   DeviceGuard guard(c->device);
   StepArgs A = make_args(c, 1.0);
   return launch_ghost(c, A);
+}
+
+int ch_set_origin(ch_ctx* c, int i0, int j0, int k0) {
+  if (!c) return fail(CH_EINVAL, "ch_set_origin: null context");
+  c->org[0] = i0; c->org[1] = j0; c->org[2] = k0;
+  return CH_OK;
+}
+
+long long ch_halo_cells(const ch_ctx* c, int d) {
+  if (!c || d < 0 || d > 2 || !c->geo.act[d]) return 0;
+  const SlabGeom S = slab_geom(c->geo, d);
+  return (long long)c->geo.g[d] * S.n1 * S.n2;
+}
+
+static int halo_launch(ch_ctx* c, int face, int mode, double* buf, const char* who) {
+  if (!c || !buf) return fail(CH_EINVAL, "ch_halo_pack / ch_halo_unpack: null argument");
+  if (face < 0 || face > 5 || !c->geo.act[face / 2]) return fail(CH_EINVAL, "ch_halo_pack / ch_halo_unpack: no such face");
+  if (!c->have_state) return fail(CH_ESTATE, "ch_halo_pack / ch_halo_unpack: no state set");
+  DeviceGuard guard(c->device);
+  StepArgs A = make_args(c, 1.0);
+  const long long per = ch_halo_cells(c, face / 2);
+  { Bracket b(c, CH_K_GHOST); k_halo<<<(unsigned)((per + 255) / 256), 256, 0, c->stream>>>(A, face / 2, face & 1, mode, buf); }
+  CH_CUDA(cudaGetLastError(), who);
+  if (mode == 1) c->dt_valid = c->dt_valid;   // ghosts do not enter Eq. 22
+  return CH_OK;
+}
+
+int ch_halo_pack(ch_ctx* c, int face, double* buf) { return halo_launch(c, face, 0, buf, "ch_halo_pack"); }
+int ch_halo_unpack(ch_ctx* c, int face, const double* buf) { return halo_launch(c, face, 1, const_cast<double*>(buf), "ch_halo_unpack"); }
+
+int ch_fill_dim(ch_ctx* c, int d) {
+  if (!c) return fail(CH_EINVAL, "ch_fill_dim: null context");
+  if (d < 0 || d > 2) return fail(CH_EINVAL, "ch_fill_dim: no such direction");
+  if (!c->have_state) return fail(CH_ESTATE, "ch_fill_dim: no state set");
+  if (!c->geo.act[d]) return CH_OK;
+  DeviceGuard guard(c->device);
+  StepArgs A = make_args(c, 1.0);
+  BcArgs B; for (int s = 0; s < 6; ++s) B.bc[s] = c->bc[s];
+  B.noh_rho0 = c->noh_rho0; B.noh_p0 = c->noh_p0; B.time = c->time;
+  B.nact = c->geo.act[0] + c->geo.act[1] + c->geo.act[2];
+  for (int e = 0; e < 3; ++e) B.org[e] = c->org[e];
+  const long long per = ch_halo_cells(c, d);
+  { Bracket b(c, CH_K_GHOST); k_fill_dim<<<(unsigned)((2 * per + 255) / 256), 256, 0, c->stream>>>(A, B, d); }
+  CH_CUDA(cudaGetLastError(), "k_fill_dim");
+  return CH_OK;
 }
 
 int ch_set_option(ch_ctx* c, int option, int value) {

@@ -709,28 +709,23 @@ def test_set_option_rejects_unknown_options_and_small_segments(ch):
     G.close()
 
 
-def test_segment_lengths_change_nothing_beyond_rounding(ch):
+def test_segment_lengths_do_not_change_the_bits(ch):
     """CH_OPT_MARCH_SEG / CH_OPT_FINAL_SEG change how the sweeps are cut into CTAs, not what a cell computes: the
-    same option values give the same bits; other segment lengths move a segment's first cell from the loop body to
-    the warm-up code (same formulas, the compiler contracts their multiply-adds differently), so the states agree
-    to rounding, far inside the one-step gate."""
-    w = wl.sweep(shape=(34, 20, 40))
-    res = []
-    for mseg, fseg in ((0, 0), (4, 8), (16, 8), (4, 32)):
-        G = ch.Grid(*w.shape, 3, w.gamma, w.bc)
-        t = G.tiling()
-        G.set_option(binding.OPT_MARCH_SEG, mseg)
-        G.set_option(binding.OPT_FINAL_SEG, fseg)
-        if (mseg, fseg) == (0, 0):
-            assert (t["march_seg_y"], t["march_seg_z"], t["final_seg"]) == (4, 4, 8), t
-        G.set_state(w.u)
-        for _ in range(2):
-            G.step(G.compute_dt(w.cfl))
-        res.append(G.get_state())
-        G.close()
-    assert np.array_equal(res[0], res[1])
-    for other in res[2:]:
-        assert max(max_rel_error(other, res[0], w.gamma)) <= 1e-14
+    functions shared by a segment's warm-up and its loop body spell out every multiply-add (ch_hydro.cuh), so a cell
+    gets the same bits wherever it sits in a segment."""
+    for w in (wl.sweep(shape=(34, 20, 40)), wl.rough_random(34, 20, 40, seed=3, decades=0.5)):
+        res = []
+        for mseg, fseg in ((0, 0), (4, 8), (16, 8), (4, 32), (64, 64)):
+            G = ch.Grid(*w.shape, 3, w.gamma, w.bc)
+            G.set_option(binding.OPT_MARCH_SEG, mseg)
+            G.set_option(binding.OPT_FINAL_SEG, fseg)
+            G.set_state(w.u)
+            for _ in range(2):
+                G.step(G.compute_dt(w.cfl))
+            res.append(G.get_padded())
+            G.close()
+        for other in res[1:]:
+            assert np.array_equal(other, res[0])
 
 
 def test_grid_on_a_device_that_is_not_current(ch):
