@@ -287,7 +287,7 @@ def main():
     import paper_1410_4194_b200 as pkg
     from paper_1410_4194_b200 import roofline as rf
     from paper_1410_4194_b200 import workloads as wl
-    from paper_1410_4194_b200.binding import fp64_peak_probe
+    from paper_1410_4194_b200.binding import fp64_peak_probe, issue_mix_probe
 
     pkg.load_library()                      # no CPU fallback: raises if the CUDA library is missing
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -302,6 +302,7 @@ def main():
 
     sampler = ClockSampler(local) if rank == 0 else None
     peak_tf, _ = fp64_peak_probe(device=device)                 # measured DFMA rate, burst
+    mix = issue_mix_probe(device=device)                        # scheduler time per FP64 / per other warp instruction
     solver = {"exact": 0, "roe": 1}[args.solver]
     recon = {"ppmc": 0, "plmc": 1, "pcm": 2}[args.recon]
     default_method = solver == 0 and recon == 0
@@ -408,7 +409,7 @@ def main():
     dfma_rate = peak_tf * 1e12 / 2.0                                    # FP64 instructions / s
     method_bytes = rf.METHOD_BYTES_PER_CELL * ghost
     capture_applies = default_method and args.size == 512 and bool(cap)
-    per_kernel, inst_step = {}, 0.0
+    per_kernel, inst_step, issue_step = {}, 0.0, 0.0
     for k, v in kern.items():
         if k not in rf.DECOMPOSITION_BYTES:
             continue
@@ -420,6 +421,12 @@ def main():
         t_a = c["inst"] * N / dfma_rate if c else 0.0
         inst_step += (c["inst"] if c else 0.0) * v["launches_per_step"]
         dec = rf.DECOMPOSITION_BYTES[k]
+        # issue ceiling of this kernel's own instruction mix (counts from the capture, scaled to this grid)
+        t_i = None
+        if c and c["warp_inst"] == c["warp_inst"]:
+            scale = N / rf.CAPTURE_N
+            t_i = scale * (c["fp64_warp_inst"] * mix["t_fp64"] + (c["warp_inst"] - c["fp64_warp_inst"]) * mix["t_alu"]) / (rf.SMS * 4)
+            issue_step += t_i * v["launches_per_step"]
         per_kernel[k] = {"ms": v["ms_avg"], "bound": "hbm" if t_h >= t_a else "alu",
                          "roofline_ms": max(t_h, t_a) * 1e3, "frac": max(t_h, t_a) / t,
                          "method_bytes_per_cell": mb, "fp64_inst_per_cell": c["inst"] if c else None,
@@ -428,6 +435,7 @@ def main():
                          "fp64_pipe_inst_per_cell_incl_compares": c["fp64_pipe_inst"] if c else None,
                          "ncu_sm__pipe_fp64_cycles_active_pct": c["pipe_pct"] if c else None,
                          "ncu_ms": c["ncu_ms"] if c else None,
+                         "issue_ceiling_ms": t_i * 1e3 if t_i else None, "issue_frac": t_i / t if t_i else None,
                          "decomposition_bytes_per_cell": dec,
                          "hbm_utilisation_of_decomposition": dec * N / t / 1e9 / hbm_gbs,
                          "traffic": c["dram_bytes"] if (c and capture_applies) else None}
@@ -454,6 +462,12 @@ def main():
                 "peak_source": psrc,
                 "kernel_ms": kern[top]["ms_avg"],
                 "kernel_share_of_step": kern[top]["ms_avg"] * kern[top]["launches_per_step"] / main_res["kernel_ms_per_step"],
+                "issue_mix_probe": {"t_fp64_scheduler_ns": mix["t_fp64"] * 1e9, "t_other_scheduler_ns": mix["t_alu"] * 1e9,
+                                    "t_other_16_scheduler_ns": mix["t_alu_16"] * 1e9, "ms": mix["ms"],
+                                    "note": "loops of 8 DFMA + {0,16,32} integer ops on 16 warps per scheduler (ch_issue_mix_probe): "
+                                            "an FP64 warp instruction costs t_fp64 of its scheduler, every other one t_other ON TOP "
+                                            "(no overlap); issue_ceiling = (F t_fp64 + O t_other) / 592 with F, O from the capture"},
+                "issue_ceiling_ms": pk["issue_ceiling_ms"], "issue_frac": pk["issue_frac"],
                 "fp64_peak_TFLOPs_measured": peak_tf, "fp64_inst_rate_measured": dfma_rate, "hbm_peak_GBps": hbm_gbs,
                 "ghost_factor": ghost,
                 "step": {"method_bytes_per_cell": method_bytes, "fp64_inst_per_cell": inst_step or None,
@@ -461,6 +475,7 @@ def main():
                          "bound": "hbm" if t_h_step >= t_a_step else "alu",
                          "roofline_ms": max(t_h_step, t_a_step) * 1e3, "measured_ms": step_ms,
                          "frac": max(t_h_step, t_a_step) * 1e3 / step_ms,
+                         "issue_ceiling_ms": issue_step * 1e3 or None, "issue_frac": issue_step * 1e3 / step_ms if issue_step else None,
                          "decomposition_bytes_per_cell": sum(rf.DECOMPOSITION_BYTES[k] for k in per_kernel),
                          "hbm_utilisation_of_decomposition":
                              sum(rf.DECOMPOSITION_BYTES[k] for k in per_kernel) * N / (step_ms * 1e-3) / 1e9 / hbm_gbs},

@@ -260,6 +260,12 @@ const char* ch_kernel_name(int kind);
  * device pointer to at least blocks*threads doubles.  FP64 flops done = 2*8*iters*blocks*threads. */
 double ch_fp64_peak_probe(double* sink, int blocks, int threads, int iters, void* stream);
 
+/* ch_issue_mix_probe — measurement helper for the second ceiling bench.py states: the same loop as
+ * ch_fp64_peak_probe (8 independent DFMA per iteration) with n_alu = 0, 16 or 32 independent 32-bit integer
+ * operations added per iteration; returns the elapsed milliseconds (negative on error).  From the three times:
+ * cost of an FP64 warp instruction and of an ALU warp instruction in scheduler cycles, and whether they overlap. */
+double ch_issue_mix_probe(double* sink, int n_alu, int blocks, int threads, int iters, void* stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -29,7 +29,7 @@ SYMBOLS = ("ch_init", "ch_free", "ch_last_error", "ch_set_spacing", "ch_padded_c
            "ch_bind", "ch_set_state", "ch_get_state", "ch_set_padded", "ch_get_padded", "ch_compute_dt",
            "ch_step", "ch_step_cfl", "ch_last_dt", "ch_elapsed", "ch_set_solver", "ch_set_reconstruction", "ch_set_hcorrection", "ch_set_option", "ch_tiling", "ch_set_noh", "ch_set_time", "ch_get_time", "ch_fill_ghosts",
            "ch_halo_cells", "ch_halo_pack", "ch_halo_unpack", "ch_fill_dim", "ch_set_origin", "ch_sync", "ch_kernel_launches", "ch_profile", "ch_profile_read", "ch_kernel_name",
-           "ch_fp64_peak_probe")
+           "ch_fp64_peak_probe", "ch_issue_mix_probe")
 K_COUNT = 11
 OPT_MARCH_SEG, OPT_FINAL_SEG, OPT_TMA, OPT_UNFUSED = 0, 1, 2, 3
 
@@ -113,6 +113,8 @@ def load_library() -> C.CDLL:
     L.ch_kernel_name.argtypes = [C.c_int]
     L.ch_fp64_peak_probe.restype = C.c_double
     L.ch_fp64_peak_probe.argtypes = [vp, C.c_int, C.c_int, C.c_int, vp]
+    L.ch_issue_mix_probe.restype = C.c_double
+    L.ch_issue_mix_probe.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.c_int, vp]
     _lib = L
     return L
 
@@ -314,3 +316,25 @@ def fp64_peak_probe(blocks=148 * 8, threads=256, iters=200000, device="cuda:0"):
     if ms <= 0:
         raise RuntimeError("ch_fp64_peak_probe: " + last_error())
     return 2.0 * 8 * iters * blocks * threads / (ms * 1e-3) / 1e12, ms
+
+
+def issue_mix_probe(blocks=148 * 4, threads=512, iters=100000, device="cuda:0"):
+    """Scheduler time per FP64 and per ALU warp instruction (seconds x schedulers, i.e. per SM sub-partition):
+    returns dict(t_fp64, t_alu, overlap) from loops of 8 DFMA + {0, 16, 32} integer operations on 4 warps per
+    scheduler.  t_fp64 = time of one DFMA warp instruction on its scheduler, t_alu = ADDED time per ALU warp
+    instruction; overlap = 1 - t_alu / (ALU-only cost) is not measured here: what matters is that the added time is
+    not hidden under the FP64 instructions."""
+    import torch
+    L = load_library()
+    sink = torch.empty(blocks * threads, dtype=torch.float64, device=device)
+    st = torch.cuda.current_stream(sink.device)
+    ms = {}
+    for n in (0, 16, 32):
+        ms[n] = L.ch_issue_mix_probe(sink.data_ptr(), n, blocks, threads, iters, st.cuda_stream)
+        if ms[n] <= 0:
+            raise RuntimeError("ch_issue_mix_probe: " + last_error())
+    warps_per_sched = (blocks / 148.0) * (threads / 32.0) / 4.0         # resident warps per scheduler (all co-resident)
+    per_iter = {n: ms[n] * 1e-3 / iters / warps_per_sched for n in ms}   # scheduler seconds per warp iteration
+    t_fp64 = per_iter[0] / 8.0
+    t_alu = (per_iter[32] - per_iter[0]) / 32.0
+    return dict(t_fp64=t_fp64, t_alu=t_alu, t_alu_16=(per_iter[16] - per_iter[0]) / 16.0, ms=ms)

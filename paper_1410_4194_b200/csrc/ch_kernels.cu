@@ -1335,6 +1335,29 @@ __global__ void k_dfma_probe(double* sink, int iters) {
   sink[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = ((a0 + a1) + (a2 + a3)) + ((a4 + a5) + (a6 + a7));
 }
 
+// Issue-mix probe: per loop iteration 8 independent DFMA plus NALU independent 32-bit integer operations (xor / add).
+// On B200 an FP64 warp instruction holds the dispatch port of its scheduler for two cycles and an ALU instruction
+// for about one, and the two do not overlap: the time of this loop is the SUM of its parts.  bench.py
+// measures the two costs with it and states every kernel's ceiling for its own instruction mix beside the FP64 one.
+template <int NALU>
+__global__ void k_mix_probe(double* sink, int iters) {
+  double a0 = threadIdx.x * 1e-9, a1 = a0 + 1, a2 = a0 + 2, a3 = a0 + 3, a4 = a0 + 4, a5 = a0 + 5, a6 = a0 + 6, a7 = a0 + 7;
+  const double b = 1.0000000001, c = 1e-12;
+  int i0 = threadIdx.x, i1 = i0 + 1, i2 = i0 + 2, i3 = i0 + 3;
+  for (int it = 0; it < iters; ++it) {
+    a0 = fma(a0, b, c); a1 = fma(a1, b, c); a2 = fma(a2, b, c); a3 = fma(a3, b, c);
+    a4 = fma(a4, b, c); a5 = fma(a5, b, c); a6 = fma(a6, b, c); a7 = fma(a7, b, c);
+#pragma unroll
+    for (int r = 0; r < NALU / 4; ++r) {
+      asm volatile("xor.b32 %0, %0, %1;" : "+r"(i0) : "r"(i1));
+      asm volatile("add.s32 %0, %0, 7;" : "+r"(i1));
+      asm volatile("xor.b32 %0, %0, %1;" : "+r"(i2) : "r"(i3));
+      asm volatile("add.s32 %0, %0, 5;" : "+r"(i3));
+    }
+  }
+  sink[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = ((a0 + a1) + (a2 + a3)) + ((a4 + a5) + (a6 + a7)) + (double)(i0 ^ i1 ^ i2 ^ i3);
+}
+
 thread_local std::string g_err;
 
 }  // namespace
@@ -2044,6 +2067,35 @@ int ch_profile_read(const ch_ctx* c, double* ms, long long* calls) {
 }
 
 const char* ch_kernel_name(int kind) { return (kind >= 0 && kind < CH_K_COUNT) ? kKernelNames[kind] : ""; }
+
+double ch_issue_mix_probe(double* sink, int n_alu, int blocks, int threads, int iters, void* stream) {
+  if (!sink || blocks < 1 || threads < 1 || threads > 1024 || iters < 1 || (n_alu != 0 && n_alu != 16 && n_alu != 32)) {
+    fail(CH_EINVAL, "ch_issue_mix_probe: bad argument (n_alu is 0, 16 or 32)"); return -1.0;
+  }
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  int dev = -1;
+  {
+    cudaPointerAttributes pa;
+    if (cudaPointerGetAttributes(&pa, sink) == cudaSuccess && pa.type == cudaMemoryTypeDevice) dev = pa.device;
+    else cudaGetLastError();
+  }
+  DeviceGuard guard(dev);
+  cudaEvent_t e0, e1;
+  if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) { fail(CH_ECUDA, "event create"); return -1.0; }
+  for (int rep = 0; rep < 2; ++rep) {      // the first launch warms up
+    if (rep == 1) cudaEventRecord(e0, st);
+    if (n_alu == 0) k_mix_probe<0><<<blocks, threads, 0, st>>>(sink, iters);
+    else if (n_alu == 16) k_mix_probe<16><<<blocks, threads, 0, st>>>(sink, iters);
+    else k_mix_probe<32><<<blocks, threads, 0, st>>>(sink, iters);
+  }
+  cudaEventRecord(e1, st);
+  cudaError_t e = cudaEventSynchronize(e1);
+  float ms = -1.f;
+  if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
+  cudaEventDestroy(e0); cudaEventDestroy(e1);
+  if (e != cudaSuccess) { cuda_fail(e, "ch_issue_mix_probe"); return -1.0; }
+  return (double)ms;
+}
 
 double ch_fp64_peak_probe(double* sink, int blocks, int threads, int iters, void* stream) {
   if (!sink || blocks < 1 || threads < 1 || threads > 1024 || iters < 1) { fail(CH_EINVAL, "ch_fp64_peak_probe: bad argument"); return -1.0; }

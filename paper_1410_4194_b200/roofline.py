@@ -12,6 +12,13 @@ The roofline of a kernel (or of the step) is the slower of two ceilings (north_s
 
     roofline time = max(80 B x Np/N x N / hbm_gbs, inst_per_cell x N / dfma_inst_rate),   frac = that / measured.
 
+A second ceiling is stated beside it because the first cannot be reached by this instruction mix: on B200 an FP64
+warp instruction holds its scheduler's dispatch port for two cycles, every other instruction for about one, and the
+two do not overlap (ch_issue_mix_probe measures both costs in the same run).  A kernel that executes F FP64-pipe and
+O other warp instructions therefore needs at least (F t_fp64 + O t_alu) / (148 x 4 schedulers): its ISSUE ceiling.
+Half of the instructions of this method are not FP64 arithmetic (selects of the limiters, compares, moves, address
+arithmetic), so the issue ceiling sits at about twice the FP64 one; `issue_frac` says how close a kernel is to it.
+
 The per-cell instruction counts are NOT typed in here: they are read from the ncu capture named by CAPTURE (a text
 file committed under profiles/, taken at 512^3 with the kernels of the commit being benched), so every roofline
 field can be reproduced from that one file and the bench line.  The same file supplies the measured DRAM traffic
@@ -123,6 +130,8 @@ def per_cell_counts(cap: dict):
             "inst": (dadd + dmul + dfma) / CAPTURE_N,
             "flops": (dadd + dmul + 2.0 * dfma) / CAPTURE_N,
             "fp64_pipe_inst": 32.0 * m.get("sm__inst_executed_pipe_fp64.sum", float("nan")) / CAPTURE_N,
+            "warp_inst": m.get("sm__inst_executed.sum", float("nan")),                 # per launch at CAPTURE_N cells
+            "fp64_warp_inst": m.get("sm__inst_executed_pipe_fp64.sum", float("nan")),
             "dram_bytes": m.get("dram__bytes_read.sum", float("nan")) + m.get("dram__bytes_write.sum", float("nan")),
             "pipe_pct": m.get("sm__pipe_fp64_cycles_active.avg.pct_of_peak_sustained_active"),
             "ncu_ms": m.get("gpu__time_duration.sum", float("nan")) * 1e3,
