@@ -641,25 +641,30 @@ CH_D void riemann_exact(const Gas& G, const double WL[5], const double WR[5], do
 // B23-B30 with B29 read as in DESIGN.md (G9); the intermediate states B31-B32 are checked for negative
 // density or pressure and the HLLE flux B33-B35 substituted if either occurs.  Square roots and quotients
 // through the branch-free rsqrt / rcp above.
+// Every multiply-add below is spelled out (fma / __dmul_rn / __dadd_rn): the solver is inlined in several places of
+// one kernel (the updating warps and the halo warp of the fused second half) and an interface on a tile seam, solved
+// once by each, must get the same bits from both (conservation to the bit, results independent of the tiling).
 CH_D void riemann_roe(const Gas& G, const double WL[5], const double WR[5], double flux[5], double etaH = 0.0) {
+#define M_ __dmul_rn
+#define A_ __dadd_rn
   const double rL = WL[0], uL = WL[1], vL = WL[2], wL = WL[3], pL = floor_p(WL[4]);
   const double rR = WR[0], uR = WR[1], vR = WR[2], wR = WR[3], pR = floor_p(WR[4]);
-  const double EL = pL * G.inv_gm1 + 0.5 * rL * ((uL * uL + vL * vL) + wL * wL);
-  const double ER = pR * G.inv_gm1 + 0.5 * rR * ((uR * uR + vR * vR) + wR * wR);
-  const double UL[5] = {rL, rL * uL, rL * vL, rL * wL, EL}, UR[5] = {rR, rR * uR, rR * vR, rR * wR, ER};
-  const double FL[5] = {UL[1], UL[1] * uL + pL, UL[1] * vL, UL[1] * wL, (EL + pL) * uL};   // Eq. 11
-  const double FR[5] = {UR[1], UR[1] * uR + pR, UR[1] * vR, UR[1] * wR, (ER + pR) * uR};
+  const double EL = fma(pL, G.inv_gm1, M_(M_(0.5, rL), fma(wL, wL, fma(vL, vL, M_(uL, uL)))));
+  const double ER = fma(pR, G.inv_gm1, M_(M_(0.5, rR), fma(wR, wR, fma(vR, vR, M_(uR, uR)))));
+  const double UL[5] = {rL, M_(rL, uL), M_(rL, vL), M_(rL, wL), EL}, UR[5] = {rR, M_(rR, uR), M_(rR, vR), M_(rR, wR), ER};
+  const double FL[5] = {UL[1], fma(UL[1], uL, pL), M_(UL[1], vL), M_(UL[1], wL), M_(A_(EL, pL), uL)};   // Eq. 11
+  const double FR[5] = {UR[1], fma(UR[1], uR, pR), M_(UR[1], vR), M_(UR[1], wR), M_(A_(ER, pR), uR)};
   // B23
   const double isl = rsqrt_pos(rL), isr = rsqrt_pos(rR);
-  const double sl = rL * isl, sr = rR * isr;
-  const double inv = rcp(sl + sr);
-  const double HL = (EL + pL) * (isl * isl), HR = (ER + pR) * (isr * isr);
-  const double ut = (sl * uL + sr * uR) * inv, vt = (sl * vL + sr * vR) * inv, wt = (sl * wL + sr * wR) * inv;
-  const double Ht = (sl * HL + sr * HR) * inv;
-  const double V2 = (ut * ut + vt * vt) + wt * wt;
-  const double at2 = G.gm1 * (Ht - 0.5 * V2);                              // B24
-  const double iat = rsqrt_pos(at2), at = at2 * iat;
-  const double lm = ut - at, l0 = ut, lp = ut + at;                        // B25
+  const double sl = M_(rL, isl), sr = M_(rR, isr);
+  const double inv = rcp(A_(sl, sr));
+  const double HL = M_(A_(EL, pL), M_(isl, isl)), HR = M_(A_(ER, pR), M_(isr, isr));
+  const double ut = M_(fma(sl, uL, M_(sr, uR)), inv), vt = M_(fma(sl, vL, M_(sr, vR)), inv), wt = M_(fma(sl, wL, M_(sr, wR)), inv);
+  const double Ht = M_(fma(sl, HL, M_(sr, HR)), inv);
+  const double V2 = fma(wt, wt, fma(vt, vt, M_(ut, ut)));
+  const double at2 = M_(G.gm1, fma(-0.5, V2, Ht));                         // B24
+  const double iat = rsqrt_pos(at2), at = M_(at2, iat);
+  const double lm = A_(ut, -at), l0 = ut, lp = A_(ut, at);                 // B25
   if (lm >= 0.0) {
 #pragma unroll
     for (int m = 0; m < 5; ++m) flux[m] = FL[m];
@@ -672,45 +677,48 @@ CH_D void riemann_roe(const Gas& G, const double WL[5], const double WR[5], doub
   }
   double dU[5];
 #pragma unroll
-  for (int m = 0; m < 5; ++m) dU[m] = UR[m] - UL[m];                       // B26
+  for (int m = 0; m < 5; ++m) dU[m] = A_(UR[m], -UL[m]);                   // B26
   // B27: acoustic strengths share  q = gamma' (0.5 V2 drho - u dmx - v dmy - w dmz + dE)
-  const double ia2 = iat * iat, Na = 0.5 * ia2, gp = G.gm1;
-  const double q = gp * ((0.5 * V2 * dU[0] - ut * dU[1]) - (vt * dU[2] + wt * dU[3]) + dU[4]);
-  const double r = at * (ut * dU[0] - dU[1]);
-  const double xi0 = Na * (q + r), xi4 = Na * (q - r);
-  const double xi1 = dU[2] - vt * dU[0], xi2 = dU[3] - wt * dU[0];
-  const double xi3 = dU[0] - q * ia2;
+  const double ia2 = M_(iat, iat), Na = M_(0.5, ia2);
+  const double q = M_(G.gm1, A_(A_(fma(-ut, dU[1], M_(M_(0.5, V2), dU[0])), -fma(vt, dU[2], M_(wt, dU[3]))), dU[4]));
+  const double r = M_(at, fma(ut, dU[0], -dU[1]));
+  const double xi0 = M_(Na, A_(q, r)), xi4 = M_(Na, A_(q, -r));
+  const double xi1 = fma(-vt, dU[0], dU[2]), xi2 = fma(-wt, dU[0], dU[3]);
+  const double xi3 = fma(-q, ia2, dU[0]);
   // B28, B29
   // C3: with the H correction |lambda| -> max(|lambda|, eta^H), here and only here (reading S18)
   const double alm = sel_max(fabs(lm), etaH), al0 = sel_max(fabs(l0), etaH), alp = sel_max(fabs(lp), etaH);
-  const double C0 = xi0 * alm, C1 = xi1 * al0, C2 = xi2 * al0, C3 = xi3 * al0, C4 = xi4 * alp;
-  const double ua = ut * at, c04 = C0 + C4;
+  const double C0 = M_(xi0, alm), C1 = M_(xi1, al0), C2 = M_(xi2, al0), C3 = M_(xi3, al0), C4 = M_(xi4, alp);
+  const double ua = M_(ut, at), c04 = A_(C0, C4), c043 = A_(c04, C3);
+  const double Hm = A_(Ht, -ua), Hp = A_(Ht, ua);
   double sv[5];
-  sv[0] = c04 + C3;
-  sv[1] = (C0 * lm + C3 * ut) + C4 * lp;
-  sv[2] = (c04 + C3) * vt + C1;
-  sv[3] = (c04 + C3) * wt + C2;
-  sv[4] = (C0 * (Ht - ua) + C4 * (Ht + ua)) + ((C1 * vt + C2 * wt) + 0.5 * C3 * V2);
+  sv[0] = c043;
+  sv[1] = fma(C4, lp, fma(C0, lm, M_(C3, ut)));
+  sv[2] = fma(c043, vt, C1);
+  sv[3] = fma(c043, wt, C2);
+  sv[4] = A_(fma(C0, Hm, M_(C4, Hp)), fma(M_(0.5, C3), V2, fma(C1, vt, M_(C2, wt))));
   // B31, B32: intermediate states
-  double Um[5] = {UL[0] + xi0, UL[1] + xi0 * lm, UL[2] + xi0 * vt, UL[3] + xi0 * wt, UL[4] + xi0 * (Ht - ua)};
-  bool hlle = !(Um[0] > 0.0) || !(Um[4] * Um[0] - 0.5 * ((Um[1] * Um[1] + Um[2] * Um[2]) + Um[3] * Um[3]) > 0.0);
-  Um[0] += xi3; Um[1] += xi3 * ut; Um[2] += xi1 + xi3 * vt; Um[3] += xi2 + xi3 * wt;
-  Um[4] += (xi1 * vt + xi2 * wt) + 0.5 * xi3 * V2;
-  hlle = hlle || !(Um[0] > 0.0) || !(Um[4] * Um[0] - 0.5 * ((Um[1] * Um[1] + Um[2] * Um[2]) + Um[3] * Um[3]) > 0.0);
+  double Um[5] = {A_(UL[0], xi0), fma(xi0, lm, UL[1]), fma(xi0, vt, UL[2]), fma(xi0, wt, UL[3]), fma(xi0, Hm, UL[4])};
+  bool hlle = !(Um[0] > 0.0) || !(fma(Um[4], Um[0], -M_(0.5, fma(Um[3], Um[3], fma(Um[2], Um[2], M_(Um[1], Um[1]))))) > 0.0);
+  Um[0] = A_(Um[0], xi3); Um[1] = fma(xi3, ut, Um[1]); Um[2] = A_(Um[2], fma(xi3, vt, xi1)); Um[3] = A_(Um[3], fma(xi3, wt, xi2));
+  Um[4] = A_(Um[4], fma(M_(0.5, xi3), V2, fma(xi1, vt, M_(xi2, wt))));
+  hlle = hlle || !(Um[0] > 0.0) || !(fma(Um[4], Um[0], -M_(0.5, fma(Um[3], Um[3], fma(Um[2], Um[2], M_(Um[1], Um[1]))))) > 0.0);
   if (!hlle) {
 #pragma unroll
-    for (int m = 0; m < 5; ++m) flux[m] = 0.5 * ((FL[m] + FR[m]) - sv[m]);   // B30
+    for (int m = 0; m < 5; ++m) flux[m] = M_(0.5, A_(A_(FL[m], FR[m]), -sv[m]));   // B30
     return;
   }
   // HLLE (B33-B35)
-  const double aL = G.gamma * pL * inv_rho_a(G, rL, pL), aR = G.gamma * pR * inv_rho_a(G, rR, pR);
-  const double bm = sel_min(sel_min(lm, uL - aL), 0.0), bp = sel_max(sel_max(lp, uR + aR), 0.0);
-  const double t = (bp + bm) * rcp(bp - bm);
+  const double aL = M_(M_(G.gamma, pL), inv_rho_a(G, rL, pL)), aR = M_(M_(G.gamma, pR), inv_rho_a(G, rR, pR));
+  const double bm = sel_min(sel_min(lm, A_(uL, -aL)), 0.0), bp = sel_max(sel_max(lp, A_(uR, aR)), 0.0);
+  const double t = M_(A_(bp, bm), rcp(A_(bp, -bm)));
 #pragma unroll
   for (int m = 0; m < 5; ++m) {
-    const double fl = FL[m] - bm * UL[m], fr = FR[m] - bp * UR[m];          // B34
-    flux[m] = 0.5 * ((fl + fr) + (fl - fr) * t);                             // B35
+    const double fl = fma(-bm, UL[m], FL[m]), fr = fma(-bp, UR[m], FR[m]);   // B34
+    flux[m] = M_(0.5, fma(A_(fl, -fr), t, A_(fl, fr)));                      // B35
   }
+#undef M_
+#undef A_
 }
 
 // Solver selection at compile time (reconstruction and solver are selectable): 0 exact, 1 Roe + HLLE.
@@ -721,16 +729,10 @@ CH_D void riemann(const Gas& G, const double WL[5], const double WR[5], double f
 }
 
 // The fused second half solves the same kind of interface in two places (the updating warps and the warp that serves
-// the two halo rows of a tile).  An interface on a tile seam is solved once by each, and both must return the same
-// bits (conservation to the bit, results independent of the tiling).  The exact solver's copies agree as inlined
-// (tested); the Roe solver's long sums contract differently from one inlining to the next, so it is called, not inlined.
-__device__ __noinline__ void riemann_roe_call(const Gas& G, const double WL[5], const double WR[5], double flux[5]) {
-  riemann_roe(G, WL, WR, flux);
-}
+// the two halo rows of a tile): both solvers spell out their multiply-adds where it matters, so the copies agree bitwise.
 template <int S>
 CH_D void riemann_tile(const Gas& G, const double WL[5], const double WR[5], double flux[5]) {
-  if (S == 0) riemann_exact(G, WL, WR, flux);
-  else riemann_roe_call(G, WL, WR, flux);
+  riemann<S>(G, WL, WR, flux);
 }
 
 }  // namespace ch
