@@ -559,6 +559,7 @@ __global__ void k_pick_dt(unsigned long long* red, double cfl, double t_left) {
   }
   r[2] = dt;
   r[3] += dt;
+  red[0] = 0ULL; red[1] = 0ULL;     // the step that follows reduces its new state into clean cells (k_reset's work)
 }
 
 __global__ void __launch_bounds__(256) k_reset(unsigned long long* red, const double* dt_dev) {
@@ -1375,6 +1376,15 @@ struct ch_ctx {
   double time = 0.0;                       // sum of the dt of ch_step calls since ch_set_state / ch_set_time
   double noh_rho0 = 1.0, noh_p0 = 1e-6;    // ambient state of the analytic (CH_BC_NOH) faces
   bool has_noh = false;
+  // ch_step_cfl replays the kernels of a step as a CUDA graph (captured on a private stream the second time a
+  // configuration is stepped): on small grids the step is launch bound
+  bool use_graph = true;
+  cudaStream_t cap_stream = nullptr;
+  cudaGraphExec_t gexec = nullptr;
+  long long gkey[8] = {-1, -1, -1, -1, -1, -1, -1, -1};   // configuration the graph / the last direct step belongs to
+  double gdx[3] = {0, 0, 0};
+  int gseen = 0;                           // direct steps taken with gkey (capture on the second)
+  long long glaunches = 0;                 // kernels in the graph
   bool has_exchange = false;               // a CH_BC_EXCHANGE face: ghost fill is driven by the caller (ch_fill_dim, ch_halo_*)
   int org[3] = {0, 0, 0};                  // global index of the first real cell (ch_set_origin)
   int device = -1;           // the device the bound buffers live on (ch_bind)
@@ -1621,9 +1631,17 @@ ch_ctx* ch_init(int nx, int ny, int nz, int nghost, double gamma, const int* bc)
   return c;
 }
 
+static void drop_graph(ch_ctx* c) {
+  if (c->gexec) { cudaGraphExecDestroy(c->gexec); c->gexec = nullptr; }
+  c->gseen = 0;
+  c->gkey[0] = -1;
+}
+
 int ch_free(ch_ctx* c) {
   if (!c) return CH_OK;
   DeviceGuard guard(c->device);
+  drop_graph(c);
+  if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
   if (c->h_red) cudaFreeHost(c->h_red);
   for (int k = 0; k < 2 * CH_K_COUNT; ++k) if (c->ev[k]) cudaEventDestroy(c->ev[k]);
   delete c;
@@ -1670,6 +1688,7 @@ int ch_bind(ch_ctx* c, const ch_buffers* b, void* stream) {
   c->stream = static_cast<cudaStream_t>(stream);
   if (!c->h_red) CH_CUDA(cudaHostAlloc((void**)&c->h_red, 16, cudaHostAllocDefault), "cudaHostAlloc");
   c->bound = true; c->have_state = false; c->dt_valid = false;
+  drop_graph(c);                           // a captured step holds the old buffers' addresses
   CH_CUDA(cudaMemsetAsync(c->red, 0, 64, c->stream), "ch_bind: clearing the reduction cells");
   c->tma_ok = build_tma_maps(c);
   return CH_OK;
@@ -1758,7 +1777,7 @@ int step_impl(ch_ctx* c, double dt, bool devdt) {
   StepArgs A = make_args(c, devdt ? 1.0 : dt);
   if (devdt) A.dt_dev = reinterpret_cast<const double*>(c->red) + 2;     // written by k_pick_dt just before
   cudaStream_t st = c->stream;
-  { Bracket b(c, CH_K_RESET); k_reset<<<1, 32, 0, st>>>(c->red, A.dt_dev); }
+  if (!devdt) { Bracket b(c, CH_K_RESET); k_reset<<<1, 32, 0, st>>>(c->red, nullptr); }   // ch_step_cfl: k_pick_dt has done it
   // pass 1
   if constexpr (R >= 3) {
     // PPMP / PLMP: faces from the gathered stencil, then the interfaces (two launches per direction)
@@ -1888,7 +1907,50 @@ int ch_step_cfl(ch_ctx* c, double cfl, double t_left) {
   }
   { Bracket b(c, CH_K_PICK_DT); k_pick_dt<<<1, 32, 0, c->stream>>>(c->red, cfl, t_left); }
   CH_CUDA(cudaGetLastError(), "k_pick_dt");
-  return step_dispatch(c, 0.0, true);
+  if (!c->use_graph || c->profiling) return step_dispatch(c, 0.0, true);
+  // The rest of the step reads dt from device memory and has no other per-step argument: one graph per
+  // configuration.  First step with a configuration: direct (sets kernel attributes); second: captured on the
+  // private stream; from then on one cudaGraphLaunch on the caller's stream.
+  const long long key[8] = {c->solver, c->recon, c->hcorr, c->unfused, c->use_tma, c->march_seg, c->final_seg, 1};
+  bool same = true;
+  for (int i = 0; i < 8; ++i) same = same && key[i] == c->gkey[i];
+  for (int d = 0; d < 3; ++d) same = same && c->gdx[d] == c->dx[d];
+  if (!same) {
+    drop_graph(c);
+    for (int i = 0; i < 8; ++i) c->gkey[i] = key[i];
+    for (int d = 0; d < 3; ++d) c->gdx[d] = c->dx[d];
+  }
+  if (c->gexec) {
+    CH_CUDA(cudaGraphLaunch(c->gexec, c->stream), "cudaGraphLaunch");
+    c->launches += c->glaunches;
+    c->dt_valid = true;
+    return CH_OK;
+  }
+  if (c->gseen++ == 0) return step_dispatch(c, 0.0, true);
+  if (!c->cap_stream) CH_CUDA(cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking), "cudaStreamCreate");
+  cudaStream_t user = c->stream;
+  const long long before = c->launches;
+  cudaGraph_t graph = nullptr;
+  CH_CUDA(cudaStreamBeginCapture(c->cap_stream, cudaStreamCaptureModeThreadLocal), "cudaStreamBeginCapture");
+  c->stream = c->cap_stream;
+  const int rc = step_dispatch(c, 0.0, true);
+  c->stream = user;
+  cudaError_t e = cudaStreamEndCapture(c->cap_stream, &graph);
+  c->glaunches = c->launches - before;
+  c->launches = before;
+  if (rc != CH_OK || e != cudaSuccess || !graph) {
+    if (graph) cudaGraphDestroy(graph);
+    cudaGetLastError();
+    c->use_graph = false;                  // fall back to direct launches for this context
+    return step_dispatch(c, 0.0, true);
+  }
+  e = cudaGraphInstantiate(&c->gexec, graph, 0);
+  cudaGraphDestroy(graph);
+  if (e != cudaSuccess) { c->gexec = nullptr; cudaGetLastError(); c->use_graph = false; return step_dispatch(c, 0.0, true); }
+  CH_CUDA(cudaGraphLaunch(c->gexec, c->stream), "cudaGraphLaunch");
+  c->launches += c->glaunches;
+  c->dt_valid = true;
+  return CH_OK;
 }
 
 double ch_last_dt(ch_ctx* c) {
@@ -2029,6 +2091,7 @@ int ch_set_option(ch_ctx* c, int option, int value) {
       c->final_seg = value; return CH_OK;
     case CH_OPT_TMA: c->use_tma = value != 0; return CH_OK;
     case CH_OPT_UNFUSED: c->unfused = value != 0; return CH_OK;
+    case CH_OPT_GRAPH: c->use_graph = value != 0; if (!c->use_graph) drop_graph(c); return CH_OK;
     default: return fail(CH_EINVAL, "ch_set_option: unknown option");
   }
 }

@@ -743,3 +743,29 @@ def test_grid_on_a_device_that_is_not_current(ch):
     assert torch.cuda.current_device() == 0
     assert np.array_equal(G0.get_padded(), G1.get_padded())
     G0.close(); G1.close()
+
+
+def test_step_cfl_graph_replay_equals_direct_launches(ch):
+    """ch_step_cfl replays a captured graph from the third step of a configuration on: same kernels, same bits, same
+    launch count as direct launches; a change of configuration (solver, options, spacing) re-captures."""
+    for w in (wl.kelvin_helmholtz(64), wl.sweep(shape=(34, 20, 20)), wl.sod(128)):
+        res = {}
+        for graph in (1, 0):
+            G = ch.Grid(*w.shape, 3, w.gamma, w.bc)
+            G.set_option(binding.OPT_GRAPH, graph)
+            G.set_state(w.u)
+            n0 = G.kernel_launches
+            for _ in range(5):
+                G.step_cfl(w.cfl)
+            n1 = G.kernel_launches - n0
+            G.set_solver(1)                       # new configuration: direct, capture, replay again
+            for _ in range(4):
+                G.step_cfl(w.cfl)
+            G.set_solver(0)
+            G.set_spacing(*(1.1 / w.shape[0],) * 3)
+            for _ in range(3):
+                G.step_cfl(w.cfl)
+            res[graph] = (G.get_padded(), n1, G.elapsed(), G.last_dt())
+            G.close()
+        assert np.array_equal(res[0][0], res[1][0]) and np.all(np.isfinite(res[0][0]))
+        assert res[0][1:] == res[1][1:]
