@@ -119,6 +119,21 @@ def test_whole_grid_parity_256_sweep(ref):
     assert max(strict) <= ONE_STEP_TOL, strict
 
 
+@pytest.mark.parametrize("n", [384, 512])
+def test_whole_grid_parity_at_the_largest_sizes(ref, n):
+    """Every cell of the 384^3 and the 512^3 grid (the size bench.py times; 1.3e8 cells x 5 fields) after one GPU
+    step, in the launch configuration the bench uses, against the oracle re-stepping the grid in 32-plane slabs
+    (about a minute of the box's host cores at 512^3)."""
+    w = wl.sweep(n)
+    post, ur, _ = whole_grid_one_step(ref, w, pre_steps=1)
+    assert post.shape == (5, n, n, n)
+    err = max_rel_error(post, ur, w.gamma)
+    strict = max_rel_error_strict(post, ur, w.gamma)
+    print(f"whole-grid {n}^3 sweep: S11 norm", err, "strict", strict)
+    assert max(err) <= ONE_STEP_TOL, err
+    assert max(strict) <= ONE_STEP_TOL, strict
+
+
 def test_whole_grid_parity_256_shock_cloud(ref):
     """The same on BASELINE.json config 4 (Mach-50 shock + lognormal cloud, outflow faces): every cell of the
     256^3 grid, after five steps (the front has entered fresh cells).  Gate in the S11 norm; the floor-free figure

@@ -265,3 +265,21 @@ def test_ppmp_and_hcorrection_exclude_each_other_and_ppmp_needs_four_ghosts(ref)
     G.set_hcorrection(False); G.set_reconstruction(PPMP)
     with pytest.raises(ValueError):
         G.set_hcorrection(True)
+
+
+def test_plmp_pure_advection_closed_form(ref):
+    """A1-A7 on a density ramp carried by a uniform flow (u, p constant): F(U_L) - F(U_R) = -u (U_R - U_L) for every
+    conserved component, so A6 / A7 give rho*_L = rho_L - (dt/2dx) u drho, rho*_R = rho_R - (dt/2dx) u drho with
+    drho = rho_R - rho_L the limited slope, and velocity and pressure stay put: the exact half-step solution of
+    linear advection at the two faces."""
+    rng = np.random.default_rng(5)
+    for _ in range(50):
+        u, v, wv, p = rng.normal(), rng.normal(), rng.normal(), rng.uniform(0.5, 2.0)
+        r0, b = rng.uniform(1.0, 2.0), rng.uniform(-0.1, 0.1)
+        w = stencil7(lambda s: np.array([r0 + b * s, u, v, wv, p]))
+        dtdx = rng.uniform(0.05, 0.4)
+        WL, WR, WLs, WRs = ref.plmp_cell(GAMMA, dtdx, w)
+        assert np.allclose(WL, [r0 - 0.5 * b, u, v, wv, p], rtol=1e-14) and np.allclose(WR, [r0 + 0.5 * b, u, v, wv, p], rtol=1e-14)
+        shift = 0.5 * dtdx * u * b
+        assert np.allclose(WLs, [r0 - 0.5 * b - shift, u, v, wv, p], rtol=1e-13, atol=1e-14)
+        assert np.allclose(WRs, [r0 + 0.5 * b - shift, u, v, wv, p], rtol=1e-13, atol=1e-14)
