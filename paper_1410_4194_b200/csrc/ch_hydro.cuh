@@ -494,6 +494,8 @@ CH_D void recon_faces_march(const Gas& G, double dtdx, const double wm[5], const
     for (int m = 0; m < 5; ++m) ifc[m] = RA[m];
   } else if (R == 1) {
     plmc_faces(G, dtdx, wm, w0, wp, dw0, s, WLs, WRs);
+  } else if (R == 4) {
+    plmp_faces(G, dtdx, wm, w0, wp, WLs, WRs);      // its own slope, in the primitive variables (A1-A4)
   } else {
 #pragma unroll
     for (int m = 0; m < 5; ++m) { WLs[m] = w0[m]; WRs[m] = w0[m]; }
@@ -507,6 +509,7 @@ CH_D void recon_faces(const Gas& G, double dtdx, const double wm[5], const doubl
                       double WRs[5]) {
   if (R == 0) ppmc_faces(G, dtdx, wm, w0, wp, dwm, dw0, dwp, s, WLs, WRs);
   else if (R == 1) plmc_faces(G, dtdx, wm, w0, wp, dw0, s, WLs, WRs);
+  else if (R == 4) plmp_faces(G, dtdx, wm, w0, wp, WLs, WRs);
   else {
 #pragma unroll
     for (int m = 0; m < 5; ++m) { WLs[m] = w0[m]; WRs[m] = w0[m]; }

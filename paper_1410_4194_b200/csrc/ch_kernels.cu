@@ -1779,7 +1779,7 @@ int step_impl(ch_ctx* c, double dt, bool devdt) {
   cudaStream_t st = c->stream;
   if (!devdt) { Bracket b(c, CH_K_RESET); k_reset<<<1, 32, 0, st>>>(c->red, nullptr); }   // ch_step_cfl: k_pick_dt has done it
   // pass 1
-  if constexpr (R >= 3) {
+  if constexpr (R == 3) {
     // PPMP / PLMP: faces from the gathered stencil, then the interfaces (two launches per direction)
     const long long cells = (long long)(g.act[0] ? g.n[0] + 2 : 1) * (g.act[1] ? g.n[1] + 2 : 1) * (g.act[2] ? g.n[2] + 2 : 1);
     const unsigned nb = (unsigned)((cells + 127) / 128);
