@@ -15,8 +15,12 @@
 // The optional OpenMP pragma on the outermost loop of each nest does not change any result (the
 // step contains no floating-point reduction; min is exact).
 //
+// Beyond the north_star path (PPMC + exact solver) it holds the paper's other method choices: the Roe solver with the
+// HLLE failsafe and the H correction (B.2, App. C), the PLMC, PCM, PPMP and PLMP reconstructions (A.1, A.2, A.4) and
+// the analytic boundary of the Noh test, each selected at run time through ref_set_*.
+//
 // Parity pins: every function below is pinned by tests/test_oracle_*.py (closed forms,
-// invariants, special cases); see DESIGN.md §5.  No function here is "parity unpinned".
+// invariants, special cases, the paper's printed observations); see DESIGN.md §5.  No function here is "parity unpinned".
 
 #include <algorithm>
 #include <cmath>
