@@ -2033,6 +2033,7 @@ double ch_get_time(const ch_ctx* c) { return c ? c->time : std::numeric_limits<d
 int ch_fill_ghosts(ch_ctx* c) {
   if (!c) return fail(CH_EINVAL, "ch_fill_ghosts: null context");
   if (!c->have_state) return fail(CH_ESTATE, "ch_fill_ghosts: no state set");
+  if (c->has_exchange) return fail(CH_ESTATE, "ch_fill_ghosts: a block of a decomposed domain is filled direction by direction (ch_halo_*, ch_fill_dim)");
   DeviceGuard guard(c->device);
   StepArgs A = make_args(c, 1.0);
   return launch_ghost(c, A);
