@@ -811,6 +811,102 @@ __global__ void __launch_bounds__(kFT, CH_F_MINB) k_final3d(const StepArgs A, in
 }
 
 // ---------------------------------------------------------------------------------------------
+// The same for x-y grids (nz = 1; BASELINE.json's Kelvin-Helmholtz box): one plane, no z carry.  A 32 x kFY tile of
+// threads: corrected x and y face states of the cell (Eq. 23 with the one transverse direction), the x problem
+// through warp shuffles, the y problem through shared memory, Eq. 24 and the Eq. 22 reduction.  It replaces
+// k_pass2 + k_update (and F, G^{n+1/2} through HBM) on grids where a step is a handful of launch-bound kernels.
+// ---------------------------------------------------------------------------------------------
+template <int S>
+__global__ void __launch_bounds__(kFT, 2) k_final2d(const StepArgs A) {
+  __shared__ double sX[5][kFT], sF[5][kFT];
+  if (step_refused(A)) return;
+  const Geom& g = A.geo;
+  double dtx[3];
+  step_dtdx(A, dtx);
+  const Gas& G = A.gas;
+  const unsigned full = 0xffffffffu;
+  const int tid = threadIdx.x, lane = tid & 31, row = tid >> 5;
+  const int nx = g.n[0], ny = g.n[1];
+  const int i = (int)blockIdx.x * (kFX - 2) - 1 + lane;
+  const int j = (int)blockIdx.y * (kFY - 2) - 1 + row;
+  const bool valid = i <= nx && j <= ny;
+  const bool realI = i >= 0 && i < nx, realJ = j >= 0 && j < ny;
+  const bool updL = lane >= 1 && lane <= kFX - 2 && realI, updR = row >= 1 && row <= kFY - 2 && realJ;
+  const bool need0 = valid && updR, need1 = valid && updL, need2 = updL && updR;
+  const bool solve0 = need0 && lane >= 1 && i >= 0, solve1 = need1 && row >= 1 && j >= 0;
+  const long long np = g.np, s1 = g.st[1];
+  const long long q = (long long)(i + g.g[0]) + (long long)(j + g.g[1]) * s1;
+  const double hx = 0.5 * dtx[0], hy = 0.5 * dtx[1];
+  double dF[3][5];
+  {
+    double fx[5] = {0.0, 0.0, 0.0, 0.0, 0.0}, fxm[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+#pragma unroll
+    for (int f = 0; f < 5; ++f) { dF[1][f] = 0.0; dF[2][f] = 0.0; }
+    if (valid) {
+#pragma unroll
+      for (int f = 0; f < 5; ++f) {
+        const long long a = f * np + q;
+        fx[f] = A.Fs[0][a];
+        if (lane == 0) fxm[f] = A.Fs[0][a - 1];
+        dF[1][f] = __dmul_rn(hy, A.Fs[1][a - s1] - A.Fs[1][a]);
+      }
+    }
+#pragma unroll
+    for (int f = 0; f < 5; ++f) {
+      const double t = __shfl_up_sync(full, fx[f], 1);
+      dF[0][f] = __dmul_rn(hx, (lane == 0 ? fxm[f] : t) - fx[f]);
+    }
+  }
+  double part[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+  if (need2) {
+#pragma unroll
+    for (int f = 0; f < 5; ++f) part[f] = A.u[f * np + q];
+  }
+  {   // ---- x: neighbours are lanes of the same warp
+    double wl[5] = {1.0, 0.0, 0.0, 0.0, 1.0}, wr[5] = {1.0, 0.0, 0.0, 0.0, 1.0}, nb[5], fl[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+    if (need0) face_states<0>(A, q, dF, wl, wr);
+#pragma unroll
+    for (int m = 0; m < 5; ++m) nb[m] = __shfl_up_sync(full, wr[m], 1);
+    if (solve0) ch::riemann<S>(G, nb, wl, fl);
+#pragma unroll
+    for (int m = 0; m < 5; ++m) {
+      const double hi = __shfl_down_sync(full, fl[m], 1);
+      part[m] += dtx[0] * (fl[m] - hi);
+    }
+  }
+  {   // ---- y: neighbours are rows of the CTA
+    double wl[5] = {1.0, 0.0, 0.0, 0.0, 1.0}, wr[5] = {1.0, 0.0, 0.0, 0.0, 1.0}, nb[5], fl[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+    if (need1) face_states<1>(A, q, dF, wl, wr);
+#pragma unroll
+    for (int m = 0; m < 5; ++m) sX[m][tid] = wr[m];
+    __syncthreads();
+    const int src = tid >= kFX ? tid - kFX : tid;
+#pragma unroll
+    for (int m = 0; m < 5; ++m) nb[m] = sX[m][src];
+    if (solve1) ch::riemann<S>(G, nb, wl, fl);
+#pragma unroll
+    for (int m = 0; m < 5; ++m) sF[m][tid] = fl[m];
+    __syncthreads();
+    if (need2) {
+      const int dst = tid + kFX;
+      // y-local order (rho, my, mz, mx, E) -> global
+      part[0] += dtx[1] * (fl[0] - sF[0][dst]);
+      part[2] += dtx[1] * (fl[1] - sF[1][dst]);
+      part[3] += dtx[1] * (fl[2] - sF[2][dst]);
+      part[1] += dtx[1] * (fl[3] - sF[3][dst]);
+      part[4] += dtx[1] * (fl[4] - sF[4][dst]);
+    }
+  }
+  double t = 0.0;
+  bool bad = false;
+  if (need2) {
+    A.u[q] = part[0]; A.u[np + q] = part[1]; A.u[2 * np + q] = part[2]; A.u[3 * np + q] = part[3]; A.u[4 * np + q] = part[4];
+    t = cell_rate(A, part[0], part[1], part[2], part[3], part[4], bad);
+  }
+  block_max_reduce(t, bad, A.red);
+}
+
+// ---------------------------------------------------------------------------------------------
 // TMA-fed form of k_final3d (used when the padded strides meet TMA's 16-byte rules).  Same tile, same
 // arithmetic, same exchanges; what changes is how a plane's 50 doubles per cell reach the SM: a
 // producer warp streams them as ten 4-D boxes {32 x, kTY y, 1 z, 5 fields} per plane
@@ -1379,7 +1475,9 @@ struct ch_ctx {
   // ch_step_cfl replays the kernels of a step as a CUDA graph (captured on a private stream the second time a
   // configuration is stepped): on small grids the step is launch bound
   bool use_graph = true;
-  cudaStream_t cap_stream = nullptr;
+  cudaStream_t cap_stream = nullptr, cap_side[2] = {nullptr, nullptr};   // the y and z sweeps of pass 1 are parallel branches of the graph
+  cudaEvent_t cap_fork = nullptr, cap_join[2] = {nullptr, nullptr};
+  bool capturing = false;
   cudaGraphExec_t gexec = nullptr;
   long long gkey[8] = {-1, -1, -1, -1, -1, -1, -1, -1};   // configuration the graph / the last direct step belongs to
   double gdx[3] = {0, 0, 0};
@@ -1642,6 +1740,11 @@ int ch_free(ch_ctx* c) {
   DeviceGuard guard(c->device);
   drop_graph(c);
   if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
+  for (int i = 0; i < 2; ++i) {
+    if (c->cap_side[i]) cudaStreamDestroy(c->cap_side[i]);
+    if (c->cap_join[i]) cudaEventDestroy(c->cap_join[i]);
+  }
+  if (c->cap_fork) cudaEventDestroy(c->cap_fork);
   if (c->h_red) cudaFreeHost(c->h_red);
   for (int k = 0; k < 2 * CH_K_COUNT; ++k) if (c->ev[k]) cudaEventDestroy(c->ev[k]);
   delete c;
@@ -1792,6 +1895,14 @@ int step_impl(ch_ctx* c, double dt, bool devdt) {
       ++c->launches;     // two launches under one bracket
     }
   } else {
+  // The three sweeps of pass 1 are independent (each reads u, writes its own arrays).  While a step is being captured
+  // into a graph (launch-bound grids only) the y and z sweeps go to side streams: parallel branches of the graph.
+  const bool fork = c->capturing && c->cap_side[0] && c->cap_side[1];
+  if (fork) {
+    cudaEventRecord(c->cap_fork, st);
+    cudaStreamWaitEvent(c->cap_side[0], c->cap_fork, 0);
+    cudaStreamWaitEvent(c->cap_side[1], c->cap_fork, 0);
+  }
   if (g.act[0]) {
     // flat run of padded cells from the first needed row to the last: rows j,k in [-1, n]
     const int j0 = g.act[1] ? g.g[1] - 1 : 0, k0 = g.act[2] ? g.g[2] - 1 : 0;
@@ -1810,8 +1921,15 @@ int step_impl(ch_ctx* c, double dt, bool devdt) {
     const int seg = march_segment(c, d);
     dim3 grid((unsigned)((cols + CH_MARCH_T - 1) / CH_MARCH_T), (unsigned)((g.n[d] + 2 * A.ext - 1 + seg - 1) / seg));
     Bracket b(c, d == 1 ? CH_K_PASS1_Y : CH_K_PASS1_Z);
-    if (d == 1) k_pass1_march<1, S, R><<<grid, CH_MARCH_T, 0, st>>>(A, seg);
-    else k_pass1_march<2, S, R><<<grid, CH_MARCH_T, 0, st>>>(A, seg);
+    cudaStream_t sd = fork ? c->cap_side[d - 1] : st;
+    if (d == 1) k_pass1_march<1, S, R><<<grid, CH_MARCH_T, 0, sd>>>(A, seg);
+    else k_pass1_march<2, S, R><<<grid, CH_MARCH_T, 0, sd>>>(A, seg);
+  }
+  if (fork) {
+    for (int i = 0; i < 2; ++i) {
+      cudaEventRecord(c->cap_join[i], c->cap_side[i]);
+      cudaStreamWaitEvent(st, c->cap_join[i], 0);
+    }
   }
   }
   CH_CUDA(cudaGetLastError(), "pass 1");
@@ -1839,6 +1957,10 @@ int step_impl(ch_ctx* c, double dt, bool devdt) {
     Bracket b(c, CH_K_FINAL);
     k_final3d<S><<<grid, kFT, smem, st>>>(A, seg);
     }
+  } else if (g.act[0] && g.act[1] && !g.act[2] && !c->unfused && !c->hcorr) {
+    dim3 grid((unsigned)((g.n[0] + kFX - 3) / (kFX - 2)), (unsigned)((g.n[1] + kFY - 3) / (kFY - 2)), 1);
+    Bracket b(c, CH_K_FINAL);
+    k_final2d<S><<<grid, kFT, 0, st>>>(A);
   } else {
     {
       const long long cells = (long long)(g.act[0] ? g.n[0] + 1 : 1) * (g.act[1] ? g.n[1] + 1 : 1) * (g.act[2] ? g.n[2] + 1 : 1);
@@ -1930,13 +2052,22 @@ int ch_step_cfl(ch_ctx* c, double cfl, double t_left) {
     return CH_OK;
   }
   if (c->gseen++ == 0) return step_dispatch(c, 0.0, true);
-  if (!c->cap_stream) CH_CUDA(cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking), "cudaStreamCreate");
+  if (!c->cap_stream) {
+    CH_CUDA(cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking), "cudaStreamCreate");
+    for (int i = 0; i < 2; ++i) {
+      CH_CUDA(cudaStreamCreateWithFlags(&c->cap_side[i], cudaStreamNonBlocking), "cudaStreamCreate");
+      CH_CUDA(cudaEventCreateWithFlags(&c->cap_join[i], cudaEventDisableTiming), "cudaEventCreate");
+    }
+    CH_CUDA(cudaEventCreateWithFlags(&c->cap_fork, cudaEventDisableTiming), "cudaEventCreate");
+  }
   cudaStream_t user = c->stream;
   const long long before = c->launches;
   cudaGraph_t graph = nullptr;
   CH_CUDA(cudaStreamBeginCapture(c->cap_stream, cudaStreamCaptureModeThreadLocal), "cudaStreamBeginCapture");
   c->stream = c->cap_stream;
+  c->capturing = true;
   const int rc = step_dispatch(c, 0.0, true);
+  c->capturing = false;
   c->stream = user;
   cudaError_t e = cudaStreamEndCapture(c->cap_stream, &graph);
   c->glaunches = c->launches - before;
