@@ -178,6 +178,8 @@ class RankBlockGrid:
             raise ValueError("world size must equal the number of blocks")
         t = self.topo
         self.device = device
+        # gloo moves host tensors only: slabs are staged through the host there; NCCL sends device tensors as they are
+        self.wire = "cpu" if dist.get_backend() == "gloo" else device
         self.G = grid_factory(*t.block_shape(self.rank), nghost, gamma, t.block_bc(self.rank), device)
         if hasattr(self.G, "set_origin"):
             self.G.set_origin(*t.origin(self.rank))
@@ -196,12 +198,15 @@ class RankBlockGrid:
                 if src == self.rank:
                     buf = torch.empty(5 * G.halo_cells(d), dtype=torch.float64, device=self.device)
                     G.halo_pack(sf, buf)
-                    sends.append((dst, df, buf))
+                    sends.append([dst, df, buf])
                 if dst == self.rank:
-                    buf = torch.empty(5 * G.halo_cells(d), dtype=torch.float64, device=self.device)
-                    recvs.append((src, df, buf))
+                    buf = torch.empty(5 * G.halo_cells(d), dtype=torch.float64, device=self.wire)
+                    recvs.append([src, df, buf])
             if hasattr(G, "sync"):
                 G.sync()                                            # packed slabs complete before they are sent
+            if self.wire != self.device:
+                for s_ in sends:
+                    s_[2] = s_[2].to(self.wire)
             local = []
             for dst, df, buf in sends:
                 if dst == self.rank:
@@ -217,8 +222,12 @@ class RankBlockGrid:
             for src, df, buf in recvs:
                 if src == self.rank:
                     buf = next(b for f, b in local if f == df)
+                if str(buf.device) != str(torch.device(self.device)):
+                    buf = buf.to(self.device)
                 G.halo_unpack(df, buf)
                 self.messages += 1
+            if hasattr(G, "sync") and self.wire != self.device:
+                G.sync()                                            # staged copies stay alive until they are unpacked
             G.fill_dim(d)
 
     def set_state(self, u_global):
@@ -228,7 +237,7 @@ class RankBlockGrid:
 
     def compute_dt(self, cfl) -> float:
         import torch
-        t = torch.tensor([self.G.compute_dt(cfl)], dtype=torch.float64, device=self.device)
+        t = torch.tensor([self.G.compute_dt(cfl)], dtype=torch.float64, device=self.wire)
         nan = torch.isnan(t).to(torch.float64)
         self.dist.all_reduce(t, op=self.dist.ReduceOp.MIN)
         self.dist.all_reduce(nan, op=self.dist.ReduceOp.MAX)        # a NaN on any rank must reach every rank

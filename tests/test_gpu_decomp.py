@@ -105,3 +105,57 @@ def test_messages_per_block_and_refusals(ch):
     with pytest.raises(RuntimeError):
         B.grids[0].step_cfl(0.4)                                  # a block needs the global minimum of dt
     B.close()
+
+
+def _gpu_rank(rank, world, port, shape, blocks, steps, out):
+    import os
+    import torch
+    import torch.distributed as dist
+    import paper_1410_4194_b200 as pkg
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    torch.cuda.set_device(0)
+    w = wl.sweep(shape=shape)
+    G = decomp.RankBlockGrid(shape, blocks, 3, w.gamma, w.bc,
+                             lambda nx, ny, nz, g, gamma, bc, dev: pkg.Grid(nx, ny, nz, g, gamma, bc, device=dev), dist, device="cuda:0")
+    G.G.set_spacing(*(1.0 / shape[0],) * 3)
+    G.set_state(w.u)
+    dts = []
+    for _ in range(steps):
+        dt = G.compute_dt(w.cfl)
+        dts.append(dt)
+        G.step(dt)
+    np.save(os.path.join(out, f"r{rank}.npy"), G.get_local_state())
+    np.save(os.path.join(out, f"dt{rank}.npy"), np.array(dts))
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+def test_one_block_per_rank_with_the_real_library(ch, tmp_path):
+    """RankBlockGrid (one block per torch.distributed rank: point-to-point slabs, all-reduce(MIN) of dt) driving the
+    CUDA library: two host processes, both on this one GPU, gloo between them (slabs staged through the host; the
+    ranks' kernels never wait on one another — each process blocks on the host in send / recv).  Periodic with two
+    blocks: both faces of a rank talk to the other rank.  Result = the undivided grid, bit for bit."""
+    import socket
+    import torch.multiprocessing as mp
+    shape, blocks, steps = (32, 24, 20), (2, 1, 1), 3
+    w = wl.sweep(shape=shape)
+    S = ch.Grid(*shape, 3, w.gamma, w.bc)
+    S.set_state(w.u)
+    dts = []
+    for _ in range(steps):
+        dt = S.compute_dt(w.cfl)
+        dts.append(dt)
+        S.step(dt)
+    want = S.get_state()
+    S.close()
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    mp.spawn(_gpu_rank, args=(2, port, shape, blocks, steps, str(tmp_path)), nprocs=2, join=True)
+    topo = decomp.Topology(shape, blocks, w.bc)
+    for r in range(2):
+        (x0, x1), (y0, y1), (z0, z1) = topo.extent(r)
+        assert np.array_equal(np.load(tmp_path / f"r{r}.npy"), want[:, z0:z1, y0:y1, x0:x1])
+        assert np.load(tmp_path / f"dt{r}.npy").tolist() == dts
