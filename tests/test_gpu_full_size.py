@@ -262,3 +262,26 @@ def test_shock_cloud_256_500_steps_stays_physical():
     front = np.max(np.nonzero(line > 0.2)[0]) + 1
     want = 16 + 204.12414523 * t * 256
     assert abs(front - want) <= 2.5, (front, want, t)
+
+
+def test_sweep_128_100_steps_match_the_oracle(ref):
+    """BASELINE.json config 5 as it is stated — 100 steps at CFL 0.4 — at the size the oracle can run in full
+    (128^3, ~90 s of the box's host cores): relative L1 per field <= 1e-8 at the end, lock-step (the oracle's dt fed
+    to the GPU) and free-running (its own Eq. 22 every step), and the two clocks agree."""
+    import paper_1410_4194_b200 as ch
+    w = wl.sweep(128)
+    w.steps = 100
+    Rg = ref.RefGrid(128, 128, 128, 3, w.gamma, w.bc)
+    dts = []
+    run(Rg, w, record_dts=dts)
+    ur = Rg.get_state()
+    G = ch.Grid(128, 128, 128, 3, w.gamma, w.bc)
+    run(G, w, dts=dts)
+    e_lock = rel_l1_error(G.get_state(), ur, w.gamma)
+    gdts = []
+    run(G, w, record_dts=gdts)
+    e_free = rel_l1_error(G.get_state(), ur, w.gamma)
+    G.close()
+    print("sweep 128^3 x 100 steps: rel L1 lock-step", e_lock, "free-running", e_free)
+    assert len(dts) == 100 and max(e_lock) <= RUN_L1_TOL and max(e_free) <= RUN_L1_TOL
+    assert np.allclose(gdts, dts, rtol=1e-9, atol=0)
