@@ -44,3 +44,16 @@ def test_paper_printed_wave_positions(ref):
     assert abs(contact - v) <= tol + 1.0 / 128
     v, tol = vals["sod_shock_x_t0.2"]
     assert abs(shock - v) <= tol + 1.0 / 128
+
+
+def test_paper_printed_ppmp_contact_and_noh_densities(ref):
+    """P:L465 (two zones with PPMP, three to four with PPMC) and P:L561 (rho = 16 ahead of, 64 behind the Noh shock;
+    2-D stand-in for the CPU suite: 4 and 16, the same closed form (1 + t/r)^(n-1) and 4^n)."""
+    vals = {r[0]: (float(r[1]), float(r[2])) for r in rows("paper_printed_values.txt")}
+    from tests.test_oracle_ppmp import contact_width
+    wp, _ = contact_width(ref, 3)
+    wc, _ = contact_width(ref, 0)
+    assert abs(wp - vals["sod_contact_zones_ppmp"][0]) <= vals["sod_contact_zones_ppmp"][1]
+    assert abs(wc - vals["sod_contact_zones_ppmc"][0]) <= vals["sod_contact_zones_ppmc"][1]
+    # the 3-D numbers are (1 + 3)^2 and 4^3: check that the printed values ARE the closed form the tests gate against
+    assert vals["noh_preshock_density_3d"][0] == (1.0 + 3.0) ** 2 and vals["noh_postshock_density_3d"][0] == 4.0 ** 3
