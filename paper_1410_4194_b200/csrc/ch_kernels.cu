@@ -990,7 +990,11 @@ __global__ void __launch_bounds__(kTT, 1) k_final3d_tma(const StepArgs A, const 
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5, row = wid + 1;
   const int sidx = row * kFX + lane;                   // this thread's slot in the staged and exchanged arrays
   const int nx = g.n[0], ny = g.n[1], nz = g.n[2];
-  const int i0 = (int)blockIdx.x * (kFX - 2) - 1, j0 = (int)blockIdx.y * (kTY - 2) - 1;
+  // With an even nghost the box of a 30-column tile would start on an odd double (not 16-byte aligned, the bulk copy
+  // faults): such grids shift the tile by one lane at each end (xs = 1): lane 0 and lane 31 idle, lane 1 supplies the
+  // left state, lanes 2..29 update, lane 30 supplies the flux; the box then starts at 28 b - 2 + nghost, an even double.
+  const int xs = (g.g[0] & 1) ? 0 : 1;
+  const int i0 = (int)blockIdx.x * (kFX - 2 - 2 * xs) - 1 - xs, j0 = (int)blockIdx.y * (kTY - 2) - 1;
   const int k0 = (int)blockIdx.z * seg;
   const int k1 = min(k0 + seg, nz);
   unsigned bfull[4], bempty[4];
@@ -1032,7 +1036,7 @@ __global__ void __launch_bounds__(kTT, 1) k_final3d_tma(const StepArgs A, const 
   if (wid == kTY - 2) {
     // ----- halo warp: rows 0 and kTY-1 of the tile -----
     const int ih = i0 + lane, jt = j0 + kTY - 1, st_ = (kTY - 1) * kFX + lane;
-    const bool laneok = lane >= 1 && lane <= kFX - 2 && ih >= 0 && ih < nx;
+    const bool laneok = lane >= 1 + xs && lane <= kFX - 2 - xs && ih >= 0 && ih < nx;
     const bool topok = laneok && jt <= ny && jt >= 0;
     const double hxh = 0.5 * dtx[0], hzh = 0.5 * dtx[2];
     double zSb[5] = {0.0, 0.0, 0.0, 0.0, 0.0}, zSt[5] = {0.0, 0.0, 0.0, 0.0, 0.0};   // F*_z of the previous plane, both rows
@@ -1083,9 +1087,9 @@ __global__ void __launch_bounds__(kTT, 1) k_final3d_tma(const StepArgs A, const 
   const int i = i0 + lane, j = j0 + row;
   const bool valid = i <= nx && j <= ny;
   const bool realI = i >= 0 && i < nx, realJ = j >= 0 && j < ny;
-  const bool updL = lane >= 1 && lane <= kFX - 2 && realI, updR = realJ;
-  const bool need0 = valid && updR, need1 = valid && updL, need2 = updL && updR;
-  const bool solve0 = need0 && lane >= 1 && i >= 0, solve1 = need1 && row >= 1 && j >= 0;
+  const bool updL = lane >= 1 + xs && lane <= kFX - 2 - xs && realI, updR = realJ;
+  const bool need0 = valid && updR && lane >= xs, need1 = valid && updL, need2 = updL && updR;
+  const bool solve0 = need0 && lane >= 1 + xs && i >= 0, solve1 = need1 && row >= 1 && j >= 0;
   const long long np = g.np, s2 = g.st[2];
   const long long qcol = (long long)(i + g.g[0]) + (long long)(j + g.g[1]) * g.st[1] + (long long)g.g[2] * s2;
   const double hx = 0.5 * dtx[0], hy = 0.5 * dtx[1], hz = 0.5 * dtx[2];
@@ -1631,9 +1635,7 @@ bool build_tma_maps(ch_ctx* c) {
   const Geom& g = c->geo;
   if (!(g.act[0] && g.act[1] && g.act[2])) return false;
   if ((g.pd[0] & 1) || (g.np & 1)) return false;
-  // a tile's box starts at padded x = 30 b - 1 + nghost: with an even nghost that is an odd number of doubles, a
-  // start address that is not 16-byte aligned, which the bulk tensor copy faults on (observed: nghost = 4)
-  if (!(g.g[0] & 1)) return false;
+  // (a tile's box must start on an even double: with an even nghost the kernel shifts its tiles, see tma_pitch_x)
   typedef CUresult (*EncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
                                const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
                                CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
@@ -1662,6 +1664,10 @@ bool build_tma_maps(ch_ctx* c) {
   return true;
 }
 
+// Updated columns per tile of k_final3d_tma: 30 with an odd nghost, 28 with an even one (the box must start on an
+// even double: 16-byte alignment of the bulk tensor copy).
+int tma_pitch_x(const Geom& g) { return (g.g[0] & 1) ? kFX - 2 : kFX - 4; }
+
 // Interfaces a thread of the marching pass-1 kernel sweeps along d: enough segments to fill the chip on small grids
 // (a segment costs ~1.5 cells of warm-up), 64 on large ones; CH_OPT_MARCH_SEG overrides.
 int march_segment(const ch_ctx* c, int d) {
@@ -1681,7 +1687,8 @@ int final_segment(const ch_ctx* c) {
   const Geom& g = c->geo;
   if (c->final_seg) return c->final_seg;
   const bool tma = c->tma_ok && c->use_tma;
-  const long long tiles = (long long)((g.n[0] + kFX - 3) / (kFX - 2)) * ((g.n[1] + (tma ? kTY : kFY) - 3) / ((tma ? kTY : kFY) - 2));
+  const int px = tma ? tma_pitch_x(g) : kFX - 2;
+  const long long tiles = (long long)((g.n[0] + px - 1) / px) * ((g.n[1] + (tma ? kTY : kFY) - 3) / ((tma ? kTY : kFY) - 2));
   const long long want = tiles * g.n[2] / (148LL * 4);
   int seg = 8;
   while (seg < 64 && seg * 2 <= want) seg *= 2;
@@ -1944,7 +1951,8 @@ int step_impl(ch_ctx* c, double dt, bool devdt) {
         CH_CUDA(cudaFuncSetAttribute(k_final3d_tma<S>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tsmem), "k_final3d_tma smem attribute");
         c->smem_attr[1][S] = true;
       }
-      dim3 tgrid((unsigned)((g.n[0] + kFX - 3) / (kFX - 2)), (unsigned)((g.n[1] + kTY - 3) / (kTY - 2)),
+      const int pitch = tma_pitch_x(g);
+      dim3 tgrid((unsigned)((g.n[0] + pitch - 1) / pitch), (unsigned)((g.n[1] + kTY - 3) / (kTY - 2)),
                  (unsigned)((g.n[2] + seg - 1) / seg));
       Bracket b(c, CH_K_FINAL);
       k_final3d_tma<S><<<tgrid, kTT, tsmem, st>>>(A, c->maps, seg);
@@ -2138,7 +2146,7 @@ int ch_tiling(const ch_ctx* c, int* out) {
   out[1] = CH_MARCH_T;                     // columns per CTA of the marching kernels
   out[2] = march_segment(c, 1);            // interfaces a marching thread sweeps along y
   out[3] = march_segment(c, 2);            // ... along z
-  out[4] = three_d ? kFX - 2 : 0;          // updated columns per tile of the fused second half along x
+  out[4] = three_d ? (tma ? tma_pitch_x(g) : kFX - 2) : 0;   // updated columns per tile of the fused second half along x
   out[5] = three_d ? (tma ? kTY : kFY) - 2 : 0;   // ... along y
   out[6] = three_d ? final_segment(c) : 0; // planes a CTA of the fused second half marches
   out[7] = tma ? 1 : 0;
