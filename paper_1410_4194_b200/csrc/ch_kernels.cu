@@ -214,6 +214,77 @@ __global__ void __launch_bounds__(CH_MARCH_T, CH_MARCH_MINB) k_pass1_march(const
   }
 }
 
+// The same march for PPMP (A.4): the thread carries the seven primitive cells c-3 .. c+3 its reconstruction reads
+// (formed with IEEE operations in the global component order, reading S21), calls the same ppmp_faces the
+// gathered-stencil kernel calls, and solves interface c-1/2 with the previous cell's right face.  y and z only (the x
+// sweep keeps the gathered form: k_faces_wide<0> + k_riemann1<0>).
+template <int D, int S>
+__global__ void __launch_bounds__(CH_MARCH_T, 2) k_pass1_march_ppmp(const StepArgs A, int seg) {
+  if (step_refused(A)) return;
+  constexpr int T = 3 - D;
+  const Geom& g = A.geo;
+  const Gas& G = A.gas;
+  const int ext0 = g.act[0] ? g.n[0] + 2 : 1, lo0 = g.act[0] ? -1 : 0;
+  const int extT = g.act[T] ? g.n[T] + 2 : 1, loT = g.act[T] ? -1 : 0;
+  const long long col = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (col >= (long long)ext0 * extT) return;
+  const int i = lo0 + (int)(col % ext0);
+  const int t = loT + (int)(col / ext0);
+  const int c0 = -1 + (int)blockIdx.y * seg;
+  const int nD = g.n[D];
+  int c1 = c0 + seg;
+  const int cend = nD;
+  const bool last = c1 >= cend;
+  if (last) c1 = cend;
+  const long long sD = g.st[D], np = g.np;
+  const long long base = (long long)(i + g.g[0]) + (long long)(t + g.g[T]) * g.st[T] + (long long)g.g[D] * sD;
+  const double dtdx = step_dtdx1(A, D);
+  const double* __restrict__ u = A.u;
+  double w[7][5], pr_prev[5], raw[5];
+#pragma unroll
+  for (int s = 0; s < 6; ++s) {
+    const long long qs = base + (long long)(c0 - 3 + s) * sD;
+    double wg[5];
+    ch::cons2prim_ieee(G, u[qs], u[np + qs], u[2 * np + qs], u[3 * np + qs], u[4 * np + qs], wg);
+#pragma unroll
+    for (int m = 0; m < 5; ++m) w[s][m] = wg[comp<D>(m)];
+  }
+  {
+    const long long qs = base + (long long)(c0 + 3) * sD;
+#pragma unroll
+    for (int f = 0; f < 5; ++f) raw[f] = u[f * np + qs];
+  }
+  for (int c = c0; c <= c1; ++c) {
+    const long long q = base + (long long)c * sD;
+    {
+      double wg[5];
+      ch::cons2prim_ieee(G, raw[0], raw[1], raw[2], raw[3], raw[4], wg);
+#pragma unroll
+      for (int m = 0; m < 5; ++m) w[6][m] = wg[comp<D>(m)];
+    }
+    if (c < c1) {                                           // cell c+4 <= n_D+3: inside the padded store (nghost >= 4)
+#pragma unroll
+      for (int f = 0; f < 5; ++f) raw[f] = u[f * np + q + 4 * sD];
+    }
+    double WLs[5], WRs[5], cl[5], cr[5];
+    ch::ppmp_faces(G, dtdx, w, WLs, WRs);
+    ch::prim2cons(G, WLs, cl);
+    ch::prim2cons(G, WRs, cr);
+    if (c < c1 || last) {
+      store_local<D>(A.UL[D], np, q, cl);
+      store_local<D>(A.UR[D], np, q, cr);
+    }
+    if (c > c0) {
+      double fl[5];
+      ch::riemann<S>(G, pr_prev, WLs, fl);
+      store_local<D>(A.Fs[D], np, q - sD, fl);
+    }
+    copy5(pr_prev, WRs);
+#pragma unroll
+    for (int s = 0; s < 6; ++s) copy5(w[s], w[s + 1]);
+  }
+}
+
 // ---------------------------------------------------------------------------------------------
 // Pass 1 along x: one thread per padded cell of a flat run of memory (x fastest, rows follow one
 // another), neighbours exchanged through shared memory in three stages (primitives -> slopes ->
@@ -1896,10 +1967,17 @@ int step_impl(ch_ctx* c, double dt, bool devdt) {
     for (int d = 0; d < 3; ++d) {
       if (!g.act[d]) continue;
       Bracket b(c, d == 0 ? CH_K_PASS1_X : d == 1 ? CH_K_PASS1_Y : CH_K_PASS1_Z);
-      if (d == 0) { k_faces_wide<0, R><<<nb, 128, 0, st>>>(A); k_riemann1<0, S><<<nb, 128, 0, st>>>(A); }
-      else if (d == 1) { k_faces_wide<1, R><<<nb, 128, 0, st>>>(A); k_riemann1<1, S><<<nb, 128, 0, st>>>(A); }
-      else { k_faces_wide<2, R><<<nb, 128, 0, st>>>(A); k_riemann1<2, S><<<nb, 128, 0, st>>>(A); }
-      ++c->launches;     // two launches under one bracket
+      if (d == 0) {
+        k_faces_wide<0, R><<<nb, 128, 0, st>>>(A); k_riemann1<0, S><<<nb, 128, 0, st>>>(A);
+        ++c->launches;     // two launches under one bracket
+      } else {
+        const int T = 3 - d;
+        const long long cols = (long long)(g.act[0] ? g.n[0] + 2 : 1) * (g.act[T] ? g.n[T] + 2 : 1);
+        const int seg = march_segment(c, d);
+        dim3 grid((unsigned)((cols + CH_MARCH_T - 1) / CH_MARCH_T), (unsigned)((g.n[d] + 1 + seg - 1) / seg));
+        if (d == 1) k_pass1_march_ppmp<1, S><<<grid, CH_MARCH_T, 0, st>>>(A, seg);
+        else k_pass1_march_ppmp<2, S><<<grid, CH_MARCH_T, 0, st>>>(A, seg);
+      }
     }
   } else {
   // The three sweeps of pass 1 are independent (each reads u, writes its own arrays).  While a step is being captured
