@@ -216,8 +216,8 @@ __global__ void __launch_bounds__(CH_MARCH_T, CH_MARCH_MINB) k_pass1_march(const
 
 // The same march for PPMP (A.4): the thread carries the seven primitive cells c-3 .. c+3 its reconstruction reads
 // (formed with IEEE operations in the global component order, reading S21), calls the same ppmp_faces the
-// gathered-stencil kernel calls, and solves interface c-1/2 with the previous cell's right face.  y and z only (the x
-// sweep keeps the gathered form: k_faces_wide<0> + k_riemann1<0>).
+// x-sweep kernel calls, and solves interface c-1/2 with the previous cell's right face.  y and z; the x sweep is
+// k_pass1_x_ppmp.
 template <int D, int S>
 __global__ void __launch_bounds__(CH_MARCH_T, 2) k_pass1_march_ppmp(const StepArgs A, int seg) {
   if (step_refused(A)) return;
@@ -372,72 +372,63 @@ __global__ void __launch_bounds__(kXT, CH_X_MINB) k_pass1_x(const StepArgs A, lo
 }
 
 // ---------------------------------------------------------------------------------------------
-// Pass 1 for the reconstructions in the primitive variables (PPMP: 7-cell stencil, g >= 4; PLMP: 3 cells),
-// a "next" row of SURVEY.md section 8(f): one thread per cell of [-1, n]^3 gathers its stencil along D (consecutive
-// lanes = consecutive x, so every load of the gather is a coalesced row segment and the re-reads of neighbouring
-// cells come from L1/L2), forms W*_L, W*_R and stores them conserved; k_riemann1 then solves the
-// interfaces.  Not marched: these kernels exist for completeness of the paper's method set, the headline path is
-// PPMC through k_pass1_x / k_pass1_march.
-// ---------------------------------------------------------------------------------------------
-template <int D, int R>     // R: 3 PPMP, 4 PLMP
-__global__ void __launch_bounds__(128) k_faces_wide(const StepArgs A) {
+// Pass 1 along x for PPMP: the flat-run form of k_pass1_x with the 7-cell stencil read from shared memory.  A CTA of
+// kXT threads stages kXT primitive cells (IEEE, reading S21), threads 3 .. kXT-4 form their cell's faces with the
+// same ppmp_faces as the marching kernels, exchange the left faces, and threads 3 .. kXT-5 solve interface i+1/2.
+constexpr int kXOutP = kXT - 7;   // interfaces produced per CTA
+template <int S>
+__global__ void __launch_bounds__(kXT, 3) k_pass1_x_ppmp(const StepArgs A, long long q_begin, long long q_end) {
+  __shared__ double sP[5][kXT];
+  __shared__ double sL[5][kXT];
   if (step_refused(A)) return;
   const Geom& g = A.geo;
-  const int e0 = g.act[0] ? g.n[0] + 2 : 1, e1 = g.act[1] ? g.n[1] + 2 : 1, e2 = g.act[2] ? g.n[2] + 2 : 1;
-  const long long id = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (id >= (long long)e0 * e1 * e2) return;
-  const int i = (int)(id % e0) - (g.act[0] ? 1 : 0);
-  const long long r = id / e0;
-  const int j = (int)(r % e1) - (g.act[1] ? 1 : 0), k = (int)(r / e1) - (g.act[2] ? 1 : 0);
-  const long long np = g.np, sD = g.st[D];
-  const long long q = (long long)(i + g.g[0]) + (long long)(j + g.g[1]) * g.st[1] + (long long)(k + g.g[2]) * g.st[2];
-  const double dtdx = step_dtdx1(A, D);
-  constexpr int H = R == 3 ? 3 : 1;     // half width of the stencil
-  double w[7][5];
-#pragma unroll
-  for (int s = 0; s < 7; ++s) {
-    if (s < 3 - H || s > 3 + H) {
-#pragma unroll
-      for (int m = 0; m < 5; ++m) w[s][m] = 0.0;
-      continue;
-    }
-    const long long qs = q + (long long)(s - 3) * sD;
-    // primitives exactly as Eq. 6-8 read in the global component order (IEEE operations): PPMP's thresholds see them
-    double wg[5];
-    ch::cons2prim_ieee(A.gas, A.u[qs], A.u[np + qs], A.u[2 * np + qs], A.u[3 * np + qs], A.u[4 * np + qs], wg);
-#pragma unroll
-    for (int m = 0; m < 5; ++m) w[s][m] = wg[comp<D>(m)];
-  }
-  double WLs[5], WRs[5], cl[5], cr[5];
-  if (R == 3) ch::ppmp_faces(A.gas, dtdx, w, WLs, WRs);
-  else ch::plmp_faces(A.gas, dtdx, w[2], w[3], w[4], WLs, WRs);
-  ch::prim2cons(A.gas, WLs, cl);
-  ch::prim2cons(A.gas, WRs, cr);
-  store_local<D>(A.UL[D], np, q, cl);
-  store_local<D>(A.UR[D], np, q, cr);
-}
-
-// First Riemann pass over stored face states: F*_D at interface c+1/2, c in [-1, n_D - 1], transverse range [-1, n].
-template <int D, int S>
-__global__ void __launch_bounds__(128) k_riemann1(const StepArgs A) {
-  if (step_refused(A)) return;
-  const Geom& g = A.geo;
-  int e[3] = {g.act[0] ? g.n[0] + 2 : 1, g.act[1] ? g.n[1] + 2 : 1, g.act[2] ? g.n[2] + 2 : 1};
-  e[D] -= 1;
-  const long long id = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (id >= (long long)e[0] * e[1] * e[2]) return;
-  const int i = (int)(id % e[0]) - (g.act[0] ? 1 : 0);
-  const long long r = id / e[0];
-  const int j = (int)(r % e[1]) - (g.act[1] ? 1 : 0), k = (int)(r / e[1]) - (g.act[2] ? 1 : 0);
+  const double dtdx0 = step_dtdx1(A, 0);
+  const Gas& G = A.gas;
   const long long np = g.np;
-  const long long q = (long long)(i + g.g[0]) + (long long)(j + g.g[1]) * g.st[1] + (long long)(k + g.g[2]) * g.st[2];
-  double ul[5], ur[5], wl[5], wr[5], fl[5];
-  load_raw<D>(A.UR[D], np, q, ul);
-  load_raw<D>(A.UL[D], np, q + g.st[D], ur);
-  ch::cons2prim(A.gas, ul[0], ul[1], ul[2], ul[3], ul[4], wl);
-  ch::cons2prim(A.gas, ur[0], ur[1], ur[2], ur[3], ur[4], wr);
-  ch::riemann<S>(A.gas, wl, wr, fl);
-  store_local<D>(A.Fs[D], np, q, fl);
+  const int tid = threadIdx.x;
+  const long long q = q_begin + (long long)blockIdx.x * kXOutP + tid - 3;
+  const bool inb = (q >= 0 && q < np);
+  int i = 0, j = 0, k = 0;
+  if (inb) {
+    long long r = q;
+    k = (int)(r / g.st[2]); r -= (long long)k * g.st[2];
+    j = (int)(r / g.st[1]);
+    i = (int)(r - (long long)j * g.st[1]);
+    i -= g.g[0]; j -= g.g[1]; k -= g.g[2];
+  }
+  const bool row_ok = inb && (!g.act[1] || (j >= -1 && j <= g.n[1])) && (!g.act[2] || (k >= -1 && k <= g.n[2]));
+  const int nx = g.n[0];
+  double w0[5] = {1.0, 0.0, 0.0, 0.0, 1.0};
+  if (row_ok) ch::cons2prim_ieee(G, A.u[q], A.u[np + q], A.u[2 * np + q], A.u[3 * np + q], A.u[4 * np + q], w0);
+#pragma unroll
+  for (int m = 0; m < 5; ++m) sP[m][tid] = w0[m];
+  __syncthreads();
+  const bool face_ok = row_ok && tid >= 3 && tid <= kXT - 4 && i >= -1 && i <= nx;
+  double prR[5] = {1.0, 0.0, 0.0, 0.0, 1.0}, prL[5] = {1.0, 0.0, 0.0, 0.0, 1.0};
+  if (face_ok) {
+    double w[7][5], WLs[5], WRs[5], cl[5], cr[5];
+#pragma unroll
+    for (int s = 0; s < 7; ++s)
+#pragma unroll
+      for (int m = 0; m < 5; ++m) w[s][m] = sP[m][tid - 3 + s];
+    ch::ppmp_faces(G, dtdx0, w, WLs, WRs);
+    ch::prim2cons(G, WLs, cl);
+    ch::prim2cons(G, WRs, cr);
+    store_local<0>(A.UL[0], np, q, cl);
+    store_local<0>(A.UR[0], np, q, cr);
+    copy5(prL, WLs);
+    copy5(prR, WRs);
+  }
+#pragma unroll
+  for (int m = 0; m < 5; ++m) sL[m][tid] = prL[m];
+  __syncthreads();
+  if (face_ok && tid <= kXT - 5 && i <= nx - 1 && q < q_end) {
+    double wr[5], fl[5];
+#pragma unroll
+    for (int m = 0; m < 5; ++m) wr[m] = sL[m][tid + 1];
+    ch::riemann<S>(G, prR, wr, fl);
+    store_local<0>(A.Fs[0], np, q, fl);
+  }
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -1961,15 +1952,17 @@ int step_impl(ch_ctx* c, double dt, bool devdt) {
   if (!devdt) { Bracket b(c, CH_K_RESET); k_reset<<<1, 32, 0, st>>>(c->red, nullptr); }   // ch_step_cfl: k_pick_dt has done it
   // pass 1
   if constexpr (R == 3) {
-    // PPMP / PLMP: faces from the gathered stencil, then the interfaces (two launches per direction)
-    const long long cells = (long long)(g.act[0] ? g.n[0] + 2 : 1) * (g.act[1] ? g.n[1] + 2 : 1) * (g.act[2] ? g.n[2] + 2 : 1);
-    const unsigned nb = (unsigned)((cells + 127) / 128);
+    // PPMP: kernels of its own (7-cell stencil, IEEE primitives), the same shapes as the PPMC ones
     for (int d = 0; d < 3; ++d) {
       if (!g.act[d]) continue;
       Bracket b(c, d == 0 ? CH_K_PASS1_X : d == 1 ? CH_K_PASS1_Y : CH_K_PASS1_Z);
       if (d == 0) {
-        k_faces_wide<0, R><<<nb, 128, 0, st>>>(A); k_riemann1<0, S><<<nb, 128, 0, st>>>(A);
-        ++c->launches;     // two launches under one bracket
+        const int j0 = g.act[1] ? g.g[1] - 1 : 0, k0 = g.act[2] ? g.g[2] - 1 : 0;
+        const int j1 = g.act[1] ? g.g[1] + g.n[1] : 0, k1 = g.act[2] ? g.g[2] + g.n[2] : 0;
+        const long long qb = (long long)j0 * g.st[1] + (long long)k0 * g.st[2];
+        const long long qe = (long long)j1 * g.st[1] + (long long)k1 * g.st[2] + g.pd[0];
+        const long long nbx = (qe - qb + kXOutP - 1) / kXOutP;
+        k_pass1_x_ppmp<S><<<(unsigned)nbx, kXT, 0, st>>>(A, qb, qe);
       } else {
         const int T = 3 - d;
         const long long cols = (long long)(g.act[0] ? g.n[0] + 2 : 1) * (g.act[T] ? g.n[T] + 2 : 1);
