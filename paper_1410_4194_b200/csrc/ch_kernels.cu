@@ -7,11 +7,15 @@
 //   k_final3d_tma      3-D grids: Eq. 23 transverse correction + second exact Riemann pass + Eq. 24
 //   (k_final3d)        update + Eq. 22 reduction of the new state, fused (steps 3-5; F,G,H^{n+1/2} stay on
 //                      chip); planes staged by TMA from a producer warp (plain loads where TMA's
-//                      16-byte stride rules do not hold, or with CH_TMA=0)
-//   k_pass2, k_update  the same two halves unfused, for 1-D / 2-D grids
-//   k_ghost            ghost fill of the new state
-// Every kernel that reconstructs or solves is a template on the reconstruction (PPMC / PLMC / PCM) and on the
-// Riemann solver (exact / Roe + HLLE); the defaults are the paper's PPMC + exact.
+//                      16-byte stride rules do not hold, or with CH_OPT_TMA = 0)
+//   k_final2d          the same for x-y grids (one plane, no z carry)
+//   k_pass2, k_update  the same two halves unfused: 1-D, x-z / y-z grids, the H-corrected step (+ k_eta)
+//   k_ghost            ghost fill of the new state, analytic (Noh) faces included
+//   k_pick_dt          ch_step_cfl: Eq. 22 finished on the device; the step is then replayed as a CUDA graph on small grids
+//   k_halo, k_fill_dim block decomposition: halo slabs and the per-direction fill
+// Every kernel that reconstructs or solves is a template on the reconstruction (PPMC / PLMC / PCM / PLMP; PPMP has
+// pass-1 kernels of its own with the 7-cell stencil: k_pass1_x_ppmp, k_pass1_march_ppmp) and on the Riemann solver
+// (exact / Roe + HLLE); the defaults are the paper's PPMC + exact.
 // Data layout: struct-of-arrays fp64, x fastest, ghosts included; every kernel maps
 // consecutive lanes to consecutive x so loads and stores coalesce.  No operand is reshaped for
 // tensor cores: this is a stencil / ALU path.
