@@ -1161,8 +1161,12 @@ __global__ void __launch_bounds__(kTT, 1) k_final3d_tma(const StepArgs A, const 
   const double hx = 0.5 * dtx[0], hy = 0.5 * dtx[1], hz = 0.5 * dtx[2];
   // carried from the previous plane (registers: one CTA per SM leaves ~150 per thread)
   double zU[5] = {1.0, 0.0, 0.0, 0.0, 1.0};    // U^{n+1/2}_R(., z) of cell k-1, primitive, z-local order
-  double zF[5] = {0.0, 0.0, 0.0, 0.0, 0.0};    // H^{n+1/2} on the low z face of cell k-1, z-local order
-  double zP[5] = {0.0, 0.0, 0.0, 0.0, 0.0};    // u + x and y flux differences of cell k-1, global order
+  // the half of the z carry that is only read when cell k-1 is finished lives in shared memory (10 doubles per slot):
+  // 164 -> 152 registers, the scheduler has room to interleave more, 2 % off this kernel
+  Arr zFs = reinterpret_cast<Arr>(s_t + 60 * kTT);    // H^{n+1/2} on the low z face of cell k-1, z-local order
+  Arr zPs = reinterpret_cast<Arr>(s_t + 65 * kTT);    // u + x and y flux differences of cell k-1, global order
+#define zF(m) zFs[m][sidx]
+#define zP(m) zPs[m][sidx]
   double zS[5] = {0.0, 0.0, 0.0, 0.0, 0.0};    // F*_z of cell k-1 (global field order)
   int n = 0;
   for (int k = k0 - 1; k <= k1; ++k, ++n) {
@@ -1212,11 +1216,11 @@ __global__ void __launch_bounds__(kTT, 1) k_final3d_tma(const StepArgs A, const 
           // finish cell k-1 (Eq. 24): z-local order (rho, mz, mx, my, E)
           const double dtd = dtx[2];
           const long long qm = q - s2;
-          const double v0 = zP[0] + dtd * (zF[0] - flz[0]);
-          const double v1 = zP[1] + dtd * (zF[2] - flz[2]);
-          const double v2 = zP[2] + dtd * (zF[3] - flz[3]);
-          const double v3 = zP[3] + dtd * (zF[1] - flz[1]);
-          const double v4 = zP[4] + dtd * (zF[4] - flz[4]);
+          const double v0 = zP(0) + dtd * (zF(0) - flz[0]);
+          const double v1 = zP(1) + dtd * (zF(2) - flz[2]);
+          const double v2 = zP(2) + dtd * (zF(3) - flz[3]);
+          const double v3 = zP(3) + dtd * (zF(1) - flz[1]);
+          const double v4 = zP(4) + dtd * (zF(4) - flz[4]);
           A.u[qm] = v0; A.u[np + qm] = v1; A.u[2 * np + qm] = v2; A.u[3 * np + qm] = v3; A.u[4 * np + qm] = v4;
           const double t = cell_rate(A, v0, v1, v2, v3, v4, bad);
           tmin = t > tmin ? t : tmin;
@@ -1276,7 +1280,7 @@ __global__ void __launch_bounds__(kTT, 1) k_final3d_tma(const StepArgs A, const 
     }
     if (need2) {
 #pragma unroll
-      for (int m = 0; m < 5; ++m) { zU[m] = wrz[m]; zF[m] = flz[m]; zP[m] = part[m]; }
+      for (int m = 0; m < 5; ++m) { zU[m] = wrz[m]; zF(m) = flz[m]; zP(m) = part[m]; }
     }
   }
   }
@@ -2021,7 +2025,7 @@ int step_impl(ch_ctx* c, double dt, bool devdt) {
     dim3 grid((unsigned)((g.n[0] + kFX - 3) / (kFX - 2)), (unsigned)((g.n[1] + kFY - 3) / (kFY - 2)),
               (unsigned)((g.n[2] + seg - 1) / seg));
     if (c->tma_ok && c->use_tma) {
-      const size_t tsmem = (size_t)60 * kTT * sizeof(double);
+      const size_t tsmem = (size_t)70 * kTT * sizeof(double);   // 50 staged + 10 exchanged + 10 carried doubles per slot
       if (!c->smem_attr[1][S]) {
         CH_CUDA(cudaFuncSetAttribute(k_final3d_tma<S>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tsmem), "k_final3d_tma smem attribute");
         c->smem_attr[1][S] = true;
