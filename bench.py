@@ -365,7 +365,7 @@ def main():
         # with PPMC, and the second-order pair PLMC + Roe the paper quotes its 2-D figure for
         for label, solver, recon, hc in ((f"sweep_{args.size} PPMC + Roe/HLLE", 1, 0, False),
                                          (f"sweep_{args.size} PLMC + Roe/HLLE", 1, 1, False),
-                                         (f"sweep_{args.size} PPMC + Roe/HLLE + H correction (4 ghost layers, unfused second half)", 1, 0, True),
+                                         (f"sweep_{args.size} PPMC + Roe/HLLE + H correction (4 ghost layers, k_eta + fused second half)", 1, 0, True),
                                          (f"sweep_{args.size} PPMP + exact (4 ghost layers)", 0, 3, False),
                                          (f"sweep_{args.size} PLMP + exact", 0, 4, False)):
             G = pkg.Grid(args.size, args.size, args.size, 4 if (hc or recon == 3) else 3, w.gamma, w.bc, device=device)

@@ -158,7 +158,8 @@ enum {
  * second Riemann pass the Roe eigenvalues of B28 become max(|lambda|, eta^H), eta^H the largest
  * eta = |(u_R + a_R) - (u_L + a_L)| / 2 over the interface and the transverse faces of the two cells that share
  * it.  Needs nghost >= 4 (CH_EINVAL otherwise) and CH_SOLVER_ROE (ch_step returns CH_ESTATE otherwise); the
- * second half of the step then runs unfused. */
+ * second half of the step then runs as k_eta + the fused TMA kernel on 3-D grids whose strides meet TMA's rules
+ * (ch_tiling reports it), unfused (k_eta, k_pass2, k_update) elsewhere. */
 int ch_set_hcorrection(ch_ctx* ctx, int on);
 
 /* ch_set_reconstruction — select the reconstruction for later steps.  CH_EINVAL for an unknown code. */

@@ -988,7 +988,7 @@ __global__ void __launch_bounds__(kFT, 2) k_final2d(const StepArgs A) {
 #define CH_T_SLEEP 200      // ns between the producer's polls of an empty barrier
 #endif
 constexpr int kTY = CH_T_TY, kTT = kFX * kTY, kTC = kTT - kFX;   // staged rows; threads = staged slots; consumer threads
-struct TmaMaps { CUtensorMap m[10]; };              // Fs0 Fs1 Fs2 | UL2 UR2 | UL0 UR0 u | UL1 UR1
+struct TmaMaps { CUtensorMap m[13]; };              // Fs0 Fs1 Fs2 | UL2 UR2 | UL0 UR0 u | UL1 UR1 | eta0 eta1 eta2 (one field each)
 __device__ __forceinline__ constexpr int group_first(int q) { return q == 0 ? 0 : q == 1 ? 3 : q == 2 ? 5 : q == 3 ? 8 : 10; }   // arrays of group q: [first(q), first(q+1))
 
 __device__ __forceinline__ void mbar_init(unsigned bar, unsigned count) {
@@ -1037,10 +1037,14 @@ __device__ __forceinline__ void tma_load_4d(unsigned dst, const CUtensorMap* map
       ::"r"(dst), "l"(map), "r"(bar), "r"(c0), "r"(c1), "r"(c2), "r"(c3) : "memory");
 }
 
-template <int S>
+// HC (Roe solver only): the H-corrected step.  k_eta has written eta of every interface (C1); a fifth staging group
+// brings eta_x and eta_y of plane k and eta_z of the faces k-1/2 and k+1/2 (slots 70..73), every thread forms the
+// three maxima of C2 for its x, y and z interface from them (the stencil stays inside the staged box) and the Roe
+// solver takes them: the same values and the same solver as k_pass2<1, true>, so the two paths agree bitwise.
+template <int S, bool HC = false>
 __global__ void __launch_bounds__(kTT, 1) k_final3d_tma(const StepArgs A, const __grid_constant__ TmaMaps M, int seg) {
   extern __shared__ __align__(1024) double s_t[];
-  __shared__ unsigned long long s_full[4], s_empty[4];
+  __shared__ unsigned long long s_full[5], s_empty[5];
   typedef double (*Arr)[kTT];
   // staging: array a (0..9) holds its 5 fields as [f][row][lane] = [f][tid]
   Arr sX = reinterpret_cast<Arr>(s_t + 50 * kTT);
@@ -1063,15 +1067,16 @@ __global__ void __launch_bounds__(kTT, 1) k_final3d_tma(const StepArgs A, const 
   const int i0 = (int)blockIdx.x * (kFX - 2 - 2 * xs) - 1 - xs, j0 = (int)blockIdx.y * (kTY - 2) - 1;
   const int k0 = (int)blockIdx.z * seg;
   const int k1 = min(k0 + seg, nz);
-  unsigned bfull[4], bempty[4];
+  constexpr int NB = HC ? 5 : 4;
+  unsigned bfull[5], bempty[5];
 #pragma unroll
-  for (int q = 0; q < 4; ++q) {
+  for (int q = 0; q < NB; ++q) {
     bfull[q] = (unsigned)__cvta_generic_to_shared(&s_full[q]);
     bempty[q] = (unsigned)__cvta_generic_to_shared(&s_empty[q]);
   }
   if (tid == 0) {
 #pragma unroll
-    for (int q = 0; q < 4; ++q) { mbar_init(bfull[q], 1); mbar_init(bempty[q], kTC); }
+    for (int q = 0; q < NB; ++q) { mbar_init(bfull[q], 1); mbar_init(bempty[q], kTC); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncthreads();
@@ -1089,6 +1094,15 @@ __global__ void __launch_bounds__(kTT, 1) k_final3d_tma(const StepArgs A, const 
           mbar_expect_tx(bfull[q], (unsigned)((a1 - a0) * 5 * kTT * sizeof(double)));
           for (int a = a0; a < a1; ++a)
             tma_load_4d(stage + (unsigned)(a * 5 * kTT * sizeof(double)), &M.m[a], bfull[q], i0 + g.g[0], j0 + g.g[1], k + g.g[2], 0);
+          if (HC && q == 0) {
+            if (n > 0) mbar_wait_relaxed(bempty[4], (unsigned)((n - 1) & 1));
+            mbar_expect_tx(bfull[4], (unsigned)(4 * kTT * sizeof(double)));
+            const unsigned e = stage + (unsigned)(70 * kTT * sizeof(double)), es = (unsigned)(kTT * sizeof(double));
+            tma_load_4d(e, &M.m[10], bfull[4], i0 + g.g[0], j0 + g.g[1], k + g.g[2], 0);
+            tma_load_4d(e + es, &M.m[11], bfull[4], i0 + g.g[0], j0 + g.g[1], k + g.g[2], 0);
+            tma_load_4d(e + 2 * es, &M.m[12], bfull[4], i0 + g.g[0], j0 + g.g[1], k - 1 + g.g[2], 0);
+            tma_load_4d(e + 3 * es, &M.m[12], bfull[4], i0 + g.g[0], j0 + g.g[1], k + g.g[2], 0);
+          }
         }
       }
     }
@@ -1122,6 +1136,16 @@ __global__ void __launch_bounds__(kTT, 1) k_final3d_tma(const StepArgs A, const 
         dxt[f] = __dmul_rn(hxh, __shfl_up_sync(full, fxt, 1) - fxt);
       }
       mbar_arrive(bempty[0]);
+      double eHt = 0.0;
+      if (HC) {
+        // C2 for the y interface below row kTY-1 (cells q = st_ - kFX and st_)
+        mbar_wait(bfull[4], ph);
+        const double* ex = s_t + 70 * kTT; const double* ey = ex + kTT; const double* ezm = ey + kTT; const double* ezp = ezm + kTT;
+        const int qb = st_ - kFX;
+        eHt = ch::sel_max(ey[qb], ch::sel_max(ch::sel_max(ch::sel_max(ezm[qb], ezp[qb]), ch::sel_max(ezm[st_], ezp[st_])),
+                                              ch::sel_max(ch::sel_max(ex[qb - 1], ex[qb]), ch::sel_max(ex[st_ - 1], ex[st_]))));
+        mbar_arrive(bempty[4]);
+      }
       mbar_wait(bfull[1], ph); mbar_arrive(bempty[1]);
       mbar_wait(bfull[2], ph); mbar_arrive(bempty[2]);
       mbar_wait(bfull[3], ph);
@@ -1142,7 +1166,10 @@ __global__ void __launch_bounds__(kTT, 1) k_final3d_tma(const StepArgs A, const 
         asm volatile("bar.sync 1, %0;" ::"n"(kTC) : "memory");
 #pragma unroll
         for (int m = 0; m < 5; ++m) nb[m] = sX[m][st_ - kFX];
-        if (topok) ch::riemann_tile<S>(G, nb, wlt, fl);
+        if (topok) {
+          if (HC) ch::riemann_roe(G, nb, wlt, fl, eHt);
+          else ch::riemann_tile<S>(G, nb, wlt, fl);
+        }
 #pragma unroll
         for (int m = 0; m < 5; ++m) sF[m][st_] = fl[m];
         asm volatile("bar.sync 1, %0;" ::"n"(kTC) : "memory");
@@ -1168,6 +1195,7 @@ __global__ void __launch_bounds__(kTT, 1) k_final3d_tma(const StepArgs A, const 
 #define zF(m) zFs[m][sidx]
 #define zP(m) zPs[m][sidx]
   double zS[5] = {0.0, 0.0, 0.0, 0.0, 0.0};    // F*_z of cell k-1 (global field order)
+  double mxyPrev = 0.0;                        // HC: largest eta on the x and y faces of cell k-1
   int n = 0;
   for (int k = k0 - 1; k <= k1; ++k, ++n) {
     const bool first = k == k0 - 1, tail = k == k1, mid = !first && !tail;
@@ -1196,6 +1224,23 @@ __global__ void __launch_bounds__(kTT, 1) k_final3d_tma(const StepArgs A, const 
         dF[0][f] = __dmul_rn(hx, t - fx[f]);
       }
     }
+    // ---- HC, group 4: C2 (reading G11) for this thread's three interfaces: i-1/2 and j-1/2 of plane k, k-1/2
+    double eHx = 0.0, eHy = 0.0, eHz = 0.0;
+    if (HC) {
+      mbar_wait(bfull[4], ph);
+      const double* ex = s_t + 70 * kTT; const double* ey = ex + kTT; const double* ezm = ey + kTT; const double* ezp = ezm + kTT;
+      const int qx = sidx - 1, qy = sidx - kFX;
+      const double ex0 = ex[sidx], exm = ex[qx], ey0 = ey[sidx], eym = ey[qy], ezm0 = ezm[sidx];
+      const double mz = ch::sel_max(ezm0, ezp[sidx]);
+      const double mxy = ch::sel_max(ch::sel_max(exm, ex0), ch::sel_max(eym, ey0));
+      eHx = ch::sel_max(exm, ch::sel_max(ch::sel_max(ch::sel_max(ey[qx - kFX], ey[qx]), ch::sel_max(eym, ey0)),
+                                         ch::sel_max(ch::sel_max(ezm[qx], ezp[qx]), mz)));
+      eHy = ch::sel_max(eym, ch::sel_max(ch::sel_max(ch::sel_max(ezm[qy], ezp[qy]), mz),
+                                         ch::sel_max(ch::sel_max(ex[qy - 1], ex[qy]), ch::sel_max(exm, ex0))));
+      eHz = ch::sel_max(ezm0, ch::sel_max(mxyPrev, mxy));
+      mxyPrev = mxy;
+      mbar_arrive(bempty[4]);
+    }
     // ---- group 1: z states; the neighbour is this thread's previous plane
     double wrz[5] = {1.0, 0.0, 0.0, 0.0, 1.0}, flz[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
     mbar_wait(bfull[1], ph);
@@ -1210,7 +1255,8 @@ __global__ void __launch_bounds__(kTT, 1) k_final3d_tma(const StepArgs A, const 
         if (!first) {
 #pragma unroll
           for (int m = 0; m < 5; ++m) nb[m] = zU[m];
-          ch::riemann_tile<S>(G, nb, wl, flz);
+          if (HC) ch::riemann_roe(G, nb, wl, flz, eHz);
+          else ch::riemann_tile<S>(G, nb, wl, flz);
         }
         if (k > k0) {
           // finish cell k-1 (Eq. 24): z-local order (rho, mz, mx, my, E)
@@ -1240,7 +1286,10 @@ __global__ void __launch_bounds__(kTT, 1) k_final3d_tma(const StepArgs A, const 
         if (need0) correct_faces<0>(A, ul, ur, dF, wl, wr);
 #pragma unroll
         for (int m = 0; m < 5; ++m) nb[m] = __shfl_up_sync(full, wr[m], 1);
-        if (solve0) ch::riemann_tile<S>(G, nb, wl, fl);
+        if (solve0) {
+          if (HC) ch::riemann_roe(G, nb, wl, fl, eHx);
+          else ch::riemann_tile<S>(G, nb, wl, fl);
+        }
 #pragma unroll
         for (int m = 0; m < 5; ++m) {
           const double hi = __shfl_down_sync(full, fl[m], 1);
@@ -1263,7 +1312,10 @@ __global__ void __launch_bounds__(kTT, 1) k_final3d_tma(const StepArgs A, const 
         asm volatile("bar.sync 1, %0;" ::"n"(kTC) : "memory");
 #pragma unroll
         for (int m = 0; m < 5; ++m) nb[m] = sX[m][sidx - kFX];
-        if (solve1) ch::riemann_tile<S>(G, nb, wl, fl);
+        if (solve1) {
+          if (HC) ch::riemann_roe(G, nb, wl, fl, eHy);
+          else ch::riemann_tile<S>(G, nb, wl, fl);
+        }
 #pragma unroll
         for (int m = 0; m < 5; ++m) sF[m][sidx] = fl[m];
         asm volatile("bar.sync 1, %0;" ::"n"(kTC) : "memory");
@@ -1561,6 +1613,7 @@ struct ch_ctx {
   int org[3] = {0, 0, 0};                  // global index of the first real cell (ch_set_origin)
   int device = -1;           // the device the bound buffers live on (ch_bind)
   bool smem_attr[2][2] = {{false, false}, {false, false}};   // [tma form][solver]: dynamic shared memory limit raised on `device`
+  bool smem_attr_hc = false;                                  // the same for the H-corrected form
   double* state = nullptr;
   double* ws = nullptr;
   unsigned long long* red = nullptr;
@@ -1574,7 +1627,7 @@ struct ch_ctx {
   TmaMaps maps;
   int solver = 0;            // CH_SOLVER_EXACT
   int recon = 0;             // CH_RECON_PPMC
-  bool hcorr = false;        // H correction (Appendix C): Roe solver, nghost >= 4, unfused second half
+  bool hcorr = false;        // H correction (Appendix C): Roe solver, nghost >= 4; fused second half where the TMA form applies
   bool unfused = false;      // CH_UNFUSED=1: k_pass2 + k_update on 3-D grids too (A/B measurements, instruction counts)
   // optional per-kernel timing (ch_profile): one event pair per kernel kind
   bool profiling = false;
@@ -1731,6 +1784,16 @@ bool build_tma_maps(ch_ctx* c) {
                CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
       return false;
   }
+  // eta_x, eta_y, eta_z of the H-corrected step: one field each
+  const cuuint64_t edims[4] = {(cuuint64_t)g.pd[0], (cuuint64_t)g.pd[1], (cuuint64_t)g.pd[2], 1};
+  const cuuint32_t ebox[4] = {(cuuint32_t)kFX, (cuuint32_t)kTY, 1, 1};
+  for (int d = 0; d < 3; ++d) {
+    double* e = c->ws + (long long)12 * blk + (long long)d * g.np;
+    if ((uintptr_t)e & 15) return false;
+    if (encode(&c->maps.m[10 + d], CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, e, edims, strides, ebox, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+               CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+      return false;
+  }
   return true;
 }
 
@@ -1858,7 +1921,7 @@ int ch_bind(ch_ctx* c, const ch_buffers* b, void* stream) {
       cudaGetLastError();
       return fail(CH_EINVAL, "ch_bind: state is not a device pointer");
     }
-    if (pa.device != c->device) { c->smem_attr[0][0] = c->smem_attr[0][1] = c->smem_attr[1][0] = c->smem_attr[1][1] = false; }
+    if (pa.device != c->device) { c->smem_attr[0][0] = c->smem_attr[0][1] = c->smem_attr[1][0] = c->smem_attr[1][1] = c->smem_attr_hc = false; }
     c->device = pa.device;
   }
   DeviceGuard guard(c->device);
@@ -2019,7 +2082,26 @@ int step_impl(ch_ctx* c, double dt, bool devdt) {
   }
   }
   CH_CUDA(cudaGetLastError(), "pass 1");
-  if (g.act[0] && g.act[1] && g.act[2] && !c->unfused && !c->hcorr) {
+  const bool three_d = g.act[0] && g.act[1] && g.act[2];
+  if (three_d && !c->unfused && c->hcorr && c->tma_ok && c->use_tma) {
+    // H-corrected step, fused: eta of every interface (C1), then the fused second half with C2's maxima taken from the
+    // staged eta planes (the plain-load kernel has no such form: without TMA the step stays unfused, below)
+    {
+      const long long ecells = (long long)(g.n[0] + 2) * (g.n[1] + 2) * (g.n[2] + 2);
+      Bracket b(c, CH_K_ETA);
+      k_eta<<<(unsigned)((ecells + CH_P2_T - 1) / CH_P2_T), CH_P2_T, 0, st>>>(A);
+    }
+    const int seg = final_segment(c);
+    const size_t tsmem = (size_t)74 * kTT * sizeof(double);     // + eta_x, eta_y and two planes of eta_z
+    if (!c->smem_attr_hc) {
+      CH_CUDA(cudaFuncSetAttribute(k_final3d_tma<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tsmem), "k_final3d_tma<HC> smem attribute");
+      c->smem_attr_hc = true;
+    }
+    const int pitch = tma_pitch_x(g);
+    dim3 tgrid((unsigned)((g.n[0] + pitch - 1) / pitch), (unsigned)((g.n[1] + kTY - 3) / (kTY - 2)), (unsigned)((g.n[2] + seg - 1) / seg));
+    Bracket b(c, CH_K_FINAL);
+    k_final3d_tma<1, true><<<tgrid, kTT, tsmem, st>>>(A, c->maps, seg);
+  } else if (three_d && !c->unfused && !c->hcorr) {
     // at least four waves of CTAs on small grids (a segment costs two light planes), 64 planes on large ones
     const int seg = final_segment(c);
     dim3 grid((unsigned)((g.n[0] + kFX - 3) / (kFX - 2)), (unsigned)((g.n[1] + kFY - 3) / (kFY - 2)),
@@ -2220,7 +2302,7 @@ int ch_tiling(const ch_ctx* c, int* out) {
   if (!c || !out) return fail(CH_EINVAL, "ch_tiling: null argument");
   const Geom& g = c->geo;
   const bool three_d = g.act[0] && g.act[1] && g.act[2];
-  const bool tma = three_d && c->tma_ok && c->use_tma && !c->unfused && !c->hcorr;
+  const bool tma = three_d && c->tma_ok && c->use_tma && !c->unfused;
   out[0] = kXOut;                          // interfaces per CTA of k_pass1_x (flat run of padded cells)
   out[1] = CH_MARCH_T;                     // columns per CTA of the marching kernels
   out[2] = march_segment(c, 1);            // interfaces a marching thread sweeps along y

@@ -74,7 +74,7 @@ def sampled_one_step(ref, w, m=12, extra=6, seed=0):
     return worst, post, dt
 
 
-def whole_grid_one_step(ref, w, slab=32, pre_steps=0):
+def whole_grid_one_step(ref, w, slab=32, pre_steps=0, g=3, setup=None, want_tma=None):
     """One GPU step of the WHOLE grid against the oracle on EVERY cell: the oracle re-steps z-slabs of `slab` planes
     (full x, y extent) cut with their 3-deep halo from the GPU's pre-step padded store (whose ghost fill is
     checked bit-exactly elsewhere), with the same dt and cell widths; a cell's update depends on nothing outside
@@ -82,8 +82,11 @@ def whole_grid_one_step(ref, w, slab=32, pre_steps=0):
     its ~95 whole-grid work arrays stay at 1/8 of their 256^3 size.  Returns the assembled oracle state."""
     import paper_1410_4194_b200 as ch
     nx, ny, nz = w.shape
-    g = 3
     G = ch.Grid(nx, ny, nz, g, w.gamma, w.bc)
+    if setup:
+        setup(G)
+    if want_tma is not None:
+        assert G.tiling()["tma"] == want_tma
     G.set_state(w.u)
     for _ in range(pre_steps):
         G.step(G.compute_dt(w.cfl))
@@ -97,6 +100,8 @@ def whole_grid_one_step(ref, w, slab=32, pre_steps=0):
     for k0 in range(0, nz, slab):
         kn = min(slab, nz - k0)
         Rg = ref.RefGrid(nx, ny, kn, g, w.gamma, (wl.OUTFLOW,) * 6)
+        if setup:
+            setup(Rg)
         Rg.set_spacing(dx, dx, dx)
         Rg.set_padded(np.ascontiguousarray(pre[:, k0:k0 + kn + 2 * g]))
         Rg.step(dt)
@@ -143,6 +148,21 @@ def test_whole_grid_parity_256_shock_cloud(ref):
     post, ur, _ = whole_grid_one_step(ref, w, pre_steps=5)
     err = max_rel_error(post, ur, w.gamma)
     print("whole-grid 256^3 shock-cloud: S11 norm", err, "strict", max_rel_error_strict(post, ur, w.gamma))
+    assert max(err) <= ONE_STEP_TOL, err
+    assert post[0].min() > 0
+
+
+def test_whole_grid_parity_256_shock_cloud_h_correction(ref):
+    """The H-corrected step (Roe solver + Appendix C, four ghost layers) in its fused form (k_eta + the TMA kernel
+    with C2's maxima taken from the staged eta planes) on every cell of the Mach-50 shock-cloud grid: the
+    grid-aligned strong shock is what the correction is for."""
+    w = wl.shock_cloud(256)
+
+    def hc(G):
+        G.set_solver(1); G.set_hcorrection(True)
+    post, ur, _ = whole_grid_one_step(ref, w, pre_steps=5, g=4, setup=hc, want_tma=1)
+    err = max_rel_error(post, ur, w.gamma)
+    print("whole-grid 256^3 shock-cloud, H correction: S11 norm", err, "strict", max_rel_error_strict(post, ur, w.gamma))
     assert max(err) <= ONE_STEP_TOL, err
     assert post[0].min() > 0
 

@@ -599,6 +599,35 @@ def test_hcorrection_one_step_parity(ch, ref, name, recon):
     G.close()
 
 
+@pytest.mark.parametrize("maker", [lambda: wl.sweep(shape=(64, 40, 36)), lambda: wl.rough_random(56, 30, 40, seed=4, decades=0.3, mach=0.8),
+                                   lambda: wl.smooth_random(28, 26, 70, seed=9, bc=(R, O, P, P, O, R)), lambda: wl.sedov(32)])
+def test_hcorrection_fused_and_unfused_forms_match_the_oracle(ch, ref, maker):
+    """The H-corrected step has two forms on 3-D grids: fused (k_eta, then the TMA kernel that takes C2's maxima from
+    the staged eta planes) where the padded strides meet TMA's alignment rules, unfused (k_eta, k_pass2, k_update)
+    elsewhere or on request.  Same grid through both, two steps, several tiles and plane segments: each within the
+    one-step gate of the oracle, and of each other."""
+    from paper_1410_4194_b200 import binding
+    w = maker()
+    out = {}
+    for form in ("fused", "unfused"):
+        G, Rg = both(ch, ref, w, nghost=4)
+        for g in (G, Rg):
+            g.set_solver(1); g.set_hcorrection(True)
+            g.set_state(w.u)
+        if form == "unfused":
+            G.set_option(binding.OPT_UNFUSED, 1)
+        else:
+            G.set_option(binding.OPT_FINAL_SEG, 8)
+            assert G.tiling()["tma"] == 1
+        for _ in range(2):
+            dt = Rg.compute_dt(w.cfl)
+            G.step(dt); Rg.step(dt)
+            assert max(max_rel_error(G.get_state(), Rg.get_state(), w.gamma)) <= ONE_STEP_TOL, form
+        out[form] = G.get_state()
+        G.close()
+    assert max(max_rel_error(out["fused"], out["unfused"], w.gamma)) <= ONE_STEP_TOL
+
+
 def test_hcorrection_run_switches_and_errors(ch, ref):
     w = wl.rough_random(48, 40, 1, seed=3, decades=0.3, mach=0.8, bc=(P,) * 6, steps=10)
     G, Rg = both(ch, ref, w, nghost=4)
