@@ -9,7 +9,9 @@
 //                      chip); planes staged by TMA from a producer warp (plain loads where TMA's
 //                      16-byte stride rules do not hold, or with CH_OPT_TMA = 0)
 //   k_final2d          the same for x-y grids (one plane, no z carry)
-//   k_pass2, k_update  the same two halves unfused: 1-D, x-z / y-z grids, the H-corrected step (+ k_eta)
+//   k_pass2, k_update  the same two halves unfused: 1-D, x-z / y-z grids, the H-corrected step without TMA (+ k_eta)
+//   k_eta3d            H correction on 3-D grids: eta of every interface (C1), tiled march; k_final3d_tma<Roe, HC> then takes
+//                      C2's maxima from the staged eta planes
 //   k_ghost            ghost fill of the new state, analytic (Noh) faces included
 //   k_pick_dt          ch_step_cfl: Eq. 22 finished on the device; the step is then replayed as a CUDA graph on small grids
 //   k_halo, k_fill_dim block decomposition: halo slabs and the per-direction fill
@@ -744,6 +746,95 @@ __device__ __forceinline__ void face_states(const StepArgs& A, long long q, cons
   correct_faces<D>(A, ul, ur, dF, wl, wr);
 }
 
+// ---------------------------------------------------------------------------------------------
+// C1 on 3-D grids, tiled (round 2; k_eta above is the one-thread-per-cell gather that 1-D / 2-D grids and
+// the unfused step use).  eta of the interface between cells c and c+1 along d is |s_L(c+1) - s_R(c)| / 2 with
+// s = u_d + a of the cell's OWN corrected face state, so a thread forms the six corrected states of its cell once
+// (as the fused second half does: the cell's three flux differences, correct_faces) and only one scalar per
+// direction crosses to the neighbour: lane+1 by shuffle, row+1 through shared memory, plane+1 is the thread's own
+// next step.  A CTA is a 32 x kEY tile of cell columns marching a segment of z; lane 31 and row kEY-1 only supply.
+// Cells [-1, n]^3, interfaces c+1/2 with c in [-1, n-1], as k_eta.
+// ---------------------------------------------------------------------------------------------
+constexpr int kEY = 8, kET = kFX * kEY;
+__device__ __forceinline__ double eta_speed(const Gas& G, const double w[5]) {   // u + a = u + gamma p / (rho a)
+  return __dadd_rn(w[1], __dmul_rn(__dmul_rn(G.gamma, w[4]), ch::inv_rho_a(G, w[0], w[4])));
+}
+
+__global__ void __launch_bounds__(kET) k_eta3d(const StepArgs A, int seg) {
+  __shared__ double sY[2][kET];
+  if (step_refused(A)) return;
+  const Geom& g = A.geo;
+  double dtx[3];
+  step_dtdx(A, dtx);
+  const unsigned full = 0xffffffffu;
+  const int tid = threadIdx.x, lane = tid & 31, row = tid >> 5;
+  const int nx = g.n[0], ny = g.n[1], nz = g.n[2];
+  const int i = (int)blockIdx.x * (kFX - 1) - 1 + lane;
+  const int j = (int)blockIdx.y * (kEY - 1) - 1 + row;
+  const int ka = (int)blockIdx.z * seg - 1;          // planes [ka, kb) of [-1, nz] are this CTA's
+  const int kb = min(ka + seg, nz + 1);
+  const bool valid = i <= nx && j <= ny;
+  const bool own = valid && lane < kFX - 1 && row < kEY - 1;
+  const long long np = g.np, s1 = g.st[1], s2 = g.st[2];
+  const long long qcol = (long long)(i + g.g[0]) + (long long)(j + g.g[1]) * s1 + (long long)g.g[2] * s2;
+  const double hx = 0.5 * dtx[0], hy = 0.5 * dtx[1], hz = 0.5 * dtx[2];
+  double zS[5] = {0.0, 0.0, 0.0, 0.0, 0.0};     // F*_z of plane k-1
+  double sRz = 0.0;                              // s_R(., z) of plane k-1
+  // a segment that does not start the grid warms up on the plane below it (its s_R(., z) only)
+  const int kstart = ka == -1 ? -1 : ka - 1;
+  for (int k = kstart; k < kb; ++k) {
+    const bool first = k == kstart, warm = k < ka;
+    const long long q = qcol + (long long)k * s2;
+    double dF[3][5];
+    {
+      double fx[5] = {0.0, 0.0, 0.0, 0.0, 0.0}, fxm[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+      if (valid) {
+#pragma unroll
+        for (int f = 0; f < 5; ++f) {
+          const long long a = f * np + q;
+          fx[f] = A.Fs[0][a];
+          if (lane == 0) fxm[f] = A.Fs[0][a - 1];
+          const double fz = A.Fs[2][a];
+          const double fzm = first ? A.Fs[2][a - s2] : zS[f];
+          zS[f] = fz;
+          dF[1][f] = __dmul_rn(hy, A.Fs[1][a - s1] - A.Fs[1][a]);
+          dF[2][f] = __dmul_rn(hz, fzm - fz);
+        }
+      }
+#pragma unroll
+      for (int f = 0; f < 5; ++f) {
+        const double t = __shfl_up_sync(full, fx[f], 1);
+        dF[0][f] = __dmul_rn(hx, (lane == 0 ? fxm[f] : t) - fx[f]);
+      }
+    }
+    double sLx = 0.0, sRx = 0.0, sLy = 0.0, sRy = 0.0, sLz = 0.0, sRzn = 0.0;
+    if (valid) {
+      double wl[5], wr[5];
+      // all thirty face values first: the kernel lives on loads in flight (two CTAs per SM), 19.4 -> 9.9 ms at 512^3
+      double ul0[5], ur0[5], ul1[5], ur1[5], ul2[5], ur2[5];
+      load_faces<2>(A, q, ul2, ur2); load_faces<0>(A, q, ul0, ur0); load_faces<1>(A, q, ul1, ur1);
+      correct_faces<2>(A, ul2, ur2, dF, wl, wr);
+      sLz = eta_speed(A.gas, wl); sRzn = eta_speed(A.gas, wr);
+      if (!warm) {
+        correct_faces<0>(A, ul0, ur0, dF, wl, wr);
+        sLx = eta_speed(A.gas, wl); sRx = eta_speed(A.gas, wr);
+        correct_faces<1>(A, ul1, ur1, dF, wl, wr);
+        sLy = eta_speed(A.gas, wl); sRy = eta_speed(A.gas, wr);
+      }
+    }
+    const double upx = __shfl_down_sync(full, sLx, 1);
+    sY[k & 1][tid] = sLy;                      // two buffers: the next plane's writes cannot pass this plane's reads
+    __syncthreads();
+    const double upy = sY[k & 1][row < kEY - 1 ? tid + kFX : tid];
+    if (own && !warm) {
+      if (i < nx) A.eta[0][q] = 0.5 * fabs(upx - sRx);
+      if (j < ny) A.eta[1][q] = 0.5 * fabs(upy - sRy);
+      if (k >= 0) A.eta[2][q - s2] = 0.5 * fabs(sLz - sRz);
+    }
+    sRz = sRzn;
+  }
+}
+
 template <int S>
 __global__ void __launch_bounds__(kFT, CH_F_MINB) k_final3d(const StepArgs A, int seg) {
   extern __shared__ double s_final[];
@@ -1037,7 +1128,7 @@ __device__ __forceinline__ void tma_load_4d(unsigned dst, const CUtensorMap* map
       ::"r"(dst), "l"(map), "r"(bar), "r"(c0), "r"(c1), "r"(c2), "r"(c3) : "memory");
 }
 
-// HC (Roe solver only): the H-corrected step.  k_eta has written eta of every interface (C1); a fifth staging group
+// HC (Roe solver only): the H-corrected step.  k_eta3d has written eta of every interface (C1); a fifth staging group
 // brings eta_x and eta_y of plane k and eta_z of the faces k-1/2 and k+1/2 (slots 70..73), every thread forms the
 // three maxima of C2 for its x, y and z interface from them (the stencil stays inside the staged box) and the Roe
 // solver takes them: the same values and the same solver as k_pass2<1, true>, so the two paths agree bitwise.
@@ -2087,9 +2178,10 @@ int step_impl(ch_ctx* c, double dt, bool devdt) {
     // H-corrected step, fused: eta of every interface (C1), then the fused second half with C2's maxima taken from the
     // staged eta planes (the plain-load kernel has no such form: without TMA the step stays unfused, below)
     {
-      const long long ecells = (long long)(g.n[0] + 2) * (g.n[1] + 2) * (g.n[2] + 2);
+      const int nseg = (g.n[2] + 2 + 63) / 64, eseg = (g.n[2] + 2 + nseg - 1) / nseg;
+      dim3 egrid((unsigned)((g.n[0] + 2 + kFX - 2) / (kFX - 1)), (unsigned)((g.n[1] + 2 + kEY - 2) / (kEY - 1)), (unsigned)nseg);
       Bracket b(c, CH_K_ETA);
-      k_eta<<<(unsigned)((ecells + CH_P2_T - 1) / CH_P2_T), CH_P2_T, 0, st>>>(A);
+      k_eta3d<<<egrid, kET, 0, st>>>(A, eseg);
     }
     const int seg = final_segment(c);
     const size_t tsmem = (size_t)74 * kTT * sizeof(double);     // + eta_x, eta_y and two planes of eta_z
