@@ -578,6 +578,12 @@ HC_CASES = {
     "sweep_ragged_3d": lambda: wl.sweep(shape=(135, 45, 37)),
     "sedov_24": lambda: wl.sedov(24),
     "smooth_mixed_bc": lambda: wl.smooth_random(41, 29, 23, seed=5, bc=(R, O, P, P, O, R)),
+    # even padded strides: the fused form (k_eta3d + the TMA kernel) on one partial tile, on a grid smaller than a tile in
+    # every direction, across two x tiles, eleven y tiles of k_eta3d and two plane segments
+    "sweep_tiny_even_tma": lambda: wl.sweep(shape=(4, 4, 4)),
+    "sweep_flat_even_tma": lambda: wl.sweep(shape=(8, 6, 4)),
+    "sweep_seams_tma": lambda: wl.sweep(shape=(34, 72, 20)),
+    "rough_reflective_tma": lambda: wl.rough_random(24, 24, 24, seed=13, bc=(R,) * 6, mach=1.0, decades=0.5),
 }
 
 
