@@ -53,6 +53,8 @@ def parse():
                     help="Riemann solver of the main measured workload (default: the metric's exact solver)")
     ap.add_argument("--recon", type=str, default="ppmc", choices=["ppmc", "plmc", "pcm"],
                     help="reconstruction of the main measured workload (default: the metric's PPM)")
+    ap.add_argument("--hcorr", action="store_true",
+                    help="main workload with the H correction of Appendix C (implies --solver roe and four ghost layers)")
     return ap.parse_args()
 
 
@@ -219,15 +221,17 @@ def timed_steps(G, cfl, steps, stream_events):
     return e0.elapsed_time(e1) * 1e-3
 
 
-def bench_size(pkg, wl, n, steps, warmup, device, dist=None, profile=True, e2e=True, solver=0, recon=0):
+def bench_size(pkg, wl, n, steps, warmup, device, dist=None, profile=True, e2e=True, solver=0, recon=0, hcorr=False):
     import numpy as np
     import torch
     from paper_1410_4194_b200.driver import max_over_ranks
     w = wl.sweep(n)
     N = n ** 3
-    G = pkg.Grid(n, n, n, 3, w.gamma, w.bc, device=device)
+    G = pkg.Grid(n, n, n, 4 if hcorr else 3, w.gamma, w.bc, device=device)
     G.set_solver(solver)
     G.set_reconstruction(recon)
+    if hcorr:
+        G.set_hcorrection(True)
     u_dev = torch.from_numpy(w.u).to(device)
     G.set_state(u_dev)
     ev = (torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
@@ -313,18 +317,20 @@ def main():
     sampler = ClockSampler(local) if rank == 0 else None
     peak_tf, _ = fp64_peak_probe(device=device)                 # measured DFMA rate, burst
     mix = issue_mix_probe(device=device)                        # scheduler time per FP64 / per other warp instruction
+    if args.hcorr:
+        args.solver = "roe"
     solver = {"exact": 0, "roe": 1}[args.solver]
     recon = {"ppmc": 0, "plmc": 1, "pcm": 2}[args.recon]
-    default_method = solver == 0 and recon == 0
+    default_method = solver == 0 and recon == 0 and not args.hcorr
     main_res, w = bench_size(pkg, wl, args.size, args.steps, args.warmup, device, dist,
-                             profile=True, e2e=not args.no_e2e, solver=solver, recon=recon)
+                             profile=True, e2e=not args.no_e2e, solver=solver, recon=recon, hcorr=args.hcorr)
     clocks = sampler.stop() if sampler else None
     others = {}
     if world == 1:
         for s in [int(x) for x in args.other_sizes.split(",") if x]:
             if s != args.size:
                 r, _ = bench_size(pkg, wl, s, args.steps, args.warmup, device, None, profile=False, e2e=False,
-                                  solver=solver, recon=recon)
+                                  solver=solver, recon=recon, hcorr=args.hcorr)
                 others[str(s)] = {"value": r["cells"] * args.steps / r["seconds"], "unit": UNIT,
                                   "ms_per_step": r["seconds"] / args.steps * 1e3,
                                   "ch_step_cfl": {"value": r["cells"] * args.steps / r["step_cfl_seconds"], "unit": UNIT,
@@ -502,7 +508,7 @@ def main():
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": f"throughput sweep (BASELINE.json config 5) {args.size}^3 periodic, "
                                    "sum of 8 seeded sinusoids, 1 replica per GPU",
-                       "gamma": w.gamma, "cfl": w.cfl, "nghost": 3, "l2": "state (5 fields) larger than L2, no flush",
+                       "gamma": w.gamma, "cfl": w.cfl, "nghost": 4 if args.hcorr else 3, "h_correction": bool(args.hcorr), "l2": "state (5 fields) larger than L2, no flush",
                        "reconstruction": args.recon, "riemann_solver": args.solver,
                        "parallelism": "replicas only" if world > 1 else "single GPU"},
             "gpu_launches": main_res["launches"], "clocks": clocks, "roofline": roofline}
