@@ -200,8 +200,10 @@ int ch_set_origin(ch_ctx* ctx, int i0, int j0, int k0);
  *   CH_OPT_UNFUSED    1: run the second half as k_pass2 + k_update on 3-D grids too (A/B measurements); default 0
  *   CH_OPT_GRAPH      1 (default): ch_step_cfl replays the kernels of a step as one CUDA graph from the third step with a
  *                     configuration on (captured on a private stream; the same kernels, the same bits); 0: direct launches
+ *   CH_OPT_FOLD_GHOST 1 (default): on x-y grids with periodic / reflective / outflow faces the update kernel also writes the
+ *                     ghost cells that copy its cells (one launch less per step, the same bits); 0: a k_ghost launch
  * CH_EINVAL for an unknown option or an out-of-range value. */
-enum { CH_OPT_MARCH_SEG = 0, CH_OPT_FINAL_SEG = 1, CH_OPT_TMA = 2, CH_OPT_UNFUSED = 3, CH_OPT_GRAPH = 4 };
+enum { CH_OPT_MARCH_SEG = 0, CH_OPT_FINAL_SEG = 1, CH_OPT_TMA = 2, CH_OPT_UNFUSED = 3, CH_OPT_GRAPH = 4, CH_OPT_FOLD_GHOST = 5 };
 int ch_set_option(ch_ctx* ctx, int option, int value);
 
 /* ch_step_cfl — one step whose size never visits the host: dt = cfl * min dx_d/(|v_d| + a) (Eq. 22, from the

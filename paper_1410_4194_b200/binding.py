@@ -31,7 +31,7 @@ SYMBOLS = ("ch_init", "ch_free", "ch_last_error", "ch_set_spacing", "ch_padded_c
            "ch_halo_cells", "ch_halo_pack", "ch_halo_unpack", "ch_fill_dim", "ch_set_origin", "ch_sync", "ch_kernel_launches", "ch_profile", "ch_profile_read", "ch_kernel_name",
            "ch_fp64_peak_probe", "ch_issue_mix_probe")
 K_COUNT = 11
-OPT_MARCH_SEG, OPT_FINAL_SEG, OPT_TMA, OPT_UNFUSED, OPT_GRAPH = 0, 1, 2, 3, 4
+OPT_MARCH_SEG, OPT_FINAL_SEG, OPT_TMA, OPT_UNFUSED, OPT_GRAPH, OPT_FOLD_GHOST = 0, 1, 2, 3, 4, 5
 
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-shared"]

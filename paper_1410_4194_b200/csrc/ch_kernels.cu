@@ -30,6 +30,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <limits>
+#include <vector>
 #include <new>
 #include <string>
 
@@ -973,8 +974,24 @@ __global__ void __launch_bounds__(kFT, CH_F_MINB) k_final3d(const StepArgs A, in
 // through warp shuffles, the y problem through shared memory, Eq. 24 and the Eq. 22 reduction.  It replaces
 // k_pass2 + k_update (and F, G^{n+1/2} through HBM) on grids where a step is a handful of launch-bound kernels.
 // ---------------------------------------------------------------------------------------------
+// Ghost images of real coordinate c (n cells, ng ghost layers, face rules lo / hi): the ghost coordinates that the
+// ghost fill maps onto c (the inverse of bc_source for periodic, reflective and outflow faces).  img[0] = c itself.
+constexpr int kMaxImg = 2 * 4 + 1;
+__device__ __forceinline__ int bc_images(int c, int n, int ng, int lo, int hi, int img[kMaxImg], bool flip[kMaxImg]) {
+  int m = 0;
+  img[m] = c; flip[m++] = false;
+  if (lo == CH_BC_PERIODIC) { if (c - n >= -ng) { img[m] = c - n; flip[m++] = false; } }
+  else if (lo == CH_BC_REFLECTIVE) { if (c < ng) { img[m] = -c - 1; flip[m++] = true; } }
+  else if (c == 0) { for (int t = 1; t <= ng; ++t) { img[m] = -t; flip[m++] = false; } }
+  if (hi == CH_BC_PERIODIC) { if (c + n < n + ng) { img[m] = c + n; flip[m++] = false; } }
+  else if (hi == CH_BC_REFLECTIVE) { if (c >= n - ng) { img[m] = 2 * n - 1 - c; flip[m++] = true; } }
+  else if (c == n - 1) { for (int t = 1; t <= ng; ++t) { img[m] = n - 1 + t; flip[m++] = false; } }
+  return m;
+}
+struct Scatter2d { int on; int bc[4]; };   // on: the update also writes the ghost images of its cells (no k_ghost launch)
+
 template <int S>
-__global__ void __launch_bounds__(kFT, 2) k_final2d(const StepArgs A) {
+__global__ void __launch_bounds__(kFT, 2) k_final2d(const StepArgs A, const Scatter2d GS) {
   __shared__ double sX[5][kFT], sF[5][kFT];
   if (step_refused(A)) return;
   const Geom& g = A.geo;
@@ -1059,6 +1076,23 @@ __global__ void __launch_bounds__(kFT, 2) k_final2d(const StepArgs A) {
   if (need2) {
     A.u[q] = part[0]; A.u[np + q] = part[1]; A.u[2 * np + q] = part[2]; A.u[3 * np + q] = part[3]; A.u[4 * np + q] = part[4];
     t = cell_rate(A, part[0], part[1], part[2], part[3], part[4], bad);
+    // the ghost fill folded into the update (launch-bound boxes: one kernel less per step): a cell within nghost of a
+    // face also writes the ghost cells that copy it -- x and y images combine as in k_ghost (each coordinate on its own)
+    if (GS.on && (i < g.g[0] || i >= nx - g.g[0] || j < g.g[1] || j >= ny - g.g[1])) {
+      int xi[kMaxImg], yj[kMaxImg];
+      bool xf[kMaxImg], yf[kMaxImg];
+      const int mx = bc_images(i, nx, g.g[0], GS.bc[0], GS.bc[1], xi, xf);
+      const int my = bc_images(j, ny, g.g[1], GS.bc[2], GS.bc[3], yj, yf);
+      for (int b = 0; b < my; ++b)
+        for (int a = (b == 0 ? 1 : 0); a < mx; ++a) {
+          const long long qd = (long long)(xi[a] + g.g[0]) + (long long)(yj[b] + g.g[1]) * s1;
+          A.u[qd] = part[0];
+          A.u[np + qd] = xf[a] ? -part[1] : part[1];
+          A.u[2 * np + qd] = yf[b] ? -part[2] : part[2];
+          A.u[3 * np + qd] = part[3];
+          A.u[4 * np + qd] = part[4];
+        }
+    }
   }
   block_max_reduce(t, bad, A.red);
 }
@@ -1692,10 +1726,14 @@ struct ch_ctx {
   // ch_step_cfl replays the kernels of a step as a CUDA graph (captured on a private stream the second time a
   // configuration is stepped): on small grids the step is launch bound
   bool use_graph = true;
+  bool fold_ghost = true;    // x-y grids: k_final2d also writes the ghost images of its cells (CH_OPT_FOLD_GHOST)
   cudaStream_t cap_stream = nullptr, cap_side[2] = {nullptr, nullptr};   // the y and z sweeps of pass 1 are parallel branches of the graph
   cudaEvent_t cap_fork = nullptr, cap_join[2] = {nullptr, nullptr};
   bool capturing = false;
   cudaGraphExec_t gexec = nullptr;
+  cudaGraph_t ggraph = nullptr;            // the captured graph (kept: its k_pick_dt node names the node of gexec to update)
+  cudaGraphNode_t gpick = nullptr;         // k_pick_dt's node
+  double gcfl = 0.0, gtleft = 0.0;         // its arguments as last set
   long long gkey[8] = {-1, -1, -1, -1, -1, -1, -1, -1};   // configuration the graph / the last direct step belongs to
   double gdx[3] = {0, 0, 0};
   int gseen = 0;                           // direct steps taken with gkey (capture on the second)
@@ -1892,6 +1930,14 @@ bool build_tma_maps(ch_ctx* c) {
 // even double: 16-byte alignment of the bulk tensor copy).
 int tma_pitch_x(const Geom& g) { return (g.g[0] & 1) ? kFX - 2 : kFX - 4; }
 
+// x-y grids whose four faces are periodic, reflective or outflow: the update kernel writes the ghost cells itself.
+bool scatter2d(const ch_ctx* c) {
+  if (!c->fold_ghost || c->has_exchange || c->has_noh || c->nghost > 4) return false;
+  for (int f = 0; f < 4; ++f)
+    if (c->bc[f] != CH_BC_PERIODIC && c->bc[f] != CH_BC_REFLECTIVE && c->bc[f] != CH_BC_OUTFLOW) return false;
+  return true;
+}
+
 // Interfaces a thread of the marching pass-1 kernel sweeps along d: enough segments to fill the chip on small grids
 // (a segment costs ~1.5 cells of warm-up), 64 on large ones; CH_OPT_MARCH_SEG overrides.
 int march_segment(const ch_ctx* c, int d) {
@@ -1962,6 +2008,8 @@ ch_ctx* ch_init(int nx, int ny, int nz, int nghost, double gamma, const int* bc)
 
 static void drop_graph(ch_ctx* c) {
   if (c->gexec) { cudaGraphExecDestroy(c->gexec); c->gexec = nullptr; }
+  if (c->ggraph) { cudaGraphDestroy(c->ggraph); c->ggraph = nullptr; }
+  c->gpick = nullptr;
   c->gseen = 0;
   c->gkey[0] = -1;
 }
@@ -2173,6 +2221,7 @@ int step_impl(ch_ctx* c, double dt, bool devdt) {
   }
   }
   CH_CUDA(cudaGetLastError(), "pass 1");
+  bool folded_ghost = false;
   const bool three_d = g.act[0] && g.act[1] && g.act[2];
   if (three_d && !c->unfused && c->hcorr && c->tma_ok && c->use_tma) {
     // H-corrected step, fused: eta of every interface (C1), then the fused second half with C2's maxima taken from the
@@ -2221,7 +2270,11 @@ int step_impl(ch_ctx* c, double dt, bool devdt) {
   } else if (g.act[0] && g.act[1] && !g.act[2] && !c->unfused && !c->hcorr) {
     dim3 grid((unsigned)((g.n[0] + kFX - 3) / (kFX - 2)), (unsigned)((g.n[1] + kFY - 3) / (kFY - 2)), 1);
     Bracket b(c, CH_K_FINAL);
-    k_final2d<S><<<grid, kFT, 0, st>>>(A);
+    Scatter2d GS;
+    GS.on = scatter2d(c) ? 1 : 0;
+    for (int f = 0; f < 4; ++f) GS.bc[f] = c->bc[f];
+    k_final2d<S><<<grid, kFT, 0, st>>>(A, GS);
+    folded_ghost = GS.on != 0;
   } else {
     {
       const long long cells = (long long)(g.act[0] ? g.n[0] + 1 : 1) * (g.act[1] ? g.n[1] + 1 : 1) * (g.act[2] ? g.n[2] + 1 : 1);
@@ -2243,7 +2296,7 @@ int step_impl(ch_ctx* c, double dt, bool devdt) {
   CH_CUDA(cudaGetLastError(), "pass 2 / update");
   if (!devdt) c->time += dt;     // analytic faces are evaluated at t^{n+1}
   // a block of a decomposed domain: its ghosts are filled by the caller, direction by direction
-  int rc = c->has_exchange ? CH_OK : launch_ghost(c, A);
+  int rc = (c->has_exchange || folded_ghost) ? CH_OK : launch_ghost(c, A);
   if (rc) return rc;
   c->dt_valid = true;
   return profile_collect(c);
@@ -2288,31 +2341,44 @@ int ch_step_cfl(ch_ctx* c, double cfl, double t_left) {
     { Bracket b(c, CH_K_DT); k_dt<<<(unsigned)blocks, 256, 0, c->stream>>>(A); }
     c->dt_valid = true;
   }
-  { Bracket b(c, CH_K_PICK_DT); k_pick_dt<<<1, 32, 0, c->stream>>>(c->red, cfl, t_left); }
-  CH_CUDA(cudaGetLastError(), "k_pick_dt");
   // launch-bound grids only: from ~256^3 up a step is tens of milliseconds of kernels and the replay measured
   // 1-3 % slower than plain launches (384^3: 15.9 against 15.4 ms)
   const long long ncell = (long long)c->geo.n[0] * c->geo.n[1] * c->geo.n[2];
-  if (!c->use_graph || c->profiling || ncell > (1LL << 24)) return step_dispatch(c, 0.0, true);
-  // The rest of the step reads dt from device memory and has no other per-step argument: one graph per
-  // configuration.  First step with a configuration: direct (sets kernel attributes); second: captured on the
-  // private stream; from then on one cudaGraphLaunch on the caller's stream.
-  const long long key[8] = {c->solver, c->recon, c->hcorr, c->unfused, c->use_tma, c->march_seg, c->final_seg, 1};
-  bool same = true;
-  for (int i = 0; i < 8; ++i) same = same && key[i] == c->gkey[i];
-  for (int d = 0; d < 3; ++d) same = same && c->gdx[d] == c->dx[d];
-  if (!same) {
-    drop_graph(c);
-    for (int i = 0; i < 8; ++i) c->gkey[i] = key[i];
-    for (int d = 0; d < 3; ++d) c->gdx[d] = c->dx[d];
+  const bool graphs = c->use_graph && !c->profiling && ncell <= (1LL << 24);
+  // The step reads dt from device memory; k_pick_dt's two arguments are the only per-step ones: one graph per
+  // configuration, k_pick_dt its first node, its arguments updated in place when they change.  First step with a
+  // configuration: direct (sets kernel attributes); second: captured on the private stream; from then on one
+  // cudaGraphLaunch on the caller's stream.
+  if (graphs) {
+    const long long key[8] = {c->solver, c->recon, c->hcorr, c->unfused, c->use_tma, c->march_seg, c->final_seg, 1};
+    bool same = true;
+    for (int i = 0; i < 8; ++i) same = same && key[i] == c->gkey[i];
+    for (int d = 0; d < 3; ++d) same = same && c->gdx[d] == c->dx[d];
+    if (!same) {
+      drop_graph(c);
+      for (int i = 0; i < 8; ++i) c->gkey[i] = key[i];
+      for (int d = 0; d < 3; ++d) c->gdx[d] = c->dx[d];
+    }
+    if (c->gexec) {
+      if (cfl != c->gcfl || t_left != c->gtleft) {
+        void* args[3] = {(void*)&c->red, (void*)&cfl, (void*)&t_left};
+        cudaKernelNodeParams kp = {};
+        kp.func = (void*)k_pick_dt;
+        kp.gridDim = dim3(1); kp.blockDim = dim3(32); kp.sharedMemBytes = 0; kp.kernelParams = args; kp.extra = nullptr;
+        CH_CUDA(cudaGraphExecKernelNodeSetParams(c->gexec, c->gpick, &kp), "cudaGraphExecKernelNodeSetParams");
+        c->gcfl = cfl; c->gtleft = t_left;
+      }
+      CH_CUDA(cudaGraphLaunch(c->gexec, c->stream), "cudaGraphLaunch");
+      c->launches += c->glaunches;
+      c->dt_valid = true;
+      return CH_OK;
+    }
   }
-  if (c->gexec) {
-    CH_CUDA(cudaGraphLaunch(c->gexec, c->stream), "cudaGraphLaunch");
-    c->launches += c->glaunches;
-    c->dt_valid = true;
-    return CH_OK;
+  if (!graphs || c->gseen++ == 0) {
+    { Bracket b(c, CH_K_PICK_DT); k_pick_dt<<<1, 32, 0, c->stream>>>(c->red, cfl, t_left); }
+    CH_CUDA(cudaGetLastError(), "k_pick_dt");
+    return step_dispatch(c, 0.0, true);
   }
-  if (c->gseen++ == 0) return step_dispatch(c, 0.0, true);
   if (!c->cap_stream) {
     CH_CUDA(cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking), "cudaStreamCreate");
     for (int i = 0; i < 2; ++i) {
@@ -2327,21 +2393,42 @@ int ch_step_cfl(ch_ctx* c, double cfl, double t_left) {
   CH_CUDA(cudaStreamBeginCapture(c->cap_stream, cudaStreamCaptureModeThreadLocal), "cudaStreamBeginCapture");
   c->stream = c->cap_stream;
   c->capturing = true;
+  { Bracket b(c, CH_K_PICK_DT); k_pick_dt<<<1, 32, 0, c->stream>>>(c->red, cfl, t_left); }
   const int rc = step_dispatch(c, 0.0, true);
   c->capturing = false;
   c->stream = user;
   cudaError_t e = cudaStreamEndCapture(c->cap_stream, &graph);
   c->glaunches = c->launches - before;
   c->launches = before;
-  if (rc != CH_OK || e != cudaSuccess || !graph) {
+  // k_pick_dt's node
+  cudaGraphNode_t pick = nullptr;
+  if (rc == CH_OK && e == cudaSuccess && graph) {
+    size_t nn = 0;
+    cudaGraphGetNodes(graph, nullptr, &nn);
+    std::vector<cudaGraphNode_t> nodes(nn);
+    if (nn) cudaGraphGetNodes(graph, nodes.data(), &nn);
+    for (size_t i = 0; i < nn && !pick; ++i) {
+      cudaGraphNodeType ty;
+      if (cudaGraphNodeGetType(nodes[i], &ty) != cudaSuccess || ty != cudaGraphNodeTypeKernel) continue;
+      cudaKernelNodeParams kp;
+      if (cudaGraphKernelNodeGetParams(nodes[i], &kp) == cudaSuccess && kp.func == (void*)k_pick_dt) pick = nodes[i];
+    }
+  }
+  if (rc != CH_OK || e != cudaSuccess || !graph || !pick) {
     if (graph) cudaGraphDestroy(graph);
     cudaGetLastError();
     c->use_graph = false;                  // fall back to direct launches for this context
+    { Bracket b(c, CH_K_PICK_DT); k_pick_dt<<<1, 32, 0, c->stream>>>(c->red, cfl, t_left); }
     return step_dispatch(c, 0.0, true);
   }
   e = cudaGraphInstantiate(&c->gexec, graph, 0);
-  cudaGraphDestroy(graph);
-  if (e != cudaSuccess) { c->gexec = nullptr; cudaGetLastError(); c->use_graph = false; return step_dispatch(c, 0.0, true); }
+  if (e != cudaSuccess) {
+    cudaGraphDestroy(graph);
+    c->gexec = nullptr; cudaGetLastError(); c->use_graph = false;
+    { Bracket b(c, CH_K_PICK_DT); k_pick_dt<<<1, 32, 0, c->stream>>>(c->red, cfl, t_left); }
+    return step_dispatch(c, 0.0, true);
+  }
+  c->ggraph = graph; c->gpick = pick; c->gcfl = cfl; c->gtleft = t_left;
   CH_CUDA(cudaGraphLaunch(c->gexec, c->stream), "cudaGraphLaunch");
   c->launches += c->glaunches;
   c->dt_valid = true;
@@ -2488,6 +2575,7 @@ int ch_set_option(ch_ctx* c, int option, int value) {
     case CH_OPT_TMA: c->use_tma = value != 0; return CH_OK;
     case CH_OPT_UNFUSED: c->unfused = value != 0; return CH_OK;
     case CH_OPT_GRAPH: c->use_graph = value != 0; if (!c->use_graph) drop_graph(c); return CH_OK;
+    case CH_OPT_FOLD_GHOST: c->fold_ghost = value != 0; drop_graph(c); return CH_OK;
     default: return fail(CH_EINVAL, "ch_set_option: unknown option");
   }
 }

@@ -79,6 +79,33 @@ def test_ghost_fill_with_four_ghost_layers(ch, ref):
     G.close()
 
 
+@pytest.mark.parametrize("shape,g", [((40, 33), 3), ((64, 70), 3), ((3, 3), 3), ((5, 4), 4), ((37, 9), 4), ((9, 37), 3)])
+@pytest.mark.parametrize("bc", [(P,) * 6, (O,) * 6, (R,) * 6, (R, O, P, P, P, P), (O, R, R, O, P, P), (P, P, O, R, P, P)])
+def test_ghost_fill_folded_into_the_2d_update_is_bit_exact(ch, shape, g, bc):
+    """x-y grids: the fused update writes the ghost cells that copy its cells (CH_OPT_FOLD_GHOST, the default) instead of a
+    k_ghost launch after it.  Every padded cell after three steps equals the k_ghost form bit for bit: faces, corners
+    (x and y images combine), grids narrower than two ghost widths (a cell is the image of both periodic sides), three
+    and four ghost layers."""
+    from paper_1410_4194_b200 import binding
+    nx, ny = shape
+    w = wl.smooth_random(nx, ny, 1, seed=21, bc=bc)
+    out = []
+    for fold in (1, 0):
+        G = ch.Grid(nx, ny, 1, g, w.gamma, bc)
+        G.set_option(binding.OPT_FOLD_GHOST, fold)
+        G.set_state(w.u)
+        dts = []
+        for _ in range(3):
+            dt = G.compute_dt(w.cfl)
+            dts.append(dt)
+            G.step(dt)
+        out.append((G.get_padded(), dts, G.kernel_launches))
+        G.close()
+    assert out[0][1] == out[1][1]
+    assert np.array_equal(out[0][0], out[1][0])
+    assert out[0][2] < out[1][2]                 # one launch less per step
+
+
 def test_device_and_pinned_sources(ch):
     import torch
     u = torch.from_numpy(np.random.default_rng(9).normal(size=(5, 6, 5, 9)))
