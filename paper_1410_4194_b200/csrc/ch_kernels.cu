@@ -304,6 +304,24 @@ __global__ void __launch_bounds__(CH_MARCH_T, 2) k_pass1_march_ppmp(const StepAr
 constexpr int kXT = CH_X_T;    // threads per CTA
 constexpr int kXOut = kXT - 5; // interfaces produced per CTA
 
+// Coordinates (relative to the first real cell) of padded index q.  Grids below 2^31 padded cells take 32-bit
+// divisions: the two 64-bit ones were 5 % of k_pass1_x's issue slots.
+__device__ __forceinline__ void padded_coords(const Geom& g, long long q, int& i, int& j, int& k) {
+  if (g.np < (1LL << 31)) {
+    unsigned r = (unsigned)q;
+    const unsigned s2 = (unsigned)g.st[2], s1 = (unsigned)g.st[1];
+    const unsigned kk = r / s2; r -= kk * s2;
+    const unsigned jj = r / s1;
+    i = (int)(r - jj * s1) - g.g[0]; j = (int)jj - g.g[1]; k = (int)kk - g.g[2];
+  } else {
+    long long r = q;
+    k = (int)(r / g.st[2]); r -= (long long)k * g.st[2];
+    j = (int)(r / g.st[1]);
+    i = (int)(r - (long long)j * g.st[1]);
+    i -= g.g[0]; j -= g.g[1]; k -= g.g[2];
+  }
+}
+
 template <int S, int R>
 __global__ void __launch_bounds__(kXT, CH_X_MINB) k_pass1_x(const StepArgs A, long long q_begin, long long q_end) {
   __shared__ double sP[5][kXT];
@@ -320,11 +338,7 @@ __global__ void __launch_bounds__(kXT, CH_X_MINB) k_pass1_x(const StepArgs A, lo
   // coordinates of q
   int i = 0, j = 0, k = 0;
   if (inb) {
-    long long r = q;
-    k = (int)(r / g.st[2]); r -= (long long)k * g.st[2];
-    j = (int)(r / g.st[1]);
-    i = (int)(r - (long long)j * g.st[1]);
-    i -= g.g[0]; j -= g.g[1]; k -= g.g[2];
+    padded_coords(g, q, i, j, k);
   }
   // rows needed: transverse indices in [-1, n] (or the single row of an inactive dimension)
   const bool row_ok = inb && (!g.act[1] || (j >= -1 && j <= g.n[1])) && (!g.act[2] || (k >= -1 && k <= g.n[2]));
@@ -397,11 +411,7 @@ __global__ void __launch_bounds__(kXT, 3) k_pass1_x_ppmp(const StepArgs A, long 
   const bool inb = (q >= 0 && q < np);
   int i = 0, j = 0, k = 0;
   if (inb) {
-    long long r = q;
-    k = (int)(r / g.st[2]); r -= (long long)k * g.st[2];
-    j = (int)(r / g.st[1]);
-    i = (int)(r - (long long)j * g.st[1]);
-    i -= g.g[0]; j -= g.g[1]; k -= g.g[2];
+    padded_coords(g, q, i, j, k);
   }
   const bool row_ok = inb && (!g.act[1] || (j >= -1 && j <= g.n[1])) && (!g.act[2] || (k >= -1 && k <= g.n[2]));
   const int nx = g.n[0];
