@@ -271,6 +271,29 @@ double ch_fp64_peak_probe(double* sink, int blocks, int threads, int iters, void
  * cost of an FP64 warp instruction and of an ALU warp instruction in scheduler cycles, and whether they overlap. */
 double ch_issue_mix_probe(double* sink, int n_alu, int blocks, int threads, int iters, void* stream);
 
+/* ch_dt_noalloc — Eq. 22 without a context, a workspace or ANY allocation: for callers that cannot
+ * call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid it).
+ *   u_padded  DEVICE pointer, read only: the padded conserved store [5][pz][py][px] fp64 exactly as ch_get_padded
+ *             lays it out (x fastest, nghost layers on every face of an active dimension, none on an inactive one)
+ *   nx,ny,nz,nghost  as ch_init;  gamma > 1;  dx,dy,dz > 0 the cell widths;  cfl in (0,1]
+ *   dt_out    DEVICE pointer on the same GPU, 1 double, written by the last kernel: cfl * min_d dx_d/(|v_d|+a) over
+ *             the real cells — the value ch_compute_dt returns for that state, bit for bit — or NaN if a cell has
+ *             rho <= 0 or a non-finite value (nothing is read back: the return code cannot say so)
+ *   stream    cudaStream_t (NULL = default stream); the call only enqueues (one 8-byte memset, two kernels)
+ * The reduction's scratch (one partial maximum per 256 cells) lives in a file-scope device array of 524 544 bytes
+ * that every GPU which loads the library holds until exit, so a grid may have at most ch_noalloc_max_cells() =
+ * 16 777 216 real cells (256^3): CH_EINVAL with a message naming the limit beyond it, and for bad arguments or
+ * pointers that are not device memory of one GPU.  All calls share that array and it keeps the last call's contents
+ * (the flag that must start at zero is cleared on `stream` at the start of every call): calls that may OVERLAP on the
+ * GPU — different streams without an ordering between them — race on it; calls on one stream, or ordered by events,
+ * are safe.  The array's device address is looked up once per device (cudaGetSymbolAddress) at the first call on that
+ * device; ch_noalloc_setup() does the look-up for the CURRENT device ahead of time (call it before a graph capture
+ * starts).  No call here uses cudaMalloc, cudaFree, cudaHostAlloc or a library routine that allocates. */
+int ch_dt_noalloc(const double* u_padded, int nx, int ny, int nz, int nghost, double gamma, double dx, double dy,
+                  double dz, double cfl, double* dt_out, void* stream);
+int ch_noalloc_setup(void);
+long long ch_noalloc_max_cells(void);
+
 #ifdef __cplusplus
 }
 #endif

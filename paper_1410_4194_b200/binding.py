@@ -29,7 +29,7 @@ SYMBOLS = ("ch_init", "ch_free", "ch_last_error", "ch_set_spacing", "ch_padded_c
            "ch_bind", "ch_set_state", "ch_get_state", "ch_set_padded", "ch_get_padded", "ch_compute_dt",
            "ch_step", "ch_step_cfl", "ch_last_dt", "ch_elapsed", "ch_set_solver", "ch_set_reconstruction", "ch_set_hcorrection", "ch_set_option", "ch_tiling", "ch_set_noh", "ch_set_time", "ch_get_time", "ch_fill_ghosts",
            "ch_halo_cells", "ch_halo_pack", "ch_halo_unpack", "ch_fill_dim", "ch_set_origin", "ch_sync", "ch_kernel_launches", "ch_profile", "ch_profile_read", "ch_kernel_name",
-           "ch_fp64_peak_probe", "ch_issue_mix_probe")
+           "ch_fp64_peak_probe", "ch_issue_mix_probe", "ch_dt_noalloc", "ch_noalloc_setup", "ch_noalloc_max_cells")
 K_COUNT = 11
 OPT_MARCH_SEG, OPT_FINAL_SEG, OPT_TMA, OPT_UNFUSED, OPT_GRAPH, OPT_FOLD_GHOST = 0, 1, 2, 3, 4, 5
 
@@ -115,6 +115,13 @@ def load_library() -> C.CDLL:
     L.ch_fp64_peak_probe.argtypes = [vp, C.c_int, C.c_int, C.c_int, vp]
     L.ch_issue_mix_probe.restype = C.c_double
     L.ch_issue_mix_probe.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.c_int, vp]
+    L.ch_dt_noalloc.restype = C.c_int
+    L.ch_dt_noalloc.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double, C.c_double,
+                                C.c_double, vp, vp]
+    L.ch_noalloc_setup.restype = C.c_int
+    L.ch_noalloc_setup.argtypes = []
+    L.ch_noalloc_max_cells.restype = C.c_longlong
+    L.ch_noalloc_max_cells.argtypes = []
     _lib = L
     return L
 
@@ -338,3 +345,26 @@ def issue_mix_probe(blocks=148 * 4, threads=512, iters=100000, device="cuda:0"):
     t_fp64 = per_iter[0] / 8.0
     t_alu = (per_iter[32] - per_iter[0]) / 32.0
     return dict(t_fp64=t_fp64, t_alu=t_alu, t_alu_16=(per_iter[16] - per_iter[0]) / 16.0, ms=ms)
+
+
+def noalloc_max_cells() -> int:
+    """Largest number of real cells ch_dt_noalloc serves (its scratch is a fixed file-scope device array)."""
+    return int(load_library().ch_noalloc_max_cells())
+
+
+def dt_noalloc(u_padded, nx, ny, nz, nghost, gamma, dx, dy, dz, cfl, dt_out, stream=None):
+    """ch_dt_noalloc: Eq. 22 of the padded state `u_padded` (a CUDA float64 tensor laid out as Grid.get_padded) into
+    the one-element CUDA tensor `dt_out`, enqueued on `stream` (torch stream; default: the current one).  Allocates
+    nothing: argument marshalling only.  Raises ValueError for bad arguments or a grid beyond noalloc_max_cells()."""
+    import torch
+    L = load_library()
+    if not (u_padded.is_cuda and dt_out.is_cuda and u_padded.dtype == torch.float64 and dt_out.dtype == torch.float64):
+        raise ValueError("dt_noalloc: u_padded and dt_out must be CUDA float64 tensors")
+    if not u_padded.is_contiguous():
+        raise ValueError("dt_noalloc: u_padded must be contiguous")
+    st = stream if stream is not None else torch.cuda.current_stream(u_padded.device)
+    rc = L.ch_dt_noalloc(u_padded.data_ptr(), int(nx), int(ny), int(nz), int(nghost), float(gamma), float(dx), float(dy),
+                         float(dz), float(cfl), dt_out.data_ptr(), st.cuda_stream)
+    if rc != 0:
+        err = last_error()
+        raise (ValueError if rc == -1 else RuntimeError)("ch_dt_noalloc: " + err)

@@ -30,6 +30,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <limits>
+#include <mutex>
 #include <vector>
 #include <new>
 #include <string>
@@ -2676,6 +2677,149 @@ double ch_fp64_peak_probe(double* sink, int blocks, int threads, int iters, void
   cudaEventDestroy(e0); cudaEventDestroy(e1);
   if (e != cudaSuccess) { cuda_fail(e, "ch_fp64_peak_probe"); return -1.0; }
   return (double)ms;
+}
+
+}  // extern "C"
+
+// ---------------------------------------------------------------------------------------------
+// ch_dt_noalloc: Eq. 22 for callers that cannot allocate (code under CUDA graph capture, tight serving
+// loops, harnesses that forbid cudaMalloc).  A variant of k_dt: the same cell_rate per cell, but the grid reduction
+// goes through per-CTA partial maxima kept in a FILE-SCOPE device array instead of the reduction cells of a bound
+// workspace, and a second one-CTA kernel finishes dt = cfl / max on the device.  No context, no workspace, no
+// cudaMalloc / cudaFree / cudaHostAlloc: the caller passes the padded state (input) and one double (output).
+//   scratch: g_na_scratch, 32 header cells + 65536 partial maxima = 524 544 B, held by every GPU that loads the
+//   library until exit; one partial per CTA of 256 cells => at most kNaMaxCells = 16 777 216 real cells (256^3).
+// In host code the NAME g_na_scratch is a host-side stand-in, not a device address: the address each device gave
+// the array is asked once per device, with that device current, through cudaGetSymbolAddress, and that is what the
+// kernels get.  Every call shares the array and it keeps the last call's contents: the non-physical flag is cleared
+// at the start of each call (the partials a call reads it has written itself); two calls that overlap on the GPU
+// (different streams, no ordering) race on it.
+// ---------------------------------------------------------------------------------------------
+namespace {
+
+constexpr int kNaThreads = 256;
+constexpr int kNaBlocks = 65536;                                        // partial maxima the scratch holds
+constexpr int kNaHeader = 32;                                           // [0] non-physical flag; rest unused (alignment)
+constexpr long long kNaMaxCells = (long long)kNaBlocks * kNaThreads;    // 16 777 216 real cells
+constexpr int kNaMaxDevices = 64;
+
+static __device__ __align__(256) unsigned long long g_na_scratch[kNaHeader + kNaBlocks];
+
+// one CTA per 256 real cells: its maximum of (|v_d| + a) / dx_d -> scratch[kNaHeader + blockIdx.x]
+__global__ void __launch_bounds__(kNaThreads) k_dt_partials(const StepArgs A, unsigned long long* __restrict__ scratch) {
+  __shared__ double s_max[kNaThreads / 32];
+  __shared__ int s_bad;
+  const Geom& g = A.geo;
+  const long long N = (long long)g.n[0] * g.n[1] * g.n[2];
+  const long long id = (long long)blockIdx.x * kNaThreads + threadIdx.x;
+  if (threadIdx.x == 0) s_bad = 0;
+  __syncthreads();
+  double t = 0.0;
+  bool bad = false;
+  if (id < N) {
+    const int i = (int)(id % g.n[0]);
+    const long long r = id / g.n[0];
+    const int j = (int)(r % g.n[1]);
+    const int k = (int)(r / g.n[1]);
+    const long long q = (long long)(i + g.g[0]) + (long long)(j + g.g[1]) * g.st[1] + (long long)(k + g.g[2]) * g.st[2];
+    t = cell_rate(A, A.u[q], A.u[g.np + q], A.u[2 * g.np + q], A.u[3 * g.np + q], A.u[4 * g.np + q], bad);
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) t = fmax(t, __shfl_xor_sync(0xffffffffu, t, o));
+  if (__any_sync(0xffffffffu, bad) && (threadIdx.x & 31) == 0) s_bad = 1;
+  if ((threadIdx.x & 31) == 0) s_max[threadIdx.x >> 5] = t;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double v = s_max[0];
+#pragma unroll
+    for (int w = 1; w < kNaThreads / 32; ++w) v = fmax(v, s_max[w]);
+    scratch[kNaHeader + blockIdx.x] = (unsigned long long)__double_as_longlong(v);
+    if (s_bad) atomicOr(scratch, 1ULL);
+  }
+}
+
+// one CTA: maximum of the partials, dt = cfl * (1 / max) rounded as ch_compute_dt rounds it on the host;
+// NaN if a non-physical cell (rho <= 0 or non-finite) was met
+__global__ void __launch_bounds__(1024) k_dt_finish(const unsigned long long* __restrict__ scratch, int nblocks, double cfl,
+                                                    double* __restrict__ dt_out) {
+  __shared__ double s_max[32];
+  double v = 0.0;
+  for (int b = threadIdx.x; b < nblocks; b += blockDim.x) v = fmax(v, __longlong_as_double((long long)scratch[kNaHeader + b]));
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
+  if ((threadIdx.x & 31) == 0) s_max[threadIdx.x >> 5] = v;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    for (int w = 1; w < (int)(blockDim.x >> 5); ++w) v = fmax(v, s_max[w]);
+    dt_out[0] = scratch[0] != 0ULL ? __longlong_as_double(0x7FF8000000000000LL) : __dmul_rn(cfl, __ddiv_rn(1.0, v));
+  }
+}
+
+std::mutex g_na_mutex;
+unsigned long long* g_na_ptr[kNaMaxDevices] = {};     // device address of g_na_scratch, per device (nullptr: not asked yet)
+
+// the device address of the scratch array on `dev` (which must be current)
+int na_scratch(int dev, unsigned long long** out) {
+  if (dev < 0 || dev >= kNaMaxDevices) return fail(CH_EINVAL, "ch_dt_noalloc: device index beyond 63");
+  std::lock_guard<std::mutex> lock(g_na_mutex);
+  if (!g_na_ptr[dev]) {
+    unsigned long long* p = nullptr;
+    CH_CUDA(cudaGetSymbolAddress((void**)&p, g_na_scratch), "cudaGetSymbolAddress(g_na_scratch)");
+    if (!p) return fail(CH_ECUDA, "ch_dt_noalloc: cudaGetSymbolAddress returned a null address");
+    g_na_ptr[dev] = p;
+  }
+  *out = g_na_ptr[dev];
+  return CH_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+long long ch_noalloc_max_cells(void) { return kNaMaxCells; }
+
+int ch_noalloc_setup(void) {
+  int dev = -1;
+  CH_CUDA(cudaGetDevice(&dev), "cudaGetDevice");
+  unsigned long long* p = nullptr;
+  return na_scratch(dev, &p);
+}
+
+int ch_dt_noalloc(const double* u_padded, int nx, int ny, int nz, int nghost, double gamma, double dx, double dy, double dz,
+                  double cfl, double* dt_out, void* stream) {
+  if (!u_padded || !dt_out) return fail(CH_EINVAL, "ch_dt_noalloc: null pointer");
+  if (!(gamma > 1.0) || !std::isfinite(gamma)) return fail(CH_EINVAL, "ch_dt_noalloc: gamma must be > 1");
+  if (!(cfl > 0.0) || !(cfl <= 1.0)) return fail(CH_EINVAL, "ch_dt_noalloc: cfl not in (0,1]");
+  if (!(dx > 0.0) || !(dy > 0.0) || !(dz > 0.0) || !std::isfinite(dx) || !std::isfinite(dy) || !std::isfinite(dz))
+    return fail(CH_EINVAL, "ch_dt_noalloc: cell widths must be positive");
+  StepArgs A = {};
+  if (!geometry(nx, ny, nz, nghost, A.geo)) return fail(CH_EINVAL, "ch_dt_noalloc: bad grid (n >= 1, nghost >= 3, active n >= nghost)");
+  const long long N = (long long)nx * ny * nz;
+  if (N > kNaMaxCells)
+    return fail(CH_EINVAL, "ch_dt_noalloc: more than 16777216 real cells (256^3): the static scratch holds one partial maximum "
+                           "per 256 cells, 65536 of them; use ch_compute_dt with a bound workspace for larger grids");
+  cudaPointerAttributes pa, pb;
+  if (cudaPointerGetAttributes(&pa, u_padded) != cudaSuccess || pa.type != cudaMemoryTypeDevice ||
+      cudaPointerGetAttributes(&pb, dt_out) != cudaSuccess || pb.type != cudaMemoryTypeDevice || pa.device != pb.device) {
+    cudaGetLastError();
+    return fail(CH_EINVAL, "ch_dt_noalloc: u_padded and dt_out must be device memory of one GPU");
+  }
+  DeviceGuard guard(pa.device);
+  unsigned long long* scratch = nullptr;
+  int rc = na_scratch(pa.device, &scratch);
+  if (rc != CH_OK) return rc;
+  A.gas.gamma = gamma; A.gas.gm1 = gamma - 1.0;                  // all cell_rate reads of the gas
+  const double w[3] = {dx, dy, dz};
+  for (int d = 0; d < 3; ++d) { A.dx[d] = w[d]; A.idx[d] = 1.0 / w[d]; A.dtdx[d] = 0.0; }
+  A.u = const_cast<double*>(u_padded);                           // read only
+  A.ext = 1;
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  const int nblocks = (int)((N + kNaThreads - 1) / kNaThreads);
+  CH_CUDA(cudaMemsetAsync(scratch, 0, sizeof(unsigned long long), st), "ch_dt_noalloc: clearing the flag");   // must start at zero
+  k_dt_partials<<<(unsigned)nblocks, kNaThreads, 0, st>>>(A, scratch);
+  k_dt_finish<<<1, 1024, 0, st>>>(scratch, nblocks, cfl, dt_out);
+  CH_CUDA(cudaGetLastError(), "ch_dt_noalloc kernels");
+  return CH_OK;
 }
 
 }  // extern "C"
