@@ -1962,18 +1962,25 @@ int march_segment(const ch_ctx* c, int d) {
   return seg;
 }
 
-// Planes a CTA of the fused second half marches: at least four waves of CTAs on small grids (a segment costs two
-// light planes), 64 planes on large ones; CH_OPT_FINAL_SEG overrides.
+// Planes a CTA of the fused second half marches (8, 16, 32 or 64); CH_OPT_FINAL_SEG overrides.
 int final_segment(const ch_ctx* c) {
   const Geom& g = c->geo;
   if (c->final_seg) return c->final_seg;
   const bool tma = c->tma_ok && c->use_tma;
   const int px = tma ? tma_pitch_x(g) : kFX - 2;
   const long long tiles = (long long)((g.n[0] + px - 1) / px) * ((g.n[1] + (tma ? kTY : kFY) - 3) / ((tma ? kTY : kFY) - 2));
-  const long long want = tiles * g.n[2] / (148LL * 4);
-  int seg = 8;
-  while (seg < 64 && seg * 2 <= want) seg *= 2;
-  return seg;
+  // a CTA costs its planes plus about three of start-up (two light planes and the fill of the staging ring), and CTAs
+  // run in waves of one per SM (two for the plain-load form): the segment with the smallest waves x (planes + 3),
+  // which reproduces the measured order at 64^3 ... 512^3 (profiles/r02_experiments.md)
+  const long long per_wave = tma ? 148 : 296;
+  int best = 8;
+  long long best_cost = -1;
+  for (int seg = 8; seg <= 64; seg *= 2) {
+    const long long ctas = tiles * ((g.n[2] + seg - 1) / seg);
+    const long long cost = ((ctas + per_wave - 1) / per_wave) * ((seg < g.n[2] ? seg : g.n[2]) + 3);
+    if (best_cost < 0 || cost <= best_cost) { best = seg; best_cost = cost; }
+  }
+  return best;
 }
 
 }  // namespace
@@ -2254,7 +2261,6 @@ int step_impl(ch_ctx* c, double dt, bool devdt) {
     Bracket b(c, CH_K_FINAL);
     k_final3d_tma<1, true><<<tgrid, kTT, tsmem, st>>>(A, c->maps, seg);
   } else if (three_d && !c->unfused && !c->hcorr) {
-    // at least four waves of CTAs on small grids (a segment costs two light planes), 64 planes on large ones
     const int seg = final_segment(c);
     dim3 grid((unsigned)((g.n[0] + kFX - 3) / (kFX - 2)), (unsigned)((g.n[1] + kFY - 3) / (kFY - 2)),
               (unsigned)((g.n[2] + seg - 1) / seg));
