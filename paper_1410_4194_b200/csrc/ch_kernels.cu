@@ -1970,13 +1970,16 @@ int final_segment(const ch_ctx* c) {
   const int px = tma ? tma_pitch_x(g) : kFX - 2;
   const long long tiles = (long long)((g.n[0] + px - 1) / px) * ((g.n[1] + (tma ? kTY : kFY) - 3) / ((tma ? kTY : kFY) - 2));
   // a CTA costs its planes plus about three of start-up (two light planes and the fill of the staging ring), and CTAs
-  // run in waves of one per SM (two for the plain-load form): the segment with the smallest waves x (planes + 3),
-  // which reproduces the measured order at 64^3 ... 512^3 (profiles/r02_experiments.md)
+  // run in waves of one per SM (two for the plain-load form): among the segments that leave at least four waves of
+  // CTAs (work that is not uniform -- a blast wave in a corner of the box -- needs them to balance: Sedov 128^3 loses
+  // 8 % with one wave of 64-plane CTAs where the uniform sweep gains 2 %) the one with the smallest
+  // waves x (planes + 3), which reproduces the measured order at 64^3 ... 512^3 (profiles/r02_experiments.md)
   const long long per_wave = tma ? 148 : 296;
   int best = 8;
   long long best_cost = -1;
   for (int seg = 8; seg <= 64; seg *= 2) {
     const long long ctas = tiles * ((g.n[2] + seg - 1) / seg);
+    if (seg > 8 && ctas < 4 * per_wave) break;
     const long long cost = ((ctas + per_wave - 1) / per_wave) * ((seg < g.n[2] ? seg : g.n[2]) + 3);
     if (best_cost < 0 || cost <= best_cost) { best = seg; best_cost = cost; }
   }
