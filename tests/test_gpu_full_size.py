@@ -124,6 +124,30 @@ def test_whole_grid_parity_256_sweep(ref):
     assert max(strict) <= ONE_STEP_TOL, strict
 
 
+# the paper's other method choices on every cell of the 256^3 grid
+METHODS_256 = {
+    "ppmc_roe": (3, lambda G: G.set_solver(1)),
+    "plmc_exact": (3, lambda G: G.set_reconstruction(1)),
+    "plmc_roe": (3, lambda G: (G.set_solver(1), G.set_reconstruction(1))),
+    "plmp_exact": (3, lambda G: G.set_reconstruction(4)),
+    "ppmp_exact": (4, lambda G: G.set_reconstruction(3)),
+}
+
+
+@pytest.mark.parametrize("name", sorted(METHODS_256))
+def test_whole_grid_parity_256_other_methods(ref, name):
+    """Every cell of the 256^3 throughput-sweep grid after one GPU step with each of the paper's other reconstructions
+    and with the Roe + HLLE solver, in the launch configuration bench.py times them in."""
+    g, setup = METHODS_256[name]
+    w = wl.sweep(256)
+    post, ur, _ = whole_grid_one_step(ref, w, pre_steps=1, g=g, setup=setup)
+    err = max_rel_error(post, ur, w.gamma)
+    strict = max_rel_error_strict(post, ur, w.gamma)
+    print(f"whole-grid 256^3 sweep, {name}: S11 norm", err, "strict", strict)
+    assert max(err) <= ONE_STEP_TOL, (name, err)
+    assert max(strict) <= ONE_STEP_TOL, (name, strict)
+
+
 @pytest.mark.parametrize("n", [384, 512])
 def test_whole_grid_parity_at_the_largest_sizes(ref, n):
     """Every cell of the 384^3 and the 512^3 grid (the size bench.py times; 1.3e8 cells x 5 fields) after one GPU
