@@ -69,12 +69,12 @@ struct StepArgs {
 };
 
 // dt / dx_d of this step: from the kernel arguments (ch_step) or from the device-resident dt (ch_step_cfl), with
-// the same correctly rounded division the host does, so the two ways of stepping agree bitwise
+// the same correctly rounded division the host does (done once, by k_pick_dt: a division per thread was 3 % of
+// k_pass1_x, whose threads live for one cell), so the two ways of stepping agree bitwise
 __device__ __forceinline__ void step_dtdx(const StepArgs& A, double out[3]) {
   if (A.dt_dev) {
-    const double dt = *A.dt_dev;
 #pragma unroll
-    for (int d = 0; d < 3; ++d) out[d] = __ddiv_rn(dt, A.dx[d]);
+    for (int d = 0; d < 3; ++d) out[d] = A.dt_dev[2 + d];      // k_pick_dt's correctly rounded dt / dx_d
   } else {
 #pragma unroll
     for (int d = 0; d < 3; ++d) out[d] = A.dtdx[d];
@@ -82,7 +82,7 @@ __device__ __forceinline__ void step_dtdx(const StepArgs& A, double out[3]) {
 }
 
 __device__ __forceinline__ double step_dtdx1(const StepArgs& A, int d) {   // one direction only (pass 1)
-  return A.dt_dev ? __ddiv_rn(*A.dt_dev, A.dx[d]) : A.dtdx[d];
+  return A.dt_dev ? A.dt_dev[2 + d] : A.dtdx[d];
 }
 
 // ch_step_cfl on a non-physical state: k_pick_dt leaves dt = NaN; every kernel of the step then returns at once,
@@ -627,8 +627,9 @@ __device__ __forceinline__ void block_max_reduce(double t, bool bad, unsigned lo
 
 // ch_step_cfl: Eq. 22 finished on the device.  red[0] holds the grid maximum of (|v_d| + a)/dx_d of the current
 // state; dt = cfl * (1 / rate) exactly as ch_compute_dt forms it on the host, clipped to t_left if that is
-// positive and smaller.  red[2] <- dt (NaN if a non-physical cell was met), red[3] += dt.
-__global__ void k_pick_dt(unsigned long long* red, double cfl, double t_left) {
+// positive and smaller.  red[2] <- dt (NaN if a non-physical cell was met), red[3] += dt, red[4..6] <- dt / dx_d.
+struct Dx3 { double v[3]; };
+__global__ void k_pick_dt(unsigned long long* red, double cfl, double t_left, Dx3 dx) {
   if (threadIdx.x != 0) return;
   double dt = __dmul_rn(cfl, __ddiv_rn(1.0, __longlong_as_double((long long)red[0])));
   if (t_left > 0.0 && dt > t_left) dt = t_left;
@@ -639,6 +640,8 @@ __global__ void k_pick_dt(unsigned long long* red, double cfl, double t_left) {
   }
   r[2] = dt;
   r[3] += dt;
+#pragma unroll
+  for (int d = 0; d < 3; ++d) r[4 + d] = __ddiv_rn(dt, dx.v[d]);
   red[0] = 0ULL; red[1] = 0ULL;     // the step that follows reduces its new state into clean cells (k_reset's work)
 }
 
@@ -2352,6 +2355,8 @@ int ch_step_cfl(ch_ctx* c, double cfl, double t_left) {
   if (c->has_exchange) return fail(CH_ESTATE, "ch_step_cfl: a block of a decomposed domain needs the global minimum of dt: use ch_compute_dt + ch_step");
   if (c->has_noh) return fail(CH_ESTATE, "ch_step_cfl: an analytic (CH_BC_NOH) face needs the time on the host: use ch_compute_dt + ch_step");
   DeviceGuard guard(c->device);
+  Dx3 dx3;
+  for (int d = 0; d < 3; ++d) dx3.v[d] = c->dx[d];
   if (!c->dt_valid) {
     StepArgs A = make_args(c, 1.0);
     { Bracket b(c, CH_K_RESET); k_reset<<<1, 32, 0, c->stream>>>(c->red, nullptr); }
@@ -2381,7 +2386,7 @@ int ch_step_cfl(ch_ctx* c, double cfl, double t_left) {
     }
     if (c->gexec) {
       if (cfl != c->gcfl || t_left != c->gtleft) {
-        void* args[3] = {(void*)&c->red, (void*)&cfl, (void*)&t_left};
+        void* args[4] = {(void*)&c->red, (void*)&cfl, (void*)&t_left, (void*)&dx3};
         cudaKernelNodeParams kp = {};
         kp.func = (void*)k_pick_dt;
         kp.gridDim = dim3(1); kp.blockDim = dim3(32); kp.sharedMemBytes = 0; kp.kernelParams = args; kp.extra = nullptr;
@@ -2395,7 +2400,7 @@ int ch_step_cfl(ch_ctx* c, double cfl, double t_left) {
     }
   }
   if (!graphs || c->gseen++ == 0) {
-    { Bracket b(c, CH_K_PICK_DT); k_pick_dt<<<1, 32, 0, c->stream>>>(c->red, cfl, t_left); }
+    { Bracket b(c, CH_K_PICK_DT); k_pick_dt<<<1, 32, 0, c->stream>>>(c->red, cfl, t_left, dx3); }
     CH_CUDA(cudaGetLastError(), "k_pick_dt");
     return step_dispatch(c, 0.0, true);
   }
@@ -2413,7 +2418,7 @@ int ch_step_cfl(ch_ctx* c, double cfl, double t_left) {
   CH_CUDA(cudaStreamBeginCapture(c->cap_stream, cudaStreamCaptureModeThreadLocal), "cudaStreamBeginCapture");
   c->stream = c->cap_stream;
   c->capturing = true;
-  { Bracket b(c, CH_K_PICK_DT); k_pick_dt<<<1, 32, 0, c->stream>>>(c->red, cfl, t_left); }
+  { Bracket b(c, CH_K_PICK_DT); k_pick_dt<<<1, 32, 0, c->stream>>>(c->red, cfl, t_left, dx3); }
   const int rc = step_dispatch(c, 0.0, true);
   c->capturing = false;
   c->stream = user;
@@ -2438,14 +2443,14 @@ int ch_step_cfl(ch_ctx* c, double cfl, double t_left) {
     if (graph) cudaGraphDestroy(graph);
     cudaGetLastError();
     c->use_graph = false;                  // fall back to direct launches for this context
-    { Bracket b(c, CH_K_PICK_DT); k_pick_dt<<<1, 32, 0, c->stream>>>(c->red, cfl, t_left); }
+    { Bracket b(c, CH_K_PICK_DT); k_pick_dt<<<1, 32, 0, c->stream>>>(c->red, cfl, t_left, dx3); }
     return step_dispatch(c, 0.0, true);
   }
   e = cudaGraphInstantiate(&c->gexec, graph, 0);
   if (e != cudaSuccess) {
     cudaGraphDestroy(graph);
     c->gexec = nullptr; cudaGetLastError(); c->use_graph = false;
-    { Bracket b(c, CH_K_PICK_DT); k_pick_dt<<<1, 32, 0, c->stream>>>(c->red, cfl, t_left); }
+    { Bracket b(c, CH_K_PICK_DT); k_pick_dt<<<1, 32, 0, c->stream>>>(c->red, cfl, t_left, dx3); }
     return step_dispatch(c, 0.0, true);
   }
   c->ggraph = graph; c->gpick = pick; c->gcfl = cfl; c->gtleft = t_left;
