@@ -66,7 +66,7 @@ typedef struct ch_buffers {
   double* state;          /* padded conserved store u, 5*Np doubles (SoA, x fastest) */
   void* workspace;        /* scratch, at least ch_workspace_bytes(...) bytes, 256-byte aligned */
   size_t workspace_bytes; /* size of `workspace` as allocated */
-  void* reduce;           /* 64 bytes, 8-byte aligned: device cells of the dt reduction (max wave rate, flag) */
+  void* reduce;           /* 64 bytes, 8-byte aligned: device cells of the dt reduction (max wave rate, flag; ch_step_cfl: dt, elapsed, dt/dx_d) */
 } ch_buffers;
 
 /* ch_init — create a context for an nx*ny*nz grid of real cells with `nghost` ghost layers on each
