@@ -128,6 +128,13 @@ CH_D void char_project(double ra, double ia2, double d0, double d1, double d2, d
   x[4] = __dmul_rn(0.5, __dadd_rn(t1, t2));
 }
 
+// The same limiter with the sign test on the high words instead of a product (limited_slope only: PPMP / PLMP keep the
+// product form above).  A vanishing one-sided difference needs no test of its own: the minimum is then zero.
+CH_D double mc_limit_bits(double dL, double dR, double dC) {
+  const double m = sel_min(fabs(dC), __dmul_rn(2.0, sel_min(fabs(dL), fabs(dR))));
+  return ((__double2hiint(dL) ^ __double2hiint(dR)) >= 0) ? copysign(m, dC) : 0.0;
+}
+
 CH_D void limited_slope(const Gas& G, const double wm[5], const double w0[5], const double wp[5], double s,
                         double dw[5]) {
   const double rho = w0[0];
@@ -145,7 +152,7 @@ CH_D void limited_slope(const Gas& G, const double wm[5], const double w0[5], co
                __dmul_rn(0.5, __dadd_rn(wp[2], -wm[2])), __dmul_rn(0.5, __dadd_rn(wp[3], -wm[3])),
                __dmul_rn(0.5, __dadd_rn(wp[4], -wm[4])), xC);
 #pragma unroll
-  for (int m = 0; m < 5; ++m) x[m] = mc_limit(xL[m], xR[m], xC[m]);
+  for (int m = 0; m < 5; ++m) x[m] = mc_limit_bits(xL[m], xR[m], xC[m]);
   const double s04 = __dadd_rn(x[0], x[4]);
   const double a2 = __dmul_rn(a, a);
   dw[0] = __dadd_rn(x[1], s04);
@@ -183,34 +190,30 @@ CH_D void ppmc_from_interfaces(const Gas& G, double dtdx, const double wm[5], co
   double WL[5], WR[5], dwi[5], w6[5];
 #pragma unroll
   for (int m = 0; m < 5; ++m) {
+    // A20-A24, A26 on the face DEVIATIONS dR = R - w, dL = w - L (round 2): every correction of A21-A23 is a clamp of
+    // a deviation, so the faces themselves are formed once, at the end.
+    //   A21: an extremum (dR dL <= 0) flattens the cell: both deviations vanish.
+    //   A22 (G8): (R - L)[L - (3w - 2R)] < 0 and (R - L)[(3w - 2L) - R] < 0 are (dR + dL)(2dR - dL) < 0 and
+    //     (dR + dL)(2dL - dR) < 0, i.e. |dL| > 2|dR| and |dR| > 2|dL| once A21 has made the signs agree; the replaced
+    //     faces 3w - 2R, 3w - 2L are the deviations 2dR, 2dL.  At most one fires; ties leave the face alone.
+    //   A23: L within [min(w_{i-1}, w), max(w_{i-1}, w)] says dL lies between 0 and tL = w - w_{i-1}:
+    //     opposite signs -> 0, |dL| > |tL| -> tL; likewise dR against tR = w_{i+1} - w.  Signs are compared on the high
+    //     words (a zero deviation passes either way and stays zero; a zero t is caught by the magnitude test).
+    //   A24 R - L = dR + dL; A26 as A50 (G2) 6[w - (L + R)/2] = 3(dL - dR), free of the cancellation.
     const double wi = w0[m];
-    double L = LA[m];                                                  // A20
-    double R = RA[m];
-    // A21 and A22 (G8) on the deviations dR = R - w, dL = w - L.  After A21 they have the same
-    // sign (or both vanish), and A22's tests (R - L)[L - (3w - 2R)] < 0, (R - L)[(3w - 2L) - R] < 0 are
-    // (dR + dL)(2dR - dL) < 0 and (dR + dL)(2dL - dR) < 0, i.e. |dL| > 2|dR| and |dR| > 2|dL|: two compares instead of
-    // two products; the replaced values 3w - 2R = w - 2dR and 3w - 2L = w + 2dL.  Ties (equality) leave the face alone
-    // in both forms; where nothing fires L and R keep the bits of A20.
-    double dR = R - wi, dL = wi - L;
-    if (dR * dL <= 0.0) { L = wi; R = wi; dR = 0.0; dL = 0.0; }
-    const double dR2 = dR + dR, dL2 = dL + dL;
-    const bool fixL = fabs(dL) > fabs(dR2);
-    const bool fixR = fabs(dR) > fabs(dL2);
-    if (fixL) L = wi - dR2;
-    if (fixR) R = wi + dL2;
-    {                                                                  // A23
-      const bool up = wm[m] < wi;
-      const double lo = up ? wm[m] : wi, hi = up ? wi : wm[m];
-      L = sel_min(hi, sel_max(lo, L));
-    }
-    {
-      const bool up = wp[m] < wi;
-      const double lo = up ? wp[m] : wi, hi = up ? wi : wp[m];
-      R = sel_min(hi, sel_max(lo, R));
-    }
-    WL[m] = L; WR[m] = R;
-    dwi[m] = R - L;                                                    // A24
-    w6[m] = 6.0 * (wi - 0.5 * (L + R));                                // A26 as A50 (G2)
+    const double dR0 = RA[m] - wi, dL0 = wi - LA[m];
+    const double tL = wi - wm[m], tR = wp[m] - wi;
+    const bool ext = dR0 * dL0 <= 0.0;
+    const double dR1 = ext ? 0.0 : dR0, dL1 = ext ? 0.0 : dL0;
+    const double dR2 = dR1 + dR1, dL2 = dL1 + dL1;
+    const bool fixL = fabs(dL1) > fabs(dR2), fixR = fabs(dR1) > fabs(dL2);
+    const double dL3 = fixL ? dR2 : dL1, dR3 = fixR ? dL2 : dR1;
+    const bool oppL = (__double2hiint(dL3) ^ __double2hiint(tL)) < 0, oppR = (__double2hiint(dR3) ^ __double2hiint(tR)) < 0;
+    const double cL = (fabs(dL3) > fabs(tL)) ? tL : dL3, cR = (fabs(dR3) > fabs(tR)) ? tR : dR3;
+    const double dL = oppL ? 0.0 : cL, dR = oppR ? 0.0 : cR;
+    WL[m] = wi - dL; WR[m] = wi + dR;
+    dwi[m] = dR + dL;
+    w6[m] = 3.0 * (dL - dR);
   }
   const double rho = w0[0];
   const double a = G.gamma * w0[4] * s;

@@ -448,14 +448,20 @@ def test_anisotropic_spacing_one_step_and_dt(ch, ref):
 def test_tma_and_plain_load_forms_of_the_fused_kernel_are_bitwise_equal(ch):
     """k_final3d_tma (TMA-staged planes, producer warp) and k_final3d (plain coalesced loads) run the same
     arithmetic in the same order on every cell: same bits, including the Eq. 22 reduction.  Shapes: even
-    padded strides (TMA applies), ragged tiles in x (30), y (TY-2) and z (64-plane segments)."""
-    for w in (wl.rough_random(44, 26, 70, seed=31, decades=0.5), wl.sweep(shape=(64, 40, 36)), wl.sedov(24)):
+    padded strides (TMA applies), ragged tiles in x (30), y (TY-2) and z (64-plane segments).
+    The rough state with jumps of a decade (decades=0.5) is compared after ONE step: the oracle's pressure is
+    already negative somewhere after that step (-1.1 before the floor) and it returns NaN two steps later, so a
+    second step of it is not a step of the method; the state with jumps of 10^0.6 stays physical (oracle: p >= 0.3
+    after three steps) and is stepped twice like the others."""
+    for w, nsteps in ((wl.rough_random(44, 26, 70, seed=31, decades=0.5), 1),
+                      (wl.rough_random(44, 26, 70, seed=31, decades=0.3, mach=0.8), 2),
+                      (wl.sweep(shape=(64, 40, 36)), 2), (wl.sedov(24), 2)):
         res = {}
         for mode in ("1", "0"):
             G = ch.Grid(*w.shape, 3, w.gamma, w.bc)
             G.set_option(binding.OPT_TMA, int(mode))
             G.set_state(w.u)
-            for _ in range(2):
+            for _ in range(nsteps):
                 G.step(G.compute_dt(w.cfl))
             res[mode] = (G.get_padded(), G.compute_dt(w.cfl))
             G.close()
