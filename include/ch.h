@@ -196,7 +196,10 @@ int ch_set_origin(ch_ctx* ctx, int i0, int j0, int k0);
  * times.  Nothing here is read from the environment.
  *   CH_OPT_MARCH_SEG  cells a thread of the marching pass-1 kernels sweeps (0 = chosen from the grid size; >= 4)
  *   CH_OPT_FINAL_SEG  planes a CTA of the fused second half marches (0 = chosen from the grid size; >= 4)
- *   CH_OPT_TMA        1 (default): the TMA-fed fused second half where the padded strides allow it; 0: plain loads
+ *   CH_OPT_TMA        the fused second half of 3-D grids where the padded strides allow TMA: 2 (default) planes staged by TMA,
+ *                     13-row tiles, the producer's work done by a lane of the warp that serves the halo rows; 1: 12-row
+ *                     tiles with a producer warp of its own (the form the H-corrected step always takes); 0: plain loads.
+ *                     The three forms give the same bits.  Other values: CH_EINVAL
  *   CH_OPT_UNFUSED    1: run the second half as k_pass2 + k_update on 3-D grids too (A/B measurements); default 0
  *   CH_OPT_GRAPH      1 (default): ch_step_cfl replays the kernels of a step as one CUDA graph from the third step with a
  *                     configuration on (captured on a private stream; the same kernels, the same bits); 0: direct launches

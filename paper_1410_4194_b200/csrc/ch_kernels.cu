@@ -6,8 +6,10 @@
 //   k_pass1_march<1|2> same along y / z, marching in registers  -> U*_L,U*_R(.,d), G*, H*
 //   k_final3d_tma      3-D grids: Eq. 23 transverse correction + second exact Riemann pass + Eq. 24
 //   (k_final3d)        update + Eq. 22 reduction of the new state, fused (steps 3-5; F,G,H^{n+1/2} stay on
-//                      chip); planes staged by TMA from a producer warp (plain loads where TMA's
-//                      16-byte stride rules do not hold, or with CH_OPT_TMA = 0)
+//                      chip); planes staged by TMA, issued by a lane of the warp that serves the halo rows
+//                      (13-row tiles, eleven updating warps; CH_OPT_TMA = 1: a producer warp of its own and
+//                      12-row tiles, the form the H-corrected step takes); plain loads where TMA's 16-byte
+//                      stride rules do not hold, or with CH_OPT_TMA = 0
 //   k_final2d          the same for x-y grids (one plane, no z carry)
 //   k_pass2, k_update  the same two halves unfused: 1-D, x-z / y-z grids, the H-corrected step without TMA (+ k_eta)
 //   k_eta3d            H correction on 3-D grids: eta of every interface (C1), tiled march; k_final3d_tma<Roe, HC> then takes
@@ -1127,6 +1129,10 @@ __global__ void __launch_bounds__(kFT, 2) k_final2d(const StepArgs A, const Scat
 #define CH_T_SLEEP 200      // ns between the producer's polls of an empty barrier
 #endif
 constexpr int kTY = CH_T_TY, kTT = kFX * kTY, kTC = kTT - kFX;   // staged rows; threads = staged slots; consumer threads
+#ifndef CH_T_TYM
+#define CH_T_TYM 13
+#endif
+constexpr int kTYM = CH_T_TYM;                                   // staged rows of the merged-producer form (kTYM - 1 warps)
 struct TmaMaps { CUtensorMap m[13]; };              // Fs0 Fs1 Fs2 | UL2 UR2 | UL0 UR0 u | UL1 UR1 | eta0 eta1 eta2 (one field each)
 __device__ __forceinline__ constexpr int group_first(int q) { return q == 0 ? 0 : q == 1 ? 3 : q == 2 ? 5 : q == 3 ? 8 : 10; }   // arrays of group q: [first(q), first(q+1))
 
@@ -1180,8 +1186,19 @@ __device__ __forceinline__ void tma_load_4d(unsigned dst, const CUtensorMap* map
 // brings eta_x and eta_y of plane k and eta_z of the faces k-1/2 and k+1/2 (slots 70..73), every thread forms the
 // three maxima of C2 for its x, y and z interface from them (the stencil stays inside the staged box) and the Roe
 // solver takes them: the same values and the same solver as k_pass2<1, true>, so the two paths agree bitwise.
-template <int S, bool HC = false>
-__global__ void __launch_bounds__(kTT, 1) k_final3d_tma(const StepArgs A, const __grid_constant__ TmaMaps M, int seg) {
+// MP (round 2, last): the producer's work moves into lane 0 of the halo warp, which is idle two thirds of a plane, and
+// the warp that used to produce updates an eleventh row: TY = 13 staged rows, still twelve warps (three per scheduler
+// is what 152 registers allow), the schedulers that held two updating warps and a helper now hold three and two + the
+// halo warp.  Lane 0 refills group 0 right after the halo warp has read it, groups 1 and 2 once every consumer has
+// released them (the slowest updating warp is then past its z solve, so the halo warp still reaches the first
+// consumer barrier before it), group 3 after that barrier.  The carried H flux and partial sums are kept for the
+// updating rows only (227 840 B of dynamic shared memory).  Same arithmetic per cell: bitwise equal to the other forms.
+template <int S, bool HC = false, int TY = CH_T_TY, bool MP = false>
+__global__ void __launch_bounds__(kFX * (MP ? TY - 1 : TY), 1) k_final3d_tma(const StepArgs A, const __grid_constant__ TmaMaps M, int seg) {
+  constexpr int kTY = TY, kTT = kFX * TY;                  // staged rows, staged slots per field (shadow the file-scope pair)
+  constexpr int kTC = MP ? kTT - kFX : kTT - kFX;          // consumer threads: all threads with MP, all but the producer warp without
+  constexpr int kZS = MP ? kTT - 2 * kFX : kTT;            // slots of the carried arrays; with MP the updating rows only
+  static_assert(!(HC && MP), "the H-corrected form keeps the producer warp");
   extern __shared__ __align__(1024) double s_t[];
   __shared__ unsigned long long s_full[5], s_empty[5];
   typedef double (*Arr)[kTT];
@@ -1220,7 +1237,15 @@ __global__ void __launch_bounds__(kTT, 1) k_final3d_tma(const StepArgs A, const 
   }
   __syncthreads();
 
-  if (wid == kTY - 1) {
+  // issue the boxes of group q for plane k (any one thread)
+  auto issue_group = [&](int q, int k) {
+    const unsigned stage = (unsigned)__cvta_generic_to_shared(s_t);
+    const int a0 = group_first(q), a1 = group_first(q + 1);
+    mbar_expect_tx(bfull[q], (unsigned)((a1 - a0) * 5 * kTT * sizeof(double)));
+    for (int a = a0; a < a1; ++a)
+      tma_load_4d(stage + (unsigned)(a * 5 * kTT * sizeof(double)), &M.m[a], bfull[q], i0 + g.g[0], j0 + g.g[1], k + g.g[2], 0);
+  };
+  if (!MP && wid == kTY - 1) {
     // ===== producer warp: one lane streams the planes =====
     if (lane == 0) {
       const unsigned stage = (unsigned)__cvta_generic_to_shared(s_t);
@@ -1260,6 +1285,11 @@ __global__ void __launch_bounds__(kTT, 1) k_final3d_tma(const StepArgs A, const 
     const double hxh = 0.5 * dtx[0], hzh = 0.5 * dtx[2];
     double zSb[5] = {0.0, 0.0, 0.0, 0.0, 0.0}, zSt[5] = {0.0, 0.0, 0.0, 0.0, 0.0};   // F*_z of the previous plane, both rows
     int n = 0;
+    if (MP && lane == 0) {
+#pragma unroll
+      for (int q = 0; q < 4; ++q) issue_group(q, k0 - 1);
+    }
+    if (MP) __syncwarp();
     for (int k = k0 - 1; k <= k1; ++k, ++n) {
       const bool mid = k != k0 - 1 && k != k1;
       const unsigned ph = (unsigned)(n & 1);
@@ -1275,6 +1305,11 @@ __global__ void __launch_bounds__(kTT, 1) k_final3d_tma(const StepArgs A, const 
         dxt[f] = __dmul_rn(hxh, __shfl_up_sync(full, fxt, 1) - fxt);
       }
       mbar_arrive(bempty[0]);
+      if (MP) {
+        // producer point A: group 0 of the next plane as soon as every consumer has read this one's (they read it first)
+        if (lane == 0 && k < k1) { mbar_wait(bempty[0], ph); issue_group(0, k + 1); }
+        __syncwarp();
+      }
       double eHt = 0.0;
       if (HC) {
         // C2 for the y interface below row kTY-1 (cells q = st_ - kFX and st_)
@@ -1296,6 +1331,17 @@ __global__ void __launch_bounds__(kTT, 1) k_final3d_tma(const StepArgs A, const 
         ct[m] = __dadd_rn(stg0[40 + comp<1>(m)][st_], __dadd_rn(dzt[comp<1>(m)], dxt[comp<1>(m)]));      // U^{n+1/2}_L(., y), row kTY-1
       }
       mbar_arrive(bempty[3]);
+      if (MP) {
+        // producer point B: groups 1 and 2 once every consumer has released them (the slowest updating warp is then
+        // past its z solve and has its x solve ahead, so this warp is still not the last at the barrier below);
+        // group 3 here too on the two planes that have no barrier (the first and the last of a segment)
+        if (lane == 0 && k < k1) {
+          mbar_wait(bempty[1], ph); issue_group(1, k + 1);
+          mbar_wait(bempty[2], ph); issue_group(2, k + 1);
+          if (!mid) { mbar_wait(bempty[3], ph); issue_group(3, k + 1); }
+        }
+        __syncwarp();
+      }
       if (mid) {
         double wr0[5] = {1.0, 0.0, 0.0, 0.0, 1.0}, wlt[5] = {1.0, 0.0, 0.0, 0.0, 1.0}, nb[5], fl[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
         if (laneok) ch::cons2prim(A.gas, cb[0], cb[1], cb[2], cb[3], cb[4], wr0);
@@ -1312,6 +1358,12 @@ __global__ void __launch_bounds__(kTT, 1) k_final3d_tma(const StepArgs A, const 
 #pragma unroll
         for (int m = 0; m < 5; ++m) sF[m][st_] = fl[m];
         asm volatile("bar.sync 1, %0;" ::"n"(kTC) : "memory");
+        if (MP) {
+          // producer point C: every consumer read group 3 before the first barrier; issued after the second so that
+          // this warp is not the one the others wait for (the y states are not needed before the end of the next plane)
+          if (lane == 0 && k < k1) { mbar_wait(bempty[3], ph); issue_group(3, k + 1); }
+          __syncwarp();
+        }
       }
     }
   } else {
@@ -1329,10 +1381,12 @@ __global__ void __launch_bounds__(kTT, 1) k_final3d_tma(const StepArgs A, const 
   double zU[5] = {1.0, 0.0, 0.0, 0.0, 1.0};    // U^{n+1/2}_R(., z) of cell k-1, primitive, z-local order
   // the half of the z carry that is only read when cell k-1 is finished lives in shared memory (10 doubles per slot):
   // 164 -> 152 registers, the scheduler has room to interleave more, 2 % off this kernel
-  Arr zFs = reinterpret_cast<Arr>(s_t + 60 * kTT);    // H^{n+1/2} on the low z face of cell k-1, z-local order
-  Arr zPs = reinterpret_cast<Arr>(s_t + 65 * kTT);    // u + x and y flux differences of cell k-1, global order
-#define zF(m) zFs[m][sidx]
-#define zP(m) zPs[m][sidx]
+  typedef double (*ArrZ)[kZS];
+  ArrZ zFs = reinterpret_cast<ArrZ>(s_t + 60 * kTT);             // H^{n+1/2} on the low z face of cell k-1, z-local order
+  ArrZ zPs = reinterpret_cast<ArrZ>(s_t + 60 * kTT + 5 * kZS);   // u + x and y flux differences of cell k-1, global order
+  const int zidx = MP ? sidx - kFX : sidx;
+#define zF(m) zFs[m][zidx]
+#define zP(m) zPs[m][zidx]
   double zS[5] = {0.0, 0.0, 0.0, 0.0, 0.0};    // F*_z of cell k-1 (global field order)
   double mxyPrev = 0.0;                        // HC: largest eta on the x and y faces of cell k-1
   int n = 0;
@@ -1765,9 +1819,12 @@ struct ch_ctx {
   long long launches = 0;
   int march_seg = 0;         // cells a marching thread sweeps; 0 = chosen per launch from the grid size
   int final_seg = 0;         // planes a k_final3d CTA marches; 0 = chosen per launch
-  bool use_tma = true;       // CH_TMA=0: plain-load k_final3d even where the TMA form applies
+  int use_tma = 2;           // CH_OPT_TMA: 0 plain-load k_final3d even where the TMA form applies, 1 the TMA form with a producer
+                             // warp (12 staged rows), 2 the producer merged into the halo warp (13 staged rows; default)
   bool tma_ok = false;       // tensor maps built for the bound buffers
-  TmaMaps maps;
+  TmaMaps maps;              // boxes of kTY rows (producer-warp form, H-corrected form)
+  TmaMaps maps_mp;           // boxes of kTYM rows (merged-producer form); arrays 0..9 only
+  bool smem_attr_mp[2] = {false, false};
   int solver = 0;            // CH_SOLVER_EXACT
   int recon = 0;             // CH_RECON_PPMC
   bool hcorr = false;        // H correction (Appendix C): Roe solver, nghost >= 4; fused second half where the TMA form applies
@@ -1920,10 +1977,14 @@ bool build_tma_maps(ch_ctx* c) {
   const cuuint64_t dims[4] = {(cuuint64_t)g.pd[0], (cuuint64_t)g.pd[1], (cuuint64_t)g.pd[2], 5};
   const cuuint64_t strides[3] = {(cuuint64_t)g.pd[0] * 8, (cuuint64_t)g.st[2] * 8, (cuuint64_t)g.np * 8};
   const cuuint32_t box[4] = {(cuuint32_t)kFX, (cuuint32_t)kTY, 1, 5};
+  const cuuint32_t box_mp[4] = {(cuuint32_t)kFX, (cuuint32_t)kTYM, 1, 5};
   const cuuint32_t estr[4] = {1, 1, 1, 1};
   for (int a = 0; a < 10; ++a) {
     if ((uintptr_t)arr[a] & 15) return false;
     if (encode(&c->maps.m[a], CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, arr[a], dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+               CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+      return false;
+    if (encode(&c->maps_mp.m[a], CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, arr[a], dims, strides, box_mp, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
                CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
       return false;
   }
@@ -1943,6 +2004,12 @@ bool build_tma_maps(ch_ctx* c) {
 // Updated columns per tile of k_final3d_tma: 30 with an odd nghost, 28 with an even one (the box must start on an
 // even double: 16-byte alignment of the bulk tensor copy).
 int tma_pitch_x(const Geom& g) { return (g.g[0] & 1) ? kFX - 2 : kFX - 4; }
+// Updated rows per tile of the fused second half: the merged-producer TMA form (not the H-corrected step), the
+// producer-warp TMA form, the plain-load form.
+int final_rows(const ch_ctx* c) {
+  if (!(c->tma_ok && c->use_tma)) return kFY - 2;
+  return (c->use_tma == 2 && !c->hcorr) ? kTYM - 2 : kTY - 2;
+}
 
 // x-y grids whose four faces are periodic, reflective or outflow: the update kernel writes the ghost cells itself.
 bool scatter2d(const ch_ctx* c) {
@@ -1971,7 +2038,8 @@ int final_segment(const ch_ctx* c) {
   if (c->final_seg) return c->final_seg;
   const bool tma = c->tma_ok && c->use_tma;
   const int px = tma ? tma_pitch_x(g) : kFX - 2;
-  const long long tiles = (long long)((g.n[0] + px - 1) / px) * ((g.n[1] + (tma ? kTY : kFY) - 3) / ((tma ? kTY : kFY) - 2));
+  const int rows = final_rows(c);
+  const long long tiles = (long long)((g.n[0] + px - 1) / px) * ((g.n[1] + rows - 1) / rows);
   // a CTA costs its planes plus about three of start-up (two light planes and the fill of the staging ring), and CTAs
   // run in waves of one per SM (two for the plain-load form): among the segments that leave at least four waves of
   // CTAs (work that is not uniform -- a blast wave in a corner of the box -- needs them to balance: Sedov 128^3 loses
@@ -2270,7 +2338,19 @@ int step_impl(ch_ctx* c, double dt, bool devdt) {
     const int seg = final_segment(c);
     dim3 grid((unsigned)((g.n[0] + kFX - 3) / (kFX - 2)), (unsigned)((g.n[1] + kFY - 3) / (kFY - 2)),
               (unsigned)((g.n[2] + seg - 1) / seg));
-    if (c->tma_ok && c->use_tma) {
+    if (c->tma_ok && c->use_tma == 2) {
+      // merged producer: kTYM staged rows, the carried arrays for the updating rows only
+      const size_t tsmem = ((size_t)60 * kFX * kTYM + (size_t)10 * kFX * (kTYM - 2)) * sizeof(double);
+      if (!c->smem_attr_mp[S]) {
+        CH_CUDA(cudaFuncSetAttribute(k_final3d_tma<S, false, kTYM, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tsmem), "k_final3d_tma<MP> smem attribute");
+        c->smem_attr_mp[S] = true;
+      }
+      const int pitch = tma_pitch_x(g);
+      dim3 tgrid((unsigned)((g.n[0] + pitch - 1) / pitch), (unsigned)((g.n[1] + kTYM - 3) / (kTYM - 2)),
+                 (unsigned)((g.n[2] + seg - 1) / seg));
+      Bracket b(c, CH_K_FINAL);
+      k_final3d_tma<S, false, kTYM, true><<<tgrid, kFX * (kTYM - 1), tsmem, st>>>(A, c->maps_mp, seg);
+    } else if (c->tma_ok && c->use_tma) {
       const size_t tsmem = (size_t)70 * kTT * sizeof(double);   // 50 staged + 10 exchanged + 10 carried doubles per slot
       if (!c->smem_attr[1][S]) {
         CH_CUDA(cudaFuncSetAttribute(k_final3d_tma<S>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tsmem), "k_final3d_tma smem attribute");
@@ -2512,7 +2592,7 @@ int ch_tiling(const ch_ctx* c, int* out) {
   out[2] = march_segment(c, 1);            // interfaces a marching thread sweeps along y
   out[3] = march_segment(c, 2);            // ... along z
   out[4] = three_d ? (tma ? tma_pitch_x(g) : kFX - 2) : 0;   // updated columns per tile of the fused second half along x
-  out[5] = three_d ? (tma ? kTY : kFY) - 2 : 0;   // ... along y
+  out[5] = three_d ? (c->unfused ? kFY - 2 : final_rows(c)) : 0;   // ... along y
   out[6] = three_d ? final_segment(c) : 0; // planes a CTA of the fused second half marches
   out[7] = tma ? 1 : 0;
   return CH_OK;
@@ -2597,7 +2677,9 @@ int ch_set_option(ch_ctx* c, int option, int value) {
     case CH_OPT_FINAL_SEG:
       if (value != 0 && value < 4) return fail(CH_EINVAL, "ch_set_option: final segment < 4");
       c->final_seg = value; return CH_OK;
-    case CH_OPT_TMA: c->use_tma = value != 0; return CH_OK;
+    case CH_OPT_TMA:
+      if (value < 0 || value > 2) return fail(CH_EINVAL, "ch_set_option: CH_OPT_TMA takes 0 (plain loads), 1 (producer warp) or 2 (merged producer)");
+      c->use_tma = value; return CH_OK;
     case CH_OPT_UNFUSED: c->unfused = value != 0; return CH_OK;
     case CH_OPT_GRAPH: c->use_graph = value != 0; if (!c->use_graph) drop_graph(c); return CH_OK;
     case CH_OPT_FOLD_GHOST: c->fold_ghost = value != 0; drop_graph(c); return CH_OK;

@@ -457,9 +457,11 @@ def test_tma_and_plain_load_forms_of_the_fused_kernel_are_bitwise_equal(ch):
                       (wl.rough_random(44, 26, 70, seed=31, decades=0.3, mach=0.8), 2),
                       (wl.sweep(shape=(64, 40, 36)), 2), (wl.sedov(24), 2)):
         res = {}
-        for mode in ("1", "0"):
+        for mode in ("2", "1", "0"):    # merged producer (13-row tiles, the default), producer warp (12-row tiles), plain loads
             G = ch.Grid(*w.shape, 3, w.gamma, w.bc)
             G.set_option(binding.OPT_TMA, int(mode))
+            t = G.tiling()
+            assert t["tma"] == (mode != "0") and t["final_tile_y"] == {"2": 11, "1": 10, "0": 8}[mode]
             G.set_state(w.u)
             for _ in range(nsteps):
                 G.step(G.compute_dt(w.cfl))
@@ -467,6 +469,7 @@ def test_tma_and_plain_load_forms_of_the_fused_kernel_are_bitwise_equal(ch):
             G.close()
         assert np.all(np.isfinite(res["0"][0]))
         assert np.array_equal(res["0"][0], res["1"][0]) and res["0"][1] == res["1"][1]
+        assert np.array_equal(res["0"][0], res["2"][0]) and res["0"][1] == res["2"][1]
 
 
 # ---- NEXT-1: Roe solver with the HLLE failsafe (B.2) ------------------------------------------------
@@ -532,7 +535,7 @@ def test_roe_tma_and_plain_forms_agree(ch):
     differently in the two, so the comparison is to rounding level rather than bitwise."""
     w = wl.sweep(shape=(64, 40, 70))
     res = {}
-    for mode in ("1", "0"):
+    for mode in ("2", "1", "0"):
         G = ch.Grid(*w.shape, 3, w.gamma, w.bc)
         G.set_option(binding.OPT_TMA, int(mode))
         G.set_solver(1)
@@ -543,6 +546,7 @@ def test_roe_tma_and_plain_forms_agree(ch):
         G.close()
     assert np.all(np.isfinite(res["0"]))
     assert max(max_rel_error(res["0"], res["1"], w.gamma)) <= 1e-14
+    assert max(max_rel_error(res["0"], res["2"], w.gamma)) <= 1e-14
 
 
 # ---- NEXT-2: PLMC and PCM reconstructions (A.2, Eq. 25-26) --------------------------------------------
