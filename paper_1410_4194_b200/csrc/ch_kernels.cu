@@ -1128,7 +1128,7 @@ __global__ void __launch_bounds__(kFT, 2) k_final2d(const StepArgs A, const Scat
 #ifndef CH_T_SLEEP
 #define CH_T_SLEEP 200      // ns between the producer's polls of an empty barrier
 #endif
-constexpr int kTY = CH_T_TY, kTT = kFX * kTY, kTC = kTT - kFX;   // staged rows; threads = staged slots; consumer threads
+constexpr int kTY = CH_T_TY, kTT = kFX * kTY;   // staged rows; threads = staged slots (producer-warp form)
 #ifndef CH_T_TYM
 #define CH_T_TYM 13
 #endif
