@@ -284,7 +284,7 @@ class Grid:
         self._check(self._L.ch_set_origin(self._h, int(i0), int(j0), int(k0)), "ch_set_origin")
 
     def set_option(self, option, value):
-        """Launch-configuration choice (OPT_MARCH_SEG, OPT_FINAL_SEG, OPT_TMA, OPT_UNFUSED); see ch_set_option."""
+        """Launch-configuration choice (OPT_MARCH_SEG, OPT_FINAL_SEG, OPT_TMA: 2 / 1 / 0, OPT_UNFUSED, OPT_GRAPH, OPT_FOLD_GHOST); see ch_set_option."""
         self._check(self._L.ch_set_option(self._h, int(option), int(value)), "ch_set_option")
 
     def tiling(self) -> dict:

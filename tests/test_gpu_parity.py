@@ -531,8 +531,9 @@ def test_roe_runs_match_oracle(ch, ref):
 
 
 def test_roe_tma_and_plain_forms_agree(ch):
-    """Same arithmetic in two kernels; with the Roe solver inlined the compiler contracts a few multiply-adds
-    differently in the two, so the comparison is to rounding level rather than bitwise."""
+    """Same arithmetic in the three forms of the fused kernel (merged producer, producer warp, plain loads), compared
+    to rounding level here; the bitwise comparison is test_tma_and_plain_load_forms_of_the_fused_kernel_are_bitwise_equal
+    (exact solver) and the decomposed Roe runs of tests/test_gpu_decomp.py."""
     w = wl.sweep(shape=(64, 40, 70))
     res = {}
     for mode in ("2", "1", "0"):
@@ -778,6 +779,11 @@ def test_set_option_rejects_unknown_options_and_small_segments(ch):
         G.set_option(binding.OPT_MARCH_SEG, 2)
     G.set_option(binding.OPT_MARCH_SEG, 8)
     G.set_option(binding.OPT_FINAL_SEG, 0)
+    for bad in (-1, 3):     # CH_OPT_TMA names one of three forms of the fused second half
+        with pytest.raises(ValueError):
+            G.set_option(binding.OPT_TMA, bad)
+    for form in (0, 1, 2):
+        G.set_option(binding.OPT_TMA, form)
     G.close()
 
 
