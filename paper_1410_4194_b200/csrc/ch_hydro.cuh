@@ -147,10 +147,10 @@ CH_D void limited_slope(const Gas& G, const double wm[5], const double w0[5], co
   for (int m = 0; m < 5; ++m) { dl[m] = __dadd_rn(w0[m], -wm[m]); dr[m] = __dadd_rn(wp[m], -w0[m]); }
   char_project(ra, ia2, dl[0], dl[1], dl[2], dl[3], dl[4], xL);
   char_project(ra, ia2, dr[0], dr[1], dr[2], dr[3], dr[4], xR);
-  // centred difference (A2) projected the same way
-  char_project(ra, ia2, __dmul_rn(0.5, __dadd_rn(wp[0], -wm[0])), __dmul_rn(0.5, __dadd_rn(wp[1], -wm[1])),
-               __dmul_rn(0.5, __dadd_rn(wp[2], -wm[2])), __dmul_rn(0.5, __dadd_rn(wp[3], -wm[3])),
-               __dmul_rn(0.5, __dadd_rn(wp[4], -wm[4])), xC);
+  // centred difference (A2): (w_{i+1} - w_{i-1})/2 is the mean of the two one-sided differences and the projection is linear,
+  // so its characteristic components are the means of theirs (one rounding apart from projecting it anew)
+#pragma unroll
+  for (int m = 0; m < 5; ++m) xC[m] = __dmul_rn(0.5, __dadd_rn(xL[m], xR[m]));
 #pragma unroll
   for (int m = 0; m < 5; ++m) x[m] = mc_limit_bits(xL[m], xR[m], xC[m]);
   const double s04 = __dadd_rn(x[0], x[4]);
