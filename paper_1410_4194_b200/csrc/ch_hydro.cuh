@@ -12,7 +12,10 @@
 //   * min / max / clamp are compare-selects (no NaN-propagating fmin/fmax emulation);
 //   * B9 and the sampling take f_k, (p/p_k)^z at the converged pressure by a first-order update
 //     from the last Newton iterate (error O(tol^2) = 1e-16) instead of a fresh evaluation;
-//   * the ten-way sampling is folded onto the left wave family by mirroring when u^m < 0.
+//   * the ten-way sampling is folded onto the left wave family by mirroring when u^m < 0;
+//   * PPMC's parabola edges are limited through their deviations from the cell average (A21-A23 are clamps of
+//     dR = R - w and dL = w - L; A24 and A26 follow without the cancellation of 6[w - (L + R)/2]), sign tests read the
+//     high words, and the centred slope's characteristic components are the mean of the one-sided ones.
 //
 // All functions work in the direction-local ordering (rho, v_n, v_t1, v_t2, p).
 #pragma once
